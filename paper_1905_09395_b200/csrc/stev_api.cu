@@ -1,0 +1,741 @@
+// stev_api.cu -- the C ABI of include/stev.h: handles, validation, table images, launch configuration,
+// the pass loop of stev_integrate (integrate -> compact active list -> integrate ...).
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+#include <new>
+
+#include "stev_host.h"
+
+namespace stev {
+
+static thread_local std::string g_error;
+static thread_local stev_stats g_stats{};
+
+void set_error(const std::string &msg) { g_error = msg; }
+int cuda_fail(cudaError_t e, const char *what) {
+  g_error = std::string("CUDA error in ") + what + ": " + cudaGetErrorString(e);
+  return STEV_ECUDA;
+}
+
+int device_sm_count() {
+  static int n = 0;
+  if (n == 0) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return 148;
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) n = 148;
+  }
+  return n;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+static int align_up(int x, int a) { return (x + a - 1) / a * a; }
+
+void build_table_image(const HostMechanism &m, const HostEstimator *e, std::vector<unsigned char> &image, DevTables &tb) {
+  const int S = m.S, R = m.R;
+  tb = DevTables{};
+  tb.S = S;
+  tb.R = R;
+  tb.Rrev = m.Rrev;
+  // gather lists: for species i, every (reaction, signed coefficient) in the caller's reaction order, reactant
+  // entries before product entries -- the order in which the plain definition omega_i = sum_j nu_ij q_j is summed.
+  std::vector<std::vector<unsigned>> gl(S);
+  for (int j = 0; j < R; ++j) {
+    for (int en = m.reac_ptr[j]; en < m.reac_ptr[j + 1]; ++en)
+      gl[m.reac_sp[en]].push_back((unsigned)m.internal_of[j] | ((unsigned)(uint8_t)(int8_t)(-m.reac_nu[en]) << 16));
+    for (int en = m.prod_ptr[j]; en < m.prod_ptr[j + 1]; ++en)
+      gl[m.prod_sp[en]].push_back((unsigned)m.internal_of[j] | ((unsigned)(uint8_t)(int8_t)(m.prod_nu[en]) << 16));
+  }
+  int n_gather = 0;
+  for (auto &v : gl) n_gather += (int)v.size();
+  tb.n_gather = n_gather;
+
+  int off = 0;
+  auto take = [&](int bytes) {
+    int o = off;
+    off = align_up(off + bytes, 16);
+    return o;
+  };
+  tb.o_invW = take(8 * S);
+  tb.o_W = take(8 * S);
+  tb.o_tmid = take(8 * S);
+  tb.o_nasa = take(8 * 2 * kNasaRows * S);
+  tb.o_lnA = take(8 * R);
+  tb.o_b = take(8 * R);
+  tb.o_Ta = take(8 * R);
+  tb.o_dnu = take(8 * R);
+  tb.o_part = take(8 * R);
+  tb.o_orig = take(2 * R);
+  tb.o_gptr = take(2 * (S + 1));
+  tb.o_gent = take(4 * n_gather);
+  if (e) {
+    tb.has_est = 1;
+    tb.H = e->H;
+    tb.n_in = e->n_in;
+    tb.n_out = e->n_out;
+    tb.act = e->act;
+    tb.input_map = e->input_map;
+    tb.h_ref_T = e->h_ref_T;
+    tb.o_eshift = take(4 * e->n_in);
+    tb.o_escale = take(4 * e->n_in);
+    tb.o_W1T = take(4 * e->n_in * e->H);
+    tb.o_b1 = take(4 * e->H);
+    tb.o_W2T = take(4 * e->H * e->n_out);
+    tb.o_b2 = take(4 * e->n_out);
+  }
+  tb.bytes = align_up(off, 128);
+  image.assign(tb.bytes, 0);
+  unsigned char *base = image.data();
+  double *invW = (double *)(base + tb.o_invW), *W = (double *)(base + tb.o_W), *tmid = (double *)(base + tb.o_tmid);
+  double *nasa = (double *)(base + tb.o_nasa);
+  for (int i = 0; i < S; ++i) {
+    invW[i] = 1.0 / m.W[i];
+    W[i] = m.W[i];
+    tmid[i] = m.t_mid[i];
+    for (int rg = 0; rg < 2; ++rg) {
+      const double *a = (rg == 0 ? m.nasa_lo.data() : m.nasa_hi.data()) + 7 * i;
+      double *row = nasa + rg * kNasaRows * S + i;
+      row[0 * S] = a[0]; row[1 * S] = a[1]; row[2 * S] = a[2]; row[3 * S] = a[3]; row[4 * S] = a[4];
+      row[5 * S] = a[1] / 2.0; row[6 * S] = a[2] / 3.0; row[7 * S] = a[3] / 4.0; row[8 * S] = a[4] / 5.0;
+      row[9 * S] = a[5];
+      row[10 * S] = a[2] / 2.0; row[11 * S] = a[3] / 3.0; row[12 * S] = a[4] / 4.0;
+      row[13 * S] = a[6];
+    }
+  }
+  double *lnA = (double *)(base + tb.o_lnA), *bb = (double *)(base + tb.o_b), *Ta = (double *)(base + tb.o_Ta);
+  double *dnu = (double *)(base + tb.o_dnu);
+  unsigned long long *part = (unsigned long long *)(base + tb.o_part);
+  unsigned short *orig = (unsigned short *)(base + tb.o_orig);
+  for (int k = 0; k < R; ++k) {
+    const int j = m.orig_of[k];
+    lnA[k] = clog(m.A[j]);
+    bb[k] = m.b[j];
+    Ta[k] = m.Ea[j] / kRcal;
+    orig[k] = (unsigned short)j;
+    unsigned long long pk = 0;
+    double d = 0.0;
+    int slot = 0;
+    for (int en = m.reac_ptr[j]; en < m.reac_ptr[j + 1]; ++en, ++slot) {
+      pk |= (unsigned long long)(m.reac_sp[en] & 0xff) << (16 * slot);
+      pk |= (unsigned long long)(m.reac_nu[en] & 0xff) << (16 * slot + 8);
+      d = d - (double)m.reac_nu[en];
+    }
+    slot = 0;
+    for (int en = m.prod_ptr[j]; en < m.prod_ptr[j + 1]; ++en, ++slot) {
+      pk |= (unsigned long long)(m.prod_sp[en] & 0xff) << (32 + 16 * slot);
+      pk |= (unsigned long long)(m.prod_nu[en] & 0xff) << (32 + 16 * slot + 8);
+      d = d + (double)m.prod_nu[en];
+    }
+    part[k] = pk;
+    dnu[k] = d;
+  }
+  unsigned short *gptr = (unsigned short *)(base + tb.o_gptr);
+  unsigned *gent = (unsigned *)(base + tb.o_gent);
+  int pos = 0;
+  for (int i = 0; i < S; ++i) {
+    gptr[i] = (unsigned short)pos;
+    for (unsigned v : gl[i]) gent[pos++] = v;
+  }
+  gptr[S] = (unsigned short)pos;
+  if (e) {
+    float *sh = (float *)(base + tb.o_eshift), *sc = (float *)(base + tb.o_escale), *W1T = (float *)(base + tb.o_W1T);
+    float *b1 = (float *)(base + tb.o_b1), *W2T = (float *)(base + tb.o_W2T), *b2 = (float *)(base + tb.o_b2);
+    for (int k = 0; k < e->n_in; ++k) {
+      sh[k] = e->in_shift[k];
+      sc[k] = e->in_scale[k];
+      for (int j = 0; j < e->H; ++j) W1T[k * e->H + j] = e->W1[j * e->n_in + k];
+    }
+    for (int j = 0; j < e->H; ++j) {
+      b1[j] = e->b1[j];
+      for (int o = 0; o < e->n_out; ++o) W2T[j * e->n_out + o] = e->W2[o * e->H + j];
+    }
+    for (int o = 0; o < e->n_out; ++o) b2[o] = e->b2[o];
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+static constexpr size_t kSmemMax = 227 * 1024;   // opt-in dynamic shared memory per block on sm_100
+static constexpr size_t kSmemPerSM = 228 * 1024;
+
+static void make_layout(const DevTables &tb, int G, CellLayout &cl) {
+  const int S = tb.S, R = tb.R, Rrev = tb.Rrev;
+  int o = 0;
+  auto take = [&](int n) {
+    int r = o;
+    o += (n + 1) & ~1;
+    return r;
+  };
+  cl.oY = take(S);
+  cl.oConc = take(S);
+  cl.oG = take(S);
+  cl.oCp = take(S);
+  cl.oH = take(S);
+  cl.oQ = take(R);
+  cl.oRof = take(Rrev);
+  cl.rrev_pad = Rrev;
+  cl.oRing = take(kWindow * Rrev);
+  cl.oHid = take(tb.has_est ? (tb.H + 1) / 2 : 0);
+  // pad the stride so that the groups of a half-warp (one 128-byte shared-memory phase) start in distinct banks
+  int stride = o;
+  if (G < 16) {
+    while (stride % (2 * G) != G) ++stride;
+  }
+  cl.stride = stride;
+}
+
+bool choose_config(const DevTables &tb, int request, LaunchConfig &cfg) {
+  auto fits = [&](int G, LaunchConfig &c) -> bool {
+    make_layout(tb, G, c.cl);
+    const size_t cell_bytes = (size_t)c.cl.stride * 8;
+    const size_t avail = kSmemMax - tb.bytes - 64;
+    const int cells_sm = (int)std::min<size_t>(avail / cell_bytes, 2048 / G);
+    const int per_warp = 32 / G;
+    if (cells_sm < per_warp) return false;
+    c.G = G;
+    if (cells_sm * G <= 512) {
+      // one block per SM holding every cell that fits
+      c.cells_per_block = cells_sm / per_warp * per_warp;
+      c.threads = c.cells_per_block * G;
+      c.blocks_per_sm = 1;
+    } else {
+      c.threads = 256;
+      c.cells_per_block = 256 / G;
+      size_t blk = tb.bytes + (size_t)c.cells_per_block * cell_bytes + 1024;
+      c.blocks_per_sm = (int)std::min<size_t>(kSmemPerSM / blk, 2048 / 256);
+      if (c.blocks_per_sm < 1) return false;
+    }
+    c.smem = tb.bytes + (size_t)c.cells_per_block * cell_bytes;
+    return c.smem <= kSmemMax;
+  };
+  if (request > 0) {
+    if (request > 32 || (request & (request - 1))) return false;
+    return fits(request, cfg);
+  }
+  // heuristic: about ten reactions per lane, then widen until an SM holds at least 12 warps (or G = 32)
+  int G = 1;
+  while (G < 32 && tb.R > 10 * G) G *= 2;
+  LaunchConfig best;
+  bool have = false;
+  for (; G <= 32; G *= 2) {
+    LaunchConfig c;
+    if (!fits(G, c)) continue;
+    best = c;
+    have = true;
+    const int warps_sm = c.threads * c.blocks_per_sm / 32;
+    if (warps_sm >= 12) break;
+  }
+  if (have) cfg = best;
+  return have;
+}
+
+}  // namespace stev
+
+using namespace stev;
+
+// =========================================================================================================
+//                                               C ABI
+// =========================================================================================================
+extern "C" {
+
+const char *stev_last_error(void) { return g_error.c_str(); }
+const char *stev_version(void) { return "stev-b200 0.1 (sm_100a)"; }
+
+void stev_params_default(stev_params *p) {
+  if (!p) return;
+  p->y_step_max = 1.0e-2;
+  p->delta_max = 1.0e-2;
+  p->alpha = 1.0e-5;
+  p->tol_ring = 0.5;
+  p->tol_freq = 0.1;
+  p->r_fac = 2.0;
+  p->rof_min = 7.888609052210118e-31;  // 2^-100
+  p->dft_first_high_bin = 4;
+  p->dft_enable = 1;
+  p->max_steps = 200000;
+  p->energy_mode = STEV_ENERGY_ADIABATIC;
+  p->chunk_steps = 0;
+  p->lanes_per_cell = 0;
+}
+
+void stev_last_stats(stev_stats *out) {
+  if (out) *out = g_stats;
+}
+
+int stev_mechanism_create(const stev_mechanism_desc *d, stev_mechanism **out) {
+  if (!d || !out) { set_error("stev_mechanism_create: null argument"); return STEV_EINVAL; }
+  *out = nullptr;
+  const int S = d->n_species, R = d->n_reactions, E = d->n_elements;
+  if (S < 1 || S > STEV_MAX_SPECIES || R < 1 || R > STEV_MAX_REACTIONS) {
+    set_error("stev_mechanism_create: n_species must be 1..64 and n_reactions 1..512");
+    return STEV_EINVAL;
+  }
+  if (!d->mol_weight || !d->nasa_lo || !d->nasa_hi || !d->t_mid || !d->A || !d->b || !d->Ea || !d->reversible ||
+      !d->reac_ptr || !d->reac_species || !d->reac_nu || !d->prod_ptr || !d->prod_species || !d->prod_nu) {
+    set_error("stev_mechanism_create: null array in descriptor");
+    return STEV_EINVAL;
+  }
+  stev_mechanism *m = new (std::nothrow) stev_mechanism;
+  if (!m) { set_error("out of host memory"); return STEV_EINVAL; }
+  HostMechanism &h = m->host;
+  h.S = S;
+  h.R = R;
+  h.W.assign(d->mol_weight, d->mol_weight + S);
+  h.nasa_lo.assign(d->nasa_lo, d->nasa_lo + 7 * S);
+  h.nasa_hi.assign(d->nasa_hi, d->nasa_hi + 7 * S);
+  h.t_mid.assign(d->t_mid, d->t_mid + S);
+  h.A.assign(d->A, d->A + R);
+  h.b.assign(d->b, d->b + R);
+  h.Ea.assign(d->Ea, d->Ea + R);
+  h.reversible.assign(d->reversible, d->reversible + R);
+  h.reac_ptr.assign(d->reac_ptr, d->reac_ptr + R + 1);
+  h.prod_ptr.assign(d->prod_ptr, d->prod_ptr + R + 1);
+  auto bad = [&](const char *msg) {
+    set_error(std::string("stev_mechanism_create: ") + msg);
+    delete m;
+    return STEV_EINVAL;
+  };
+  for (int i = 0; i < S; ++i)
+    if (!(h.W[i] > 0.0) || !std::isfinite(h.W[i])) return bad("mol_weight must be positive");
+  if (h.reac_ptr[0] != 0 || h.prod_ptr[0] != 0) return bad("CSR pointers must start at 0");
+  for (int j = 0; j < R; ++j) {
+    const int nr = h.reac_ptr[j + 1] - h.reac_ptr[j], np = h.prod_ptr[j + 1] - h.prod_ptr[j];
+    if (nr < 1 || nr > 2 || np < 1 || np > 2) return bad("each reaction needs 1..2 reactant and 1..2 product entries");
+    if (!(h.A[j] > 0.0) || !std::isfinite(h.A[j])) return bad("A must be positive and finite");
+  }
+  h.reac_sp.assign(d->reac_species, d->reac_species + h.reac_ptr[R]);
+  h.reac_nu.assign(d->reac_nu, d->reac_nu + h.reac_ptr[R]);
+  h.prod_sp.assign(d->prod_species, d->prod_species + h.prod_ptr[R]);
+  h.prod_nu.assign(d->prod_nu, d->prod_nu + h.prod_ptr[R]);
+  for (int j = 0; j < R; ++j) {
+    int seen[4], ns = 0;
+    for (int side = 0; side < 2; ++side) {
+      const std::vector<int> &ptr = side ? h.prod_ptr : h.reac_ptr, &sp = side ? h.prod_sp : h.reac_sp,
+                             &nu = side ? h.prod_nu : h.reac_nu;
+      for (int en = ptr[j]; en < ptr[j + 1]; ++en) {
+        if (sp[en] < 0 || sp[en] >= S) return bad("species index out of range");
+        if (nu[en] < 1 || nu[en] > 3) return bad("stoichiometric coefficients must be 1..3");
+        for (int q = 0; q < ns; ++q)
+          if (seen[q] == sp[en]) return bad("a species may appear only once per reaction");
+        seen[ns++] = sp[en];
+      }
+    }
+    if (d->elem_comp && E > 0) {
+      for (int el = 0; el < E; ++el) {
+        double bal = 0.0;
+        for (int en = h.reac_ptr[j]; en < h.reac_ptr[j + 1]; ++en) bal -= h.reac_nu[en] * d->elem_comp[h.reac_sp[en] * E + el];
+        for (int en = h.prod_ptr[j]; en < h.prod_ptr[j + 1]; ++en) bal += h.prod_nu[en] * d->elem_comp[h.prod_sp[en] * E + el];
+        if (std::fabs(bal) > 1e-9) return bad("reaction does not conserve elements");
+      }
+    }
+  }
+  h.internal_of.assign(R, 0);
+  h.orig_of.clear();
+  for (int j = 0; j < R; ++j)
+    if (h.reversible[j]) h.orig_of.push_back(j);
+  h.Rrev = (int)h.orig_of.size();
+  for (int j = 0; j < R; ++j)
+    if (!h.reversible[j]) h.orig_of.push_back(j);
+  for (int k = 0; k < R; ++k) h.internal_of[h.orig_of[k]] = k;
+
+  std::vector<unsigned char> image;
+  build_table_image(h, nullptr, image, m->tb);
+  cudaError_t e = cudaMalloc(&m->d_table, image.size());
+  if (e == cudaSuccess) e = cudaMemcpy(m->d_table, image.data(), image.size(), cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) {
+    delete m;
+    return cuda_fail(e, "mechanism table upload");
+  }
+  *out = m;
+  return STEV_OK;
+}
+
+void stev_mechanism_destroy(stev_mechanism *m) {
+  if (!m) return;
+  if (m->d_table) cudaFree(m->d_table);
+  delete m;
+}
+
+int stev_mechanism_sizes(const stev_mechanism *m, int32_t *S, int32_t *R, int32_t *Rrev) {
+  if (!m) { set_error("null mechanism"); return STEV_EINVAL; }
+  if (S) *S = m->host.S;
+  if (R) *R = m->host.R;
+  if (Rrev) *Rrev = m->host.Rrev;
+  return STEV_OK;
+}
+
+int stev_estimator_load(const stev_mechanism *m, const stev_estimator_desc *d, stev_estimator **out) {
+  if (!d || !out) { set_error("stev_estimator_load: null argument"); return STEV_EINVAL; }
+  *out = nullptr;
+  if (d->n_in < 1 || d->n_in > 64 || d->n_hidden < 8 || d->n_hidden > 128 || d->n_hidden % 8 || d->n_out < 1 || d->n_out > 256) {
+    set_error("stev_estimator_load: need 1 <= n_in <= 64, 8 <= n_hidden <= 128 (multiple of 8), 1 <= n_out <= 256");
+    return STEV_EINVAL;
+  }
+  if (d->activation != STEV_ACT_TANH && d->activation != STEV_ACT_SIGMOID) { set_error("unknown activation"); return STEV_EINVAL; }
+  if (d->input_map != STEV_IN_T && d->input_map != STEV_IN_T_P_Y) { set_error("unknown input_map"); return STEV_EINVAL; }
+  if (!d->in_shift || !d->in_scale || !d->W1 || !d->b1 || !d->W2 || !d->b2) { set_error("null weight array"); return STEV_EINVAL; }
+  if (m) {
+    const int S = m->host.S;
+    if (d->n_out != 2 * S) { set_error("an estimator attached to a mechanism must have n_out = 2 * n_species"); return STEV_EINVAL; }
+    if ((d->input_map == STEV_IN_T && d->n_in != 1) || (d->input_map == STEV_IN_T_P_Y && d->n_in != 2 + S)) {
+      set_error("n_in does not match input_map");
+      return STEV_EINVAL;
+    }
+  }
+  stev_estimator *e = new (std::nothrow) stev_estimator;
+  if (!e) { set_error("out of host memory"); return STEV_EINVAL; }
+  HostEstimator &h = e->host;
+  h.n_in = d->n_in; h.H = d->n_hidden; h.n_out = d->n_out; h.act = d->activation; h.input_map = d->input_map;
+  h.h_ref_T = d->h_ref_temperature;
+  h.in_shift.assign(d->in_shift, d->in_shift + h.n_in);
+  h.in_scale.assign(d->in_scale, d->in_scale + h.n_in);
+  h.W1.assign(d->W1, d->W1 + (size_t)h.H * h.n_in);
+  h.b1.assign(d->b1, d->b1 + h.H);
+  h.W2.assign(d->W2, d->W2 + (size_t)h.n_out * h.H);
+  h.b2.assign(d->b2, d->b2 + h.n_out);
+  e->mech = m;
+  cudaError_t ce = cudaSuccess;
+  if (m) {
+    std::vector<unsigned char> image;
+    build_table_image(m->host, &h, image, e->tb);
+    ce = cudaMalloc(&e->d_table, image.size());
+    if (ce == cudaSuccess) ce = cudaMemcpy(e->d_table, image.data(), image.size(), cudaMemcpyHostToDevice);
+  }
+  if (ce == cudaSuccess) {
+    // standalone parameter block: in_shift, in_scale, W1T [n_in][H], b1, W2T [H][n_out], b2
+    std::vector<float> pb;
+    pb.insert(pb.end(), h.in_shift.begin(), h.in_shift.end());
+    pb.insert(pb.end(), h.in_scale.begin(), h.in_scale.end());
+    for (int k = 0; k < h.n_in; ++k)
+      for (int j = 0; j < h.H; ++j) pb.push_back(h.W1[(size_t)j * h.n_in + k]);
+    pb.insert(pb.end(), h.b1.begin(), h.b1.end());
+    for (int j = 0; j < h.H; ++j)
+      for (int o = 0; o < h.n_out; ++o) pb.push_back(h.W2[(size_t)o * h.H + j]);
+    pb.insert(pb.end(), h.b2.begin(), h.b2.end());
+    e->params_floats = pb.size();
+    ce = cudaMalloc(&e->d_params, pb.size() * sizeof(float));
+    if (ce == cudaSuccess) ce = cudaMemcpy(e->d_params, pb.data(), pb.size() * sizeof(float), cudaMemcpyHostToDevice);
+  }
+  if (ce != cudaSuccess) {
+    stev_estimator_destroy(e);
+    return cuda_fail(ce, "estimator upload");
+  }
+  *out = e;
+  return STEV_OK;
+}
+
+void stev_estimator_destroy(stev_estimator *e) {
+  if (!e) return;
+  if (e->d_table) cudaFree(e->d_table);
+  if (e->d_params) cudaFree(e->d_params);
+  delete e;
+}
+
+}  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------
+// Workspace carving
+// ---------------------------------------------------------------------------------------------------------
+namespace {
+struct Workspace {
+  int *counters;            // [0] queue head, [1] worst status, [2] active count
+  int *list[2];
+  unsigned char *flags;
+  int *block_counts;
+  double *spill;
+  long long spill_stride;
+  size_t bytes;
+};
+size_t rnd256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+Workspace carve(void *base, const DevTables &tb, const stev_params *p, int64_t n) {
+  Workspace w{};
+  size_t off = 0;
+  auto take = [&](size_t bytes) {
+    size_t o = off;
+    off += rnd256(bytes);
+    return base ? (unsigned char *)base + o : (unsigned char *)nullptr;
+  };
+  w.counters = (int *)take(256);
+  if (p->chunk_steps > 0) {
+    w.list[0] = (int *)take(4 * (size_t)n);
+    w.list[1] = (int *)take(4 * (size_t)n);
+    w.flags = take((size_t)n);
+    w.block_counts = (int *)take(4 * ((size_t)n / 1024 + 2));
+    w.spill_stride = 3 + (long long)tb.Rrev * (1 + kWindow);
+    w.spill = (double *)take(8 * (size_t)n * (size_t)w.spill_stride);
+  }
+  w.bytes = off;
+  return w;
+}
+
+int check_params(const stev_params *p) {
+  if (!p) { set_error("null params"); return STEV_EINVAL; }
+  if (!(p->y_step_max > 0) || !(p->delta_max > 0 && p->delta_max <= 1) || !(p->alpha >= 0) || !(p->r_fac > 1) ||
+      !(p->rof_min > 0 && p->rof_min <= 1) || p->dft_first_high_bin < 1 || p->dft_first_high_bin > 6 || p->max_steps < 1 ||
+      (p->energy_mode != 0 && p->energy_mode != 1) || p->chunk_steps < 0) {
+    set_error("stev_params out of range");
+    return STEV_EINVAL;
+  }
+  return STEV_OK;
+}
+
+SolverConsts make_consts(const stev_params *p) {
+  SolverConsts sc;
+  sc.y_step_max = p->y_step_max;
+  sc.delta_max = p->delta_max;
+  sc.alpha = p->alpha;
+  sc.tol_ring = p->tol_ring;
+  sc.tol_freq = p->tol_freq;
+  sc.r_fac = p->r_fac;
+  sc.inv_r_fac = 1.0 / p->r_fac;
+  sc.rof_min = p->rof_min;
+  sc.nhf = p->dft_first_high_bin;
+  sc.dft_enable = p->dft_enable;
+  sc.max_steps = p->max_steps;
+  sc.energy_mode = p->energy_mode;
+  return sc;
+}
+
+int pick_tables(const stev_mechanism *m, const stev_estimator *e, const DevTables **tb, const unsigned char **table) {
+  if (!m) { set_error("null mechanism"); return STEV_EINVAL; }
+  if (e) {
+    if (e->mech != m || !e->d_table) { set_error("estimator was not loaded against this mechanism"); return STEV_EINVAL; }
+    *tb = &e->tb;
+    *table = e->d_table;
+  } else {
+    *tb = &m->tb;
+    *table = m->d_table;
+  }
+  return STEV_OK;
+}
+
+template <typename Args>
+using KernelPtr = void (*)(const Args);
+
+template <int G> void *integrate_fn() { return (void *)stev_integrate_kernel<G>; }
+template <int G> void *rates_fn() { return (void *)stev_rates_kernel<G>; }
+
+void *integrate_kernel_for(int G) {
+  switch (G) {
+    case 1: return integrate_fn<1>();
+    case 2: return integrate_fn<2>();
+    case 4: return integrate_fn<4>();
+    case 8: return integrate_fn<8>();
+    case 16: return integrate_fn<16>();
+    default: return integrate_fn<32>();
+  }
+}
+void *rates_kernel_for(int G) {
+  switch (G) {
+    case 1: return rates_fn<1>();
+    case 2: return rates_fn<2>();
+    case 4: return rates_fn<4>();
+    case 8: return rates_fn<8>();
+    case 16: return rates_fn<16>();
+    default: return rates_fn<32>();
+  }
+}
+}  // namespace
+
+// compaction kernels live in stev_compact.cu
+namespace stev {
+int compact_launch(const unsigned char *flags, const int *list_in, int n, int *list_out, int *count_out, int *block_counts,
+                   cudaStream_t s);
+}
+
+namespace {
+std::mutex g_scratch_mutex;
+void *g_scratch = nullptr;
+size_t g_scratch_bytes = 0;
+cudaStream_t g_host_stream = nullptr;
+}  // namespace
+
+extern "C" {
+
+size_t stev_workspace_bytes(const stev_mechanism *m, const stev_estimator *e, const stev_params *p, int64_t n_cells) {
+  const DevTables *tb;
+  const unsigned char *table;
+  if (!p || n_cells < 0 || pick_tables(m, e, &tb, &table) != STEV_OK) return 0;
+  return carve(nullptr, *tb, p, n_cells).bytes;
+}
+
+int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const stev_params *p, int64_t n, int64_t ld,
+                   double *T, const double *pressure, double *Y, double dt_cfd, int32_t *steps_out, uint8_t *status_out,
+                   void *workspace, size_t workspace_bytes, void *cuda_stream) {
+  const DevTables *tb;
+  const unsigned char *table;
+  int rc = pick_tables(m, est, &tb, &table);
+  if (rc) return rc;
+  if ((rc = check_params(p))) return rc;
+  if (n < 0 || n > 0x7fffffff || ld < n || !(dt_cfd > 0.0) || !std::isfinite(dt_cfd)) {
+    set_error("stev_integrate: need 0 <= n_cells <= 2^31-1, ld >= n_cells, dt_cfd > 0");
+    return STEV_EINVAL;
+  }
+  g_stats = stev_stats{};
+  g_stats.total_steps = -1;
+  if (n == 0) return STEV_OK;
+  if (!T || !pressure || !Y || !steps_out) { set_error("stev_integrate: null state pointer"); return STEV_EINVAL; }
+  Workspace need = carve(nullptr, *tb, p, n);
+  if (!workspace || workspace_bytes < need.bytes || ((uintptr_t)workspace & 255)) {
+    set_error("stev_integrate: workspace missing, misaligned or smaller than stev_workspace_bytes()");
+    return STEV_EWORKSPACE;
+  }
+  LaunchConfig cfg;
+  if (!choose_config(*tb, p->lanes_per_cell, cfg)) {
+    set_error("stev_integrate: no launch configuration fits shared memory for this mechanism / lanes_per_cell");
+    return STEV_EINVAL;
+  }
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  Workspace w = carve(workspace, *tb, p, n);
+  void *fn = integrate_kernel_for(cfg.G);
+  STEV_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem));
+
+  IntegrateArgs a{};
+  a.tb = *tb;
+  a.table = table;
+  a.cl = cfg.cl;
+  a.sc = make_consts(p);
+  a.t_f = dt_cfd;
+  a.ld = ld;
+  a.T = T;
+  a.p = pressure;
+  a.Y = Y;
+  a.steps = steps_out;
+  a.status = status_out;
+  a.queue_head = w.counters;
+  a.worst_status = w.counters + 1;
+  a.chunk_steps = p->chunk_steps;
+  a.flags = w.flags;
+  a.spill = w.spill;
+  a.spill_stride = w.spill_stride;
+
+  const int sms = device_sm_count();
+  long long n_active = n;
+  int cur = 0;
+  STEV_CUDA(cudaMemsetAsync(w.counters, 0, 256, s));
+  for (int pass = 0; n_active > 0; ++pass) {
+    a.n_active = n_active;
+    a.list = (pass == 0) ? nullptr : w.list[cur];
+    a.restore = (pass > 0);
+    long long blocks = std::min<long long>((long long)sms * cfg.blocks_per_sm, (n_active + cfg.cells_per_block - 1) / cfg.cells_per_block);
+    if (pass > 0) STEV_CUDA(cudaMemsetAsync(w.counters, 0, 4, s));
+    void *args[] = {&a};
+    STEV_CUDA(cudaLaunchKernel(fn, dim3((unsigned)blocks), dim3(cfg.threads), args, cfg.smem, s));
+    g_stats.passes += 1;
+    g_stats.kernel_launches += 1;
+    g_stats.blocks = (int)blocks;
+    if (p->chunk_steps <= 0) break;
+    int rcc = compact_launch(w.flags, a.list, (int)n_active, w.list[cur ^ 1], w.counters + 2, w.block_counts, s);
+    if (rcc) return rcc;
+    g_stats.kernel_launches += 3;
+    int count = 0;
+    STEV_CUDA(cudaMemcpyAsync(&count, w.counters + 2, 4, cudaMemcpyDeviceToHost, s));
+    STEV_CUDA(cudaStreamSynchronize(s));
+    n_active = count;
+    cur ^= 1;
+  }
+  int worst = 0;
+  STEV_CUDA(cudaMemcpyAsync(&worst, w.counters + 1, 4, cudaMemcpyDeviceToHost, s));
+  STEV_CUDA(cudaStreamSynchronize(s));
+  STEV_CUDA(cudaGetLastError());
+  g_stats.lanes_per_cell = cfg.G;
+  g_stats.threads_per_block = cfg.threads;
+  g_stats.cells_per_block = cfg.cells_per_block;
+  g_stats.smem_bytes = (int64_t)cfg.smem;
+  if (worst == 2) { set_error("some cells produced non-finite values (status 2)"); return STEV_WNONFINITE; }
+  if (worst == 1) { set_error("some cells stopped at max_steps (status 1)"); return STEV_WMAXSTEPS; }
+  return STEV_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Host-buffer entry point: grow-only device scratch owned by the library.
+// ---------------------------------------------------------------------------------------------------------
+int stev_integrate_host(const stev_mechanism *m, const stev_estimator *est, const stev_params *p, int64_t n, int64_t ld,
+                        double *T, const double *pressure, double *Y, double dt_cfd, int32_t *steps_out, uint8_t *status_out) {
+  if (!m) { set_error("null mechanism"); return STEV_EINVAL; }
+  if (n == 0) return STEV_OK;
+  if (n < 0 || ld < n || !T || !pressure || !Y || !steps_out) { set_error("stev_integrate_host: bad argument"); return STEV_EINVAL; }
+  std::lock_guard<std::mutex> lock(g_scratch_mutex);
+  const int S = m->host.S;
+  const size_t ws = stev_workspace_bytes(m, est, p, n);
+  if (p == nullptr) { set_error("null params"); return STEV_EINVAL; }
+  size_t off = 0;
+  auto take = [&](size_t b) { size_t o = off; off += rnd256(b); return o; };
+  const size_t oT = take(8 * (size_t)n), oP = take(8 * (size_t)n), oY = take(8 * (size_t)n * S), oS = take(4 * (size_t)n),
+               oSt = take((size_t)n), oW = take(ws);
+  if (off > g_scratch_bytes) {
+    if (g_scratch) cudaFree(g_scratch);
+    g_scratch = nullptr;
+    g_scratch_bytes = 0;
+    STEV_CUDA(cudaMalloc(&g_scratch, off));
+    g_scratch_bytes = off;
+  }
+  if (!g_host_stream) STEV_CUDA(cudaStreamCreateWithFlags(&g_host_stream, cudaStreamNonBlocking));
+  unsigned char *b = (unsigned char *)g_scratch;
+  cudaStream_t s = g_host_stream;
+  STEV_CUDA(cudaMemcpyAsync(b + oT, T, 8 * (size_t)n, cudaMemcpyHostToDevice, s));
+  STEV_CUDA(cudaMemcpyAsync(b + oP, pressure, 8 * (size_t)n, cudaMemcpyHostToDevice, s));
+  if (ld == n) {
+    STEV_CUDA(cudaMemcpyAsync(b + oY, Y, 8 * (size_t)n * S, cudaMemcpyHostToDevice, s));
+  } else {
+    STEV_CUDA(cudaMemcpy2DAsync(b + oY, 8 * (size_t)n, Y, 8 * (size_t)ld, 8 * (size_t)n, S, cudaMemcpyHostToDevice, s));
+  }
+  int rc = stev_integrate(m, est, p, n, n, (double *)(b + oT), (const double *)(b + oP), (double *)(b + oY), dt_cfd,
+                          (int32_t *)(b + oS), (uint8_t *)(b + oSt), b + oW, ws, s);
+  if (rc < 0) return rc;
+  stev_stats keep = g_stats;
+  STEV_CUDA(cudaMemcpyAsync(T, b + oT, 8 * (size_t)n, cudaMemcpyDeviceToHost, s));
+  if (ld == n) {
+    STEV_CUDA(cudaMemcpyAsync(Y, b + oY, 8 * (size_t)n * S, cudaMemcpyDeviceToHost, s));
+  } else {
+    STEV_CUDA(cudaMemcpy2DAsync(Y, 8 * (size_t)ld, b + oY, 8 * (size_t)n, 8 * (size_t)n, S, cudaMemcpyDeviceToHost, s));
+  }
+  STEV_CUDA(cudaMemcpyAsync(steps_out, b + oS, 4 * (size_t)n, cudaMemcpyDeviceToHost, s));
+  if (status_out) STEV_CUDA(cudaMemcpyAsync(status_out, b + oSt, (size_t)n, cudaMemcpyDeviceToHost, s));
+  STEV_CUDA(cudaStreamSynchronize(s));
+  long long tot = 0;
+  for (int64_t c = 0; c < n; ++c) tot += steps_out[c];
+  keep.total_steps = tot;
+  g_stats = keep;
+  return rc;
+}
+
+int stev_rates_eval(const stev_mechanism *m, const stev_estimator *est, const stev_params *p, int64_t n, int64_t ld,
+                    const double *T, const double *pressure, const double *Y, const double *rOF, double *dYdt, double *dTdt,
+                    double *q, void *cuda_stream) {
+  const DevTables *tb;
+  const unsigned char *table;
+  int rc = pick_tables(m, est, &tb, &table);
+  if (rc) return rc;
+  if ((rc = check_params(p))) return rc;
+  if (n < 0 || ld < n) { set_error("stev_rates_eval: bad sizes"); return STEV_EINVAL; }
+  if (n == 0) return STEV_OK;
+  if (!T || !pressure || !Y || !dYdt || !dTdt || !q) { set_error("stev_rates_eval: null pointer"); return STEV_EINVAL; }
+  LaunchConfig cfg;
+  if (!choose_config(*tb, p->lanes_per_cell, cfg)) { set_error("no launch configuration fits"); return STEV_EINVAL; }
+  void *fn = rates_kernel_for(cfg.G);
+  STEV_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem));
+  RatesArgs a{};
+  a.tb = *tb;
+  a.table = table;
+  a.cl = cfg.cl;
+  a.sc = make_consts(p);
+  a.n = n;
+  a.ld = ld;
+  a.T = T;
+  a.p = pressure;
+  a.Y = Y;
+  a.rOF = rOF;
+  a.dYdt = dYdt;
+  a.dTdt = dTdt;
+  a.q = q;
+  long long blocks = std::min<long long>((long long)device_sm_count() * cfg.blocks_per_sm, (n + cfg.cells_per_block - 1) / cfg.cells_per_block);
+  void *args[] = {&a};
+  STEV_CUDA(cudaLaunchKernel(fn, dim3((unsigned)blocks), dim3(cfg.threads), args, cfg.smem, (cudaStream_t)cuda_stream));
+  STEV_CUDA(cudaGetLastError());
+  return STEV_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,67 @@
+// stev_host.h -- host-side handle types and helpers shared by the translation units of libstev_b200.so.
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+#include "../../include/stev.h"
+#include "stev_device.cuh"
+
+namespace stev {
+
+void set_error(const std::string &msg);
+int cuda_fail(cudaError_t e, const char *what);
+#define STEV_CUDA(call)                                        \
+  do {                                                         \
+    cudaError_t e__ = (call);                                  \
+    if (e__ != cudaSuccess) return ::stev::cuda_fail(e__, #call); \
+  } while (0)
+
+struct HostEstimator {
+  int n_in = 0, H = 0, n_out = 0, act = 0, input_map = 0;
+  float h_ref_T = 1000.f;
+  std::vector<float> in_shift, in_scale, W1, b1, W2, b2;  // caller's row-major layouts
+};
+
+// Host copy of a mechanism in the caller's ordering plus derived quantities.
+struct HostMechanism {
+  int S = 0, R = 0, Rrev = 0;
+  std::vector<double> W, nasa_lo, nasa_hi, t_mid, A, b, Ea;
+  std::vector<uint8_t> reversible;
+  std::vector<int> reac_ptr, reac_sp, reac_nu, prod_ptr, prod_sp, prod_nu;
+  std::vector<int> internal_of;  // caller reaction index -> internal index (reversible first)
+  std::vector<int> orig_of;      // internal -> caller
+};
+
+// Builds the table image for a mechanism and, optionally, an estimator.
+void build_table_image(const HostMechanism &m, const HostEstimator *e, std::vector<unsigned char> &image, DevTables &tb);
+
+struct LaunchConfig {
+  int G = 1, threads = 128, cells_per_block = 128, blocks_per_sm = 1;
+  size_t smem = 0;
+  CellLayout cl{};
+};
+// Chooses lanes per cell, block shape and the per-cell shared-memory layout.  Returns false if nothing fits.
+bool choose_config(const DevTables &tb, int lanes_per_cell_request, LaunchConfig &cfg);
+
+int device_sm_count();
+
+}  // namespace stev
+
+struct stev_mechanism {
+  stev::HostMechanism host;
+  stev::DevTables tb{};
+  unsigned char *d_table = nullptr;
+};
+
+struct stev_estimator {
+  stev::HostEstimator host;
+  const stev_mechanism *mech = nullptr;  // the mechanism it was loaded against (may be null)
+  stev::DevTables tb{};                  // mechanism + estimator image (only if mech != null)
+  unsigned char *d_table = nullptr;
+  // standalone evaluation (stev_estimator_eval): device copies in kernel-friendly layouts
+  float *d_params = nullptr;             // in_shift, in_scale, W1T [n_in][H], b1, W2T [H][n_out], b2
+  size_t params_floats = 0;
+};
