@@ -1,0 +1,316 @@
+#!/usr/bin/env python
+"""bench.py -- cells advanced through dt_cfd per second (BASELINE.json's metric) on N B200s.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--cells n] [--impl reference]
+
+A "step" is one pass of the whole hot path (rows a1-a7) over one batch of synthetic cells:
+one `stev_integrate` call that takes every cell from t = 0 to t = dt_cfd.  The default workload is BASELINE.json's
+config 3 (1,048,576 cells, 53 species / 325 reactions, MLP cp/h), the configuration the north star's target is stated
+on.  State is resident in HBM when the timed region starts and is restored from a pristine device copy between steps
+(outside the CUDA-event pairs).  Under torchrun every rank integrates its own interleaved shard of an N-times larger
+field (weak scaling; cells are independent, so there is no data-path collective); the time is the max
+over ranks.
+
+`--impl reference` times the CPU oracle (oracle/, test infrastructure) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "cells advanced through dt_cfd per second"
+UNIT = "cells/s"
+
+
+def _env_int(name, default):
+    try:
+        return int(os.environ.get(name, default))
+    except ValueError:
+        return default
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config index 0..4 (default 3: the target config)")
+    ap.add_argument("--cells", type=int, default=None, help="cells per GPU (default: the config's full size)")
+    ap.add_argument("--impl", default="stev", choices=["stev", "reference"])
+    ap.add_argument("--chunk-steps", type=int, default=0)
+    ap.add_argument("--lanes", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--ref-cells", type=int, default=None, help="cells per step of the --impl reference arm")
+    return ap.parse_args()
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# clocks: nvidia-smi sampled DURING the timed region (B200_PROFILING.md "clocks line")
+# ----------------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.proc = None
+        self.path = f"/tmp/stev_clocks_{os.getpid()}.csv"
+        try:
+            self.f = open(self.path, "w")
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.FIELDS}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f,
+                                         stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self) -> dict:
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        self.f.close()
+        sm, smax, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        try:
+            for line in open(self.path):
+                parts = [x.strip() for x in line.split(",")]
+                if len(parts) < 7:
+                    continue
+                try:
+                    sm.append(float(parts[0]))
+                    smax.append(float(parts[1]))
+                    power.append(float(parts[2]))
+                except ValueError:
+                    continue
+                for nm, v in zip(names, parts[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+            os.unlink(self.path)
+        except OSError:
+            pass
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(smax)), reasons=sorted(reasons), samples=len(sm),
+                       power_w_max=float(max(power)))
+        return out
+
+
+# ----------------------------------------------------------------------------------------------------------------
+def oracle_time(w, n_cells: int, n_threads: int | None = None):
+    """Times the CPU oracle, as it stands, on the first n_cells of workload w.  Returns (cells/s, seconds, cell_steps, threads)."""
+    from oracle import stev_oracle
+    n = min(n_cells, w.n_cells)
+    t0 = time.perf_counter()
+    r = stev_oracle.integrate(w.mech, w.estimator, w.params, w.T[:n], w.p[:n], np.ascontiguousarray(w.Y[:, :n]), w.dt_cfd,
+                              n_threads=n_threads)
+    dt = time.perf_counter() - t0
+    return n / dt, dt, int(r["steps"].sum()), r["n_threads"]
+
+
+def run_reference(args):
+    """The reference arm of this tier IS the oracle: plain CPU fp64 STEV on the box's host cores, bounded sample."""
+    rank = _env_int("RANK", 0)
+    if rank != 0:
+        return 0
+    from stev_inputs.configs import make_workload, FULL_CELLS
+    from oracle import stev_oracle
+    stev_oracle.build()
+    cores = os.cpu_count() or 1
+    per_step = args.ref_cells or {0: 4096, 1: 256, 2: 256, 3: 32 * cores, 4: 128}[args.config]
+    w = make_workload(args.config, per_step * (args.steps + args.warmup))
+    times, steps_total = [], 0
+    for s in range(args.warmup + args.steps):
+        lo = s * per_step
+        sub = type(w)(config=w.config, name=w.name, mech=w.mech, estimator=w.estimator, params=w.params, dt_cfd=w.dt_cfd,
+                      T=w.T[lo:lo + per_step], p=w.p[lo:lo + per_step], Y=np.ascontiguousarray(w.Y[:, lo:lo + per_step]),
+                      blocks=w.blocks)
+        cps, dt, cs, thr = oracle_time(sub, per_step, cores)
+        if s >= args.warmup:
+            times.append(dt)
+            steps_total += cs
+    total = sum(times)
+    value = per_step * args.steps / total
+    sample = f"{per_step} cells per step (consecutive seeded cells of {w.name}), {args.steps} steps"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "cells_full": FULL_CELLS[args.config], "cells_per_step": per_step,
+                       "species": w.mech.n_species, "reactions": w.mech.n_reactions, "dt_cfd": w.dt_cfd},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": thr, "kind": "oracle", "sample": sample,
+                             "cell_steps_per_s": steps_total / total},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ----------------------------------------------------------------------------------------------------------------
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import paper_1905_09395_b200 as stev
+    from paper_1905_09395_b200 import multi, workmodel
+    from stev_inputs.configs import make_workload, FULL_CELLS
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback (use --impl reference for the oracle arm)")
+    ctx = multi.init(args.gpus)
+    rank, world, dev = ctx.rank, ctx.world, ctx.device
+    stev.load()
+
+    n = FULL_CELLS[args.config] if args.cells is None else args.cells
+    w = make_workload(args.config, n, rank=rank, world=world, weak=True)
+    S = w.mech.n_species
+    mech = stev.Mechanism(w.mech)
+    est = stev.Estimator(mech, w.estimator) if w.estimator is not None else None
+    prm = stev.stev_params_default(chunk_steps=args.chunk_steps, lanes_per_cell=args.lanes, **w.params)
+
+    T0 = torch.tensor(w.T, dtype=torch.float64, device=dev)
+    p = torch.tensor(w.p, dtype=torch.float64, device=dev)
+    Y0 = torch.tensor(w.Y, dtype=torch.float64, device=dev)
+    T, Y = torch.empty_like(T0), torch.empty_like(Y0)
+    steps = torch.zeros(n, dtype=torch.int32, device=dev)
+    status = torch.zeros(n, dtype=torch.uint8, device=dev)
+    ws = torch.empty(max(stev.stev_workspace_bytes(mech, est, prm, n), 256), dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+
+    def one_step(timed: bool):
+        T.copy_(T0)
+        Y.copy_(Y0)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        rc = stev.stev_integrate(mech, est, prm, T, p, Y, w.dt_cfd, steps, status, workspace=ws, stream=stream)
+        e1.record(stream)
+        e1.synchronize()
+        return e0.elapsed_time(e1), rc, stev.stev_last_stats()
+
+    for _ in range(max(args.warmup, 0)):
+        one_step(False)
+
+    # fp64 throughput probes for the roofline denominator (outside the timed region)
+    dfma_per_s = stev.stev_microbench(0, 4096)
+    cexp_per_s = stev.stev_microbench(1, 512)
+
+    multi.barrier(ctx)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(ctx.local_rank) if rank == 0 else None
+    t_wall0 = time.perf_counter()
+    ms, launches, rc = [], 0, 0
+    for _ in range(args.steps):
+        m, rc, st = one_step(True)
+        ms.append(m)
+        launches += st["kernel_launches"]
+    torch.cuda.synchronize()
+    multi.barrier(ctx)
+    t_wall = time.perf_counter() - t_wall0
+    clocks = sampler.stop() if sampler else None
+
+    total_ms = multi.max_over_ranks(ctx, float(sum(ms)))
+    steps_h = steps.cpu().numpy().astype(np.int64)
+    status_h = status.cpu().numpy()
+    cell_steps_rank = int(steps_h.sum())
+    finished_rank = int((status_h == 0).sum())
+    cell_steps_all = multi.sum_over_ranks(ctx, cell_steps_rank)
+    finished_all = multi.sum_over_ranks(ctx, finished_rank)
+    ms_per_step = total_ms / args.steps
+    value = world * n / (ms_per_step * 1e-3)
+
+    # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        Th0 = torch.tensor(w.T, dtype=torch.float64).pin_memory()
+        ph = torch.tensor(w.p, dtype=torch.float64).pin_memory()
+        Yh0 = torch.tensor(w.Y, dtype=torch.float64).pin_memory()
+        Th, Yh = torch.empty_like(Th0).pin_memory(), torch.empty_like(Yh0).pin_memory()
+        sh = torch.zeros(n, dtype=torch.int32).pin_memory()
+        sth = torch.zeros(n, dtype=torch.uint8).pin_memory()
+        reps = max(1, min(args.steps, 2))
+        tt = []
+        for k in range(1 + reps):
+            Th.copy_(Th0)
+            Yh.copy_(Yh0)
+            multi.barrier(ctx)
+            t0 = time.perf_counter()
+            stev.stev_integrate_host(mech, est, prm, Th, ph, Yh, w.dt_cfd, sh, sth)
+            dt = time.perf_counter() - t0
+            if k > 0:
+                tt.append(dt)
+        e2e_s = multi.max_over_ranks(ctx, float(sum(tt))) / reps
+        same = bool(np.array_equal(sh.numpy(), steps_h) and np.array_equal(Yh.numpy(), Y.cpu().numpy()))
+        e2e = {"value": world * n / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 8 * n * (2 + S),
+               "d2h_bytes_per_step": 8 * n * (1 + S) + 5 * n, "steps": reps, "ms_per_step": 1e3 * e2e_s,
+               "matches_device_path_bitwise": same, "api": "stev_integrate_host (pinned host buffers)"}
+
+    if rank != 0:
+        multi.finish(ctx)
+        return 0
+
+    # ---- roofline of the dominant kernel (stev_integrate_kernel: one launch per step when chunk_steps = 0)
+    work = workmodel.cell_step_work(w.mech, w.estimator, dft_enable=bool(w.params["dft_enable"]),
+                                    first_high_bin=w.params["dft_first_high_bin"], alpha_on=w.params["alpha"] > 0,
+                                    adiabatic=w.params["energy_mode"] == 0)
+    kernel_s = (sum(ms) / args.steps) * 1e-3  # CUDA events on the launching stream around the launch(es) of one step
+    flop = work.fp64_flop * cell_steps_rank
+    instr = work.fp64_instr * cell_steps_rank
+    sm_max = (clocks or {}).get("sm_max_mhz") or 1965.0
+    peak_instr = workmodel.fp64_peak_instr_per_s(sm_max)
+    peak_tflops = 2.0 * peak_instr / 1e12
+    roofline = {"bound": "alu", "kernel": f"stev_integrate_kernel<{st['lanes_per_cell']}>",
+                "achieved": flop / kernel_s / 1e12, "peak": peak_tflops, "unit": "TFLOP/s",
+                "frac": flop / kernel_s / 1e12 / peak_tflops, "traffic": None,
+                "peak_source": f"derived: 148 SM x 64 DFMA/clk x 2 x {sm_max:.0f} MHz (DESIGN.md section 8); not in MEASURED_PEAKS.json",
+                "fp64_instr": {"achieved_per_s": instr / kernel_s, "peak_per_s": peak_instr,
+                               "frac": instr / kernel_s / peak_instr, "measured_dfma_per_s": dfma_per_s,
+                               "frac_of_measured_dfma": instr / kernel_s / dfma_per_s,
+                               "measured_contract_exp_per_s": cexp_per_s},
+                "per_cell_step": {"fp64_fma": work.fma, "fp64_other": work.other, "fp32_fma": work.fp32_fma,
+                                  "hbm_bytes": 0},
+                "cell_steps_per_launch": cell_steps_rank / max(1, st["passes"]),
+                "hbm_bytes_per_launch": n * (8 * (2 + S) + 8 * (1 + S) + 5)}
+
+    cpu_baseline = None
+    if not args.no_cpu_baseline:
+        cores = os.cpu_count() or 1
+        n_s = {0: 4096, 1: 1024, 2: 512, 3: 96 * cores, 4: 256}[args.config]
+        n_s = min(n_s, n)
+        cps, dt, cs, thr = oracle_time(w, n_s, cores)
+        cpu_baseline = {"value": cps, "unit": UNIT, "cores": thr, "kind": "oracle",
+                        "sample": f"first {n_s} cells of this rank's field, {dt:.1f} s", "cell_steps_per_s": cs / dt}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": w.name, "cells_per_gpu": n, "species": S, "reactions": w.mech.n_reactions,
+                       "reversible": w.mech.n_reversible, "dt_cfd": w.dt_cfd,
+                       "estimator": None if w.estimator is None else f"mlp {w.estimator.n_in}-{w.estimator.n_hidden}-{w.estimator.n_out} fp32",
+                       "parallelism": f"cells sharded over {world} GPU(s), no collective",
+                       "l2": f"inputs larger than L2 ({(8 * n * (2 + S)) >> 20} MiB of state per GPU, restored between steps)",
+                       "chunk_steps": args.chunk_steps, "lanes_per_cell": st["lanes_per_cell"],
+                       "threads_per_block": st["threads_per_block"], "blocks": st["blocks"], "smem_bytes": st["smem_bytes"]},
+            "cell_steps_per_s": cell_steps_all / (ms_per_step * 1e-3), "mean_steps_per_cell": cell_steps_all / (world * n),
+            "finished_fraction": finished_all / (world * n), "return_code": rc,
+            "wall_s_timed_region": t_wall, "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
+            "roofline": roofline, "cpu_baseline": cpu_baseline}
+    print(json.dumps(line), flush=True)
+    multi.finish(ctx)
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -190,7 +190,8 @@ def test_mechanism_validation(stev):
     import copy
     m = copy.deepcopy(make_mechanism(1))
     m.prod_species = m.prod_species.copy()
-    m.prod_species[0] = (m.prod_species[0] + 1) % 9      # break element conservation
+    used = set(m.reac_species[:2]) | set(m.prod_species[:2])
+    m.prod_species[0] = next(i for i in range(9) if i not in used)   # break element conservation of reaction 0
     with pytest.raises(stev.StevError):
         stev.Mechanism(m)
     stev.Mechanism(m, validate_elements=False).close()
