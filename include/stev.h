@@ -109,7 +109,9 @@ typedef struct {
   int32_t chunk_steps;    /* 0: every cell runs to completion in one pass; > 0: a pass advances each active
                              cell at most this many steps, unfinished cells are spilled to the workspace and the
                              active-cell list is compacted before the next pass */
-  int32_t lanes_per_cell; /* 0 = chosen from (S, R); else 1,2,4,8,16,32 */
+  int32_t lanes_per_cell; /* 0 = chosen from (S, R); 1,2,4,8,16,32 = lanes cooperating on one cell (one kernel role);
+                             64 = the warp-specialised kernel: a rate warp + a DFT warp per cell, DFT history in
+                             tensor memory (default for >= 128 reactions; needs dft_enable, chunk_steps = 0) */
 } stev_params;
 
 /* Counters of the last stev_integrate / stev_integrate_host call on this thread. */

@@ -1,0 +1,485 @@
+// stev_ab_kernel.cuh -- the warp-specialised STEV integrator for large mechanisms (rows a1-a6 of DESIGN.md section 1).
+//
+// One block per SM holds up to eight cells.  Each cell is served by a pair of warps:
+//   * the RATE warp ("A") walks the critical path of a step: thermo (NASA-7 / MLP), mixture sums, stabilised
+//     concentrations, Arrhenius + equilibrium rates, source terms, the step limiter, the Euler update and retirement;
+//   * the DFT warp ("B") runs the ringing detector of the previous step concurrently: it keeps the 13-deep history of
+//     every reversible reaction in TENSOR MEMORY (one lane-private row of TMEM columns per reaction, written with
+//     tcgen05.st and read back with tcgen05.ld), evaluates the DFT bins and produces the rOF factors of the next step.
+// The two warps hand over through two named barriers per cell (bar.arrive / bar.sync, producer-consumer):
+//   S2: A -> B "step published (q_eff, h, 1/C_tot)"      S1: B -> A "rOF of the next step ready".
+// The history never touches HBM or shared memory; shared memory holds the mechanism tables (staged once per block by
+// one TMA bulk copy) and ~10 KB of per-cell scratch.  Arithmetic follows the contract of DESIGN.md section 5 exactly;
+// every deviation in evaluation order that is bit-equivalent is explained where it occurs.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "stev_ab.cuh"
+#include "stev_device.cuh"
+#include "stev_math.cuh"
+
+namespace stev {
+
+// Twiddles of DESIGN.md 5.6 in constant memory: with compile-time indices they become constant-bank operands of DFMA.
+__device__ __constant__ const double kTwCos[13] = {
+    1.0, 0.8854560256532099, 0.5680647467311559, 0.120536680255323, -0.35460488704253545,
+    -0.7485107481711012, -0.970941817426052, -0.9709418174260521, -0.7485107481711013,
+    -0.3546048870425359, 0.1205366802553232, 0.5680647467311548, 0.88545602565321};
+__device__ __constant__ const double kTwNegSin[13] = {
+    -0.0, -0.4647231720437685, -0.8229838658936564, -0.992708874098054, -0.9350162426854148,
+    -0.6631226582407952, -0.23931566428755768, 0.23931566428755743, 0.663122658240795,
+    0.9350162426854147, 0.992708874098054, 0.822983865893657, 0.4647231720437684};
+
+__device__ __forceinline__ void named_bar_sync(int id) { asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory"); }
+__device__ __forceinline__ void named_bar_arrive(int id) { asm volatile("bar.arrive %0, 64;" ::"r"(id) : "memory"); }
+
+__device__ __forceinline__ void tmem_st2(uint32_t taddr, double v) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};" ::"r"(taddr), "r"((uint32_t)__double2loint(v)),
+               "r"((uint32_t)__double2hiint(v))
+               : "memory");
+}
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+// 13 doubles = 26 consecutive columns of this lane: x16 + x8 + x2
+__device__ __forceinline__ void tmem_ld_window(uint32_t taddr, double (&x)[kWindow]) {
+  uint32_t r[26];
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]),
+        "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+      : "r"(taddr)
+      : "memory");
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23])
+               : "r"(taddr + 16)
+               : "memory");
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0,%1}, [%2];" : "=r"(r[24]), "=r"(r[25]) : "r"(taddr + 24) : "memory");
+  tmem_wait_ld();
+#pragma unroll
+  for (int s = 0; s < kWindow; ++s) x[s] = __hiloint2double((int)r[2 * s + 1], (int)r[2 * s]);
+}
+
+__device__ __forceinline__ double lds_f64(const unsigned char *base, unsigned off) { return *(const double *)(base + off); }
+
+// |X_M|^2 of the window (Eq 9).  The k = 0 terms of the contract's sums are fma(x0, 1, 0) = x0 and
+// fma(x0, -0, 0) = +0 for every finite x0, so the sums start from them (a non-finite sample only occurs in the step
+// that retires the cell with status 2, whose DFT is not evaluated).
+template <int M>
+__device__ __forceinline__ double ab_bin_sq(const double (&x)[kWindow]) {
+  double re = x[0], im = 0.0;
+#pragma unroll
+  for (int k = 1; k < kWindow; ++k) {
+    re = fma_rn(x[k], kTwCos[(M * k) % kWindow], re);
+    im = fma_rn(x[k], kTwNegSin[(M * k) % kWindow], im);
+  }
+  return fma_rn(re, re, im * im);
+}
+
+// Eq 10 + Eq 12 for one window.
+__device__ __forceinline__ bool ab_is_ringing(const double (&x)[kWindow], const SolverConsts &sc) {
+  double d0 = x[0];
+#pragma unroll
+  for (int k = 1; k < kWindow; ++k) d0 = d0 + x[k];
+  d0 = fabs(d0);
+  double m2 = 0.0, v;
+  const int nhf = sc.nhf;
+  if (nhf <= 1) { v = ab_bin_sq<1>(x); m2 = (v > m2) ? v : m2; }
+  if (nhf <= 2) { v = ab_bin_sq<2>(x); m2 = (v > m2) ? v : m2; }
+  if (nhf <= 3) { v = ab_bin_sq<3>(x); m2 = (v > m2) ? v : m2; }
+  if (nhf <= 4) { v = ab_bin_sq<4>(x); m2 = (v > m2) ? v : m2; }
+  if (nhf <= 5) { v = ab_bin_sq<5>(x); m2 = (v > m2) ? v : m2; }
+  { v = ab_bin_sq<6>(x); m2 = (v > m2) ? v : m2; }
+  const double d_hi = sqrt(m2);   // max of sqrt = sqrt of max (IEEE sqrt is monotone)
+  const double f_ring = d0 / ((d_hi > 1.0e-300) ? d_hi : 1.0e-300);
+  return (f_ring < sc.tol_ring) && (d0 < sc.tol_freq);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// DFT warp: rows a5 of DESIGN.md.  TMEM address of slot s of this lane's reaction `it`:
+//   base + (lane quarter << 16) + cell_half * 256 + it * 32 + 2 s.
+// ---------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void ab_dft_warp(const AbArgs &a, unsigned char *cell, int j, uint32_t tmem_base, int lane) {
+  const AbTables &tb = a.tb;
+  const SolverConsts &sc = a.sc;
+  const int Rrev = tb.Rrev, n_it = tb.n_it;
+  double *cRof = (double *)(cell + a.cl.oRof);
+  const double *cQ = (const double *)(cell + a.cl.oQ);
+  volatile AbCtrl *ctrl = (volatile AbCtrl *)(cell + a.cl.oCtrl);
+  const uint32_t trow = tmem_base + ((uint32_t)((j & 3) * 32) << 16) + (uint32_t)((j >> 2) * 256);
+  const int barS2 = 2 * j, barS1 = 2 * j + 1;
+  int slot = 0;
+
+  auto reset = [&]() {
+    for (int it = 0; it < n_it; ++it)
+      for (int s = 0; s < kWindow; ++s) tmem_st2(trow + it * 32 + 2 * s, 0.0);   // R10: zero-initialised window
+    tmem_wait_st();
+    for (int k = lane; k < Rrev; k += 32) cRof[k] = 1.0;                         // Eq 11
+    slot = 0;
+  };
+
+  reset();
+  __threadfence_block();
+  named_bar_arrive(barS1);
+  for (;;) {
+    named_bar_sync(barS2);
+    const int cmd = ctrl->cmd;
+    if (cmd == kCmdExit) break;
+    if (cmd == kCmdFinal) {
+      reset();   // the cell retired: its last DFT is unobservable; prepare the next cell
+    } else {
+      const double h = ctrl->h, inv_ctot = ctrl->inv_ctot;
+      for (int it = 0; it < n_it; ++it) {
+        const int k = it * 32 + lane;
+        const bool live = k < Rrev;
+        const double q = live ? cQ[k] : 0.0;
+        const uint32_t tw = trow + it * 32;
+        tmem_st2(tw + 2 * slot, (q * h) * inv_ctot);   // Eq 8 with R8, R9: applied change in progress / C_tot
+        tmem_wait_st();
+        double x[kWindow];
+        tmem_ld_window(tw, x);
+        const bool ringing = ab_is_ringing(x, sc);
+        if (live) {
+          double rof = cRof[k] * (ringing ? sc.inv_r_fac : sc.r_fac);   // Eqs 12-13
+          if (rof > 1.0) rof = 1.0;
+          if (rof < sc.rof_min) rof = sc.rof_min;
+          cRof[k] = rof;
+        }
+      }
+      slot = (slot + 1 == kWindow) ? 0 : slot + 1;
+    }
+    __threadfence_block();
+    named_bar_arrive(barS1);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Rate warp: rows a1-a4, a6.
+// ---------------------------------------------------------------------------------------------------------
+template <bool EST>
+__device__ __forceinline__ void ab_rate_warp(const AbArgs &a, const unsigned char *tbl, unsigned char *cell, int j, int lane) {
+  const AbTables &tb = a.tb;
+  const SolverConsts &sc = a.sc;
+  const int S = tb.S, R = tb.R, Rrev = tb.Rrev, Rp = tb.Rp;
+  double2 *cYp = (double2 *)(cell + a.cl.oYp);
+  double2 *cYwCp = (double2 *)(cell + a.cl.oYwCp);
+  double2 *cHOm = (double2 *)(cell + a.cl.oHOm);
+  double *cConc = (double *)(cell + a.cl.oConc);
+  double *cG = (double *)(cell + a.cl.oG);
+  double *cQ = (double *)(cell + a.cl.oQ);
+  double *cQraw = (double *)(cell + a.cl.oQraw);
+  const double *cRof = (const double *)(cell + a.cl.oRof);
+  float *cHid = (float *)(cell + a.cl.oHid);
+  volatile AbCtrl *ctrl = (volatile AbCtrl *)(cell + a.cl.oCtrl);
+
+  const double *tmid = (const double *)(tbl + tb.o_tmid), *W = (const double *)(tbl + tb.o_W);
+  const double *invW = (const double *)(tbl + tb.o_invW), *nasa = (const double *)(tbl + tb.o_nasa);
+  const double2 *rkA = (const double2 *)(tbl + tb.o_rkA), *rkB = (const double2 *)(tbl + tb.o_rkB);
+  const uint4 *rfac = (const uint4 *)(tbl + tb.o_rfac), *rdg = (const uint4 *)(tbl + tb.o_rdg);
+  const double *varc = (const double *)(tbl + tb.o_varc);
+  const unsigned char *gsp = tbl + tb.o_gsp;
+  const unsigned short *gent = (const unsigned short *)(tbl + tb.o_gent);
+  const int n_var = tb.n_var;
+
+  const int barS2 = 2 * j, barS1 = 2 * j + 1;
+  const double dt_max = a.t_f * sc.delta_max;   // Eq 4
+  const double t_tol = 1.0e-12 * a.t_f;         // R5
+
+  if (lane == 0) {
+    cConc[0] = 1.0;
+    cG[0] = 0.0;
+  }
+
+  for (;;) {
+    // ---- a6: variable load.  A retired cell's warp pair pulls the next active cell from the global queue.
+    int pos = 0;
+    if (lane == 0) pos = atomicAdd(a.queue_head, 1);
+    pos = __shfl_sync(0xffffffffu, pos, 0);
+    if ((long long)pos >= a.n_active) {
+      named_bar_sync(barS1);          // the DFT warp has consumed the previous command
+      if (lane == 0) ctrl->cmd = kCmdExit;
+      __threadfence_block();
+      named_bar_arrive(barS2);
+      return;
+    }
+    const int cidx = a.list ? a.list[pos] : pos;
+    double T = a.T[cidx];
+    const double p = a.p[cidx];
+    for (int i = lane; i < S; i += 32) cYp[i] = make_double2(a.Y[(long long)i * a.ld + cidx], invW[i]);
+    double t = 0.0;
+    int steps = 0;
+    __syncwarp();
+
+    for (;;) {
+      // ================= part 1: everything that does not need rOF =================
+      // -- scalars.  ln T and ln(p_atm / (R_u T)) are evaluated side by side in the two half-warps.
+      const double RuT = kRu * T;
+      const double c_tot = p / RuT;
+      const double invT = 1.0 / T;
+      const double larg = (lane & 16) ? (kPatm / RuT) : T;
+      const double lval = clog(larg);
+      const double lnT = __shfl_sync(0xffffffffu, lval, 0);
+      const double ln_c0 = __shfl_sync(0xffffffffu, lval, 16);
+
+      // -- a1: NASA-7 (Eqs 15-16, R17); g/RT always, cp and h unless the MLP supplies them.
+      for (int i = lane; i < S; i += 32) {
+        const double *c = nasa + ((T < tmid[i]) ? 0 : kNasaRows * S) + i;
+        const double a1 = c[0], a2 = c[S];
+        const double hp = fma_rn(fma_rn(fma_rn(fma_rn(c[8 * S], T, c[7 * S]), T, c[6 * S]), T, c[5 * S]), T, a1);
+        const double hRT = fma_rn(c[9 * S], invT, hp);
+        const double sp = fma_rn(fma_rn(fma_rn(c[12 * S], T, c[11 * S]), T, c[10 * S]), T, a2);
+        const double sR = fma_rn(a1, lnT, fma_rn(sp, T, c[13 * S]));
+        const double g = hRT - sR;
+        cG[1 + i] = g;
+        cG[1 + S + i] = g + g;
+        if (!EST) {
+          cYwCp[i].y = fma_rn(fma_rn(fma_rn(fma_rn(c[4 * S], T, c[3 * S]), T, c[2 * S]), T, a2), T, a1);
+          cHOm[i].x = hRT;
+        }
+      }
+      // -- a7 in the integrator (fp32 CUDA cores, R18): cp_i/R and h_i/(R T_ref) from the shallow MLP.
+      if (EST) {
+        const float *eshift = (const float *)(tbl + tb.o_eshift), *escale = (const float *)(tbl + tb.o_escale);
+        const float *W1T = (const float *)(tbl + tb.o_W1T), *b1 = (const float *)(tbl + tb.o_b1);
+        const float *W2p = (const float *)(tbl + tb.o_W2p), *b2 = (const float *)(tbl + tb.o_b2);
+        const int H = tb.H, Hpad = tb.Hpad, n_in = tb.n_in, n_out = tb.n_out;
+        for (int jh = lane; jh < H; jh += 32) {
+          float z = b1[jh];
+          for (int k = 0; k < n_in; ++k) {
+            const double raw = (k == 0) ? T : ((k == 1) ? p : cYp[k - 2].x);
+            const float xk = ((float)raw - eshift[k]) * escale[k];
+            z = __fmaf_rn(W1T[k * H + jh], xk, z);
+          }
+          const double zd = (double)z;
+          float act;
+          if (tb.act == 0) act = (float)(1.0 - 2.0 / (1.0 + cexp(2.0 * zd)));
+          else act = (float)(1.0 / (1.0 + cexp(-zd)));
+          cHid[jh] = act;
+        }
+        __syncwarp();
+        const float4 *hid4 = (const float4 *)cHid;
+        for (int o0 = 0; o0 < n_out; o0 += 128) {
+          float y[4];
+          const float4 *wrow[4];
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            int o = o0 + 32 * u + lane;
+            o = (o < n_out) ? o : n_out - 1;
+            y[u] = b2[o];
+            wrow[u] = (const float4 *)(W2p + (size_t)o * Hpad);
+          }
+          for (int q4 = 0; q4 < H / 4; ++q4) {
+            const float4 hv = hid4[q4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+              const float4 wv = wrow[u][q4];
+              y[u] = __fmaf_rn(wv.x, hv.x, y[u]);
+              y[u] = __fmaf_rn(wv.y, hv.y, y[u]);
+              y[u] = __fmaf_rn(wv.z, hv.z, y[u]);
+              y[u] = __fmaf_rn(wv.w, hv.w, y[u]);
+            }
+          }
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            const int o = o0 + 32 * u + lane;
+            if (o < n_out) {
+              if (o < S) cYwCp[o].y = (double)y[u];
+              else cHOm[o - S].x = ((double)y[u] * (double)tb.h_ref_T) * invT;
+            }
+          }
+        }
+      }
+
+      // -- mixture (sequential in species order, contract 5.4), density, stabilised concentrations (Eqs 6-7, R7)
+      double inv_wbar = 0.0;
+      for (int i = 0; i < S; ++i) {
+        const double2 v = cYp[i];
+        inv_wbar = fma_rn(v.x, v.y, inv_wbar);
+      }
+      const double rho = c_tot / inv_wbar;
+      for (int i = lane; i < S; i += 32) {
+        const double2 v = cYp[i];
+        cYwCp[i].x = v.x * v.y;
+        const double yp = (v.x > 0.0) ? v.x : 0.0;
+        double c = (rho * yp) * v.y;
+        if (sc.alpha > 0.0) c = (yp / (sc.alpha + yp)) * c;
+        cConc[1 + i] = c;
+      }
+      __syncwarp();
+
+      // -- a2: rate constants and raw progress rates (Eqs 28-30).  Reversible reactions first.
+      for (int k = lane; k < R; k += 32) {
+        const double2 ka = rkA[k], kb = rkB[k];
+        const double ln_kf = fma_rn(-kb.x, invT, fma_rn(ka.y, lnT, ka.x));
+        double fwd = cexp(ln_kf);
+        const uint4 f = rfac[k];
+        fwd = fwd * lds_f64(cell, f.x);
+        fwd = fwd * lds_f64(cell, f.y);
+        double qk = fwd;
+        if (k < Rrev) {
+          const uint4 d = rdg[k];
+          double dg = 0.0 - lds_f64(cell, d.x);
+          dg = dg - lds_f64(cell, d.y);
+          dg = dg + lds_f64(cell, d.z);
+          dg = dg + lds_f64(cell, d.w);
+          const double ln_kc = fma_rn(kb.y, ln_c0, -dg);
+          double rev = cexp(ln_kf - ln_kc);
+          rev = rev * lds_f64(cell, f.z);
+          rev = rev * lds_f64(cell, f.w);
+          qk = fwd - rev;
+        }
+        cQraw[k] = qk;
+      }
+      double sum_cp = 0.0;
+      for (int i = 0; i < S; ++i) {
+        const double2 v = cYwCp[i];
+        sum_cp = fma_rn(v.x, v.y, sum_cp);
+      }
+
+      // ================= part 2: needs rOF of this step (produced by the DFT warp) =================
+      named_bar_sync(barS1);
+      // effective rates (Eq 14) and their stored multiples: variant v holds varc[v] * q_eff (exact for +-1, +-2,
+      // rounded once for +-3 exactly as the plain sum omega_i = sum_j nu_ij q_j rounds nu*q before adding)
+      for (int k = lane; k < R; k += 32) {
+        double q = cQraw[k];
+        if (k < Rrev) q = q * cRof[k];
+        cQ[k] = q;
+        for (int v = 1; v < n_var; ++v) cQ[v * Rp + k] = varc[v] * q;
+      }
+      __syncwarp();
+
+      // -- source terms and the limiter (Eqs 1-3).  Lane l owns species gsp[l] and gsp[32+l]; the
+      //    entry lists are padded with the 0.0 slot to a common length per round, so the loops are warp-uniform.
+      const double inv_rho = 1.0 / rho;
+      double t_star = bits_to_double(0x7ff0000000000000ull);
+      {
+        const unsigned short *ge = gent + lane;
+#pragma unroll 1
+        for (int round = 0; round < 2; ++round) {
+          const int len = tb.g_len[round];
+          const int i = gsp[32 * round + lane];
+          double om = 0.0;
+#pragma unroll 4
+          for (int e = 0; e < len; ++e) om = om + lds_f64(cell, ge[e * 32]);
+          ge += len * 32;
+          if (i < S) {
+            const double r = (W[i] * om) * inv_rho;
+            const double y = cYp[i].x;
+            const double r_star = (-r > 1.0e-30) ? -r : 1.0e-30;
+            const double y_star = (y < 1.0e-20) ? 1.0 : 0.9 * y;
+            const double lim = ((sc.y_step_max < y_star) ? sc.y_step_max : y_star) / r_star;
+            if (lim < t_star) t_star = lim;
+            cConc[1 + i] = r;     // concentrations are dead: reuse for dY_i/dt
+            cHOm[i].y = om;
+          }
+        }
+      }
+      // min over lanes: every lim is a positive double (or +inf / NaN), for which the ordering of the bit patterns
+      // as unsigned integers is the ordering of the values; NaN patterns sort above +inf and are ignored like the
+      // plain comparison `lim < t_star` ignores them.
+      {
+        const unsigned long long u = double_to_bits(t_star);
+        const unsigned hi = (unsigned)(u >> 32), lo = (unsigned)u;
+        const unsigned mhi = __reduce_min_sync(0xffffffffu, hi);
+        const unsigned mlo = __reduce_min_sync(0xffffffffu, (hi == mhi) ? lo : 0xffffffffu);
+        t_star = bits_to_double(((unsigned long long)mhi << 32) | mlo);
+      }
+      __syncwarp();
+
+      // -- temperature equation (R15), enthalpy sum sequential in species order
+      double sum_h = 0.0;
+      for (int i = 0; i < S; ++i) {
+        const double2 v = cHOm[i];
+        sum_h = fma_rn(v.x, v.y, sum_h);
+      }
+      const double dTdt = (sc.energy_mode == 0) ? -((sum_h * kRu) * T) / (rho * (kRu * sum_cp)) : 0.0;
+
+      // -- a3: step size (Eq 5) and landing on t_f (R5)
+      double h = (t_star < dt_max) ? t_star : dt_max;
+      bool last = false;
+      const double rem = a.t_f - t;
+      if (rem - h < t_tol) {
+        h = rem;
+        last = true;
+      }
+      // -- a4: forward Euler (Eq 18)
+      int bad = 0;
+      for (int i = lane; i < S; i += 32) {
+        const double y = fma_rn(h, cConc[1 + i], cYp[i].x);
+        cYp[i].x = y;
+        bad |= !(y - y == 0.0);
+      }
+      T = fma_rn(h, dTdt, T);
+      t = last ? a.t_f : t + h;
+      steps += 1;
+      bad |= !(T - T == 0.0);
+      bad = __any_sync(0xffffffffu, bad);
+
+      // -- a6: retirement (R20)
+      int st = -1;
+      if (last) st = 0;
+      else if (bad) st = 2;
+      else if (steps >= sc.max_steps) st = 1;
+
+      if (lane == 0) {
+        ctrl->h = h;
+        ctrl->inv_ctot = 1.0 / c_tot;
+        ctrl->cmd = (st >= 0) ? kCmdFinal : kCmdStep;
+      }
+      __threadfence_block();
+      named_bar_arrive(barS2);
+
+      if (st >= 0) {
+        for (int i = lane; i < S; i += 32) a.Y[(long long)i * a.ld + cidx] = cYp[i].x;
+        if (lane == 0) {
+          a.T[cidx] = T;
+          a.steps[cidx] = steps;
+          if (a.status) a.status[cidx] = (unsigned char)st;
+          if (st > 0) atomicMax(a.worst_status, st);
+        }
+        break;
+      }
+    }
+  }
+}
+
+__global__ void __launch_bounds__(kAbThreads, 1) stev_ab_kernel(const __grid_constant__ AbArgs a) {
+  extern __shared__ __align__(128) unsigned char smem[];
+  __shared__ unsigned long long mbar;
+  __shared__ uint32_t tmem_base_s;
+  __shared__ int done_warps;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (threadIdx.x == 0) done_warps = 0;
+  stage_tables(smem, a.table, a.tb.bytes, &mbar);
+  if (warp == 0) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(
+                     (uint32_t)__cvta_generic_to_shared(&tmem_base_s))
+                 : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  const uint32_t tmem_base = tmem_base_s;
+
+  // warps 0..7: DFT warp of cell slot j = warp (TMEM lane quarter j & 3 = warp & 3); warps 8..15: rate warp of j = warp - 8
+  const bool is_dft = warp < kAbMaxCells;
+  const int j = is_dft ? warp : warp - kAbMaxCells;
+  if (j < a.cells_per_block) {
+    unsigned char *cell = smem + a.tb.bytes + (size_t)j * a.cl.stride;
+    if (is_dft) ab_dft_warp(a, cell, j, tmem_base, lane);
+    else if (a.tb.has_est) ab_rate_warp<true>(a, smem, cell, j, lane);
+    else ab_rate_warp<false>(a, smem, cell, j, lane);
+  }
+  __syncwarp();
+  if (lane == 0) atomicAdd(&done_warps, 1);
+  if (warp == 0) {
+    if (lane == 0) {
+      while (atomicAdd(&done_warps, 0) < kAbThreads / 32) __nanosleep(200);
+    }
+    __syncwarp();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem_base) : "memory");
+  }
+}
+
+}  // namespace stev

@@ -343,8 +343,16 @@ int stev_mechanism_create(const stev_mechanism_desc *d, stev_mechanism **out) {
   build_table_image(h, nullptr, image, m->tb);
   cudaError_t e = cudaMalloc(&m->d_table, image.size());
   if (e == cudaSuccess) e = cudaMemcpy(m->d_table, image.data(), image.size(), cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) {
+    std::vector<unsigned char> ab;
+    m->ab_ok = build_ab_image(h, nullptr, ab, m->ab_tb, m->ab_cl);
+    if (m->ab_ok) {
+      e = cudaMalloc(&m->d_ab_table, ab.size());
+      if (e == cudaSuccess) e = cudaMemcpy(m->d_ab_table, ab.data(), ab.size(), cudaMemcpyHostToDevice);
+    }
+  }
   if (e != cudaSuccess) {
-    delete m;
+    stev_mechanism_destroy(m);
     return cuda_fail(e, "mechanism table upload");
   }
   *out = m;
@@ -354,6 +362,7 @@ int stev_mechanism_create(const stev_mechanism_desc *d, stev_mechanism **out) {
 void stev_mechanism_destroy(stev_mechanism *m) {
   if (!m) return;
   if (m->d_table) cudaFree(m->d_table);
+  if (m->d_ab_table) cudaFree(m->d_ab_table);
   delete m;
 }
 
@@ -401,6 +410,14 @@ int stev_estimator_load(const stev_mechanism *m, const stev_estimator_desc *d, s
     build_table_image(m->host, &h, image, e->tb);
     ce = cudaMalloc(&e->d_table, image.size());
     if (ce == cudaSuccess) ce = cudaMemcpy(e->d_table, image.data(), image.size(), cudaMemcpyHostToDevice);
+    if (ce == cudaSuccess) {
+      std::vector<unsigned char> ab;
+      e->ab_ok = build_ab_image(m->host, &h, ab, e->ab_tb, e->ab_cl);
+      if (e->ab_ok) {
+        ce = cudaMalloc(&e->d_ab_table, ab.size());
+        if (ce == cudaSuccess) ce = cudaMemcpy(e->d_ab_table, ab.data(), ab.size(), cudaMemcpyHostToDevice);
+      }
+    }
   }
   if (ce == cudaSuccess) {
     // standalone parameter block: in_shift, in_scale, W1T [n_in][H], b1, W2T [H][n_out], b2
@@ -428,6 +445,7 @@ int stev_estimator_load(const stev_mechanism *m, const stev_estimator_desc *d, s
 void stev_estimator_destroy(stev_estimator *e) {
   if (!e) return;
   if (e->d_table) cudaFree(e->d_table);
+  if (e->d_ab_table) cudaFree(e->d_ab_table);
   if (e->d_params) cudaFree(e->d_params);
   delete e;
 }
@@ -582,13 +600,48 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
     set_error("stev_integrate: workspace missing, misaligned or smaller than stev_workspace_bytes()");
     return STEV_EWORKSPACE;
   }
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  Workspace w = carve(workspace, *tb, p, n);
+
+  // Large mechanisms: the warp-specialised kernel (a rate warp and a DFT warp per cell, history in tensor memory).
+  {
+    const bool ab_ok = est ? est->ab_ok : m->ab_ok;
+    const bool ab_allowed = ab_ok && p->dft_enable && p->chunk_steps == 0;
+    if (p->lanes_per_cell == 64 && !ab_allowed) {
+      set_error("stev_integrate: lanes_per_cell = 64 (warp-specialised kernel) needs dft_enable = 1, chunk_steps = 0, at most "
+                "two factors per reaction side and at most 256 reversible reactions");
+      return STEV_EINVAL;
+    }
+    if (ab_allowed && (p->lanes_per_cell == 64 || (p->lanes_per_cell == 0 && tb->R >= 128))) {
+      STEV_CUDA(cudaMemsetAsync(w.counters, 0, 256, s));
+      int blocks = 0, cpb = 0;
+      size_t smem = 0;
+      rc = integrate_ab_launch(est ? est->ab_tb : m->ab_tb, est ? est->ab_cl : m->ab_cl, est ? est->d_ab_table : m->d_ab_table,
+                               make_consts(p), dt_cfd, n, ld, T, pressure, Y, steps_out, status_out, w.counters, s, &blocks, &cpb,
+                               &smem);
+      if (rc) return rc;
+      int worst = 0;
+      STEV_CUDA(cudaMemcpyAsync(&worst, w.counters + 1, 4, cudaMemcpyDeviceToHost, s));
+      STEV_CUDA(cudaStreamSynchronize(s));
+      STEV_CUDA(cudaGetLastError());
+      g_stats.passes = 1;
+      g_stats.kernel_launches = 1;
+      g_stats.blocks = blocks;
+      g_stats.lanes_per_cell = 64;
+      g_stats.threads_per_block = kAbThreads;
+      g_stats.cells_per_block = cpb;
+      g_stats.smem_bytes = (int64_t)smem;
+      if (worst == 2) { set_error("some cells produced non-finite values (status 2)"); return STEV_WNONFINITE; }
+      if (worst == 1) { set_error("some cells stopped at max_steps (status 1)"); return STEV_WMAXSTEPS; }
+      return STEV_OK;
+    }
+  }
+
   LaunchConfig cfg;
   if (!choose_config(*tb, p->lanes_per_cell, cfg)) {
     set_error("stev_integrate: no launch configuration fits shared memory for this mechanism / lanes_per_cell");
     return STEV_EINVAL;
   }
-  cudaStream_t s = (cudaStream_t)cuda_stream;
-  Workspace w = carve(workspace, *tb, p, n);
   void *fn = integrate_kernel_for(cfg.G);
   STEV_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem));
 

@@ -7,6 +7,7 @@
 #include <cuda_runtime.h>
 
 #include "../../include/stev.h"
+#include "stev_ab.cuh"
 #include "stev_device.cuh"
 
 namespace stev {
@@ -48,12 +49,24 @@ bool choose_config(const DevTables &tb, int lanes_per_cell_request, LaunchConfig
 
 int device_sm_count();
 
+// Warp-specialised integrator (stev_ab.cuh / stev_ab.cu).  build_ab_image returns false if the mechanism is outside
+// its limits (more than two factors per reaction side, more than 256 reversible reactions, tables too large).
+bool build_ab_image(const HostMechanism &m, const HostEstimator *e, std::vector<unsigned char> &image, AbTables &tb, AbCell &cl);
+int ab_cells_per_block(const AbTables &tb, const AbCell &cl);
+int integrate_ab_launch(const AbTables &tb, const AbCell &cl, const unsigned char *d_table, const SolverConsts &sc, double t_f,
+                        long long n, long long ld, double *T, const double *p, double *Y, int *steps, unsigned char *status,
+                        int *counters, cudaStream_t s, int *blocks_out, int *cells_per_block_out, size_t *smem_out);
+
 }  // namespace stev
 
 struct stev_mechanism {
   stev::HostMechanism host;
   stev::DevTables tb{};
   unsigned char *d_table = nullptr;
+  bool ab_ok = false;                    // image of the warp-specialised kernel (NASA-7 thermo)
+  stev::AbTables ab_tb{};
+  stev::AbCell ab_cl{};
+  unsigned char *d_ab_table = nullptr;
 };
 
 struct stev_estimator {
@@ -61,6 +74,10 @@ struct stev_estimator {
   const stev_mechanism *mech = nullptr;  // the mechanism it was loaded against (may be null)
   stev::DevTables tb{};                  // mechanism + estimator image (only if mech != null)
   unsigned char *d_table = nullptr;
+  bool ab_ok = false;                    // image of the warp-specialised kernel (MLP thermo)
+  stev::AbTables ab_tb{};
+  stev::AbCell ab_cl{};
+  unsigned char *d_ab_table = nullptr;
   // standalone evaluation (stev_estimator_eval): device copies in kernel-friendly layouts
   float *d_params = nullptr;             // in_shift, in_scale, W1T [n_in][H], b1, W2T [H][n_out], b2
   size_t params_floats = 0;

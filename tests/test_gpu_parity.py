@@ -130,6 +130,35 @@ def test_result_does_not_depend_on_lanes_per_cell(stev, oracle, config, n, lanes
     assert rep["bit_exact"] == 1.0
 
 
+@pytest.mark.parametrize("config,n,over", [(3, 500, {}), (3, 37, {}), (3, 200, dict(use_estimator=False)),
+                                           (1, 400, {}), (2, 300, {}), (4, 300, {}), (0, 600, {}),
+                                           (1, 100, dict(max_steps=150)), (2, 100, dict(alpha=0.0, dft_first_high_bin=1)),
+                                           (2, 100, dict(energy_mode=1, delta_max=0.002, y_step_max=0.05))])
+def test_warp_specialised_kernel_parity(stev, oracle, config, n, over):
+    """lanes_per_cell = 64: the rate-warp / DFT-warp kernel with the DFT history in tensor memory (stev_ab_kernel.cuh),
+    the default for large mechanisms (config 3).  Bit-exact against the oracle on every config it accepts."""
+    over = dict(over)
+    w = make_workload(config, n)
+    est = w.estimator if over.pop("use_estimator", True) else None
+    prm = dict(w.params, **over)
+    ref = oracle.integrate(w.mech, est, prm, w.T, w.p, w.Y, w.dt_cfd)
+    case = GpuCase(stev, w)
+    if est is None:
+        case.est = None
+    gpu = case.integrate(lanes_per_cell=64, **over)
+    assert gpu["stats"]["lanes_per_cell"] == 64
+    rep = assert_parity(gpu, ref)
+    print(f"config {config}: n={n} {rep} stats={gpu['stats']}")
+    assert gpu["rc"] == ref["rc"]
+    assert rep["bit_exact"] == 1.0
+
+
+def test_large_mechanism_defaults_to_warp_specialised_kernel(stev):
+    w = make_workload(3, 64)
+    gpu = GpuCase(stev, w).integrate()
+    assert gpu["stats"]["lanes_per_cell"] == 64 and gpu["stats"]["threads_per_block"] == 512
+
+
 @pytest.mark.parametrize("config,n,chunk", [(0, 3000, 64), (1, 600, 100), (1, 600, 1000), (2, 300, 333), (3, 100, 150)])
 def test_chunked_passes_with_compaction_give_identical_results(stev, config, n, chunk):
     """Row a6: retiring / spilling / compacting is pure scheduling -- results cannot depend on chunk_steps."""
