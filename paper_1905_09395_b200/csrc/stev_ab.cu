@@ -69,21 +69,24 @@ bool build_ab_image(const HostMechanism &m, const HostEstimator *e, std::vector<
   // which the plain definition omega_i = sum_j nu_ij q_j adds them (same as the oracle's scatter, per species)
   struct Ent { int k, coef; };
   std::vector<std::vector<Ent>> gl(S);
-  std::vector<int> variants = {1};
+  // stored multiples of q, fixed order: +1, -1 (always), +2, -2 (if any coefficient is +-2)
+  const int variants[4] = {1, -1, 2, -2};
+  bool has2 = false;
   auto variant_of = [&](int coef) {
-    for (size_t v = 0; v < variants.size(); ++v)
-      if (variants[v] == coef) return (int)v;
-    variants.push_back(coef);
-    return (int)variants.size() - 1;
+    for (int v = 0; v < 4; ++v)
+      if (variants[v] == coef) return v;
+    return -1;
   };
   for (int j = 0; j < R; ++j) {
     for (int en = m.reac_ptr[j]; en < m.reac_ptr[j + 1]; ++en) gl[m.reac_sp[en]].push_back({m.internal_of[j], -m.reac_nu[en]});
     for (int en = m.prod_ptr[j]; en < m.prod_ptr[j + 1]; ++en) gl[m.prod_sp[en]].push_back({m.internal_of[j], m.prod_nu[en]});
   }
   for (auto &v : gl)
-    for (auto &en : v) variant_of(en.coef);
-  tb.n_var = (int)variants.size();
-  if (tb.n_var > kAbMaxVariants) return false;
+    for (auto &en : v) {
+      if (variant_of(en.coef) < 0) return false;
+      has2 = has2 || en.coef == 2 || en.coef == -2;
+    }
+  tb.n_var = has2 ? 4 : 2;
   ab_layout(tb, cl);
 
   // species -> (round, lane): the 32 longest lists in round 0, the rest in round 1 (each round is as long as its
@@ -116,7 +119,6 @@ bool build_ab_image(const HostMechanism &m, const HostEstimator *e, std::vector<
   tb.o_rkB = take(16 * R);
   tb.o_rfac = take(16 * R);
   tb.o_rdg = take(16 * Rrev);
-  tb.o_varc = take(8 * tb.n_var);
   tb.o_gsp = take(64);
   tb.o_gent = take(2 * 32 * std::max(g_total, 1));
   if (e) {
@@ -177,8 +179,6 @@ bool build_ab_image(const HostMechanism &m, const HostEstimator *e, std::vector<
     std::memcpy(rfac + 4 * k, fac, 16);
     if (k < Rrev) std::memcpy(rdg + 4 * k, dgo, 16);
   }
-  double *varc = (double *)(base + tb.o_varc);
-  for (int v = 0; v < tb.n_var; ++v) varc[v] = (double)variants[v];
   std::memcpy(base + tb.o_gsp, gsp, 64);
   unsigned short *gent = (unsigned short *)(base + tb.o_gent);
   for (int round = 0, row0 = 0; round < 2; ++round) {

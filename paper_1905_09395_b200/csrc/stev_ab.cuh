@@ -9,21 +9,19 @@ namespace stev {
 constexpr int kAbMaxCells = 8;       // cells per block: 2 per TMEM lane quarter x 4 quarters
 constexpr int kAbMaxIt = 8;          // reversible reactions per lane (32 TMEM columns each, 256 columns per cell)
 constexpr int kAbThreads = 64 * kAbMaxCells;
-constexpr int kAbMaxVariants = 6;    // stored multiples of q: +-1, +-2, +-3
 
 // Table image of the AB kernel (one contiguous buffer, copied verbatim to shared memory).  Byte offsets.
 struct AbTables {
   int S, R, Rrev, n_it, Rp;            // Rp: row length of the q-variant array (R rounded up to even)
   int has_est, H, Hpad, n_in, n_out, act, input_map;
   float h_ref_T;
-  int n_var;                           // stored multiples of q (variant 0 is +1)
+  int n_var;                           // stored multiples of q: 2 (+q, -q) or 4 (+q, -q, +2q, -2q)
   int g_len[2];                        // padded entries per lane in gather round 0 / 1 (species lane, lane + 32)
   int o_tmid, o_W, o_invW, o_nasa;     // double [S] each; nasa [2][14][S]
   int o_rkA, o_rkB;                    // double2 [R]: {ln A, b}, {Ea/R_cal, dnu}
   int o_rfac;                          // uint4 [R]: byte offsets (from the cell base) of the two reactant and two
                                        //            product concentration factors (the 1.0 slot if absent)
   int o_rdg;                           // uint4 [Rrev]: byte offsets of nu*g of the <=2 reactant / <=2 product entries
-  int o_varc;                          // double [n_var]: the multiples
   int o_gsp;                           // uint8 [64]: species handled by lane l in round 0 ([l]) and round 1 ([32+l]); 255 = none
   int o_gent;                          // uint16 [(g_len[0]+g_len[1])][32]: byte offsets (from the cell base) of the
                                        //            stored multiple coef*q_j, or of the 0.0 slot (padding)

@@ -21,15 +21,67 @@
 
 namespace stev {
 
-// Twiddles of DESIGN.md 5.6 in constant memory: with compile-time indices they become constant-bank operands of DFMA.
-__device__ __constant__ const double kTwCos[13] = {
+// Twiddles of DESIGN.md 5.6 and the contract's exp / log coefficients in constant memory.  The arrays
+// are deliberately NOT const-qualified: a const array is folded into 64-bit immediates, which sm_100 has to build with
+// two moves per DFMA; a plain __constant__ array stays a constant-bank operand of the DFMA itself (no extra
+// instruction, no register).  Nothing ever writes them.
+__device__ __constant__ double kTwCos[13] = {
     1.0, 0.8854560256532099, 0.5680647467311559, 0.120536680255323, -0.35460488704253545,
     -0.7485107481711012, -0.970941817426052, -0.9709418174260521, -0.7485107481711013,
     -0.3546048870425359, 0.1205366802553232, 0.5680647467311548, 0.88545602565321};
-__device__ __constant__ const double kTwNegSin[13] = {
+__device__ __constant__ double kTwNegSin[13] = {
     -0.0, -0.4647231720437685, -0.8229838658936564, -0.992708874098054, -0.9350162426854148,
     -0.6631226582407952, -0.23931566428755768, 0.23931566428755743, 0.663122658240795,
     0.9350162426854147, 0.992708874098054, 0.822983865893657, 0.4647231720437684};
+// exp: [0] log2 e, [1] 1.5*2^52, [2] ln2_hi, [3] ln2_lo, [4..17] 1/13! .. 1/0!
+__device__ __constant__ double kExpC[18] = {
+    1.4426950408889634, 6755399441055744.0, 6.93147180369123816490e-01, 1.90821492927058770002e-10,
+    1.6059043836821613e-10, 2.08767569878681e-09, 2.505210838544172e-08, 2.755731922398589e-07,
+    2.7557319223985893e-06, 2.48015873015873e-05, 0.0001984126984126984, 0.001388888888888889,
+    0.008333333333333333, 0.041666666666666664, 0.16666666666666666, 0.5, 1.0, 1.0};
+// log: [0] sqrt 2, [1] ln2_hi, [2] ln2_lo, [3..13] 1/23, 1/21, .. 1/3
+__device__ __constant__ double kLogC[14] = {
+    1.4142135623730951, 6.93147180369123816490e-01, 1.90821492927058770002e-10,
+    0.043478260869565216, 0.047619047619047616, 0.05263157894736842, 0.058823529411764705,
+    0.06666666666666667, 0.07692307692307693, 0.09090909090909091, 0.1111111111111111,
+    0.14285714285714285, 0.2, 0.3333333333333333};
+
+// The contract's exp (same operations, same order as stev_math.cuh / DESIGN.md 5.3).  p * 2^k is formed by adding k
+// to the exponent field of p, which is the same number whenever the product is a normal double: p lies in
+// [0.70, 1.42] and |x| <= 708 gives |k| <= 1022 with e^x >= 2^-1021.4.  Everything else takes the generic routine.
+__device__ __forceinline__ double ab_exp(double x) {
+  if (__builtin_expect(!(fabs(x) <= 708.0), 0)) return cexp(x);
+  const double t = fma_rn(x, kExpC[0], kExpC[1]);
+  const double k = t - kExpC[1];
+  double r = fma_rn(-k, kExpC[2], x);
+  r = fma_rn(-k, kExpC[3], r);
+  double p = kExpC[4];
+#pragma unroll
+  for (int n = 5; n < 18; ++n) p = fma_rn(p, r, kExpC[n]);
+  const int ki = __double2loint(t);
+  return __hiloint2double(__double2hiint(p) + ki * 1048576, __double2loint(p));
+}
+
+// The contract's log for positive finite normal x (T and p_atm/(R_u T) on this path); other inputs take the generic routine.
+__device__ __forceinline__ double ab_log(double x) {
+  const int hi = __double2hiint(x);
+  if (__builtin_expect(hi < 0x00100000 || hi >= 0x7ff00000, 0)) return clog(x);
+  int e = (hi >> 20) - 1023;
+  double m = __hiloint2double((hi & 0x000fffff) | 0x3ff00000, __double2loint(x));
+  if (m > kLogC[0]) {
+    m = m * 0.5;
+    e = e + 1;
+  }
+  const double f = (m - 1.0) / (m + 1.0);
+  const double s = f * f;
+  double P = kLogC[3];
+#pragma unroll
+  for (int n = 4; n < 14; ++n) P = fma_rn(P, s, kLogC[n]);
+  const double two_f = f + f;
+  const double log_m = fma_rn(two_f, s * P, two_f);
+  const double ed = (double)e;
+  return fma_rn(ed, kLogC[1], fma_rn(ed, kLogC[2], log_m));
+}
 
 __device__ __forceinline__ void named_bar_sync(int id) { asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory"); }
 __device__ __forceinline__ void named_bar_arrive(int id) { asm volatile("bar.arrive %0, 64;" ::"r"(id) : "memory"); }
@@ -176,10 +228,9 @@ __device__ __forceinline__ void ab_rate_warp(const AbArgs &a, const unsigned cha
   const double *invW = (const double *)(tbl + tb.o_invW), *nasa = (const double *)(tbl + tb.o_nasa);
   const double2 *rkA = (const double2 *)(tbl + tb.o_rkA), *rkB = (const double2 *)(tbl + tb.o_rkB);
   const uint4 *rfac = (const uint4 *)(tbl + tb.o_rfac), *rdg = (const uint4 *)(tbl + tb.o_rdg);
-  const double *varc = (const double *)(tbl + tb.o_varc);
   const unsigned char *gsp = tbl + tb.o_gsp;
   const unsigned short *gent = (const unsigned short *)(tbl + tb.o_gent);
-  const int n_var = tb.n_var;
+  const bool has2 = tb.n_var > 2;
 
   const int barS2 = 2 * j, barS1 = 2 * j + 1;
   const double dt_max = a.t_f * sc.delta_max;   // Eq 4
@@ -217,7 +268,7 @@ __device__ __forceinline__ void ab_rate_warp(const AbArgs &a, const unsigned cha
       const double c_tot = p / RuT;
       const double invT = 1.0 / T;
       const double larg = (lane & 16) ? (kPatm / RuT) : T;
-      const double lval = clog(larg);
+      const double lval = ab_log(larg);
       const double lnT = __shfl_sync(0xffffffffu, lval, 0);
       const double ln_c0 = __shfl_sync(0xffffffffu, lval, 16);
 
@@ -252,8 +303,8 @@ __device__ __forceinline__ void ab_rate_warp(const AbArgs &a, const unsigned cha
           }
           const double zd = (double)z;
           float act;
-          if (tb.act == 0) act = (float)(1.0 - 2.0 / (1.0 + cexp(2.0 * zd)));
-          else act = (float)(1.0 / (1.0 + cexp(-zd)));
+          if (tb.act == 0) act = (float)(1.0 - 2.0 / (1.0 + ab_exp(2.0 * zd)));
+          else act = (float)(1.0 / (1.0 + ab_exp(-zd)));
           cHid[jh] = act;
         }
         __syncwarp();
@@ -268,6 +319,7 @@ __device__ __forceinline__ void ab_rate_warp(const AbArgs &a, const unsigned cha
             y[u] = b2[o];
             wrow[u] = (const float4 *)(W2p + (size_t)o * Hpad);
           }
+#pragma unroll 2
           for (int q4 = 0; q4 < H / 4; ++q4) {
             const float4 hv = hid4[q4];
 #pragma unroll
@@ -288,18 +340,23 @@ __device__ __forceinline__ void ab_rate_warp(const AbArgs &a, const unsigned cha
             }
           }
         }
+        __syncwarp();
       }
 
-      // -- mixture (sequential in species order, contract 5.4), density, stabilised concentrations (Eqs 6-7, R7)
-      double inv_wbar = 0.0;
+      // -- mixture sums, sequential in species order (contract 5.4): 1/Wbar = sum Y_i/W_i and sum (Y_i/W_i) cp_i/R,
+      //    two independent chains walked together
+      double inv_wbar = 0.0, sum_cp = 0.0;
+#pragma unroll 4
       for (int i = 0; i < S; ++i) {
         const double2 v = cYp[i];
+        const double cp = cYwCp[i].y;
         inv_wbar = fma_rn(v.x, v.y, inv_wbar);
+        sum_cp = fma_rn(v.x * v.y, cp, sum_cp);
       }
       const double rho = c_tot / inv_wbar;
+      // -- small-species stabilisation (Eqs 6-7, R7): C** = gamma(y) rho y / W
       for (int i = lane; i < S; i += 32) {
         const double2 v = cYp[i];
-        cYwCp[i].x = v.x * v.y;
         const double yp = (v.x > 0.0) ? v.x : 0.0;
         double c = (rho * yp) * v.y;
         if (sc.alpha > 0.0) c = (yp / (sc.alpha + yp)) * c;
@@ -307,44 +364,63 @@ __device__ __forceinline__ void ab_rate_warp(const AbArgs &a, const unsigned cha
       }
       __syncwarp();
 
-      // -- a2: rate constants and raw progress rates (Eqs 28-30).  Reversible reactions first.
-      for (int k = lane; k < R; k += 32) {
+      // -- a2: rate constants and raw progress rates (Eqs 28-30).  Reversible reactions occupy
+      //    internal indices [0, Rrev): one loop without branches for them (lanes past Rrev recompute the last one and
+      //    store nothing), one for the irreversible rest.
+      for (int k0 = 0; k0 < Rrev; k0 += 32) {
+        const int kk = k0 + lane;
+        const int k = (kk < Rrev) ? kk : Rrev - 1;
         const double2 ka = rkA[k], kb = rkB[k];
+        const uint4 f = rfac[k], d = rdg[k];
         const double ln_kf = fma_rn(-kb.x, invT, fma_rn(ka.y, lnT, ka.x));
-        double fwd = cexp(ln_kf);
-        const uint4 f = rfac[k];
+        double dg = 0.0 - lds_f64(cell, d.x);
+        dg = dg - lds_f64(cell, d.y);
+        dg = dg + lds_f64(cell, d.z);
+        dg = dg + lds_f64(cell, d.w);
+        const double ln_kc = fma_rn(kb.y, ln_c0, -dg);
+        double fwd = ab_exp(ln_kf);
+        double rev = ab_exp(ln_kf - ln_kc);
         fwd = fwd * lds_f64(cell, f.x);
         fwd = fwd * lds_f64(cell, f.y);
-        double qk = fwd;
-        if (k < Rrev) {
-          const uint4 d = rdg[k];
-          double dg = 0.0 - lds_f64(cell, d.x);
-          dg = dg - lds_f64(cell, d.y);
-          dg = dg + lds_f64(cell, d.z);
-          dg = dg + lds_f64(cell, d.w);
-          const double ln_kc = fma_rn(kb.y, ln_c0, -dg);
-          double rev = cexp(ln_kf - ln_kc);
-          rev = rev * lds_f64(cell, f.z);
-          rev = rev * lds_f64(cell, f.w);
-          qk = fwd - rev;
-        }
-        cQraw[k] = qk;
+        rev = rev * lds_f64(cell, f.z);
+        rev = rev * lds_f64(cell, f.w);
+        if (kk < Rrev) cQraw[k] = fwd - rev;
       }
-      double sum_cp = 0.0;
-      for (int i = 0; i < S; ++i) {
-        const double2 v = cYwCp[i];
-        sum_cp = fma_rn(v.x, v.y, sum_cp);
+      for (int k0 = Rrev; k0 < R; k0 += 32) {
+        const int kk = k0 + lane;
+        const int k = (kk < R) ? kk : R - 1;
+        const double2 ka = rkA[k];
+        const double ta = rkB[k].x;
+        const uint4 f = rfac[k];
+        const double ln_kf = fma_rn(-ta, invT, fma_rn(ka.y, lnT, ka.x));
+        double fwd = ab_exp(ln_kf);
+        fwd = fwd * lds_f64(cell, f.x);
+        fwd = fwd * lds_f64(cell, f.y);
+        // irreversible: q_eff = q; its stored multiples can be written right away (the DFT warp never reads them)
+        if (kk < R) {
+          cQ[k] = fwd;
+          cQ[Rp + k] = -fwd;
+          if (has2) {
+            const double f2 = fwd + fwd;
+            cQ[2 * Rp + k] = f2;
+            cQ[3 * Rp + k] = -f2;
+          }
+        }
       }
 
       // ================= part 2: needs rOF of this step (produced by the DFT warp) =================
       named_bar_sync(barS1);
-      // effective rates (Eq 14) and their stored multiples: variant v holds varc[v] * q_eff (exact for +-1, +-2,
-      // rounded once for +-3 exactly as the plain sum omega_i = sum_j nu_ij q_j rounds nu*q before adding)
-      for (int k = lane; k < R; k += 32) {
-        double q = cQraw[k];
-        if (k < Rrev) q = q * cRof[k];
+      // effective rates (Eq 14) and their stored multiples +q, -q, +2q, -2q (all exact), which turn the sum
+      // omega_i = sum_j nu_ij q_j into plain additions in the contract's order
+      for (int k = lane; k < Rrev; k += 32) {
+        const double q = cQraw[k] * cRof[k];
         cQ[k] = q;
-        for (int v = 1; v < n_var; ++v) cQ[v * Rp + k] = varc[v] * q;
+        cQ[Rp + k] = -q;
+        if (has2) {
+          const double q2 = q + q;
+          cQ[2 * Rp + k] = q2;
+          cQ[3 * Rp + k] = -q2;
+        }
       }
       __syncwarp();
 
@@ -359,7 +435,7 @@ __device__ __forceinline__ void ab_rate_warp(const AbArgs &a, const unsigned cha
           const int len = tb.g_len[round];
           const int i = gsp[32 * round + lane];
           double om = 0.0;
-#pragma unroll 4
+#pragma unroll 8
           for (int e = 0; e < len; ++e) om = om + lds_f64(cell, ge[e * 32]);
           ge += len * 32;
           if (i < S) {
@@ -386,14 +462,6 @@ __device__ __forceinline__ void ab_rate_warp(const AbArgs &a, const unsigned cha
       }
       __syncwarp();
 
-      // -- temperature equation (R15), enthalpy sum sequential in species order
-      double sum_h = 0.0;
-      for (int i = 0; i < S; ++i) {
-        const double2 v = cHOm[i];
-        sum_h = fma_rn(v.x, v.y, sum_h);
-      }
-      const double dTdt = (sc.energy_mode == 0) ? -((sum_h * kRu) * T) / (rho * (kRu * sum_cp)) : 0.0;
-
       // -- a3: step size (Eq 5) and landing on t_f (R5)
       double h = (t_star < dt_max) ? t_star : dt_max;
       bool last = false;
@@ -402,13 +470,21 @@ __device__ __forceinline__ void ab_rate_warp(const AbArgs &a, const unsigned cha
         h = rem;
         last = true;
       }
-      // -- a4: forward Euler (Eq 18)
+      // -- a4: forward Euler (Eq 18) for the species; the enthalpy sum of the temperature equation
+      //    (R15) is sequential in species order
       int bad = 0;
       for (int i = lane; i < S; i += 32) {
         const double y = fma_rn(h, cConc[1 + i], cYp[i].x);
         cYp[i].x = y;
         bad |= !(y - y == 0.0);
       }
+      double sum_h = 0.0;
+#pragma unroll 4
+      for (int i = 0; i < S; ++i) {
+        const double2 v = cHOm[i];
+        sum_h = fma_rn(v.x, v.y, sum_h);
+      }
+      const double dTdt = (sc.energy_mode == 0) ? -((sum_h * kRu) * T) / (rho * (kRu * sum_cp)) : 0.0;
       T = fma_rn(h, dTdt, T);
       t = last ? a.t_f : t + h;
       steps += 1;
@@ -429,6 +505,7 @@ __device__ __forceinline__ void ab_rate_warp(const AbArgs &a, const unsigned cha
       __threadfence_block();
       named_bar_arrive(barS2);
 
+      __syncwarp();
       if (st >= 0) {
         for (int i = lane; i < S; i += 32) a.Y[(long long)i * a.ld + cidx] = cYp[i].x;
         if (lane == 0) {
@@ -448,7 +525,7 @@ __global__ void __launch_bounds__(kAbThreads, 1) stev_ab_kernel(const __grid_con
   __shared__ unsigned long long mbar;
   __shared__ uint32_t tmem_base_s;
   __shared__ int done_warps;
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;   // warp-uniform for the compiler
   if (threadIdx.x == 0) done_warps = 0;
   stage_tables(smem, a.table, a.tb.bytes, &mbar);
   if (warp == 0) {
