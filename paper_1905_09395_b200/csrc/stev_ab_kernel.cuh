@@ -93,9 +93,23 @@ __device__ __forceinline__ void tmem_st2(uint32_t taddr, double v) {
 }
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-// 13 doubles = 26 consecutive columns of this lane: x16 + x8 + x2
-__device__ __forceinline__ void tmem_ld_window(uint32_t taddr, double (&x)[kWindow]) {
-  uint32_t r[26];
+__device__ __forceinline__ double lds_f64(const unsigned char *base, unsigned off) { return *(const double *)(base + off); }
+
+// exp without the range check (the caller checks |x| <= 708 for the whole batch and falls back to ab_exp)
+__device__ __forceinline__ double ab_exp_core(double x) {
+  const double t = fma_rn(x, kExpC[0], kExpC[1]);
+  const double k = t - kExpC[1];
+  double r = fma_rn(-k, kExpC[2], x);
+  r = fma_rn(-k, kExpC[3], r);
+  double p = kExpC[4];
+#pragma unroll
+  for (int n = 5; n < 18; ++n) p = fma_rn(p, r, kExpC[n]);
+  return __hiloint2double(__double2hiint(p) + __double2loint(t) * 1048576, __double2loint(p));
+}
+__device__ __forceinline__ bool ab_exp_out_of_range(double x) { return !(fabs(x) <= 708.0); }
+
+// 13 doubles = 26 consecutive columns of this lane, issued as x16 + x8 + x2 (no wait)
+__device__ __forceinline__ void tmem_ld26(uint32_t taddr, uint32_t (&r)[26]) {
   asm volatile(
       "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
       : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]),
@@ -107,12 +121,11 @@ __device__ __forceinline__ void tmem_ld_window(uint32_t taddr, double (&x)[kWind
                : "r"(taddr + 16)
                : "memory");
   asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0,%1}, [%2];" : "=r"(r[24]), "=r"(r[25]) : "r"(taddr + 24) : "memory");
-  tmem_wait_ld();
+}
+__device__ __forceinline__ void unpack_window(const uint32_t (&r)[26], double (&x)[kWindow]) {
 #pragma unroll
   for (int s = 0; s < kWindow; ++s) x[s] = __hiloint2double((int)r[2 * s + 1], (int)r[2 * s]);
 }
-
-__device__ __forceinline__ double lds_f64(const unsigned char *base, unsigned off) { return *(const double *)(base + off); }
 
 // |X_M|^2 of the window (Eq 9).  The k = 0 terms of the contract's sums are fma(x0, 1, 0) = x0 and
 // fma(x0, -0, 0) = +0 for every finite x0, so the sums start from them (a non-finite sample only occurs in the step
@@ -128,29 +141,50 @@ __device__ __forceinline__ double ab_bin_sq(const double (&x)[kWindow]) {
   return fma_rn(re, re, im * im);
 }
 
-// Eq 10 + Eq 12 for one window.
-__device__ __forceinline__ bool ab_is_ringing(const double (&x)[kWindow], const SolverConsts &sc) {
-  double d0 = x[0];
+// D^0 = |sum x| and the largest |X_m|^2 over the high bins NHF..6 (Eqs 9-10).  max of sqrt = sqrt of max (IEEE sqrt
+// is monotone), so one square root at most is needed per window.
+template <int NHF>
+__device__ __forceinline__ void ab_window_stats(const double (&x)[kWindow], double &d0, double &m2) {
+  double s = x[0];
 #pragma unroll
-  for (int k = 1; k < kWindow; ++k) d0 = d0 + x[k];
-  d0 = fabs(d0);
-  double m2 = 0.0, v;
-  const int nhf = sc.nhf;
-  if (nhf <= 1) { v = ab_bin_sq<1>(x); m2 = (v > m2) ? v : m2; }
-  if (nhf <= 2) { v = ab_bin_sq<2>(x); m2 = (v > m2) ? v : m2; }
-  if (nhf <= 3) { v = ab_bin_sq<3>(x); m2 = (v > m2) ? v : m2; }
-  if (nhf <= 4) { v = ab_bin_sq<4>(x); m2 = (v > m2) ? v : m2; }
-  if (nhf <= 5) { v = ab_bin_sq<5>(x); m2 = (v > m2) ? v : m2; }
-  { v = ab_bin_sq<6>(x); m2 = (v > m2) ? v : m2; }
-  const double d_hi = sqrt(m2);   // max of sqrt = sqrt of max (IEEE sqrt is monotone)
+  for (int k = 1; k < kWindow; ++k) s = s + x[k];
+  d0 = fabs(s);
+  double m = 0.0, v;   // the contract's running maximum starts at 0 and ignores NaN
+  if (NHF <= 1) { v = ab_bin_sq<1>(x); m = (v > m) ? v : m; }
+  if (NHF <= 2) { v = ab_bin_sq<2>(x); m = (v > m) ? v : m; }
+  if (NHF <= 3) { v = ab_bin_sq<3>(x); m = (v > m) ? v : m; }
+  if (NHF <= 4) { v = ab_bin_sq<4>(x); m = (v > m) ? v : m; }
+  if (NHF <= 5) { v = ab_bin_sq<5>(x); m = (v > m) ? v : m; }
+  { v = ab_bin_sq<6>(x); m = (v > m) ? v : m; }
+  m2 = m;
+}
+
+// Eq 10 + Eq 12 exactly as written: f_ring = D^0 / max(sqrt(m2), 1e-300) < Tol_ring and D^0 < Tol_freq.
+__device__ __forceinline__ bool ab_ring_exact(double d0, double m2, const SolverConsts &sc) {
+  const double d_hi = sqrt(m2);
   const double f_ring = d0 / ((d_hi > 1.0e-300) ? d_hi : 1.0e-300);
   return (f_ring < sc.tol_ring) && (d0 < sc.tol_freq);
 }
+// The same decision without the square root and the division whenever it is not close: with u = 2^-53,
+// fl(d0/fl(sqrt m2)) = (d0/sqrt m2)(1 + 2.1u) at worst, while d0^2 and Tol_ring^2 m2 are each formed with at most
+// three roundings, so  d0^2 < Tol_ring^2 m2 (1 - 1e-14)  implies f_ring < Tol_ring (1 - 4e-15) < Tol_ring, and
+// symmetrically for >.  `sure` is false inside that band, when m2 or Tol_ring^2 m2 leave [1e-290, 1e290] (so that
+// no underflow, overflow or the 1e-300 guard is involved) and for NaN; the caller then evaluates ab_ring_exact.
+__device__ __forceinline__ bool ab_ring_filter(double d0, double m2, const SolverConsts &sc, bool &sure) {
+  const double lhs = d0 * d0, rhs = sc.tol_ring2 * m2;
+  const bool below = lhs < rhs * sc.ring_lo, above = lhs > rhs * sc.ring_hi;
+  const bool in_range = (m2 >= 1.0e-280) && (rhs >= 1.0e-290) && (rhs <= 1.0e290);
+  const bool small = d0 < sc.tol_freq;
+  sure = !small || (sc.ring_filter_ok && in_range && (below || above));
+  return below && small;
+}
 
 // ---------------------------------------------------------------------------------------------------------
-// DFT warp: rows a5 of DESIGN.md.  TMEM address of slot s of this lane's reaction `it`:
+// DFT warp: row a5 of DESIGN.md.  TMEM address of slot s of this lane's reaction `it`:
 //   base + (lane quarter << 16) + cell_half * 256 + it * 32 + 2 s.
+// Two windows are processed side by side (independent dependency chains for the scheduler).
 // ---------------------------------------------------------------------------------------------------------
+template <int NHF>
 __device__ __forceinline__ void ab_dft_warp(const AbArgs &a, unsigned char *cell, int j, uint32_t tmem_base, int lane) {
   const AbTables &tb = a.tb;
   const SolverConsts &sc = a.sc;
@@ -169,6 +203,12 @@ __device__ __forceinline__ void ab_dft_warp(const AbArgs &a, unsigned char *cell
     for (int k = lane; k < Rrev; k += 32) cRof[k] = 1.0;                         // Eq 11
     slot = 0;
   };
+  auto update_rof = [&](int k, bool ringing) {
+    double rof = cRof[k] * (ringing ? sc.inv_r_fac : sc.r_fac);   // Eqs 12-13
+    if (rof > 1.0) rof = 1.0;
+    if (rof < sc.rof_min) rof = sc.rof_min;
+    cRof[k] = rof;
+  };
 
   reset();
   __threadfence_block();
@@ -181,22 +221,49 @@ __device__ __forceinline__ void ab_dft_warp(const AbArgs &a, unsigned char *cell
       reset();   // the cell retired: its last DFT is unobservable; prepare the next cell
     } else {
       const double h = ctrl->h, inv_ctot = ctrl->inv_ctot;
+      // Eq 8 with R8, R9: the applied change in progress / C_tot of every reversible reaction goes into its window
       for (int it = 0; it < n_it; ++it) {
         const int k = it * 32 + lane;
-        const bool live = k < Rrev;
-        const double q = live ? cQ[k] : 0.0;
-        const uint32_t tw = trow + it * 32;
-        tmem_st2(tw + 2 * slot, (q * h) * inv_ctot);   // Eq 8 with R8, R9: applied change in progress / C_tot
-        tmem_wait_st();
-        double x[kWindow];
-        tmem_ld_window(tw, x);
-        const bool ringing = ab_is_ringing(x, sc);
-        if (live) {
-          double rof = cRof[k] * (ringing ? sc.inv_r_fac : sc.r_fac);   // Eqs 12-13
-          if (rof > 1.0) rof = 1.0;
-          if (rof < sc.rof_min) rof = sc.rof_min;
-          cRof[k] = rof;
+        const double q = (k < Rrev) ? cQ[k] : 0.0;
+        tmem_st2(trow + it * 32 + 2 * slot, (q * h) * inv_ctot);
+      }
+      tmem_wait_st();
+      int it = 0;
+      for (; it + 2 <= n_it; it += 2) {
+        uint32_t ra[26], rb[26];
+        tmem_ld26(trow + it * 32, ra);
+        tmem_ld26(trow + it * 32 + 32, rb);
+        tmem_wait_ld();
+        double xa[kWindow], xb[kWindow];
+        unpack_window(ra, xa);
+        unpack_window(rb, xb);
+        double d0a, m2a, d0b, m2b;
+        ab_window_stats<NHF>(xa, d0a, m2a);
+        ab_window_stats<NHF>(xb, d0b, m2b);
+        const int ka = it * 32 + lane, kb = ka + 32;
+        bool sure_a, sure_b;
+        bool ring_a = ab_ring_filter(d0a, m2a, sc, sure_a);
+        bool ring_b = ab_ring_filter(d0b, m2b, sc, sure_b);
+        if (__any_sync(0xffffffffu, (!sure_a && ka < Rrev) || (!sure_b && kb < Rrev))) {
+          ring_a = ab_ring_exact(d0a, m2a, sc);
+          ring_b = ab_ring_exact(d0b, m2b, sc);
         }
+        if (ka < Rrev) update_rof(ka, ring_a);
+        if (kb < Rrev) update_rof(kb, ring_b);
+      }
+      if (it < n_it) {
+        uint32_t ra[26];
+        tmem_ld26(trow + it * 32, ra);
+        tmem_wait_ld();
+        double xa[kWindow];
+        unpack_window(ra, xa);
+        double d0a, m2a;
+        ab_window_stats<NHF>(xa, d0a, m2a);
+        const int ka = it * 32 + lane;
+        bool sure_a;
+        bool ring_a = ab_ring_filter(d0a, m2a, sc, sure_a);
+        if (__any_sync(0xffffffffu, !sure_a && ka < Rrev)) ring_a = ab_ring_exact(d0a, m2a, sc);
+        if (ka < Rrev) update_rof(ka, ring_a);
       }
       slot = (slot + 1 == kWindow) ? 0 : slot + 1;
     }
@@ -273,19 +340,33 @@ __device__ __forceinline__ void ab_rate_warp(const AbArgs &a, const unsigned cha
       const double ln_c0 = __shfl_sync(0xffffffffu, lval, 16);
 
       // -- a1: NASA-7 (Eqs 15-16, R17); g/RT always, cp and h unless the MLP supplies them.
-      for (int i = lane; i < S; i += 32) {
-        const double *c = nasa + ((T < tmid[i]) ? 0 : kNasaRows * S) + i;
-        const double a1 = c[0], a2 = c[S];
-        const double hp = fma_rn(fma_rn(fma_rn(fma_rn(c[8 * S], T, c[7 * S]), T, c[6 * S]), T, c[5 * S]), T, a1);
-        const double hRT = fma_rn(c[9 * S], invT, hp);
-        const double sp = fma_rn(fma_rn(fma_rn(c[12 * S], T, c[11 * S]), T, c[10 * S]), T, a2);
-        const double sR = fma_rn(a1, lnT, fma_rn(sp, T, c[13 * S]));
-        const double g = hRT - sR;
-        cG[1 + i] = g;
-        cG[1 + S + i] = g + g;
+      //    Two species per lane side by side; lanes past the end recompute the last species and store nothing.
+      for (int ia = lane; ia < S; ia += 64) {
+        const int ib_ = ia + 32;
+        const int ib = (ib_ < S) ? ib_ : S - 1;
+        const double *ca = nasa + ((T < tmid[ia]) ? 0 : kNasaRows * S) + ia;
+        const double *cb = nasa + ((T < tmid[ib]) ? 0 : kNasaRows * S) + ib;
+        const double a1a = ca[0], a2a = ca[S], a1b = cb[0], a2b = cb[S];
+        const double hpa = fma_rn(fma_rn(fma_rn(fma_rn(ca[8 * S], T, ca[7 * S]), T, ca[6 * S]), T, ca[5 * S]), T, a1a);
+        const double hpb = fma_rn(fma_rn(fma_rn(fma_rn(cb[8 * S], T, cb[7 * S]), T, cb[6 * S]), T, cb[5 * S]), T, a1b);
+        const double hRTa = fma_rn(ca[9 * S], invT, hpa), hRTb = fma_rn(cb[9 * S], invT, hpb);
+        const double spa = fma_rn(fma_rn(fma_rn(ca[12 * S], T, ca[11 * S]), T, ca[10 * S]), T, a2a);
+        const double spb = fma_rn(fma_rn(fma_rn(cb[12 * S], T, cb[11 * S]), T, cb[10 * S]), T, a2b);
+        const double sRa = fma_rn(a1a, lnT, fma_rn(spa, T, ca[13 * S])), sRb = fma_rn(a1b, lnT, fma_rn(spb, T, cb[13 * S]));
+        const double ga = hRTa - sRa, gb = hRTb - sRb;
+        cG[1 + ia] = ga;
+        cG[1 + S + ia] = ga + ga;
+        if (ib_ < S) {
+          cG[1 + ib] = gb;
+          cG[1 + S + ib] = gb + gb;
+        }
         if (!EST) {
-          cYwCp[i].y = fma_rn(fma_rn(fma_rn(fma_rn(c[4 * S], T, c[3 * S]), T, c[2 * S]), T, a2), T, a1);
-          cHOm[i].x = hRT;
+          cYwCp[ia].y = fma_rn(fma_rn(fma_rn(fma_rn(ca[4 * S], T, ca[3 * S]), T, ca[2 * S]), T, a2a), T, a1a);
+          cHOm[ia].x = hRTa;
+          if (ib_ < S) {
+            cYwCp[ib].y = fma_rn(fma_rn(fma_rn(fma_rn(cb[4 * S], T, cb[3 * S]), T, cb[2 * S]), T, a2b), T, a1b);
+            cHOm[ib].x = hRTb;
+          }
         }
       }
       // -- a7 in the integrator (fp32 CUDA cores, R18): cp_i/R and h_i/(R T_ref) from the shallow MLP.
@@ -319,7 +400,7 @@ __device__ __forceinline__ void ab_rate_warp(const AbArgs &a, const unsigned cha
             y[u] = b2[o];
             wrow[u] = (const float4 *)(W2p + (size_t)o * Hpad);
           }
-#pragma unroll 2
+#pragma unroll 4
           for (int q4 = 0; q4 < H / 4; ++q4) {
             const float4 hv = hid4[q4];
 #pragma unroll
@@ -346,7 +427,7 @@ __device__ __forceinline__ void ab_rate_warp(const AbArgs &a, const unsigned cha
       // -- mixture sums, sequential in species order (contract 5.4): 1/Wbar = sum Y_i/W_i and sum (Y_i/W_i) cp_i/R,
       //    two independent chains walked together
       double inv_wbar = 0.0, sum_cp = 0.0;
-#pragma unroll 4
+#pragma unroll 8
       for (int i = 0; i < S; ++i) {
         const double2 v = cYp[i];
         const double cp = cYwCp[i].y;
@@ -355,55 +436,98 @@ __device__ __forceinline__ void ab_rate_warp(const AbArgs &a, const unsigned cha
       }
       const double rho = c_tot / inv_wbar;
       // -- small-species stabilisation (Eqs 6-7, R7): C** = gamma(y) rho y / W
-      for (int i = lane; i < S; i += 32) {
-        const double2 v = cYp[i];
-        const double yp = (v.x > 0.0) ? v.x : 0.0;
-        double c = (rho * yp) * v.y;
-        if (sc.alpha > 0.0) c = (yp / (sc.alpha + yp)) * c;
-        cConc[1 + i] = c;
+      for (int ia = lane; ia < S; ia += 64) {
+        const int ib_ = ia + 32;
+        const int ib = (ib_ < S) ? ib_ : S - 1;
+        const double2 va = cYp[ia], vb = cYp[ib];
+        const double ypa = (va.x > 0.0) ? va.x : 0.0, ypb = (vb.x > 0.0) ? vb.x : 0.0;
+        double ca = (rho * ypa) * va.y, cb = (rho * ypb) * vb.y;
+        if (sc.alpha > 0.0) {
+          const double gam_a = ypa / (sc.alpha + ypa), gam_b = ypb / (sc.alpha + ypb);
+          ca = gam_a * ca;
+          cb = gam_b * cb;
+        }
+        cConc[1 + ia] = ca;
+        if (ib_ < S) cConc[1 + ib] = cb;
       }
       __syncwarp();
 
       // -- a2: rate constants and raw progress rates (Eqs 28-30).  Reversible reactions occupy
-      //    internal indices [0, Rrev): one loop without branches for them (lanes past Rrev recompute the last one and
-      //    store nothing), one for the irreversible rest.
-      for (int k0 = 0; k0 < Rrev; k0 += 32) {
-        const int kk = k0 + lane;
-        const int k = (kk < Rrev) ? kk : Rrev - 1;
-        const double2 ka = rkA[k], kb = rkB[k];
-        const uint4 f = rfac[k], d = rdg[k];
-        const double ln_kf = fma_rn(-kb.x, invT, fma_rn(ka.y, lnT, ka.x));
-        double dg = 0.0 - lds_f64(cell, d.x);
-        dg = dg - lds_f64(cell, d.y);
-        dg = dg + lds_f64(cell, d.z);
-        dg = dg + lds_f64(cell, d.w);
-        const double ln_kc = fma_rn(kb.y, ln_c0, -dg);
-        double fwd = ab_exp(ln_kf);
-        double rev = ab_exp(ln_kf - ln_kc);
-        fwd = fwd * lds_f64(cell, f.x);
-        fwd = fwd * lds_f64(cell, f.y);
-        rev = rev * lds_f64(cell, f.z);
-        rev = rev * lds_f64(cell, f.w);
-        if (kk < Rrev) cQraw[k] = fwd - rev;
+      //    internal indices [0, Rrev).  Each lane evaluates two reversible reactions side by side (four independent
+      //    exp chains for the scheduler); lanes past the end recompute the last reaction and store nothing.
+      for (int k0 = 0; k0 < Rrev; k0 += 64) {
+        const int ka_ = k0 + lane, kb_ = ka_ + 32;
+        const int ka = (ka_ < Rrev) ? ka_ : Rrev - 1, kb = (kb_ < Rrev) ? kb_ : Rrev - 1;
+        const double2 pa0 = rkA[ka], pa1 = rkB[ka], pb0 = rkA[kb], pb1 = rkB[kb];
+        const uint4 fa = rfac[ka], da = rdg[ka], fb = rfac[kb], db = rdg[kb];
+        const double lkf_a = fma_rn(-pa1.x, invT, fma_rn(pa0.y, lnT, pa0.x));
+        const double lkf_b = fma_rn(-pb1.x, invT, fma_rn(pb0.y, lnT, pb0.x));
+        double dga = 0.0 - lds_f64(cell, da.x), dgb = 0.0 - lds_f64(cell, db.x);
+        dga = dga - lds_f64(cell, da.y);
+        dgb = dgb - lds_f64(cell, db.y);
+        dga = dga + lds_f64(cell, da.z);
+        dgb = dgb + lds_f64(cell, db.z);
+        dga = dga + lds_f64(cell, da.w);
+        dgb = dgb + lds_f64(cell, db.w);
+        const double lkr_a = lkf_a - fma_rn(pa1.y, ln_c0, -dga);
+        const double lkr_b = lkf_b - fma_rn(pb1.y, ln_c0, -dgb);
+        double fwd_a, rev_a, fwd_b, rev_b;
+        if (__any_sync(0xffffffffu, ab_exp_out_of_range(lkf_a) || ab_exp_out_of_range(lkr_a) ||
+                                        ab_exp_out_of_range(lkf_b) || ab_exp_out_of_range(lkr_b))) {
+          fwd_a = cexp(lkf_a); rev_a = cexp(lkr_a); fwd_b = cexp(lkf_b); rev_b = cexp(lkr_b);
+        } else {
+          fwd_a = ab_exp_core(lkf_a); rev_a = ab_exp_core(lkr_a); fwd_b = ab_exp_core(lkf_b); rev_b = ab_exp_core(lkr_b);
+        }
+        fwd_a = fwd_a * lds_f64(cell, fa.x);
+        fwd_b = fwd_b * lds_f64(cell, fb.x);
+        rev_a = rev_a * lds_f64(cell, fa.z);
+        rev_b = rev_b * lds_f64(cell, fb.z);
+        fwd_a = fwd_a * lds_f64(cell, fa.y);
+        fwd_b = fwd_b * lds_f64(cell, fb.y);
+        rev_a = rev_a * lds_f64(cell, fa.w);
+        rev_b = rev_b * lds_f64(cell, fb.w);
+        if (ka_ < Rrev) cQraw[ka] = fwd_a - rev_a;
+        if (kb_ < Rrev) cQraw[kb] = fwd_b - rev_b;
       }
-      for (int k0 = Rrev; k0 < R; k0 += 32) {
-        const int kk = k0 + lane;
-        const int k = (kk < R) ? kk : R - 1;
-        const double2 ka = rkA[k];
-        const double ta = rkB[k].x;
-        const uint4 f = rfac[k];
-        const double ln_kf = fma_rn(-ta, invT, fma_rn(ka.y, lnT, ka.x));
-        double fwd = ab_exp(ln_kf);
-        fwd = fwd * lds_f64(cell, f.x);
-        fwd = fwd * lds_f64(cell, f.y);
-        // irreversible: q_eff = q; its stored multiples can be written right away (the DFT warp never reads them)
-        if (kk < R) {
-          cQ[k] = fwd;
-          cQ[Rp + k] = -fwd;
-          if (has2) {
-            const double f2 = fwd + fwd;
-            cQ[2 * Rp + k] = f2;
-            cQ[3 * Rp + k] = -f2;
+      // irreversible reactions: four per lane side by side; q_eff = q, so the stored multiples are written right
+      // away (the DFT warp never reads them)
+      for (int k0 = Rrev; k0 < R; k0 += 128) {
+        double lk[4], fw[4];
+        uint4 f[4];
+        int kk[4];
+        bool oor = false;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          kk[u] = k0 + 32 * u + lane;
+          const int k = (kk[u] < R) ? kk[u] : R - 1;
+          const double2 p0 = rkA[k];
+          const double ta = rkB[k].x;
+          f[u] = rfac[k];
+          lk[u] = fma_rn(-ta, invT, fma_rn(p0.y, lnT, p0.x));
+          oor = oor || ab_exp_out_of_range(lk[u]);
+        }
+        if (__any_sync(0xffffffffu, oor)) {
+#pragma unroll
+          for (int u = 0; u < 4; ++u) fw[u] = cexp(lk[u]);
+        } else {
+#pragma unroll
+          for (int u = 0; u < 4; ++u) fw[u] = ab_exp_core(lk[u]);
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) fw[u] = fw[u] * lds_f64(cell, f[u].x);
+#pragma unroll
+        for (int u = 0; u < 4; ++u) fw[u] = fw[u] * lds_f64(cell, f[u].y);
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          if (kk[u] < R) {
+            const int k = kk[u];
+            cQ[k] = fw[u];
+            cQ[Rp + k] = -fw[u];
+            if (has2) {
+              const double f2 = fw[u] + fw[u];
+              cQ[2 * Rp + k] = f2;
+              cQ[3 * Rp + k] = -f2;
+            }
           }
         }
       }
@@ -427,27 +551,38 @@ __device__ __forceinline__ void ab_rate_warp(const AbArgs &a, const unsigned cha
       // -- source terms and the limiter (Eqs 1-3).  Lane l owns species gsp[l] and gsp[32+l]; the
       //    entry lists are padded with the 0.0 slot to a common length per round, so the loops are warp-uniform.
       const double inv_rho = 1.0 / rho;
-      double t_star = bits_to_double(0x7ff0000000000000ull);
+      double t_star;
       {
-        const unsigned short *ge = gent + lane;
-#pragma unroll 1
-        for (int round = 0; round < 2; ++round) {
-          const int len = tb.g_len[round];
-          const int i = gsp[32 * round + lane];
-          double om = 0.0;
+        const int len0 = tb.g_len[0], len1 = tb.g_len[1];   // len1 <= len0 (the longest lists are in round 0)
+        const unsigned short *ge0 = gent + lane, *ge1 = gent + len0 * 32 + lane;
+        const int i0 = gsp[lane], i1 = gsp[32 + lane];
+        double om0 = 0.0, om1 = 0.0;
+        int e = 0;
+#pragma unroll 4
+        for (; e < len1; ++e) {
+          om0 = om0 + lds_f64(cell, ge0[e * 32]);
+          om1 = om1 + lds_f64(cell, ge1[e * 32]);
+        }
 #pragma unroll 8
-          for (int e = 0; e < len; ++e) om = om + lds_f64(cell, ge[e * 32]);
-          ge += len * 32;
-          if (i < S) {
-            const double r = (W[i] * om) * inv_rho;
-            const double y = cYp[i].x;
-            const double r_star = (-r > 1.0e-30) ? -r : 1.0e-30;
-            const double y_star = (y < 1.0e-20) ? 1.0 : 0.9 * y;
-            const double lim = ((sc.y_step_max < y_star) ? sc.y_step_max : y_star) / r_star;
-            if (lim < t_star) t_star = lim;
-            cConc[1 + i] = r;     // concentrations are dead: reuse for dY_i/dt
-            cHOm[i].y = om;
-          }
+        for (; e < len0; ++e) om0 = om0 + lds_f64(cell, ge0[e * 32]);
+        // lanes without a species (i = 255) work on species 0 and discard the result
+        const int j0 = (i0 < S) ? i0 : 0, j1 = (i1 < S) ? i1 : 0;
+        const double r0 = (W[j0] * om0) * inv_rho, r1 = (W[j1] * om1) * inv_rho;
+        const double y0 = cYp[j0].x, y1 = cYp[j1].x;
+        const double rs0 = (-r0 > 1.0e-30) ? -r0 : 1.0e-30, rs1 = (-r1 > 1.0e-30) ? -r1 : 1.0e-30;
+        const double ys0 = (y0 < 1.0e-20) ? 1.0 : 0.9 * y0, ys1 = (y1 < 1.0e-20) ? 1.0 : 0.9 * y1;
+        const double lim0 = ((sc.y_step_max < ys0) ? sc.y_step_max : ys0) / rs0;
+        const double lim1 = ((sc.y_step_max < ys1) ? sc.y_step_max : ys1) / rs1;
+        const double inf = bits_to_double(0x7ff0000000000000ull);
+        const double l0 = (i0 < S && lim0 < inf) ? lim0 : inf, l1 = (i1 < S) ? lim1 : inf;
+        t_star = (l1 < l0) ? l1 : l0;
+        if (i0 < S) {
+          cConc[1 + i0] = r0;     // concentrations are dead: reuse for dY_i/dt
+          cHOm[i0].y = om0;
+        }
+        if (i1 < S) {
+          cConc[1 + i1] = r1;
+          cHOm[i1].y = om1;
         }
       }
       // min over lanes: every lim is a positive double (or +inf / NaN), for which the ordering of the bit patterns
@@ -479,7 +614,7 @@ __device__ __forceinline__ void ab_rate_warp(const AbArgs &a, const unsigned cha
         bad |= !(y - y == 0.0);
       }
       double sum_h = 0.0;
-#pragma unroll 4
+#pragma unroll 8
       for (int i = 0; i < S; ++i) {
         const double2 v = cHOm[i];
         sum_h = fma_rn(v.x, v.y, sum_h);
@@ -544,7 +679,16 @@ __global__ void __launch_bounds__(kAbThreads, 1) stev_ab_kernel(const __grid_con
   const int j = is_dft ? warp : warp - kAbMaxCells;
   if (j < a.cells_per_block) {
     unsigned char *cell = smem + a.tb.bytes + (size_t)j * a.cl.stride;
-    if (is_dft) ab_dft_warp(a, cell, j, tmem_base, lane);
+    if (is_dft) {
+      switch (a.sc.nhf) {
+        case 1: ab_dft_warp<1>(a, cell, j, tmem_base, lane); break;
+        case 2: ab_dft_warp<2>(a, cell, j, tmem_base, lane); break;
+        case 3: ab_dft_warp<3>(a, cell, j, tmem_base, lane); break;
+        case 4: ab_dft_warp<4>(a, cell, j, tmem_base, lane); break;
+        case 5: ab_dft_warp<5>(a, cell, j, tmem_base, lane); break;
+        default: ab_dft_warp<6>(a, cell, j, tmem_base, lane); break;
+      }
+    }
     else if (a.tb.has_est) ab_rate_warp<true>(a, smem, cell, j, lane);
     else ab_rate_warp<false>(a, smem, cell, j, lane);
   }

@@ -509,6 +509,10 @@ SolverConsts make_consts(const stev_params *p) {
   sc.r_fac = p->r_fac;
   sc.inv_r_fac = 1.0 / p->r_fac;
   sc.rof_min = p->rof_min;
+  sc.tol_ring2 = p->tol_ring * p->tol_ring;
+  sc.ring_lo = 1.0 - 1.0e-14;
+  sc.ring_hi = 1.0 + 1.0e-14;
+  sc.ring_filter_ok = (p->tol_ring > 1.0e-100 && p->tol_ring < 1.0e100) ? 1 : 0;
   sc.nhf = p->dft_first_high_bin;
   sc.dft_enable = p->dft_enable;
   sc.max_steps = p->max_steps;

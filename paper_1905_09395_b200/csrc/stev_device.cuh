@@ -47,7 +47,9 @@ struct CellLayout {
 
 struct SolverConsts {
   double y_step_max, delta_max, alpha, tol_ring, tol_freq, r_fac, inv_r_fac, rof_min;
+  double tol_ring2, ring_lo, ring_hi;   // Tol_ring^2 and the 1 -+ 1e-14 band of the square-root-free ringing test
   int nhf, dft_enable, max_steps, energy_mode;
+  int ring_filter_ok;                   // Tol_ring^2 is a normal number far from overflow and underflow
 };
 
 struct IntegrateArgs {
