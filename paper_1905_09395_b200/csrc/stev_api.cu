@@ -434,6 +434,10 @@ int stev_estimator_load(const stev_mechanism *m, const stev_estimator_desc *d, s
     ce = cudaMalloc(&e->d_params, pb.size() * sizeof(float));
     if (ce == cudaSuccess) ce = cudaMemcpy(e->d_params, pb.data(), pb.size() * sizeof(float), cudaMemcpyHostToDevice);
   }
+  if (ce == cudaSuccess && estimator_tensor_prepare(e) != STEV_OK) {
+    stev_estimator_destroy(e);
+    return STEV_ECUDA;
+  }
   if (ce != cudaSuccess) {
     stev_estimator_destroy(e);
     return cuda_fail(ce, "estimator upload");
@@ -447,6 +451,8 @@ void stev_estimator_destroy(stev_estimator *e) {
   if (e->d_table) cudaFree(e->d_table);
   if (e->d_ab_table) cudaFree(e->d_ab_table);
   if (e->d_params) cudaFree(e->d_params);
+  for (int k = 0; k < 2; ++k)
+    if (e->d_tc_image[k]) cudaFree(e->d_tc_image[k]);
   delete e;
 }
 

@@ -10,6 +10,8 @@
 #include "stev_ab.cuh"
 #include "stev_device.cuh"
 
+struct stev_estimator;
+
 namespace stev {
 
 void set_error(const std::string &msg);
@@ -57,6 +59,8 @@ int integrate_ab_launch(const AbTables &tb, const AbCell &cl, const unsigned cha
                         long long n, long long ld, double *T, const double *p, double *Y, int *steps, unsigned char *status,
                         int *counters, cudaStream_t s, int *blocks_out, int *cells_per_block_out, size_t *smem_out);
 
+int estimator_tensor_prepare(stev_estimator *e);
+
 }  // namespace stev
 
 struct stev_mechanism {
@@ -81,4 +85,7 @@ struct stev_estimator {
   // standalone evaluation (stev_estimator_eval): device copies in kernel-friendly layouts
   float *d_params = nullptr;             // in_shift, in_scale, W1T [n_in][H], b1, W2T [H][n_out], b2
   size_t params_floats = 0;
+  // tensor-core path (stev_mlp_tc.cu): weight images in the canonical UMMA layout, [0] TF32, [1] BF16
+  bool tc_ok[2] = {false, false};
+  unsigned char *d_tc_image[2] = {nullptr, nullptr};
 };

@@ -106,6 +106,59 @@ def test_estimator_fp32_matches_cpu_forward_pass(stev, oracle, config):
     np.testing.assert_array_equal(out, ref)   # and in fact bit for bit (R18)
 
 
+def _estimator_inputs(w):
+    X = np.zeros((w.n_cells, w.estimator.n_in), np.float32)
+    X[:, 0] = w.T
+    if w.estimator.n_in > 1:
+        X[:, 1] = w.p
+        X[:, 2:] = w.Y.T
+    return X
+
+
+@pytest.mark.parametrize("config,n", [(3, 1000), (4, 1000), (4, 1), (4, 128), (3, 129), (4, 70001)])
+@pytest.mark.parametrize("precision", ["TF32", "BF16"])
+def test_estimator_tensor_core_path(stev, oracle, config, n, precision):
+    """Row a7, tcgen05 path (stev_mlp_tc.cu).  North star: 'the MLP path must match a CPU forward pass of the same
+    weights to ... 1e-2 relative where TF32/BF16 tensor cores are used'; relative error in the R24 norm
+    (|a - b| / max(|b|, RMS of that output over the batch))."""
+    w = make_workload(config, n)
+    est = stev.Estimator(None, w.estimator)
+    X = _estimator_inputs(w)
+    prec = getattr(stev, "STEV_PREC_" + precision)
+    out = stev.stev_estimator_eval(est, _dev(X), prec).cpu().numpy()
+    ref = oracle.estimator_eval(w.estimator, X)
+    assert out.shape == ref.shape and np.isfinite(out).all()
+    scale = np.maximum(np.abs(ref), np.sqrt(np.mean(ref.astype(np.float64) ** 2, axis=0, keepdims=True)))
+    err = float(np.max(np.abs(out - ref) / scale))
+    print(f"config {config} n={n} {precision}: max rel err (R24) {err:.3e}")
+    assert err <= 1e-2
+    # the tensor path really rounds its operands: it is not the fp32 path in disguise
+    if n >= 1000:
+        assert err > 1e-7
+
+
+def test_estimator_tensor_core_path_sigmoid_and_odd_widths(stev, oracle):
+    """Sigmoid activation (the paper's choice) and widths that are not multiples of the MMA shapes."""
+    import copy
+    rng = np.random.default_rng(5)
+    w = make_workload(4, 777)
+    e = copy.deepcopy(w.estimator)
+    e.activation = 1
+    e.n_hidden, e.n_out = 24, 13          # 24 -> padded to 32 columns, 13 outputs -> scalar row stores
+    e.W1 = rng.uniform(-1, 1, (e.n_hidden, e.n_in)).astype(np.float32)
+    e.b1 = rng.uniform(-1, 1, e.n_hidden).astype(np.float32)
+    e.W2 = rng.uniform(-1, 1, (e.n_out, e.n_hidden)).astype(np.float32)
+    e.b2 = rng.uniform(-1, 1, e.n_out).astype(np.float32)
+    est = stev.Estimator(None, e)
+    X = _estimator_inputs(w)
+    ref = oracle.estimator_eval(e, X)
+    scale = np.maximum(np.abs(ref), np.sqrt(np.mean(ref.astype(np.float64) ** 2, axis=0, keepdims=True)))
+    for prec in (stev.STEV_PREC_FP32, stev.STEV_PREC_TF32, stev.STEV_PREC_BF16):
+        out = stev.stev_estimator_eval(est, _dev(X), prec).cpu().numpy()
+        err = float(np.max(np.abs(out - ref) / scale))
+        assert err <= (1e-5 if prec == stev.STEV_PREC_FP32 else 1e-2), (prec, err)
+
+
 # ------------------------------------------------------------------------------------------------ the integrator
 @pytest.mark.parametrize("config,n", [(0, 4096), (1, 1500), (2, 700), (3, 300), (4, 300)])
 def test_integrate_parity(stev, oracle, config, n):
