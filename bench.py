@@ -52,6 +52,8 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--ref-cells", type=int, default=None, help="cells per step of the --impl reference arm")
+    ap.add_argument("--what", default="integrate", choices=["integrate", "estimator"],
+                    help="estimator: time the standalone MLP forward pass (row a7) of config 3/4 on the fp32, TF32 and BF16 paths")
     return ap.parse_args()
 
 
@@ -158,10 +160,74 @@ def run_reference(args):
 
 
 # ----------------------------------------------------------------------------------------------------------------
+def run_estimator(args):
+    """Row a7 on its own (BASELINE.json config 4: 'run on the tensor-core (TF32/BF16) path vs the fp32 CUDA-core path'):
+    one step = one stev_estimator_eval call over all cells of the config; inputs and outputs resident in HBM."""
+    import torch
+    import paper_1905_09395_b200 as stev
+    from stev_inputs.configs import make_workload, FULL_CELLS
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device")
+    stev.load()
+    config = args.config if args.config in (3, 4) else 4
+    n = FULL_CELLS[config] if args.cells is None else args.cells
+    w = make_workload(config, n)
+    e = w.estimator
+    est = stev.Estimator(None, e)
+    dev = torch.device("cuda:0")
+    X = torch.empty((n, e.n_in), dtype=torch.float32, device=dev)
+    X[:, 0] = torch.tensor(w.T, dtype=torch.float32, device=dev)
+    if e.n_in > 1:
+        X[:, 1] = torch.tensor(w.p, dtype=torch.float32, device=dev)
+        X[:, 2:] = torch.tensor(w.Y.T, dtype=torch.float32, device=dev)
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    bytes_per_call = 4 * n * (e.n_in + e.n_out)
+    flop_per_call = 2.0 * n * (e.n_in * e.n_hidden + e.n_hidden * e.n_out)
+    stream = torch.cuda.current_stream()
+    res = {}
+    for name in ("FP32", "TF32", "BF16"):
+        prec = getattr(stev, "STEV_PREC_" + name)
+        for _ in range(max(args.warmup, 3)):
+            out = stev.stev_estimator_eval(est, X, prec)
+        ms = []
+        for _ in range(max(args.steps, 3)):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            out = stev.stev_estimator_eval(est, X, prec)
+            e1.record(stream)
+            e1.synchronize()
+            ms.append(e0.elapsed_time(e1))
+        t = float(np.mean(ms)) * 1e-3
+        res[name] = {"ms": 1e3 * t, "cells_per_s": n / t, "hbm_gbs": bytes_per_call / t / 1e9,
+                     "hbm_frac_of_measured": bytes_per_call / t / 1e9 / hbm_peak, "tflops": flop_per_call / t / 1e12}
+        del out
+    best = max(("TF32", "BF16"), key=lambda k: res[k]["cells_per_s"])
+    line = {"metric": "cells evaluated per second by the standalone MLP estimator (row a7)", "value": res[best]["cells_per_s"],
+            "unit": "cells/s", "n_gpus": 1, "steps": max(args.steps, 3), "warmup": max(args.warmup, 3),
+            "ms_per_step": res[best]["ms"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": best.lower(), "data": "synthetic",
+            "config": {"workload": f"{w.name}: estimator {e.n_in}-{e.n_hidden}-{e.n_out}", "cells": n,
+                       "l2": f"inputs + outputs {bytes_per_call >> 20} MiB, larger than L2"},
+            "paths": res, "gpu_launches": max(args.steps, 3),
+            "roofline": {"bound": "hbm", "kernel": "estimator_tc_kernel", "achieved": res[best]["hbm_gbs"], "peak": hbm_peak,
+                         "unit": "GB/s", "frac": res[best]["hbm_frac_of_measured"], "traffic": None,
+                         "peak_source": "MEASURED_PEAKS.json hbm_gbs (of measured)" if peaks else "fallback 6650 GB/s (of fallback)",
+                         "bytes_per_cell": 4 * (e.n_in + e.n_out)}}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.what == "estimator":
+        return run_estimator(args)
 
     import torch
     import paper_1905_09395_b200 as stev
@@ -287,7 +353,7 @@ def main():
     cpu_baseline = None
     if not args.no_cpu_baseline:
         cores = os.cpu_count() or 1
-        n_s = {0: 4096, 1: 1024, 2: 512, 3: 96 * cores, 4: 256}[args.config]
+        n_s = {0: 4096, 1: 4096, 2: 2048, 3: 768 * cores, 4: 1024}[args.config]   # about 10-30 s of oracle time
         n_s = min(n_s, n)
         cps, dt, cs, thr = oracle_time(w, n_s, cores)
         cpu_baseline = {"value": cps, "unit": UNIT, "cores": thr, "kind": "oracle",
