@@ -109,9 +109,13 @@ typedef struct {
   int32_t chunk_steps;    /* 0: every cell runs to completion in one pass; > 0: a pass advances each active
                              cell at most this many steps, unfinished cells are spilled to the workspace and the
                              active-cell list is compacted before the next pass */
-  int32_t lanes_per_cell; /* 0 = chosen from (S, R); 1,2,4,8,16,32 = lanes cooperating on one cell (one kernel role);
-                             64 = the warp-specialised kernel: a rate warp + a DFT warp per cell, DFT history in
-                             tensor memory (default for >= 128 reactions; needs dft_enable, chunk_steps = 0) */
+  int32_t lanes_per_cell; /* 0 = chosen from (S, R).  1,2,4,8,16,32 = lanes cooperating on one cell, DFT history in
+                             shared memory (any mechanism, any chunk_steps).  Kernels that keep the DFT history in tensor
+                             memory (need chunk_steps = 0, at most two factors per reaction side):
+                             33 = one warp per cell, 16 cells per SM (<= 32 species, 1..128 reversible reactions);
+                             64 = a warp pair per cell, 8 cells per SM, both warps split every phase of a step
+                                  (<= 64 species, 1..256 reversible reactions; the default for >= 128 reactions);
+                             66 = warp-specialised variant of 64 (a rate warp + a DFT warp; also needs dft_enable) */
 } stev_params;
 
 /* Counters of the last stev_integrate / stev_integrate_host call on this thread. */

@@ -9,8 +9,8 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libstev_b200.so")
-SOURCES = ["stev_api.cu", "stev_ab.cu", "stev_compact.cu", "stev_aux.cu", "stev_mlp_tc.cu"]
-HEADERS = ["stev_math.cuh", "stev_device.cuh", "stev_ab.cuh", "stev_ab_kernel.cuh", "stev_host.h", os.path.join("..", "..", "include", "stev.h")]
+SOURCES = ["stev_api.cu", "stev_ab.cu", "stev_pk.cu", "stev_compact.cu", "stev_aux.cu", "stev_mlp_tc.cu"]
+HEADERS = ["stev_math.cuh", "stev_device.cuh", "stev_ab.cuh", "stev_ab_kernel.cuh", "stev_fast.cuh", "stev_pk.cuh", "stev_pk_kernel.cuh", "stev_host.h", os.path.join("..", "..", "include", "stev.h")]
 
 # --fmad=false: no implicit FMA contraction anywhere (arithmetic contract); FMAs are explicit.
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "--fmad=false",
@@ -42,7 +42,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
             f.write(r.stderr)
         return obj
 
-    with ThreadPoolExecutor(max_workers=4) as ex:
+    with ThreadPoolExecutor(max_workers=6) as ex:
         objs = list(ex.map(compile_one, SOURCES))
     cmd = ["nvcc", "-shared", "-o", LIB, *objs, "-lcudart"]
     r = subprocess.run(cmd, capture_output=True, text=True)

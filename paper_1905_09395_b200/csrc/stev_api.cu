@@ -351,6 +351,14 @@ int stev_mechanism_create(const stev_mechanism_desc *d, stev_mechanism **out) {
       if (e == cudaSuccess) e = cudaMemcpy(m->d_ab_table, ab.data(), ab.size(), cudaMemcpyHostToDevice);
     }
   }
+  for (int w = 1; w >= 0 && e == cudaSuccess; --w) {   // the pair image first: it chooses the reaction order
+    std::vector<unsigned char> pk;
+    m->pk_ok[w] = build_pk_image(h, nullptr, w + 1, pk, m->pk_tb[w], m->pk_cl[w]);
+    if (m->pk_ok[w]) {
+      e = cudaMalloc(&m->d_pk_table[w], pk.size());
+      if (e == cudaSuccess) e = cudaMemcpy(m->d_pk_table[w], pk.data(), pk.size(), cudaMemcpyHostToDevice);
+    }
+  }
   if (e != cudaSuccess) {
     stev_mechanism_destroy(m);
     return cuda_fail(e, "mechanism table upload");
@@ -363,6 +371,8 @@ void stev_mechanism_destroy(stev_mechanism *m) {
   if (!m) return;
   if (m->d_table) cudaFree(m->d_table);
   if (m->d_ab_table) cudaFree(m->d_ab_table);
+  for (int w = 0; w < 2; ++w)
+    if (m->d_pk_table[w]) cudaFree(m->d_pk_table[w]);
   delete m;
 }
 
@@ -418,6 +428,14 @@ int stev_estimator_load(const stev_mechanism *m, const stev_estimator_desc *d, s
         if (ce == cudaSuccess) ce = cudaMemcpy(e->d_ab_table, ab.data(), ab.size(), cudaMemcpyHostToDevice);
       }
     }
+    for (int w = 1; w >= 0 && ce == cudaSuccess; --w) {
+      std::vector<unsigned char> pk;
+      e->pk_ok[w] = build_pk_image(m->host, &h, w + 1, pk, e->pk_tb[w], e->pk_cl[w]);
+      if (e->pk_ok[w]) {
+        ce = cudaMalloc(&e->d_pk_table[w], pk.size());
+        if (ce == cudaSuccess) ce = cudaMemcpy(e->d_pk_table[w], pk.data(), pk.size(), cudaMemcpyHostToDevice);
+      }
+    }
   }
   if (ce == cudaSuccess) {
     // standalone parameter block: in_shift, in_scale, W1T [n_in][H], b1, W2T [H][n_out], b2
@@ -450,6 +468,8 @@ void stev_estimator_destroy(stev_estimator *e) {
   if (!e) return;
   if (e->d_table) cudaFree(e->d_table);
   if (e->d_ab_table) cudaFree(e->d_ab_table);
+  for (int w = 0; w < 2; ++w)
+    if (e->d_pk_table[w]) cudaFree(e->d_pk_table[w]);
   if (e->d_params) cudaFree(e->d_params);
   for (int k = 0; k < 2; ++k)
     if (e->d_tc_image[k]) cudaFree(e->d_tc_image[k]);
@@ -613,22 +633,41 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
   cudaStream_t s = (cudaStream_t)cuda_stream;
   Workspace w = carve(workspace, *tb, p, n);
 
-  // Large mechanisms: the warp-specialised kernel (a rate warp and a DFT warp per cell, history in tensor memory).
+  // The whole-cell-on-chip kernels with the DFT history in tensor memory.
+  //   lanes_per_cell = 33: one warp per cell, 16 cells per SM (the default when the mechanism fits: <= 32 species,
+  //                        <= 128 reversible reactions)
+  //   lanes_per_cell = 64: warp pair per cell, 8 cells per SM (both warps split every phase; the default for >= 128 reactions)
+  //   lanes_per_cell = 66: warp-specialised kernel (a rate warp and a DFT warp per cell)
   {
-    const bool ab_ok = est ? est->ab_ok : m->ab_ok;
-    const bool ab_allowed = ab_ok && p->dft_enable && p->chunk_steps == 0;
-    if (p->lanes_per_cell == 64 && !ab_allowed) {
-      set_error("stev_integrate: lanes_per_cell = 64 (warp-specialised kernel) needs dft_enable = 1, chunk_steps = 0, at most "
-                "two factors per reaction side and at most 256 reversible reactions");
+    const bool tm_common = p->chunk_steps == 0;
+    const bool pk1_ok = (est ? est->pk_ok[0] : m->pk_ok[0]) && tm_common;
+    const bool pk2_ok = (est ? est->pk_ok[1] : m->pk_ok[1]) && tm_common;
+    const bool ab_ok = (est ? est->ab_ok : m->ab_ok) && p->dft_enable && tm_common;
+    int kind = 0;   // 1: one warp per cell, 2: warp pair, 3: warp-specialised
+    if (p->lanes_per_cell == 33) kind = 1;
+    else if (p->lanes_per_cell == 64) kind = 2;
+    else if (p->lanes_per_cell == 66) kind = 3;
+    else if (p->lanes_per_cell == 0) kind = (tb->R >= 128 && pk2_ok) ? 2 : (pk1_ok ? 1 : (pk2_ok && tb->R >= 64 ? 2 : 0));
+    if ((kind == 1 && !pk1_ok) || (kind == 2 && !pk2_ok) || (kind == 3 && !ab_ok)) {
+      set_error("stev_integrate: lanes_per_cell = 33 / 64 / 66 (tensor-memory kernels) need chunk_steps = 0, at most two factors "
+                "per reaction side, 1..128 (33) or 1..256 (64, 66) reversible reactions, at most 32 (33) or 64 species "
+                "(66 also dft_enable = 1)");
       return STEV_EINVAL;
     }
-    if (ab_allowed && (p->lanes_per_cell == 64 || (p->lanes_per_cell == 0 && tb->R >= 128))) {
+    if (kind) {
       STEV_CUDA(cudaMemsetAsync(w.counters, 0, 256, s));
       int blocks = 0, cpb = 0;
       size_t smem = 0;
-      rc = integrate_ab_launch(est ? est->ab_tb : m->ab_tb, est ? est->ab_cl : m->ab_cl, est ? est->d_ab_table : m->d_ab_table,
-                               make_consts(p), dt_cfd, n, ld, T, pressure, Y, steps_out, status_out, w.counters, s, &blocks, &cpb,
-                               &smem);
+      if (kind == 3) {
+        rc = integrate_ab_launch(est ? est->ab_tb : m->ab_tb, est ? est->ab_cl : m->ab_cl, est ? est->d_ab_table : m->d_ab_table,
+                                 make_consts(p), dt_cfd, n, ld, T, pressure, Y, steps_out, status_out, w.counters, s, &blocks, &cpb,
+                                 &smem);
+      } else {
+        const int wi = kind - 1;
+        rc = integrate_pk_launch(est ? est->pk_tb[wi] : m->pk_tb[wi], est ? est->pk_cl[wi] : m->pk_cl[wi],
+                                 est ? est->d_pk_table[wi] : m->d_pk_table[wi], make_consts(p), dt_cfd, n, ld, T, pressure, Y,
+                                 steps_out, status_out, w.counters, s, &blocks, &cpb, &smem);
+      }
       if (rc) return rc;
       int worst = 0;
       STEV_CUDA(cudaMemcpyAsync(&worst, w.counters + 1, 4, cudaMemcpyDeviceToHost, s));
@@ -637,8 +676,8 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
       g_stats.passes = 1;
       g_stats.kernel_launches = 1;
       g_stats.blocks = blocks;
-      g_stats.lanes_per_cell = 64;
-      g_stats.threads_per_block = kAbThreads;
+      g_stats.lanes_per_cell = kind == 1 ? 33 : (kind == 2 ? 64 : 66);
+      g_stats.threads_per_block = kind == 3 ? kAbThreads : kPkThreads;
       g_stats.cells_per_block = cpb;
       g_stats.smem_bytes = (int64_t)smem;
       if (worst == 2) { set_error("some cells produced non-finite values (status 2)"); return STEV_WNONFINITE; }

@@ -8,6 +8,7 @@
 
 #include "../../include/stev.h"
 #include "stev_ab.cuh"
+#include "stev_pk.cuh"
 #include "stev_device.cuh"
 
 struct stev_estimator;
@@ -36,6 +37,7 @@ struct HostMechanism {
   std::vector<int> reac_ptr, reac_sp, reac_nu, prod_ptr, prod_sp, prod_nu;
   std::vector<int> internal_of;  // caller reaction index -> internal index (reversible first)
   std::vector<int> orig_of;      // internal -> caller
+  mutable std::vector<int> pk_order;     // internal -> caller of the warp-pair kernel (bank-conflict-aware, chosen once)
 };
 
 // Builds the table image for a mechanism and, optionally, an estimator.
@@ -61,6 +63,14 @@ int integrate_ab_launch(const AbTables &tb, const AbCell &cl, const unsigned cha
 
 int estimator_tensor_prepare(stev_estimator *e);
 
+// Warp-pair integrator (stev_pk.cuh / stev_pk.cu): both warps of a cell split every phase.  Same limits as above
+// plus at most 64 species.
+bool build_pk_image(const HostMechanism &m, const HostEstimator *e, int nw, std::vector<unsigned char> &image, PkTables &tb,
+                    PkCell &cl);
+int integrate_pk_launch(const PkTables &tb, const PkCell &cl, const unsigned char *d_table, const SolverConsts &sc, double t_f,
+                        long long n, long long ld, double *T, const double *p, double *Y, int *steps, unsigned char *status,
+                        int *counters, cudaStream_t s, int *blocks_out, int *cells_per_block_out, size_t *smem_out);
+
 }  // namespace stev
 
 struct stev_mechanism {
@@ -71,6 +81,10 @@ struct stev_mechanism {
   stev::AbTables ab_tb{};
   stev::AbCell ab_cl{};
   unsigned char *d_ab_table = nullptr;
+  bool pk_ok[2] = {false, false};        // images of the tensor-memory kernel, [0] one warp per cell, [1] warp pair (NASA-7 thermo)
+  stev::PkTables pk_tb[2]{};
+  stev::PkCell pk_cl[2]{};
+  unsigned char *d_pk_table[2] = {nullptr, nullptr};
 };
 
 struct stev_estimator {
@@ -82,6 +96,10 @@ struct stev_estimator {
   stev::AbTables ab_tb{};
   stev::AbCell ab_cl{};
   unsigned char *d_ab_table = nullptr;
+  bool pk_ok[2] = {false, false};        // images of the tensor-memory kernel (MLP thermo)
+  stev::PkTables pk_tb[2]{};
+  stev::PkCell pk_cl[2]{};
+  unsigned char *d_pk_table[2] = {nullptr, nullptr};
   // standalone evaluation (stev_estimator_eval): device copies in kernel-friendly layouts
   float *d_params = nullptr;             // in_shift, in_scale, W1T [n_in][H], b1, W2T [H][n_out], b2
   size_t params_floats = 0;

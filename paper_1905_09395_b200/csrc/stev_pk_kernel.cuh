@@ -1,0 +1,576 @@
+// stev_pk_kernel.cuh -- the warp-pair STEV integrator for large mechanisms (rows a1-a7 of DESIGN.md section 1).
+//
+// One block per SM holds up to eight cells.  Each cell is served by a PAIR of warps that split every phase of a step
+// between them (no idle role), meeting at a 64-thread named barrier between phases:
+//   A  warp 0: scalars, ln T, ln(p_atm/R_u T), NASA-7 g/RT, 1/Wbar, stabilised concentrations
+//      warp 1: the cp / h estimator (MLP on fp32 CUDA cores, or the NASA-7 polynomials)
+//   B  both:   Arrhenius + equilibrium rates of their own 32-blocks of reactions, q_eff = q rOF, stored multiples
+//   C  both:   source terms of their own species (one species per lane), step limiter, warp minimum
+//   D  both:   step size, Euler update of their own species, DFT ringing filter of their own 32-blocks of
+//              reversible reactions; warp 0 also evaluates the two sequential sums of the temperature equation
+// The 13-deep history of every reversible reaction lives in TENSOR MEMORY (one lane-private row of TMEM columns per
+// reaction, tcgen05.st / tcgen05.ld); both warps of a pair sit in the same TMEM lane quarter.  Shared memory holds the
+// mechanism tables (one TMA bulk copy per block) and ~17 KB of per-cell scratch; the hot loop has no HBM traffic.
+// Arithmetic follows the contract of DESIGN.md section 5 exactly; every bit-equivalent deviation in evaluation order
+// is explained where it occurs.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "stev_device.cuh"
+#include "stev_fast.cuh"
+#include "stev_math.cuh"
+#include "stev_pk.cuh"
+
+namespace stev {
+
+// ---------------------------------------------------------------------------------------------------------
+// a1: NASA-7 (Eqs 15-16, R17) by one warp: g/RT (and 2 g/RT) always, cp/R and h/RT if CPH.
+// Two species per lane side by side; lanes past the end recompute the last species and store nothing.
+// ---------------------------------------------------------------------------------------------------------
+template <bool CPH>
+__device__ __forceinline__ void pk_nasa(const PkTables &tb, const unsigned char *tbl, double *cG, double2 *cYwCp, double2 *cHOm,
+                                        double T, double invT, double lnT, int lane) {
+  const int S = tb.S;
+  const double *tmid = (const double *)(tbl + tb.o_tmid), *nasa = (const double *)(tbl + tb.o_nasa);
+  for (int ia = lane; ia < S; ia += 64) {
+    const int ib_ = ia + 32;
+    const int ib = (ib_ < S) ? ib_ : S - 1;
+    const double *ca = nasa + ((T < tmid[ia]) ? 0 : kNasaRows * S) + ia;
+    const double *cb = nasa + ((T < tmid[ib]) ? 0 : kNasaRows * S) + ib;
+    const double a1a = ca[0], a2a = ca[S], a1b = cb[0], a2b = cb[S];
+    const double hpa = fma_rn(fma_rn(fma_rn(fma_rn(ca[8 * S], T, ca[7 * S]), T, ca[6 * S]), T, ca[5 * S]), T, a1a);
+    const double hpb = fma_rn(fma_rn(fma_rn(fma_rn(cb[8 * S], T, cb[7 * S]), T, cb[6 * S]), T, cb[5 * S]), T, a1b);
+    const double hRTa = fma_rn(ca[9 * S], invT, hpa), hRTb = fma_rn(cb[9 * S], invT, hpb);
+    const double spa = fma_rn(fma_rn(fma_rn(ca[12 * S], T, ca[11 * S]), T, ca[10 * S]), T, a2a);
+    const double spb = fma_rn(fma_rn(fma_rn(cb[12 * S], T, cb[11 * S]), T, cb[10 * S]), T, a2b);
+    const double sRa = fma_rn(a1a, lnT, fma_rn(spa, T, ca[13 * S])), sRb = fma_rn(a1b, lnT, fma_rn(spb, T, cb[13 * S]));
+    const double ga = hRTa - sRa, gb = hRTb - sRb;
+    cG[1 + ia] = ga;
+    cG[1 + S + ia] = ga + ga;
+    if (ib_ < S) {
+      cG[1 + ib] = gb;
+      cG[1 + S + ib] = gb + gb;
+    }
+    if (CPH) {
+      cYwCp[ia].y = fma_rn(fma_rn(fma_rn(fma_rn(ca[4 * S], T, ca[3 * S]), T, ca[2 * S]), T, a2a), T, a1a);
+      cHOm[ia].x = hRTa;
+      if (ib_ < S) {
+        cYwCp[ib].y = fma_rn(fma_rn(fma_rn(fma_rn(cb[4 * S], T, cb[3 * S]), T, cb[2 * S]), T, a2b), T, a1b);
+        cHOm[ib].x = hRTb;
+      }
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// a7 in the integrator (fp32 CUDA cores, R18): cp_i/R and h_i/(R T_ref) from the shallow MLP, by one warp.
+// ---------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void pk_mlp(const PkTables &tb, const unsigned char *tbl, const double2 *cYp, double2 *cYwCp,
+                                       double2 *cHOm, float *cHid, double T, double p, double invT, int lane) {
+  const int S = tb.S;
+  const float *eshift = (const float *)(tbl + tb.o_eshift), *escale = (const float *)(tbl + tb.o_escale);
+  const float *W1T = (const float *)(tbl + tb.o_W1T), *b1 = (const float *)(tbl + tb.o_b1);
+  const float *W2p = (const float *)(tbl + tb.o_W2p), *b2 = (const float *)(tbl + tb.o_b2);
+  const int H = tb.H, Hpad = tb.Hpad, n_in = tb.n_in, n_out = tb.n_out;
+  for (int jh = lane; jh < H; jh += 32) {
+    float z = b1[jh];
+    for (int k = 0; k < n_in; ++k) {
+      const double raw = (k == 0) ? T : ((k == 1) ? p : cYp[k - 2].x);
+      const float xk = ((float)raw - eshift[k]) * escale[k];
+      z = __fmaf_rn(W1T[k * H + jh], xk, z);
+    }
+    const double zd = (double)z;
+    float act;
+    if (tb.act == 0) act = (float)(1.0 - 2.0 / (1.0 + ab_exp(2.0 * zd)));
+    else act = (float)(1.0 / (1.0 + ab_exp(-zd)));
+    cHid[jh] = act;
+  }
+  __syncwarp();
+  const float4 *hid4 = (const float4 *)cHid;
+  for (int o0 = 0; o0 < n_out; o0 += 128) {
+    float y[4];
+    const float4 *wrow[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      int o = o0 + 32 * u + lane;
+      o = (o < n_out) ? o : n_out - 1;
+      y[u] = b2[o];
+      wrow[u] = (const float4 *)(W2p + (size_t)o * Hpad);
+    }
+#pragma unroll 4
+    for (int q4 = 0; q4 < H / 4; ++q4) {
+      const float4 hv = hid4[q4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const float4 wv = wrow[u][q4];
+        y[u] = __fmaf_rn(wv.x, hv.x, y[u]);
+        y[u] = __fmaf_rn(wv.y, hv.y, y[u]);
+        y[u] = __fmaf_rn(wv.z, hv.z, y[u]);
+        y[u] = __fmaf_rn(wv.w, hv.w, y[u]);
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int o = o0 + 32 * u + lane;
+      if (o < n_out) {
+        if (o < S) cYwCp[o].y = (double)y[u];
+        else cHOm[o - S].x = ((double)y[u] * (double)tb.h_ref_T) * invT;
+      }
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// a5: the ringing filter (Eqs 8-13) of the 32-blocks [it_lo, it_hi) of reversible reactions, by one
+// warp.  TMEM address of slot s of this lane's reaction in block `it`:  trow + it * 32 + 2 s.
+// Two windows are processed side by side (independent dependency chains for the scheduler).
+// ---------------------------------------------------------------------------------------------------------
+template <int NHF>
+__device__ __forceinline__ void pk_dft(const SolverConsts &sc, const double *cQ, double *cRof, int Rrev, int it_lo, int it_hi,
+                                       uint32_t trow, int slot, double h, double inv_ctot, int lane) {
+  auto update_rof = [&](int k, bool ringing) {
+    double rof = cRof[k] * (ringing ? sc.inv_r_fac : sc.r_fac);   // Eqs 12-13
+    if (rof > 1.0) rof = 1.0;
+    if (rof < sc.rof_min) rof = sc.rof_min;
+    cRof[k] = rof;
+  };
+  // Eq 8 with R8, R9: the applied change in progress / C_tot of every reversible reaction goes into its window
+  for (int it = it_lo; it < it_hi; ++it) {
+    const int k = it * 32 + lane;
+    const double q = (k < Rrev) ? cQ[k] : 0.0;
+    tmem_st2(trow + it * 32 + 2 * slot, (q * h) * inv_ctot);
+  }
+  tmem_wait_st();
+  int it = it_lo;
+  for (; it + 2 <= it_hi; it += 2) {
+    uint32_t ra[26], rb[26];
+    tmem_ld26(trow + it * 32, ra);
+    tmem_ld26(trow + it * 32 + 32, rb);
+    tmem_wait_ld();
+    double xa[kWindow], xb[kWindow];
+    unpack_window(ra, xa);
+    unpack_window(rb, xb);
+    double d0a, m2a, d0b, m2b;
+    ab_window_stats<NHF>(xa, d0a, m2a);
+    ab_window_stats<NHF>(xb, d0b, m2b);
+    const int ka = it * 32 + lane, kb = ka + 32;
+    bool sure_a, sure_b;
+    bool ring_a = ab_ring_filter(d0a, m2a, sc, sure_a);
+    bool ring_b = ab_ring_filter(d0b, m2b, sc, sure_b);
+    if (__any_sync(0xffffffffu, (!sure_a && ka < Rrev) || (!sure_b && kb < Rrev))) {
+      ring_a = ab_ring_exact(d0a, m2a, sc);
+      ring_b = ab_ring_exact(d0b, m2b, sc);
+    }
+    if (ka < Rrev) update_rof(ka, ring_a);
+    if (kb < Rrev) update_rof(kb, ring_b);
+  }
+  if (it < it_hi) {
+    uint32_t ra[26];
+    tmem_ld26(trow + it * 32, ra);
+    tmem_wait_ld();
+    double xa[kWindow];
+    unpack_window(ra, xa);
+    double d0a, m2a;
+    ab_window_stats<NHF>(xa, d0a, m2a);
+    const int ka = it * 32 + lane;
+    bool sure_a;
+    bool ring_a = ab_ring_filter(d0a, m2a, sc, sure_a);
+    if (__any_sync(0xffffffffu, !sure_a && ka < Rrev)) ring_a = ab_ring_exact(d0a, m2a, sc);
+    if (ka < Rrev) update_rof(ka, ring_a);
+  }
+}
+
+// unsigned-bit-pattern minimum of positive doubles (NaN patterns sort above +inf and are thereby ignored, like the
+// contract's plain comparison `lim < t_star` ignores them)
+__device__ __forceinline__ double pk_min_bits(double a, double b) {
+  return (double_to_bits(b) < double_to_bits(a)) ? b : a;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// One warp of the NW (1 or 2) warps that serve a cell.  `half` (0 .. NW-1) is warp-uniform.  With NW = 1 the pair
+// barriers degenerate to __syncwarp and the warp walks both halves of every phase (mid-size mechanisms: 16 cells per SM).
+// ---------------------------------------------------------------------------------------------------------
+template <bool EST, int NW>
+__device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *tbl, unsigned char *cell, int j, int half,
+                                          uint32_t tmem_base, int lane) {
+  const PkTables &tb = a.tb;
+  const SolverConsts &sc = a.sc;
+  const int S = tb.S, R = tb.R, Rrev = tb.Rrev, Rp = tb.Rp, n_it = tb.n_it;
+  double2 *cYp = (double2 *)(cell + a.cl.oYp);
+  double2 *cYwCp = (double2 *)(cell + a.cl.oYwCp);
+  double2 *cHOm = (double2 *)(cell + a.cl.oHOm);
+  double *cConc = (double *)(cell + a.cl.oConc);
+  double *cG = (double *)(cell + a.cl.oG);
+  double *cQ = (double *)(cell + a.cl.oQ);
+  double *cRof = (double *)(cell + a.cl.oRof);
+  float *cHid = (float *)(cell + a.cl.oHid);
+  volatile PkScal *scal = (volatile PkScal *)(cell + a.cl.oSc);
+
+  const double *W = (const double *)(tbl + tb.o_W), *invW = (const double *)(tbl + tb.o_invW);
+  const double2 *rkA = (const double2 *)(tbl + tb.o_rkA), *rkB = (const double2 *)(tbl + tb.o_rkB);
+  const uint4 *rfac = (const uint4 *)(tbl + tb.o_rfac), *rdg = (const uint4 *)(tbl + tb.o_rdg);
+  const unsigned char *gsp = tbl + tb.o_gsp;
+  const bool has2 = tb.n_var > 2;
+
+  const int bar = 1 + j;                        // named barrier of this pair (0 is __syncthreads)
+  auto cell_sync = [&]() {
+    if (NW == 2) named_bar_sync(bar);
+    else __syncwarp();
+  };
+  const double dt_max = a.t_f * sc.delta_max;   // Eq 4
+  const double t_tol = 1.0e-12 * a.t_f;         // R5
+  const uint32_t trow = tmem_base + ((uint32_t)((j & 3) * 32) << 16) + (uint32_t)((j >> 2) * (NW == 2 ? 256 : 128));
+  const int it_lo = half ? tb.it_half0 : 0, it_hi = half ? n_it : tb.it_half0;   // DFT blocks of this warp
+  const int my_sp = half * 32 + lane;           // species this lane loads, updates and writes back
+  const int g_sp = gsp[half * 32 + lane];       // species whose source term this lane gathers (255 = none)
+  const uint4 *ge = (const uint4 *)(tbl + tb.o_gent) + (half ? tb.g_len4[0] * 32 : 0) + lane;
+  const int g_len4 = tb.g_len4[half];
+  const int g_mylen = ((const unsigned short *)(tbl + tb.o_glen))[half * 32 + lane];   // entries of this lane's list
+
+  if (half == 0 && lane == 0) {
+    cConc[0] = 1.0;
+    cG[0] = 0.0;
+  }
+
+  for (;;) {
+    // ---- a6: variable load.  A pair whose cell retired pulls the next active cell from the global queue.
+    if (half == 0 && lane == 0) scal->pos = atomicAdd(a.queue_head, 1);
+    cell_sync();
+    const int pos = scal->pos;
+    if ((long long)pos >= a.n_active) return;
+    const int cidx = a.list ? a.list[pos] : pos;
+    double T = a.T[cidx];
+    const double p = a.p[cidx];
+    if (my_sp < S) cYp[my_sp] = make_double2(a.Y[(long long)my_sp * a.ld + cidx], invW[my_sp]);
+    for (int it = it_lo; it < it_hi; ++it) {
+#pragma unroll
+      for (int s = 0; s < kWindow; ++s) tmem_st2(trow + it * 32 + 2 * s, 0.0);   // R10: zero-initialised window
+      const int k = it * 32 + lane;
+      if (k < Rrev) cRof[k] = 1.0;                                                // Eq 11
+    }
+    tmem_wait_st();
+    double t = 0.0;
+    int steps = 0, slot = 0;
+    cell_sync();
+
+    for (;;) {
+      // ================= phase A =================
+      double lnT, ln_c0, invT, inv_ctot, rho;
+      if (NW == 1 || half == 0) {
+        // -- scalars.  ln T and ln(p_atm / (R_u T)) are evaluated side by side in the two half-warps.
+        const double RuT = kRu * T;
+        const double c_tot = p / RuT;
+        invT = 1.0 / T;
+        const double larg = (lane & 16) ? (kPatm / RuT) : T;
+        const double lval = ab_log(larg);
+        lnT = __shfl_sync(0xffffffffu, lval, 0);
+        ln_c0 = __shfl_sync(0xffffffffu, lval, 16);
+        inv_ctot = 1.0 / c_tot;
+        if (EST) pk_nasa<false>(tb, tbl, cG, cYwCp, cHOm, T, invT, lnT, lane);
+        else if (NW == 1) pk_nasa<true>(tb, tbl, cG, cYwCp, cHOm, T, invT, lnT, lane);
+        // -- 1/Wbar = sum Y_i/W_i, sequential in species order (contract 5.4)
+        double inv_wbar = 0.0;
+#pragma unroll 8
+        for (int i = 0; i < S; ++i) {
+          const double2 v = cYp[i];
+          inv_wbar = fma_rn(v.x, v.y, inv_wbar);
+        }
+        rho = c_tot / inv_wbar;
+        if (lane == 0) {
+          scal->lnT = lnT;
+          scal->ln_c0 = ln_c0;
+          scal->invT = invT;
+          scal->inv_ctot = inv_ctot;
+          scal->rho = rho;
+        }
+        // -- Y_i/W_i (for the cp sum) and the small-species stabilisation (Eqs 6-7, R7):
+        //    C** = gamma(y) rho y / W
+        for (int ia = lane; ia < S; ia += 64) {
+          const int ib_ = ia + 32;
+          const int ib = (ib_ < S) ? ib_ : S - 1;
+          const double2 va = cYp[ia], vb = cYp[ib];
+          const double ypa = (va.x > 0.0) ? va.x : 0.0, ypb = (vb.x > 0.0) ? vb.x : 0.0;
+          double ca = (rho * ypa) * va.y, cb = (rho * ypb) * vb.y;
+          if (sc.alpha > 0.0) {
+            const double gam_a = ypa / (sc.alpha + ypa), gam_b = ypb / (sc.alpha + ypb);
+            ca = gam_a * ca;
+            cb = gam_b * cb;
+          }
+          cYwCp[ia].x = va.x * va.y;
+          cConc[1 + ia] = ca;
+          if (ib_ < S) {
+            cYwCp[ib].x = vb.x * vb.y;
+            cConc[1 + ib] = cb;
+          }
+        }
+      }
+      if (NW == 1) {
+        if (EST) pk_mlp(tb, tbl, cYp, cYwCp, cHOm, cHid, T, p, invT, lane);
+      } else if (half == 1) {
+        if (EST) {
+          pk_mlp(tb, tbl, cYp, cYwCp, cHOm, cHid, T, p, 1.0 / T, lane);
+        } else {
+          pk_nasa<true>(tb, tbl, cG, cYwCp, cHOm, T, 1.0 / T, ab_log(T), lane);
+        }
+      }
+      cell_sync();
+      if (NW == 2 && half) {
+        lnT = scal->lnT;
+        ln_c0 = scal->ln_c0;
+        invT = scal->invT;
+        inv_ctot = scal->inv_ctot;
+        rho = scal->rho;
+      }
+
+      // ================= phase B: a2, rate constants and effective progress rates (Eqs 28-30, Eq 14) =================
+      // Reversible reactions occupy internal indices [0, Rrev) in 32-blocks; blocks b = half (mod 2) belong to this
+      // warp and are evaluated two at a time (four independent exp chains for the scheduler).  Lanes past the end
+      // recompute the last reaction and store nothing.  The stored multiples +q, -q, +2q, -2q (all exact) turn the sum
+      // omega_i = sum_j nu_ij q_j into plain additions in the contract's order.
+      for (int b0 = half; b0 < n_it; b0 += 2 * NW) {
+        const int ka_ = b0 * 32 + lane, kb_ = ka_ + 32 * NW;
+        const int ka = (ka_ < Rrev) ? ka_ : Rrev - 1, kb = (kb_ < Rrev) ? kb_ : Rrev - 1;
+        const double2 pa0 = rkA[ka], pa1 = rkB[ka], pb0 = rkA[kb], pb1 = rkB[kb];
+        const uint4 fa = rfac[ka], da = rdg[ka], fb = rfac[kb], db = rdg[kb];
+        const double lkf_a = fma_rn(-pa1.x, invT, fma_rn(pa0.y, lnT, pa0.x));
+        const double lkf_b = fma_rn(-pb1.x, invT, fma_rn(pb0.y, lnT, pb0.x));
+        double dga = 0.0 - lds_f64(cell, da.x), dgb = 0.0 - lds_f64(cell, db.x);
+        dga = dga - lds_f64(cell, da.y);
+        dgb = dgb - lds_f64(cell, db.y);
+        dga = dga + lds_f64(cell, da.z);
+        dgb = dgb + lds_f64(cell, db.z);
+        dga = dga + lds_f64(cell, da.w);
+        dgb = dgb + lds_f64(cell, db.w);
+        const double lkr_a = lkf_a - fma_rn(pa1.y, ln_c0, -dga);
+        const double lkr_b = lkf_b - fma_rn(pb1.y, ln_c0, -dgb);
+        double fwd_a, rev_a, fwd_b, rev_b;
+        if (__any_sync(0xffffffffu, ab_exp_out_of_range(lkf_a) || ab_exp_out_of_range(lkr_a) ||
+                                        ab_exp_out_of_range(lkf_b) || ab_exp_out_of_range(lkr_b))) {
+          fwd_a = cexp(lkf_a); rev_a = cexp(lkr_a); fwd_b = cexp(lkf_b); rev_b = cexp(lkr_b);
+        } else {
+          fwd_a = ab_exp_core(lkf_a); rev_a = ab_exp_core(lkr_a); fwd_b = ab_exp_core(lkf_b); rev_b = ab_exp_core(lkr_b);
+        }
+        fwd_a = fwd_a * lds_f64(cell, fa.x);
+        fwd_b = fwd_b * lds_f64(cell, fb.x);
+        rev_a = rev_a * lds_f64(cell, fa.z);
+        rev_b = rev_b * lds_f64(cell, fb.z);
+        fwd_a = fwd_a * lds_f64(cell, fa.y);
+        fwd_b = fwd_b * lds_f64(cell, fb.y);
+        rev_a = rev_a * lds_f64(cell, fa.w);
+        rev_b = rev_b * lds_f64(cell, fb.w);
+        const double qa = (fwd_a - rev_a) * cRof[ka], qb = (fwd_b - rev_b) * cRof[kb];   // Eq 14
+        if (ka_ < Rrev) {
+          cQ[ka] = qa;
+          cQ[Rp + ka] = -qa;
+          if (has2) {
+            const double q2 = qa + qa;
+            cQ[2 * Rp + ka] = q2;
+            cQ[3 * Rp + ka] = -q2;
+          }
+        }
+        if (kb_ < Rrev) {
+          cQ[kb] = qb;
+          cQ[Rp + kb] = -qb;
+          if (has2) {
+            const double q2 = qb + qb;
+            cQ[2 * Rp + kb] = q2;
+            cQ[3 * Rp + kb] = -q2;
+          }
+        }
+      }
+      // irreversible reactions [Rrev, R): 32-blocks c = half (mod 2), two at a time
+      for (int k0 = Rrev + half * 32; k0 < R; k0 += 64 * NW) {
+        double lk[2], fw[2];
+        uint4 f[2];
+        int kk[2];
+        bool oor = false;
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+          kk[u] = k0 + 32 * NW * u + lane;
+          const int k = (kk[u] < R) ? kk[u] : R - 1;
+          const double2 p0 = rkA[k];
+          const double ta = rkB[k].x;
+          f[u] = rfac[k];
+          lk[u] = fma_rn(-ta, invT, fma_rn(p0.y, lnT, p0.x));
+          oor = oor || ab_exp_out_of_range(lk[u]);
+        }
+        if (__any_sync(0xffffffffu, oor)) {
+#pragma unroll
+          for (int u = 0; u < 2; ++u) fw[u] = cexp(lk[u]);
+        } else {
+#pragma unroll
+          for (int u = 0; u < 2; ++u) fw[u] = ab_exp_core(lk[u]);
+        }
+#pragma unroll
+        for (int u = 0; u < 2; ++u) fw[u] = fw[u] * lds_f64(cell, f[u].x);
+#pragma unroll
+        for (int u = 0; u < 2; ++u) fw[u] = fw[u] * lds_f64(cell, f[u].y);
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+          if (kk[u] < R) {
+            const int k = kk[u];
+            cQ[k] = fw[u];
+            cQ[Rp + k] = -fw[u];
+            if (has2) {
+              const double f2 = fw[u] + fw[u];
+              cQ[2 * Rp + k] = f2;
+              cQ[3 * Rp + k] = -f2;
+            }
+          }
+        }
+      }
+      cell_sync();
+
+      // ================= phase C: source terms and the limiter (Eqs 1-3) =================
+      // One species per lane; the entry lists hold the byte offsets of the stored multiples in the caller's reaction
+      // order and are padded with the 0.0 slot to the longest list of the warp, so the loop is warp-uniform.
+      {
+        const double inv_rho = 1.0 / rho;
+        double om = 0.0;
+        // lists are sorted by length over the lanes, so whole quarter- and half-warps drop out of the shared-memory
+        // loads as the loop proceeds (skipping a padding entry is the same as adding its +0.0: om is never -0.0)
+#pragma unroll 2
+        for (int e4 = 0; e4 < g_len4; ++e4) {
+          const int left = g_mylen - 4 * e4;
+          if (left > 0) {
+            const uint4 o = ge[e4 * 32];
+            om = om + lds_f64(cell, o.x);
+            if (left > 1) om = om + lds_f64(cell, o.y);
+            if (left > 2) om = om + lds_f64(cell, o.z);
+            if (left > 3) om = om + lds_f64(cell, o.w);
+          }
+        }
+        // lanes without a species (255) work on species 0 and discard the result
+        const int i0 = (g_sp < S) ? g_sp : 0;
+        const double r0 = (W[i0] * om) * inv_rho;
+        const double y0 = cYp[i0].x;
+        const double rs0 = (-r0 > 1.0e-30) ? -r0 : 1.0e-30;
+        const double ys0 = (y0 < 1.0e-20) ? 1.0 : 0.9 * y0;
+        const double lim0 = ((sc.y_step_max < ys0) ? sc.y_step_max : ys0) / rs0;
+        const double inf = bits_to_double(0x7ff0000000000000ull);
+        double t_star = (g_sp < S && lim0 < inf) ? lim0 : inf;
+        if (g_sp < S) {
+          cConc[1 + g_sp] = r0;     // concentrations are dead: reuse for dY_i/dt
+          cHOm[g_sp].y = om;
+        }
+        // min over lanes: every lim is a positive double or +inf, for which the ordering of the bit patterns as
+        // unsigned integers is the ordering of the values
+        const unsigned long long u = double_to_bits(t_star);
+        const unsigned hi = (unsigned)(u >> 32), lo = (unsigned)u;
+        const unsigned mhi = __reduce_min_sync(0xffffffffu, hi);
+        const unsigned mlo = __reduce_min_sync(0xffffffffu, (hi == mhi) ? lo : 0xffffffffu);
+        if (lane == 0) scal->t_star[half] = bits_to_double(((unsigned long long)mhi << 32) | mlo);
+      }
+      cell_sync();
+
+      // ================= phase D =================
+      // -- a3: step size (Eq 5) and landing on t_f (R5)
+      const double t_star = (NW == 2) ? pk_min_bits(scal->t_star[0], scal->t_star[1]) : scal->t_star[0];
+      double h = (t_star < dt_max) ? t_star : dt_max;
+      bool last = false;
+      const double rem = a.t_f - t;
+      if (rem - h < t_tol) {
+        h = rem;
+        last = true;
+      }
+      // -- a4: forward Euler (Eq 18), one species per lane
+      int bad = 0;
+      if (my_sp < S) {
+        const double y = fma_rn(h, cConc[1 + my_sp], cYp[my_sp].x);
+        cYp[my_sp].x = y;
+        bad |= !(y - y == 0.0);
+      }
+      if (half == 0) {
+        // temperature equation (R15): sum (Y_i/W_i) cp_i/R and sum (h_i/RT) omega_i, each sequential in species order
+        // (contract 5.4); the two chains run in the even and the odd lanes of the same instruction stream
+        const double2 *arr = (lane & 1) ? cHOm : cYwCp;
+        double acc = 0.0;
+#pragma unroll 8
+        for (int i = 0; i < S; ++i) {
+          const double2 v = arr[i];
+          acc = fma_rn(v.x, v.y, acc);
+        }
+        const double sum_cp = __shfl_sync(0xffffffffu, acc, 0), sum_h = __shfl_sync(0xffffffffu, acc, 1);
+        const double dTdt = (sc.energy_mode == 0) ? -((sum_h * kRu) * T) / (rho * (kRu * sum_cp)) : 0.0;
+        T = fma_rn(h, dTdt, T);
+        bad |= !(T - T == 0.0);
+        if (lane == 0) scal->T_new = T;
+      }
+      bad = __any_sync(0xffffffffu, bad);
+      if (lane == 0) scal->bad[half] = bad;
+      // -- a5: DFT ringing filter of this warp's blocks (skipped on the landing step: the cell retires)
+      if (!last && sc.dft_enable) {
+        switch (sc.nhf) {
+          case 1: pk_dft<1>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h, inv_ctot, lane); break;
+          case 2: pk_dft<2>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h, inv_ctot, lane); break;
+          case 3: pk_dft<3>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h, inv_ctot, lane); break;
+          case 4: pk_dft<4>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h, inv_ctot, lane); break;
+          case 5: pk_dft<5>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h, inv_ctot, lane); break;
+          default: pk_dft<6>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h, inv_ctot, lane); break;
+        }
+        slot = (slot + 1 == kWindow) ? 0 : slot + 1;
+      }
+      cell_sync();
+      if (NW == 2 && half) T = scal->T_new;
+      t = last ? a.t_f : t + h;
+      steps += 1;
+
+      // -- a6: retirement (R20)
+      int st = -1;
+      if (last) st = 0;
+      else if (scal->bad[0] | (NW == 2 ? scal->bad[1] : 0)) st = 2;
+      else if (steps >= sc.max_steps) st = 1;
+      if (st >= 0) {
+        if (my_sp < S) a.Y[(long long)my_sp * a.ld + cidx] = cYp[my_sp].x;
+        if (half == 0 && lane == 0) {
+          a.T[cidx] = T;
+          a.steps[cidx] = steps;
+          if (a.status) a.status[cidx] = (unsigned char)st;
+          if (st > 0) atomicMax(a.worst_status, st);
+        }
+        break;
+      }
+    }
+  }
+}
+
+template <int NW>
+__global__ void __launch_bounds__(kPkThreads, 1) stev_pk_kernel(const __grid_constant__ PkArgs a) {
+  extern __shared__ __align__(128) unsigned char smem[];
+  __shared__ unsigned long long mbar;
+  __shared__ uint32_t tmem_base_s;
+  __shared__ int done_warps;
+  const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;   // warp-uniform for the compiler
+  if (threadIdx.x == 0) done_warps = 0;
+  stage_tables(smem, a.table, a.tb.bytes, &mbar);
+  if (warp == 0) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(
+                     (uint32_t)__cvta_generic_to_shared(&tmem_base_s))
+                 : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  const uint32_t tmem_base = tmem_base_s;
+
+  // NW = 2: warps j and j + 8 form the pair of cell slot j; both sit in TMEM lane quarter j & 3.  NW = 1: warp j is cell slot j.
+  const int j = (NW == 2) ? (warp & 7) : warp, half = (NW == 2) ? (warp >> 3) : 0;
+  if (j < a.cells_per_block) {
+    unsigned char *cell = smem + a.tb.bytes + (size_t)j * a.cl.stride;
+    if (a.tb.has_est) pk_worker<true, NW>(a, smem, cell, j, half, tmem_base, lane);
+    else pk_worker<false, NW>(a, smem, cell, j, half, tmem_base, lane);
+  }
+  __syncwarp();
+  if (lane == 0) atomicAdd(&done_warps, 1);
+  if (warp == 0) {
+    if (lane == 0) {
+      while (atomicAdd(&done_warps, 0) < kPkThreads / 32) __nanosleep(200);
+    }
+    __syncwarp();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem_base) : "memory");
+  }
+}
+
+}  // namespace stev

@@ -186,11 +186,19 @@ def test_result_does_not_depend_on_lanes_per_cell(stev, oracle, config, n, lanes
 @pytest.mark.parametrize("config,n,over", [(3, 500, {}), (3, 37, {}), (3, 200, dict(use_estimator=False)),
                                            (1, 400, {}), (2, 300, {}), (4, 300, {}), (0, 600, {}),
                                            (1, 100, dict(max_steps=150)), (2, 100, dict(alpha=0.0, dft_first_high_bin=1)),
-                                           (2, 100, dict(energy_mode=1, delta_max=0.002, y_step_max=0.05))])
-def test_warp_specialised_kernel_parity(stev, oracle, config, n, over):
-    """lanes_per_cell = 64: the rate-warp / DFT-warp kernel with the DFT history in tensor memory (stev_ab_kernel.cuh),
-    the default for large mechanisms (config 3).  Bit-exact against the oracle on every config it accepts."""
+                                           (2, 100, dict(energy_mode=1, delta_max=0.002, y_step_max=0.05)),
+                                           (1, 100, dict(dft_enable=0, max_steps=3000))])
+@pytest.mark.parametrize("kernel", [33, 64, 66])
+def test_tensor_memory_kernels_parity(stev, oracle, kernel, config, n, over):
+    """lanes_per_cell = 33: one warp per cell (stev_pk_kernel.cuh, NW = 1), the default for small and mid-size mechanisms;
+    lanes_per_cell = 64: the warp-pair kernel (stev_pk_kernel.cuh, NW = 2), the default for large mechanisms (config 3);
+    lanes_per_cell = 66: the rate-warp / DFT-warp kernel (stev_ab_kernel.cuh).  Both keep the DFT history in tensor
+    memory and are bit-exact against the oracle on every config they accept."""
     over = dict(over)
+    if kernel == 66 and over.get("dft_enable", 1) == 0:
+        pytest.skip("the warp-specialised kernel needs the DFT filter on")
+    if kernel == 33 and config == 3:
+        pytest.skip("one warp per cell holds at most 32 species / 128 reversible reactions")
     w = make_workload(config, n)
     est = w.estimator if over.pop("use_estimator", True) else None
     prm = dict(w.params, **over)
@@ -198,18 +206,21 @@ def test_warp_specialised_kernel_parity(stev, oracle, config, n, over):
     case = GpuCase(stev, w)
     if est is None:
         case.est = None
-    gpu = case.integrate(lanes_per_cell=64, **over)
-    assert gpu["stats"]["lanes_per_cell"] == 64
+    gpu = case.integrate(lanes_per_cell=kernel, **over)
+    assert gpu["stats"]["lanes_per_cell"] == kernel
     rep = assert_parity(gpu, ref)
-    print(f"config {config}: n={n} {rep} stats={gpu['stats']}")
+    print(f"kernel {kernel} config {config}: n={n} {rep} stats={gpu['stats']}")
     assert gpu["rc"] == ref["rc"]
     assert rep["bit_exact"] == 1.0
 
 
-def test_large_mechanism_defaults_to_warp_specialised_kernel(stev):
-    w = make_workload(3, 64)
-    gpu = GpuCase(stev, w).integrate()
+def test_default_kernel_selection(stev):
+    gpu = GpuCase(stev, make_workload(3, 64)).integrate()
     assert gpu["stats"]["lanes_per_cell"] == 64 and gpu["stats"]["threads_per_block"] == 512
+    gpu = GpuCase(stev, make_workload(2, 64)).integrate()
+    assert gpu["stats"]["lanes_per_cell"] == 33 and gpu["stats"]["cells_per_block"] == 16
+    gpu = GpuCase(stev, make_workload(2, 64)).integrate(chunk_steps=50)
+    assert gpu["stats"]["lanes_per_cell"] <= 32
 
 
 @pytest.mark.parametrize("config,n,chunk", [(0, 3000, 64), (1, 600, 100), (1, 600, 1000), (2, 300, 333), (3, 100, 150)])
