@@ -114,9 +114,11 @@ bool build_pk_image(const HostMechanism &m, const HostEstimator *e, int nw, std:
     glen[32 * half + lane] = (unsigned short)gl[order[n]].size();
     g_len[half] = std::max(g_len[half], (int)gl[order[n]].size());
   }
-  tb.g_len4[0] = (g_len[0] + 3) / 4;
-  tb.g_len4[1] = (g_len[1] + 3) / 4;
-  const int g_rows = tb.g_len4[0] + tb.g_len4[1];
+  // rows of four entries, an even number per warp (the kernel walks two rows per trip) plus two spare rows that the
+  // kernel prefetches past the end
+  tb.g_len4[0] = (g_len[0] + 7) / 8 * 2;
+  tb.g_len4[1] = (g_len[1] + 7) / 8 * 2;
+  const int g_rows = tb.g_len4[0] + tb.g_len4[1] + 2;
 
   // Internal reaction order: reversible reactions first (lanes never diverge on reversibility); within each group the
   // order is free, because every table is indexed through it.  It decides which shared-memory banks the lanes of a
@@ -292,6 +294,7 @@ bool build_pk_image(const HostMechanism &m, const HostEstimator *e, int nw, std:
   std::memcpy(base + tb.o_gsp, gsp, 64);
   std::memcpy(base + tb.o_glen, glen, 128);
   unsigned *gent = (unsigned *)(base + tb.o_gent);   // [row][lane][4]
+  for (int n = 0; n < 4 * 32 * g_rows; ++n) gent[n] = zero_slot;
   for (int half = 0, row0 = 0; half < 2; ++half) {
     for (int lane = 0; lane < 32; ++lane) {
       const int i = gsp[32 * half + lane];

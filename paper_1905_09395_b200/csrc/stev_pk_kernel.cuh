@@ -2,8 +2,8 @@
 //
 // One block per SM holds up to eight cells.  Each cell is served by a PAIR of warps that split every phase of a step
 // between them (no idle role), meeting at a 64-thread named barrier between phases:
-//   A  warp 0: scalars, ln T, ln(p_atm/R_u T), NASA-7 g/RT, 1/Wbar, stabilised concentrations
-//      warp 1: the cp / h estimator (MLP on fp32 CUDA cores, or the NASA-7 polynomials)
+//   A  warp 0: scalars, ln T, ln(p_atm/R_u T), 1/Wbar, stabilised concentrations
+//      warp 1: NASA-7 g/RT and the cp / h estimator (MLP on fp32 CUDA cores, or the NASA-7 polynomials)
 //   B  both:   Arrhenius + equilibrium rates of their own 32-blocks of reactions, q_eff = q rOF, stored multiples
 //   C  both:   source terms of their own species (one species per lane), step limiter, warp minimum
 //   D  both:   step size, Euler update of their own species, DFT ringing filter of their own 32-blocks of
@@ -226,7 +226,6 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
   const int g_sp = gsp[half * 32 + lane];       // species whose source term this lane gathers (255 = none)
   const uint4 *ge = (const uint4 *)(tbl + tb.o_gent) + (half ? tb.g_len4[0] * 32 : 0) + lane;
   const int g_len4 = tb.g_len4[half];
-  const int g_mylen = ((const unsigned short *)(tbl + tb.o_glen))[half * 32 + lane];   // entries of this lane's list
 
   if (half == 0 && lane == 0) {
     cConc[0] = 1.0;
@@ -267,8 +266,10 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
         lnT = __shfl_sync(0xffffffffu, lval, 0);
         ln_c0 = __shfl_sync(0xffffffffu, lval, 16);
         inv_ctot = 1.0 / c_tot;
-        if (EST) pk_nasa<false>(tb, tbl, cG, cYwCp, cHOm, T, invT, lnT, lane);
-        else if (NW == 1) pk_nasa<true>(tb, tbl, cG, cYwCp, cHOm, T, invT, lnT, lane);
+        if (NW == 1) {
+          if (EST) pk_nasa<false>(tb, tbl, cG, cYwCp, cHOm, T, invT, lnT, lane);
+          else pk_nasa<true>(tb, tbl, cG, cYwCp, cHOm, T, invT, lnT, lane);
+        }
         // -- 1/Wbar = sum Y_i/W_i, sequential in species order (contract 5.4)
         double inv_wbar = 0.0;
 #pragma unroll 8
@@ -308,10 +309,13 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
       if (NW == 1) {
         if (EST) pk_mlp(tb, tbl, cYp, cYwCp, cHOm, cHid, T, p, invT, lane);
       } else if (half == 1) {
+        // warp 1 of the pair: all of the thermodynamics (its own ln T and 1/T: same operations, same bits)
+        const double invT1 = 1.0 / T;
         if (EST) {
-          pk_mlp(tb, tbl, cYp, cYwCp, cHOm, cHid, T, p, 1.0 / T, lane);
+          pk_nasa<false>(tb, tbl, cG, cYwCp, cHOm, T, invT1, ab_log(T), lane);
+          pk_mlp(tb, tbl, cYp, cYwCp, cHOm, cHid, T, p, invT1, lane);
         } else {
-          pk_nasa<true>(tb, tbl, cG, cYwCp, cHOm, T, 1.0 / T, ab_log(T), lane);
+          pk_nasa<true>(tb, tbl, cG, cYwCp, cHOm, T, invT1, ab_log(T), lane);
         }
       }
       cell_sync();
@@ -344,6 +348,10 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
         dgb = dgb + lds_f64(cell, db.w);
         const double lkr_a = lkf_a - fma_rn(pa1.y, ln_c0, -dga);
         const double lkr_b = lkf_b - fma_rn(pb1.y, ln_c0, -dgb);
+        // the concentration factors and rOF are fetched before the exponentials so that their latency is hidden
+        const double ca0 = lds_f64(cell, fa.x), cb0 = lds_f64(cell, fb.x), ca2 = lds_f64(cell, fa.z), cb2 = lds_f64(cell, fb.z);
+        const double ca1 = lds_f64(cell, fa.y), cb1 = lds_f64(cell, fb.y), ca3 = lds_f64(cell, fa.w), cb3 = lds_f64(cell, fb.w);
+        const double rof_a = cRof[ka], rof_b = cRof[kb];
         double fwd_a, rev_a, fwd_b, rev_b;
         if (__any_sync(0xffffffffu, ab_exp_out_of_range(lkf_a) || ab_exp_out_of_range(lkr_a) ||
                                         ab_exp_out_of_range(lkf_b) || ab_exp_out_of_range(lkr_b))) {
@@ -351,15 +359,15 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
         } else {
           fwd_a = ab_exp_core(lkf_a); rev_a = ab_exp_core(lkr_a); fwd_b = ab_exp_core(lkf_b); rev_b = ab_exp_core(lkr_b);
         }
-        fwd_a = fwd_a * lds_f64(cell, fa.x);
-        fwd_b = fwd_b * lds_f64(cell, fb.x);
-        rev_a = rev_a * lds_f64(cell, fa.z);
-        rev_b = rev_b * lds_f64(cell, fb.z);
-        fwd_a = fwd_a * lds_f64(cell, fa.y);
-        fwd_b = fwd_b * lds_f64(cell, fb.y);
-        rev_a = rev_a * lds_f64(cell, fa.w);
-        rev_b = rev_b * lds_f64(cell, fb.w);
-        const double qa = (fwd_a - rev_a) * cRof[ka], qb = (fwd_b - rev_b) * cRof[kb];   // Eq 14
+        fwd_a = fwd_a * ca0;
+        fwd_b = fwd_b * cb0;
+        rev_a = rev_a * ca2;
+        rev_b = rev_b * cb2;
+        fwd_a = fwd_a * ca1;
+        fwd_b = fwd_b * cb1;
+        rev_a = rev_a * ca3;
+        rev_b = rev_b * cb3;
+        const double qa = (fwd_a - rev_a) * rof_a, qb = (fwd_b - rev_b) * rof_b;   // Eq 14
         if (ka_ < Rrev) {
           cQ[ka] = qa;
           cQ[Rp + ka] = -qa;
@@ -428,18 +436,23 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
       {
         const double inv_rho = 1.0 / rho;
         double om = 0.0;
-        // lists are sorted by length over the lanes, so whole quarter- and half-warps drop out of the shared-memory
-        // loads as the loop proceeds (skipping a padding entry is the same as adding its +0.0: om is never -0.0)
-#pragma unroll 2
-        for (int e4 = 0; e4 < g_len4; ++e4) {
-          const int left = g_mylen - 4 * e4;
-          if (left > 0) {
-            const uint4 o = ge[e4 * 32];
-            om = om + lds_f64(cell, o.x);
-            if (left > 1) om = om + lds_f64(cell, o.y);
-            if (left > 2) om = om + lds_f64(cell, o.z);
-            if (left > 3) om = om + lds_f64(cell, o.w);
-          }
+        // Two rows of four entries per trip: the eight loads of a trip are independent and the offsets of the next
+        // trip are fetched before the additions of this one (the table carries two spare rows).  Lists are sorted by
+        // length over the lanes; padding entries read the 0.0 slot, and adding +0.0 changes nothing (om is never -0.0).
+        uint4 o0 = ge[0], o1 = ge[32];
+        for (int e4 = 0; e4 < g_len4; e4 += 2) {
+          const double v0 = lds_f64(cell, o0.x), v1 = lds_f64(cell, o0.y), v2 = lds_f64(cell, o0.z), v3 = lds_f64(cell, o0.w);
+          const double v4 = lds_f64(cell, o1.x), v5 = lds_f64(cell, o1.y), v6 = lds_f64(cell, o1.z), v7 = lds_f64(cell, o1.w);
+          o0 = ge[(e4 + 2) * 32];
+          o1 = ge[(e4 + 3) * 32];
+          om = om + v0;
+          om = om + v1;
+          om = om + v2;
+          om = om + v3;
+          om = om + v4;
+          om = om + v5;
+          om = om + v6;
+          om = om + v7;
         }
         // lanes without a species (255) work on species 0 and discard the result
         const int i0 = (g_sp < S) ? g_sp : 0;
