@@ -327,7 +327,7 @@ def main():
         multi.finish(ctx)
         return 0
 
-    # ---- roofline of the dominant kernel (stev_integrate_kernel: one launch per step when chunk_steps = 0)
+    # ---- roofline of the dominant kernel (the integrator: one launch per step when chunk_steps = 0)
     work = workmodel.cell_step_work(w.mech, w.estimator, dft_enable=bool(w.params["dft_enable"]),
                                     first_high_bin=w.params["dft_first_high_bin"], alpha_on=w.params["alpha"] > 0,
                                     adiabatic=w.params["energy_mode"] == 0)
@@ -337,7 +337,11 @@ def main():
     sm_max = (clocks or {}).get("sm_max_mhz") or 1965.0
     peak_instr = workmodel.fp64_peak_instr_per_s(sm_max)
     peak_tflops = 2.0 * peak_instr / 1e12
-    roofline = {"bound": "alu", "kernel": f"stev_integrate_kernel<{st['lanes_per_cell']}>",
+    kernel_name = {33: "stev_pk_kernel<1> (one warp per cell, DFT history in tensor memory)",
+                   64: "stev_pk_kernel<2> (warp pair per cell, DFT history in tensor memory)",
+                   66: "stev_ab_kernel (rate warp + DFT warp per cell)"}.get(st["lanes_per_cell"],
+                                                                             f"stev_integrate_kernel<{st['lanes_per_cell']}>")
+    roofline = {"bound": "alu", "kernel": kernel_name,
                 "achieved": flop / kernel_s / 1e12, "peak": peak_tflops, "unit": "TFLOP/s",
                 "frac": flop / kernel_s / 1e12 / peak_tflops, "traffic": None,
                 "peak_source": f"derived: 148 SM x 64 DFMA/clk x 2 x {sm_max:.0f} MHz (DESIGN.md section 8); not in MEASURED_PEAKS.json",
