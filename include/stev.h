@@ -179,8 +179,9 @@ STEV_API int stev_compact_active(const uint8_t *flags, const int32_t *list_in, i
 STEV_API int stev_dft_mag(const double *ring, int64_t n, double *D, void *cuda_stream);
 /* The arithmetic contract's exp / log on device arrays. */
 STEV_API int stev_contract_exp_log(const double *x, int64_t n, double *exp_out, double *log_out, void *cuda_stream);
-/* Throughput microbenchmarks used for the roofline denominators: runs `iters` dependent-chain-free DFMA (kind 0)
- * or contract-exp (kind 1) operations per thread on a full grid; returns operations per second in *ops_per_s. */
+/* Microbenchmarks used for the roofline denominators: kind 0 runs 8 x `iters` independent DFMAs per thread on a full
+ * grid, kind 1 4 x `iters` contract exps; kind 2 runs one dependent chain of 8 x `iters` DFMAs in one warp per SM (a
+ * latency probe: ops per second per thread = clock / DFMA latency).  Returns operations per second in *ops_per_s. */
 STEV_API int stev_microbench(int32_t kind, int32_t iters, double *ops_per_s, void *cuda_stream);
 
 STEV_API const char *stev_last_error(void); /* thread-local, valid until the next call on this thread */

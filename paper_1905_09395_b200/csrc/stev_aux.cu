@@ -46,10 +46,14 @@ __global__ void __launch_bounds__(256) microbench_kernel(int kind, int iters, do
       a0 = fma_rn(a0, m, c); a1 = fma_rn(a1, m, c); a2 = fma_rn(a2, m, c); a3 = fma_rn(a3, m, c);
       a4 = fma_rn(a4, m, c); a5 = fma_rn(a5, m, c); a6 = fma_rn(a6, m, c); a7 = fma_rn(a7, m, c);
     }
-  } else {
+  } else if (kind == 1) {
     for (int i = 0; i < iters; ++i) {
       a0 = cexp(a0 * -0.5); a1 = cexp(a1 * -0.5); a2 = cexp(a2 * -0.5); a3 = cexp(a3 * -0.5);
     }
+  } else {
+    // kind 2: one dependent DFMA chain per thread (latency probe; launched with one warp per SM)
+#pragma unroll 16
+    for (int i = 0; i < 8 * iters; ++i) a0 = fma_rn(a0, m, c);
   }
   const double r = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
   if (r == 123456.789) sink[0] = r;
@@ -125,11 +129,11 @@ int stev_contract_exp_log(const double *x, int64_t n, double *exp_out, double *l
 }
 
 int stev_microbench(int32_t kind, int32_t iters, double *ops_per_s, void *cuda_stream) {
-  if ((kind != 0 && kind != 1) || iters < 1 || !ops_per_s) { set_error("stev_microbench: bad argument"); return STEV_EINVAL; }
+  if ((kind < 0 || kind > 2) || iters < 1 || !ops_per_s) { set_error("stev_microbench: bad argument"); return STEV_EINVAL; }
   cudaStream_t s = (cudaStream_t)cuda_stream;
   double *sink = nullptr;
   STEV_CUDA(cudaMalloc(&sink, 8));
-  const int blocks = device_sm_count() * 8, threads = 256;
+  const int blocks = (kind == 2) ? device_sm_count() : device_sm_count() * 8, threads = (kind == 2) ? 32 : 256;
   cudaEvent_t e0, e1;
   STEV_CUDA(cudaEventCreate(&e0));
   STEV_CUDA(cudaEventCreate(&e1));
@@ -140,7 +144,7 @@ int stev_microbench(int32_t kind, int32_t iters, double *ops_per_s, void *cuda_s
   STEV_CUDA(cudaEventSynchronize(e1));
   float ms = 0.f;
   STEV_CUDA(cudaEventElapsedTime(&ms, e0, e1));
-  const double per_thread = (kind == 0) ? 8.0 * iters : 4.0 * iters;
+  const double per_thread = (kind == 1) ? 4.0 * iters : 8.0 * iters;
   *ops_per_s = per_thread * (double)blocks * threads / (ms * 1e-3);
   cudaEventDestroy(e0);
   cudaEventDestroy(e1);

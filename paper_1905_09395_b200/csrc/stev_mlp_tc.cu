@@ -6,12 +6,14 @@
 // Both contractions run on the 5th-generation tensor cores: tcgen05.mma (kind::tf32, or kind::f16 with BF16
 // operands), M = 128 cells per instruction, fp32 accumulators in tensor memory.  One CTA of 128 threads owns a tile of
 // 128 cells: thread t is cell row t and TMEM lane t.  Per tile
-//   1. the raw inputs are read coalesced, normalised in fp32, rounded to the operand type and written to shared
-//      memory in the canonical K-major core-matrix layout (8 rows x 16 bytes per core matrix, no swizzle);
+//   1. the raw input tile arrives by one TMA bulk copy (cp.async.bulk on an mbarrier, issued one tile ahead), is
+//      normalised in fp32, rounded to the operand type and written to shared memory in the canonical K-major
+//      core-matrix layout (8 rows x 16 bytes per core matrix, no swizzle);
 //   2. one elected thread issues the layer-1 MMAs (accumulator D1: 128 x Hp in TMEM) and commits to an mbarrier;
 //   3. every thread reads its row of D1 with tcgen05.ld, adds the bias in fp32, applies the activation (MUFU
 //      tanh / ex2) and writes the hidden activations back to shared memory as the A operand of layer 2;
-//   4. layer-2 MMAs (D2: 128 x Np), then the epilogue adds b2 in fp32 and stores the rows.
+//   4. layer-2 MMAs (D2: 128 x Np), then the epilogue adds b2 in fp32, stages the rows in shared memory and one TMA
+//      bulk store writes the tile (a ragged last tile is read and written row by row).
 // BF16 keeps only 8 mantissa bits, which alone would put the result at the edge of the 1e-2 tolerance, so on that
 // path both contractions are compensated: a = a_hi + a_lo and w = w_hi + w_lo (all BF16) and the K axis carries the
 // three products a_hi w_hi + a_lo w_hi + a_hi w_lo side by side (the tensor cores have an order of magnitude of slack).
@@ -43,6 +45,8 @@ struct TcArgs {
   int kstep_elems;               // K elements per MMA: 8 (TF32) or 16 (BF16) = 32 bytes
   int lbo_a1, lbo_a2, lbo_w1, lbo_w2;   // byte distance between K-adjacent core matrices
   int o_a1, o_a2;                // shared-memory offsets of the two A operands
+  int o_xs, o_os;                // staging of one raw input tile (TMA bulk load) and one output tile (TMA bulk store;
+                                 // aliases A2 when it fits: A2 is dead once the layer-2 MMAs have completed)
   uint32_t idesc1, idesc2;
   int tmem_cols;
   const float *X;
@@ -142,7 +146,7 @@ __device__ __forceinline__ int canon_off(int r, int c, int esize, int lbo) {
 template <bool BF16>
 __global__ void __launch_bounds__(kTcThreads) estimator_tc_kernel(const __grid_constant__ TcArgs a) {
   extern __shared__ __align__(128) unsigned char smem[];
-  __shared__ unsigned long long mbar;
+  __shared__ unsigned long long mbar, mbar_x;
   __shared__ uint32_t tmem_base_s;
   const int t = threadIdx.x, warp = t >> 5;
 
@@ -152,6 +156,7 @@ __global__ void __launch_bounds__(kTcThreads) estimator_tc_kernel(const __grid_c
   for (int i = a.o_a1 + t * 16; i < a.o_a2 + a.lbo_a2 * (a.K2 * a.esize / 16); i += kTcThreads * 16) *(uint4 *)(smem + i) = make_uint4(0, 0, 0, 0);
   if (t == 0) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&mbar)));
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&mbar_x)));
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 0) {
@@ -170,16 +175,35 @@ __global__ void __launch_bounds__(kTcThreads) estimator_tc_kernel(const __grid_c
   unsigned char *A1 = smem + a.o_a1, *A2 = smem + a.o_a2;
   const uint32_t sA1 = smem_u32(A1), sA2 = smem_u32(A2), sW1 = smem_u32(smem + a.im.o_w1), sW2 = smem_u32(smem + a.im.o_w2);
   const int n_in = a.n_in;
-  uint32_t parity = 0;
+  uint32_t parity = 0, parity_x = 0;
+  float *Xs = (float *)(smem + a.o_xs), *Os = (float *)(smem + a.o_os);
+  const int tile_in_bytes = kTcRows * n_in * 4, tile_out_bytes = kTcRows * a.n_out * 4;
+  const int r_first = t / n_in, c_first = t - r_first * n_in, r_step = kTcThreads / n_in, c_step = kTcThreads - r_step * n_in;
 
   const long long n_tiles = (a.n + kTcRows - 1) / kTcRows;
+  // raw input tiles arrive by TMA bulk copy (one instruction per tile, signalled on mbar_x), one tile ahead
+  auto prefetch = [&](long long tile) {
+    if (tile < n_tiles && (tile + 1) * kTcRows <= a.n) {
+      const uint32_t mb = smem_u32(&mbar_x);
+      asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mb), "r"(tile_in_bytes) : "memory");
+      asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(Xs)),
+                   "l"(a.X + tile * kTcRows * n_in), "r"(tile_in_bytes), "r"(mb)
+                   : "memory");
+    }
+  };
+  if (t == 0) prefetch(blockIdx.x);
   for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
     const long long row0 = tile * kTcRows;
     const int rows = (int)((a.n - row0 < kTcRows) ? (a.n - row0) : kTcRows);
-    // ---- 1. inputs: coalesced read, fp32 normalisation, operand rounding, canonical layout
+    const bool full = rows == kTcRows;
+    // ---- 1. inputs: fp32 normalisation, operand rounding, canonical layout (a ragged last tile is read directly)
     const float *Xt = a.X + row0 * n_in;
-    for (int e = t; e < kTcRows * n_in; e += kTcThreads) {
-      const int r = e / n_in, c = e - r * n_in;
+    if (full) {
+      mbar_wait(&mbar_x, parity_x);
+      parity_x ^= 1;
+      Xt = Xs;
+    }
+    for (int e = t, r = r_first, c = c_first; e < kTcRows * n_in; e += kTcThreads) {
       const float x = (r < rows) ? (Xt[e] - shift[c]) * scale[c] : 0.f;
       if (BF16) {
         const unsigned short hi = to_bf16(x);
@@ -190,12 +214,21 @@ __global__ void __launch_bounds__(kTcThreads) estimator_tc_kernel(const __grid_c
       } else {
         *(uint32_t *)(A1 + canon_off(r, c, 4, a.lbo_a1)) = to_tf32(x);
       }
+      r += r_step;
+      c += c_step;
+      if (c >= n_in) {
+        c -= n_in;
+        r += 1;
+      }
     }
+    // the previous tile's bulk store must have finished reading the output staging (it may alias A2)
+    if (t == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes -> visible to the tensor core
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
     // ---- 2. layer 1: D1[128 x Hp] = A1[128 x K1] * W1^T
     if (t == 0) {
+      prefetch(tile + gridDim.x);   // the staging buffer is free: every thread has converted its part
       asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
       const int ksteps = a.K1 / a.kstep_elems;
       for (int ks = 0; ks < ksteps; ++ks) {
@@ -260,8 +293,9 @@ __global__ void __launch_bounds__(kTcThreads) estimator_tc_kernel(const __grid_c
     mbar_wait(&mbar, parity);
     parity ^= 1;
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-    // ---- epilogue 2: bias in fp32, rows out
-    float *orow = a.out + (row0 + t) * a.n_out;
+    // ---- epilogue 2: bias in fp32; a full tile is staged in shared memory and leaves by one TMA bulk store, a ragged
+    //      last tile is written row by row
+    float *orow = full ? (Os + t * a.n_out) : (a.out + (row0 + t) * a.n_out);
     const bool vec = (a.n_out % 4) == 0;
     for (int c0 = 0; c0 < a.Np; c0 += 16) {
       uint32_t v[16];
@@ -287,9 +321,17 @@ __global__ void __launch_bounds__(kTcThreads) estimator_tc_kernel(const __grid_c
         }
       }
     }
+    if (full) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-    __syncthreads();   // D1, D2, A1, A2 are free again
+    __syncthreads();   // D1, D2, A1 are free again; the output tile is complete in shared memory
+    if (full && t == 0) {
+      asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(a.out + row0 * a.n_out), "r"(smem_u32(Os)),
+                   "r"(tile_out_bytes)
+                   : "memory");
+      asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    }
   }
+  if (t == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
   __syncthreads();
   if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(a.tmem_cols) : "memory");
@@ -363,7 +405,10 @@ bool make_plan(const HostEstimator &h, bool bf16, TcPlan &p) {
   a.im.o_scale = take(4 * h.n_in);
   a.im.bytes = off;
   a.o_a1 = take(a.lbo_a1 * (a.K1 / per));
-  a.o_a2 = take(a.lbo_a2 * (a.K2 / per));
+  const int a2_bytes = a.lbo_a2 * (a.K2 / per);
+  a.o_a2 = take(a2_bytes);
+  a.o_xs = take(kTcRows * h.n_in * 4);
+  a.o_os = (kTcRows * h.n_out * 4 <= a2_bytes) ? a.o_a2 : take(kTcRows * h.n_out * 4);
   p.smem = (size_t)off;
   if (p.smem > 200 * 1024) return false;
   a.idesc1 = make_idesc(bf16, kTcRows, a.Hp);

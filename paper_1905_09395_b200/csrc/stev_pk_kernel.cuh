@@ -9,8 +9,9 @@
 //   D  both:   step size, Euler update of their own species, DFT ringing filter of their own 32-blocks of
 //              reversible reactions; warp 0 also evaluates the two sequential sums of the temperature equation
 // The 13-deep history of every reversible reaction lives in TENSOR MEMORY (one lane-private row of TMEM columns per
-// reaction, tcgen05.st / tcgen05.ld); both warps of a pair sit in the same TMEM lane quarter.  Shared memory holds the
-// mechanism tables (one TMA bulk copy per block) and ~17 KB of per-cell scratch; the hot loop has no HBM traffic.
+// reaction, tcgen05.st / tcgen05.ld); each warp keeps the windows of its own blocks in its own TMEM lane quarter.
+// Shared memory holds the mechanism tables (one TMA bulk copy per block) and ~17 KB of per-cell scratch; the hot loop
+// has no HBM traffic.
 // Arithmetic follows the contract of DESIGN.md section 5 exactly; every bit-equivalent deviation in evaluation order
 // is explained where it occurs.
 #pragma once
@@ -193,7 +194,7 @@ __device__ __forceinline__ double pk_min_bits(double a, double b) {
 // ---------------------------------------------------------------------------------------------------------
 template <bool EST, int NW>
 __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *tbl, unsigned char *cell, int j, int half,
-                                          uint32_t tmem_base, int lane) {
+                                          int tmem_quarter, uint32_t tmem_base, int lane) {
   const PkTables &tb = a.tb;
   const SolverConsts &sc = a.sc;
   const int S = tb.S, R = tb.R, Rrev = tb.Rrev, Rp = tb.Rp, n_it = tb.n_it;
@@ -220,8 +221,11 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
   };
   const double dt_max = a.t_f * sc.delta_max;   // Eq 4
   const double t_tol = 1.0e-12 * a.t_f;         // R5
-  const uint32_t trow = tmem_base + ((uint32_t)((j & 3) * 32) << 16) + (uint32_t)((j >> 2) * (NW == 2 ? 256 : 128));
-  const int it_lo = half ? tb.it_half0 : 0, it_hi = half ? n_it : tb.it_half0;   // DFT blocks of this warp
+  const int it_lo = half ? tb.it_half0 : 0, it_hi = half ? n_it : tb.it_half0;   // DFT blocks of this warp (at most four)
+  // TMEM: a warp reaches the lane quarter (warp id mod 4); it keeps the windows of its own blocks in 128 columns of
+  // that quarter: columns [128 (j / 4), +128) for warp 0 of a cell (or the only warp), [256 + 128 (j / 4), +128) for warp 1.
+  const uint32_t trow = tmem_base + ((uint32_t)((tmem_quarter & 3) * 32) << 16) + (uint32_t)((j >> 2) * 128 + half * 256) -
+                        (uint32_t)(it_lo * 32);
   const int my_sp = half * 32 + lane;           // species this lane loads, updates and writes back
   const int g_sp = gsp[half * 32 + lane];       // species whose source term this lane gathers (255 = none)
   const uint4 *ge = (const uint4 *)(tbl + tb.o_gent) + (half ? tb.g_len4[0] * 32 : 0) + lane;
@@ -568,12 +572,15 @@ __global__ void __launch_bounds__(kPkThreads, 1) stev_pk_kernel(const __grid_con
   asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
   const uint32_t tmem_base = tmem_base_s;
 
-  // NW = 2: warps j and j + 8 form the pair of cell slot j; both sit in TMEM lane quarter j & 3.  NW = 1: warp j is cell slot j.
-  const int j = (NW == 2) ? (warp & 7) : warp, half = (NW == 2) ? (warp >> 3) : 0;
+  // NW = 1: warp j is cell slot j.  NW = 2: warps j and 8 + (j + 1) % 8 form the pair of cell slot j.  The two warps of a
+  // pair run the same phase at the same time, so they are placed on DIFFERENT schedulers (warp id mod 4): a scheduler
+  // then interleaves four cells in four different phases (fp64-bound DFT against latency-bound gather and rates).
+  const int half = (NW == 2) ? (warp >> 3) : 0;
+  const int j = (NW == 2) ? (half ? ((warp - 8 + 7) & 7) : warp) : warp;
   if (j < a.cells_per_block) {
     unsigned char *cell = smem + a.tb.bytes + (size_t)j * a.cl.stride;
-    if (a.tb.has_est) pk_worker<true, NW>(a, smem, cell, j, half, tmem_base, lane);
-    else pk_worker<false, NW>(a, smem, cell, j, half, tmem_base, lane);
+    if (a.tb.has_est) pk_worker<true, NW>(a, smem, cell, j, half, warp & 3, tmem_base, lane);
+    else pk_worker<false, NW>(a, smem, cell, j, half, warp & 3, tmem_base, lane);
   }
   __syncwarp();
   if (lane == 0) atomicAdd(&done_warps, 1);
