@@ -217,7 +217,7 @@ def stev_integrate(mechanism: Mechanism, estimator: Estimator | None, params: st
     n = int(T.shape[0])
     assert T.is_cuda and T.dtype == torch.float64 and T.is_contiguous()
     assert p.is_cuda and p.dtype == torch.float64 and p.is_contiguous() and p.shape[0] == n
-    assert Y.is_cuda and Y.dtype == torch.float64 and Y.dim() == 2 and Y.stride(1) == 1 and Y.shape[0] == mechanism.n_species
+    assert Y.is_cuda and Y.dtype == torch.float64 and Y.dim() == 2 and (Y.stride(1) == 1 or Y.shape[1] <= 1) and Y.shape[0] == mechanism.n_species
     assert steps_out.is_cuda and steps_out.dtype == torch.int32 and steps_out.is_contiguous()
     ld = int(Y.stride(0)) if Y.shape[0] > 1 else int(Y.shape[1])
     need = stev_workspace_bytes(mechanism, estimator, params, n)

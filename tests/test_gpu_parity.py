@@ -307,5 +307,6 @@ def test_host_buffer_entry_point_matches_device_entry_point(stev):
 def test_fp64_microbenchmarks_run(stev):
     dfma = stev.stev_microbench(0, 2048)
     cexp = stev.stev_microbench(1, 256)
-    print(f"DFMA {dfma / 1e12:.2f} T/s, contract exp {cexp / 1e9:.1f} G/s")
-    assert dfma > 1e12 and cexp > 1e10
+    chain = stev.stev_microbench(2, 2048)   # one dependent DFMA chain in one warp per SM
+    print(f"DFMA {dfma / 1e12:.2f} T/s, contract exp {cexp / 1e9:.1f} G/s, dependent DFMA chain {chain / 1e9:.1f} G/s")
+    assert dfma > 1e12 and cexp > 1e10 and 1e10 < chain < dfma
