@@ -56,8 +56,8 @@ bool build_pk_image(const HostMechanism &m, const HostEstimator *e, int nw, std:
   tb.Rrev = Rrev;
   tb.n_it = (Rrev + 31) / 32;
   tb.Rp = (R + 1) & ~1;
-  // DFT blocks: warp 0 of the pair also walks the two sequential sums of the temperature equation (about half a
-  // block's worth of instructions), so it takes the smaller half
+  // DFT blocks: each warp keeps at most four blocks (128 TMEM columns); warp 0 takes the smaller half because it also
+  // walks the two sequential sums of the temperature equation
   tb.it_half0 = (nw == 2) ? tb.n_it / 2 : tb.n_it;
   tb.nw = nw;
   if (e) {
