@@ -182,6 +182,77 @@ __device__ __forceinline__ void pk_dft(const SolverConsts &sc, const double *cQ,
   }
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// a2 for U reversible reactions per lane side by side (blocks b0, b0 + bs, ..): rate constants, equilibrium
+// constants, effective progress rates and their stored multiples.  One pass = one trip through the latency chain
+// table load -> g loads -> exponentials -> concentration loads -> stores, with 2 U independent exp chains in flight.
+// Lanes past the end recompute the last reaction and store nothing.
+// ---------------------------------------------------------------------------------------------------------
+template <int U>
+__device__ __forceinline__ void pk_rev_batch(const unsigned char *cell, const double2 *rkA, const double2 *rkB, const uint4 *rfac,
+                                             const uint4 *rdg, const double *cRof, double *cQ, int Rp, int Rrev, bool has2,
+                                             double invT, double lnT, double ln_c0, int b0, int bs, int lane) {
+  int k_[U], k[U];
+  double lkf[U], lkr[U];
+  uint4 f[U];
+  bool oor = false;
+#pragma unroll
+  for (int u = 0; u < U; ++u) {
+    k_[u] = (b0 + u * bs) * 32 + lane;
+    k[u] = (k_[u] < Rrev) ? k_[u] : Rrev - 1;
+  }
+#pragma unroll
+  for (int u = 0; u < U; ++u) {
+    const double2 p0 = rkA[k[u]], p1 = rkB[k[u]];
+    const uint4 d = rdg[k[u]];
+    f[u] = rfac[k[u]];
+    lkf[u] = fma_rn(-p1.x, invT, fma_rn(p0.y, lnT, p0.x));
+    double dg = 0.0 - lds_f64(cell, d.x);
+    dg = dg - lds_f64(cell, d.y);
+    dg = dg + lds_f64(cell, d.z);
+    dg = dg + lds_f64(cell, d.w);
+    lkr[u] = lkf[u] - fma_rn(p1.y, ln_c0, -dg);
+    oor = oor || ab_exp_out_of_range(lkf[u]) || ab_exp_out_of_range(lkr[u]);
+  }
+  double fwd[U], rev[U];
+  if (__any_sync(0xffffffffu, oor)) {
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      fwd[u] = cexp(lkf[u]);
+      rev[u] = cexp(lkr[u]);
+    }
+  } else {
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      fwd[u] = ab_exp_core(lkf[u]);
+      rev[u] = ab_exp_core(lkr[u]);
+    }
+  }
+#pragma unroll
+  for (int u = 0; u < U; ++u) {
+    fwd[u] = fwd[u] * lds_f64(cell, f[u].x);
+    rev[u] = rev[u] * lds_f64(cell, f[u].z);
+  }
+#pragma unroll
+  for (int u = 0; u < U; ++u) {
+    fwd[u] = fwd[u] * lds_f64(cell, f[u].y);
+    rev[u] = rev[u] * lds_f64(cell, f[u].w);
+  }
+#pragma unroll
+  for (int u = 0; u < U; ++u) {
+    const double q = (fwd[u] - rev[u]) * cRof[k[u]];   // Eq 14
+    if (k_[u] < Rrev) {
+      cQ[k[u]] = q;
+      cQ[Rp + k[u]] = -q;
+      if (has2) {
+        const double q2 = q + q;
+        cQ[2 * Rp + k[u]] = q2;
+        cQ[3 * Rp + k[u]] = -q2;
+      }
+    }
+  }
+}
+
 // unsigned-bit-pattern minimum of positive doubles (NaN patterns sort above +inf and are thereby ignored, like the
 // contract's plain comparison `lim < t_star` ignores them)
 __device__ __forceinline__ double pk_min_bits(double a, double b) {
@@ -333,63 +404,15 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
 
       // ================= phase B: a2, rate constants and effective progress rates (Eqs 28-30, Eq 14) =================
       // Reversible reactions occupy internal indices [0, Rrev) in 32-blocks; blocks b = half (mod 2) belong to this
-      // warp and are evaluated two at a time (four independent exp chains for the scheduler).  Lanes past the end
-      // recompute the last reaction and store nothing.  The stored multiples +q, -q, +2q, -2q (all exact) turn the sum
+      // warp and are evaluated four (small mechanisms: two) at a time, i.e. eight independent exp chains and one trip
+      // through the load -> exp -> load -> store latency chain.  The stored multiples +q, -q, +2q, -2q (all exact) turn the sum
       // omega_i = sum_j nu_ij q_j into plain additions in the contract's order.
-      for (int b0 = half; b0 < n_it; b0 += 2 * NW) {
-        const int ka_ = b0 * 32 + lane, kb_ = ka_ + 32 * NW;
-        const int ka = (ka_ < Rrev) ? ka_ : Rrev - 1, kb = (kb_ < Rrev) ? kb_ : Rrev - 1;
-        const double2 pa0 = rkA[ka], pa1 = rkB[ka], pb0 = rkA[kb], pb1 = rkB[kb];
-        const uint4 fa = rfac[ka], da = rdg[ka], fb = rfac[kb], db = rdg[kb];
-        const double lkf_a = fma_rn(-pa1.x, invT, fma_rn(pa0.y, lnT, pa0.x));
-        const double lkf_b = fma_rn(-pb1.x, invT, fma_rn(pb0.y, lnT, pb0.x));
-        double dga = 0.0 - lds_f64(cell, da.x), dgb = 0.0 - lds_f64(cell, db.x);
-        dga = dga - lds_f64(cell, da.y);
-        dgb = dgb - lds_f64(cell, db.y);
-        dga = dga + lds_f64(cell, da.z);
-        dgb = dgb + lds_f64(cell, db.z);
-        dga = dga + lds_f64(cell, da.w);
-        dgb = dgb + lds_f64(cell, db.w);
-        const double lkr_a = lkf_a - fma_rn(pa1.y, ln_c0, -dga);
-        const double lkr_b = lkf_b - fma_rn(pb1.y, ln_c0, -dgb);
-        // the concentration factors and rOF are fetched before the exponentials so that their latency is hidden
-        const double ca0 = lds_f64(cell, fa.x), cb0 = lds_f64(cell, fb.x), ca2 = lds_f64(cell, fa.z), cb2 = lds_f64(cell, fb.z);
-        const double ca1 = lds_f64(cell, fa.y), cb1 = lds_f64(cell, fb.y), ca3 = lds_f64(cell, fa.w), cb3 = lds_f64(cell, fb.w);
-        const double rof_a = cRof[ka], rof_b = cRof[kb];
-        double fwd_a, rev_a, fwd_b, rev_b;
-        if (__any_sync(0xffffffffu, ab_exp_out_of_range(lkf_a) || ab_exp_out_of_range(lkr_a) ||
-                                        ab_exp_out_of_range(lkf_b) || ab_exp_out_of_range(lkr_b))) {
-          fwd_a = cexp(lkf_a); rev_a = cexp(lkr_a); fwd_b = cexp(lkf_b); rev_b = cexp(lkr_b);
-        } else {
-          fwd_a = ab_exp_core(lkf_a); rev_a = ab_exp_core(lkr_a); fwd_b = ab_exp_core(lkf_b); rev_b = ab_exp_core(lkr_b);
-        }
-        fwd_a = fwd_a * ca0;
-        fwd_b = fwd_b * cb0;
-        rev_a = rev_a * ca2;
-        rev_b = rev_b * cb2;
-        fwd_a = fwd_a * ca1;
-        fwd_b = fwd_b * cb1;
-        rev_a = rev_a * ca3;
-        rev_b = rev_b * cb3;
-        const double qa = (fwd_a - rev_a) * rof_a, qb = (fwd_b - rev_b) * rof_b;   // Eq 14
-        if (ka_ < Rrev) {
-          cQ[ka] = qa;
-          cQ[Rp + ka] = -qa;
-          if (has2) {
-            const double q2 = qa + qa;
-            cQ[2 * Rp + ka] = q2;
-            cQ[3 * Rp + ka] = -q2;
-          }
-        }
-        if (kb_ < Rrev) {
-          cQ[kb] = qb;
-          cQ[Rp + kb] = -qb;
-          if (has2) {
-            const double q2 = qb + qb;
-            cQ[2 * Rp + kb] = q2;
-            cQ[3 * Rp + kb] = -q2;
-          }
-        }
+      if (n_it > 2 * NW) {
+        for (int b0 = half; b0 < n_it; b0 += 4 * NW)
+          pk_rev_batch<4>(cell, rkA, rkB, rfac, rdg, cRof, cQ, Rp, Rrev, has2, invT, lnT, ln_c0, b0, NW, lane);
+      } else {
+        for (int b0 = half; b0 < n_it; b0 += 2 * NW)
+          pk_rev_batch<2>(cell, rkA, rkB, rfac, rdg, cRof, cQ, Rp, Rrev, has2, invT, lnT, ln_c0, b0, NW, lane);
       }
       // irreversible reactions [Rrev, R): 32-blocks c = half (mod 2), two at a time
       for (int k0 = Rrev + half * 32; k0 < R; k0 += 64 * NW) {
