@@ -214,6 +214,29 @@ def test_tensor_memory_kernels_parity(stev, oracle, kernel, config, n, over):
     assert rep["bit_exact"] == 1.0
 
 
+@pytest.mark.parametrize("config,kernel,n_rev", [(3, 64, 1), (3, 64, 31), (3, 64, 32), (3, 64, 33), (3, 64, 64), (3, 64, 65),
+                                                 (3, 64, 128), (3, 64, 129), (3, 64, 193), (3, 64, 224), (3, 66, 33),
+                                                 (2, 33, 1), (2, 33, 31), (2, 33, 32), (2, 33, 33), (2, 64, 33), (1, 33, 1)])
+def test_tensor_memory_kernels_block_boundaries(stev, oracle, config, kernel, n_rev):
+    """The tensor-memory kernels walk the reversible reactions in 32-blocks split over the warps of a cell; this runs
+    them with the number of reversible reactions at and around every block boundary (the first n_rev reversible
+    reactions of the config's mechanism stay reversible, the others become irreversible)."""
+    import dataclasses
+    w = make_workload(config, 48)
+    rev = np.array(w.mech.reversible).copy()
+    idx = np.nonzero(rev)[0]
+    assert n_rev <= idx.size
+    rev[idx[n_rev:]] = 0
+    mech = dataclasses.replace(w.mech, reversible=rev)
+    prm = dict(w.params, max_steps=4000)
+    ref = oracle.integrate(mech, None, prm, w.T, w.p, w.Y, w.dt_cfd)
+    w2 = dataclasses.replace(w, mech=mech, estimator=None)
+    gpu = GpuCase(stev, w2).integrate(lanes_per_cell=kernel, max_steps=4000)
+    assert gpu["stats"]["lanes_per_cell"] == kernel
+    rep = assert_parity(gpu, ref)
+    assert rep["bit_exact"] == 1.0, rep
+
+
 def test_default_kernel_selection(stev):
     gpu = GpuCase(stev, make_workload(3, 64)).integrate()
     assert gpu["stats"]["lanes_per_cell"] == 64 and gpu["stats"]["threads_per_block"] == 512
