@@ -339,7 +339,8 @@ def main():
     peak_tflops = 2.0 * peak_instr / 1e12
     kernel_name = {33: "stev_pk_kernel<1> (one warp per cell, DFT history in tensor memory)",
                    64: "stev_pk_kernel<2> (warp pair per cell, DFT history in tensor memory)",
-                   66: "stev_ab_kernel (rate warp + DFT warp per cell)"}.get(st["lanes_per_cell"],
+                   66: "stev_ab_kernel (rate warp + DFT warp per cell)",
+                   128: "stev_pk_kernel<4> (warp quad per cell, DFT history in tensor memory)"}.get(st["lanes_per_cell"],
                                                                              f"stev_integrate_kernel<{st['lanes_per_cell']}>")
     roofline = {"bound": "alu", "kernel": kernel_name,
                 "achieved": flop / kernel_s / 1e12, "peak": peak_tflops, "unit": "TFLOP/s",

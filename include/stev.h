@@ -115,7 +115,8 @@ typedef struct {
                              33 = one warp per cell, 16 cells per SM (<= 32 species, 1..128 reversible reactions);
                              64 = a warp pair per cell, 8 cells per SM, both warps split every phase of a step
                                   (<= 64 species, 1..256 reversible reactions; the default for >= 128 reactions);
-                             66 = warp-specialised variant of 64 (a rate warp + a DFT warp; also needs dft_enable) */
+                             66 = warp-specialised variant of 64 (a rate warp + a DFT warp; also needs dft_enable);
+                             128 = a warp quad per cell, 8 cells per SM, 32 warps of 64 registers per SM (same limits as 64) */
 } stev_params;
 
 /* Counters of the last stev_integrate / stev_integrate_host call on this thread. */

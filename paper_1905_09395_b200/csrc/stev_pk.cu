@@ -15,7 +15,8 @@ static constexpr size_t kSmemMax = 227 * 1024;
 // The pair kernel keeps at most two concentration factors per reaction side (total nu per side <= 2, so nu*g is exact
 // for the equilibrium sum), 8 reversible reactions per TMEM lane (Rrev <= 256) and one species per lane (S <= 64).
 static bool pk_mechanism_ok(const HostMechanism &m, int nw) {
-  if (m.S > 32 * nw || m.Rrev < 1 || m.Rrev > 16 * nw * kPkMaxIt) return false;
+  const int nw2 = std::min(nw, 2);   // species and gather lists live in at most two warps, histories in 256 TMEM columns
+  if (m.S > 32 * nw2 || m.Rrev < 1 || m.Rrev > 16 * nw2 * kPkMaxIt) return false;
   for (int j = 0; j < m.R; ++j) {
     int nr = 0, np = 0;
     for (int e = m.reac_ptr[j]; e < m.reac_ptr[j + 1]; ++e) nr += m.reac_nu[e];
@@ -48,7 +49,7 @@ static void pk_layout(const PkTables &tb, PkCell &cl) {
 
 bool build_pk_image(const HostMechanism &m, const HostEstimator *e, int nw, std::vector<unsigned char> &image, PkTables &tb,
                     PkCell &cl) {
-  if ((nw != 1 && nw != 2) || !pk_mechanism_ok(m, nw)) return false;
+  if ((nw != 1 && nw != 2 && nw != 4) || !pk_mechanism_ok(m, nw)) return false;
   const int S = m.S, R = m.R, Rrev = m.Rrev;
   tb = PkTables{};
   tb.S = S;
@@ -58,8 +59,16 @@ bool build_pk_image(const HostMechanism &m, const HostEstimator *e, int nw, std:
   tb.Rp = (R + 1) & ~1;
   // DFT blocks: each warp keeps at most four blocks (128 TMEM columns); warp 0 takes the smaller half because it also
   // walks the two sequential sums of the temperature equation
-  tb.it_half0 = (nw == 2) ? tb.n_it / 2 : tb.n_it;
+  // (quad: warps 2 and 3 run the filter of the previous step while warps 0 and 1 run phase A of the next one)
   tb.nw = nw;
+  tb.it_split[0] = 0;
+  for (int h = 0; h < kPkMaxNw; ++h) {
+    int cnt = 0;
+    if (nw == 1) cnt = (h == 0) ? tb.n_it : 0;
+    else if (nw == 2) cnt = (h == 0) ? tb.n_it / 2 : (h == 1 ? tb.n_it - tb.n_it / 2 : 0);
+    else cnt = (h == 2) ? tb.n_it / 2 : (h == 3 ? tb.n_it - tb.n_it / 2 : 0);   // the filter runs on warps 2 and 3
+    tb.it_split[h + 1] = tb.it_split[h] + cnt;
+  }
   if (e) {
     tb.has_est = 1;
     tb.H = e->H;
@@ -102,23 +111,30 @@ bool build_pk_image(const HostMechanism &m, const HostEstimator *e, int nw, std:
   std::vector<int> order(S);
   std::iota(order.begin(), order.end(), 0);
   std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return gl[x].size() > gl[y].size(); });
-  unsigned char gsp[64];
-  unsigned short glen[64];
+  // With four warps per cell the gather stays in two of them (warps 2 and 3; a sequential sum cannot be split, so more
+  // warps would add instructions without shortening the longest list); warps 0 and 1 skip phase C.
+  unsigned char gsp[32 * kPkMaxNw];
+  unsigned short glen[32 * kPkMaxNw];
   std::memset(gsp, 255, sizeof(gsp));
   std::memset(glen, 0, sizeof(glen));
-  int g_len[2] = {0, 0};
+  int g_len[kPkMaxNw] = {0, 0, 0, 0};
+  const int g_short = (nw == 4) ? 2 : 0, g_long = (nw == 4) ? 3 : 1;
   for (int n = 0; n < S; ++n) {
     const int group = n / 16;
-    const int half = (nw == 2 && group < 2) ? 1 : 0, lane = (nw == 2) ? (group & 1) * 16 + n % 16 : n;
+    const int half = (nw >= 2) ? (group < 2 ? g_long : g_short) : 0, lane = (nw >= 2) ? (group & 1) * 16 + n % 16 : n;
     gsp[32 * half + lane] = (unsigned char)order[n];
     glen[32 * half + lane] = (unsigned short)gl[order[n]].size();
     g_len[half] = std::max(g_len[half], (int)gl[order[n]].size());
   }
   // rows of four entries, an even number per warp (the kernel walks two rows per trip) plus two spare rows that the
   // kernel prefetches past the end
-  tb.g_len4[0] = (g_len[0] + 7) / 8 * 2;
-  tb.g_len4[1] = (g_len[1] + 7) / 8 * 2;
-  const int g_rows = tb.g_len4[0] + tb.g_len4[1] + 2;
+  int g_rows = 0;
+  for (int h = 0; h < kPkMaxNw; ++h) {
+    tb.g_len4[h] = (g_len[h] + 7) / 8 * 2;
+    tb.g_row0[h] = g_rows;
+    g_rows += tb.g_len4[h];
+  }
+  g_rows += 2;
 
   // Internal reaction order: reversible reactions first (lanes never diverge on reversibility); within each group the
   // order is free, because every table is indexed through it.  It decides which shared-memory banks the lanes of a
@@ -169,7 +185,7 @@ bool build_pk_image(const HostMechanism &m, const HostEstimator *e, int nw, std:
     for (int k = 0; k < R; ++k) internal_of[orig_of[k]] = k;
     long long total = 0;
     unsigned addr[16];
-    for (int half = 0; half < 2; ++half)            // gather: step e of the lists of one half-warp
+    for (int half = 0; half < kPkMaxNw; ++half)     // gather: step e of the lists of one half-warp
       for (int hw = 0; hw < 2; ++hw)
         for (int e = 0;; ++e) {
           int n = 0;
@@ -248,8 +264,8 @@ bool build_pk_image(const HostMechanism &m, const HostEstimator *e, int nw, std:
   tb.o_rkB = take(16 * R);
   tb.o_rfac = take(16 * R);
   tb.o_rdg = take(16 * Rrev);
-  tb.o_gsp = take(64);
-  tb.o_glen = take(128);
+  tb.o_gsp = take(sizeof(gsp));
+  tb.o_glen = take(sizeof(glen));
   tb.o_gent = take(16 * 32 * std::max(g_rows, 1));
   if (e) {
     tb.o_eshift = take(4 * e->n_in);
@@ -291,11 +307,11 @@ bool build_pk_image(const HostMechanism &m, const HostEstimator *e, int nw, std:
     std::memcpy(rfac + 4 * k, &fac_of[4 * (size_t)j], 16);
     if (k < Rrev) std::memcpy(rdg + 4 * k, &dg_of[4 * (size_t)j], 16);
   }
-  std::memcpy(base + tb.o_gsp, gsp, 64);
-  std::memcpy(base + tb.o_glen, glen, 128);
+  std::memcpy(base + tb.o_gsp, gsp, sizeof(gsp));
+  std::memcpy(base + tb.o_glen, glen, sizeof(glen));
   unsigned *gent = (unsigned *)(base + tb.o_gent);   // [row][lane][4]
   for (int n = 0; n < 4 * 32 * g_rows; ++n) gent[n] = zero_slot;
-  for (int half = 0, row0 = 0; half < 2; ++half) {
+  for (int half = 0, row0 = 0; half < kPkMaxNw; ++half) {
     for (int lane = 0; lane < 32; ++lane) {
       const int i = gsp[32 * half + lane];
       for (int en = 0; en < 4 * tb.g_len4[half]; ++en) {
@@ -325,7 +341,7 @@ bool build_pk_image(const HostMechanism &m, const HostEstimator *e, int nw, std:
 
 int pk_cells_per_block(const PkTables &tb, const PkCell &cl) {
   const size_t avail = kSmemMax - (size_t)tb.bytes - 256;
-  return (int)std::min<size_t>(kPkMaxCells * 2 / tb.nw, avail / (size_t)cl.stride);
+  return (int)std::min<size_t>(tb.nw == 1 ? 2 * kPkMaxCells : kPkMaxCells, avail / (size_t)cl.stride);
 }
 
 int integrate_pk_launch(const PkTables &tb, const PkCell &cl, const unsigned char *d_table, const SolverConsts &sc, double t_f,
@@ -350,11 +366,12 @@ int integrate_pk_launch(const PkTables &tb, const PkCell &cl, const unsigned cha
   a.cells_per_block = pk_cells_per_block(tb, cl);
   if (a.cells_per_block < 1) { set_error("pair kernel: shared memory too small"); return STEV_EINVAL; }
   const size_t smem = (size_t)tb.bytes + (size_t)a.cells_per_block * cl.stride;
-  void *fn = (tb.nw == 2) ? (void *)stev_pk_kernel<2> : (void *)stev_pk_kernel<1>;
+  void *fn = (tb.nw == 4) ? (void *)stev_pk_kernel<4> : ((tb.nw == 2) ? (void *)stev_pk_kernel<2> : (void *)stev_pk_kernel<1>);
+  const int threads = (tb.nw == 4) ? kPkThreads4 : kPkThreads;
   STEV_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   const long long blocks = std::min<long long>(device_sm_count(), (n + a.cells_per_block - 1) / a.cells_per_block);
   void *args[] = {&a};
-  STEV_CUDA(cudaLaunchKernel(fn, dim3((unsigned)blocks), dim3(kPkThreads), args, smem, s));
+  STEV_CUDA(cudaLaunchKernel(fn, dim3((unsigned)blocks), dim3(threads), args, smem, s));
   *blocks_out = (int)blocks;
   *cells_per_block_out = a.cells_per_block;
   *smem_out = smem;

@@ -10,25 +10,28 @@ constexpr int kPkMaxCells = 8;       // cells per block with two warps per cell:
                                      // (one warp per cell: 16 cells, 4 per quarter)
 constexpr int kPkMaxIt = 8;          // 32-blocks of reversible reactions per cell with two warps per cell (32 TMEM columns
                                      // each, 256 columns per cell); 4 with one warp per cell
-constexpr int kPkThreads = 64 * kPkMaxCells;
+constexpr int kPkThreads = 64 * kPkMaxCells;   // block size with one or two warps per cell
+constexpr int kPkThreads4 = 128 * kPkMaxCells;  // block size with four warps per cell (8 cells, 64 registers per thread)
+constexpr int kPkMaxNw = 4;
 
 // Table image of the pair kernel (one contiguous buffer, copied verbatim to shared memory).  Byte offsets.
 struct PkTables {
-  int nw;                              // warps per cell: 2 (pair, 8 cells per block) or 1 (16 cells per block)
+  int nw;                              // warps per cell: 4 (quad, 8 cells per block), 2 (pair, 8 cells) or 1 (16 cells)
   int S, R, Rrev, n_it, Rp;            // n_it: 32-blocks of reversible reactions; Rp: row length of the q-variant array
   int has_est, H, Hpad, n_in, n_out, act, input_map;
   float h_ref_T;
   int n_var;                           // stored multiples of q: 2 (+q, -q) or 4 (+q, -q, +2q, -2q)
-  int g_len4[2];                       // per warp of the pair: rows of four gather entries per lane (longest list, rounded up)
-  int it_half0;                        // DFT blocks [0, it_half0) belong to warp 0 of the pair, [it_half0, n_it) to warp 1
+  int g_len4[kPkMaxNw];                // per warp of the cell: rows of four gather entries per lane (longest list, rounded up)
+  int g_row0[kPkMaxNw];                // first row of that warp's entries in o_gent
+  int it_split[kPkMaxNw + 1];          // DFT blocks [it_split[h], it_split[h + 1]) belong to warp h of the cell
   int o_tmid, o_W, o_invW, o_nasa;     // double [S] each; nasa [2][14][S]
   int o_rkA, o_rkB;                    // double2 [R]: {ln A, b}, {Ea/R_cal, dnu}
   int o_rfac;                          // uint4 [R]: byte offsets (from the cell base) of the two reactant and two
                                        //            product concentration factors (the 1.0 slot if absent)
   int o_rdg;                           // uint4 [Rrev]: byte offsets of nu*g of the <=2 reactant / <=2 product entries
-  int o_gsp;                           // uint8 [64]: species whose source term lane l of warp h gathers ([32 h + l]); 255 = none
-  int o_glen;                          // uint16 [64]: number of entries of that species' list
-  int o_gent;                          // uint4 [g_len4[0] + g_len4[1]][32]: byte offsets (from the cell base) of the
+  int o_gsp;                           // uint8 [128]: species whose source term lane l of warp h gathers ([32 h + l]); 255 = none
+  int o_glen;                          // uint16 [128]: number of entries of that species' list
+  int o_gent;                          // uint4 [sum of g_len4 + 2][32]: byte offsets (from the cell base) of the
                                        //            stored multiples coef*q_j, or of the 0.0 slot (padding)
   int o_eshift, o_escale, o_W1T, o_b1, o_W2p, o_b2;  // float: [n_in],[n_in],[n_in][H],[H],[n_out][Hpad],[n_out]
   int bytes;
@@ -51,9 +54,9 @@ struct PkCell {
 // Scalars the two warps of a pair hand to each other (each field has one writer per step, read after a pair barrier).
 struct PkScal {
   double lnT, ln_c0, invT, inv_ctot, rho;
-  double t_star[2];
+  double t_star[kPkMaxNw];
   double T_new;
-  int bad[2];
+  int bad[kPkMaxNw];
   int pos;
   int pad;
 };

@@ -67,13 +67,14 @@ __device__ __forceinline__ void pk_nasa(const PkTables &tb, const unsigned char 
 // ---------------------------------------------------------------------------------------------------------
 // a7 in the integrator (fp32 CUDA cores, R18): cp_i/R and h_i/(R T_ref) from the shallow MLP, by one warp.
 // ---------------------------------------------------------------------------------------------------------
+template <int MU>
 __device__ __forceinline__ void pk_mlp(const PkTables &tb, const unsigned char *tbl, const double2 *cYp, double2 *cYwCp,
-                                       double2 *cHOm, float *cHid, double T, double p, double invT, int lane) {
+                                       double2 *cHOm, float *cHid, double T, double p, double invT, int lane, int o_lo, int o_hi) {
   const int S = tb.S;
   const float *eshift = (const float *)(tbl + tb.o_eshift), *escale = (const float *)(tbl + tb.o_escale);
   const float *W1T = (const float *)(tbl + tb.o_W1T), *b1 = (const float *)(tbl + tb.o_b1);
   const float *W2p = (const float *)(tbl + tb.o_W2p), *b2 = (const float *)(tbl + tb.o_b2);
-  const int H = tb.H, Hpad = tb.Hpad, n_in = tb.n_in, n_out = tb.n_out;
+  const int H = tb.H, Hpad = tb.Hpad, n_in = tb.n_in;
   for (int jh = lane; jh < H; jh += 32) {
     float z = b1[jh];
     for (int k = 0; k < n_in; ++k) {
@@ -89,13 +90,13 @@ __device__ __forceinline__ void pk_mlp(const PkTables &tb, const unsigned char *
   }
   __syncwarp();
   const float4 *hid4 = (const float4 *)cHid;
-  for (int o0 = 0; o0 < n_out; o0 += 128) {
-    float y[4];
-    const float4 *wrow[4];
+  for (int o0 = o_lo; o0 < o_hi; o0 += 32 * MU) {
+    float y[MU];
+    const float4 *wrow[MU];
 #pragma unroll
-    for (int u = 0; u < 4; ++u) {
+    for (int u = 0; u < MU; ++u) {
       int o = o0 + 32 * u + lane;
-      o = (o < n_out) ? o : n_out - 1;
+      o = (o < o_hi) ? o : o_hi - 1;
       y[u] = b2[o];
       wrow[u] = (const float4 *)(W2p + (size_t)o * Hpad);
     }
@@ -103,7 +104,7 @@ __device__ __forceinline__ void pk_mlp(const PkTables &tb, const unsigned char *
     for (int q4 = 0; q4 < H / 4; ++q4) {
       const float4 hv = hid4[q4];
 #pragma unroll
-      for (int u = 0; u < 4; ++u) {
+      for (int u = 0; u < MU; ++u) {
         const float4 wv = wrow[u][q4];
         y[u] = __fmaf_rn(wv.x, hv.x, y[u]);
         y[u] = __fmaf_rn(wv.y, hv.y, y[u]);
@@ -112,9 +113,9 @@ __device__ __forceinline__ void pk_mlp(const PkTables &tb, const unsigned char *
       }
     }
 #pragma unroll
-    for (int u = 0; u < 4; ++u) {
+    for (int u = 0; u < MU; ++u) {
       const int o = o0 + 32 * u + lane;
-      if (o < n_out) {
+      if (o < o_hi) {
         if (o < S) cYwCp[o].y = (double)y[u];
         else cHOm[o - S].x = ((double)y[u] * (double)tb.h_ref_T) * invT;
       }
@@ -127,7 +128,7 @@ __device__ __forceinline__ void pk_mlp(const PkTables &tb, const unsigned char *
 // warp.  TMEM address of slot s of this lane's reaction in block `it`:  trow + it * 32 + 2 s.
 // Two windows are processed side by side (independent dependency chains for the scheduler).
 // ---------------------------------------------------------------------------------------------------------
-template <int NHF>
+template <int NHF, bool PAIRWIN>
 __device__ __forceinline__ void pk_dft(const SolverConsts &sc, const double *cQ, double *cRof, int Rrev, int it_lo, int it_hi,
                                        uint32_t trow, int slot, double h, double inv_ctot, int lane) {
   auto update_rof = [&](int k, bool ringing) {
@@ -144,7 +145,7 @@ __device__ __forceinline__ void pk_dft(const SolverConsts &sc, const double *cQ,
   }
   tmem_wait_st();
   int it = it_lo;
-  for (; it + 2 <= it_hi; it += 2) {
+  for (; PAIRWIN && it + 2 <= it_hi; it += 2) {
     uint32_t ra[26], rb[26];
     tmem_ld26(trow + it * 32, ra);
     tmem_ld26(trow + it * 32 + 32, rb);
@@ -166,7 +167,7 @@ __device__ __forceinline__ void pk_dft(const SolverConsts &sc, const double *cQ,
     if (ka < Rrev) update_rof(ka, ring_a);
     if (kb < Rrev) update_rof(kb, ring_b);
   }
-  if (it < it_hi) {
+  auto one_window = [&](int it) {
     uint32_t ra[26];
     tmem_ld26(trow + it * 32, ra);
     tmem_wait_ld();
@@ -179,6 +180,12 @@ __device__ __forceinline__ void pk_dft(const SolverConsts &sc, const double *cQ,
     bool ring_a = ab_ring_filter(d0a, m2a, sc, sure_a);
     if (__any_sync(0xffffffffu, !sure_a && ka < Rrev)) ring_a = ab_ring_exact(d0a, m2a, sc);
     if (ka < Rrev) update_rof(ka, ring_a);
+  };
+  if (PAIRWIN) {
+    if (it < it_hi) one_window(it);
+  } else {
+#pragma unroll 1
+    for (; it < it_hi; ++it) one_window(it);
   }
 }
 
@@ -285,22 +292,31 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
   const unsigned char *gsp = tbl + tb.o_gsp;
   const bool has2 = tb.n_var > 2;
 
-  const int bar = 1 + j;                        // named barrier of this pair (0 is __syncthreads)
+  const int bar = 1 + j;                        // named barrier of this cell's warps (0 is __syncthreads)
   auto cell_sync = [&]() {
-    if (NW == 2) named_bar_sync(bar);
+    if (NW >= 2) asm volatile("bar.sync %0, %1;" ::"r"(bar), "n"(32 * NW) : "memory");
     else __syncwarp();
   };
   const double dt_max = a.t_f * sc.delta_max;   // Eq 4
   const double t_tol = 1.0e-12 * a.t_f;         // R5
-  const int it_lo = half ? tb.it_half0 : 0, it_hi = half ? n_it : tb.it_half0;   // DFT blocks of this warp (at most four)
+  const int it_lo = (NW == 1 || half == 0) ? 0 : tb.it_split[half], it_hi = (NW == 1) ? n_it : tb.it_split[half + 1];   // DFT blocks of this warp (at most four; quad: two)
   // TMEM: a warp reaches the lane quarter (warp id mod 4); it keeps the windows of its own blocks in 128 columns of
   // that quarter: columns [128 (j / 4), +128) for warp 0 of a cell (or the only warp), [256 + 128 (j / 4), +128) for warp 1.
-  const uint32_t trow = tmem_base + ((uint32_t)((tmem_quarter & 3) * 32) << 16) + (uint32_t)((j >> 2) * 128 + half * 256) -
-                        (uint32_t)(it_lo * 32);
-  const int my_sp = half * 32 + lane;           // species this lane loads, updates and writes back
+  // Quad: the four warps of cell j sit in the four quarters; warps 2 and 3 keep four blocks each, and since the role
+  // rotates with j every quarter holds four such warps: columns [128 rank, +128), rank = earlier cells with a filter
+  // warp in this quarter.
+  uint32_t tcol = (uint32_t)((j >> 2) * 128 + half * 256);
+  if (NW == 4) {
+    int rank = 0;
+    for (int jj = 0; jj < j; ++jj) rank += (((tmem_quarter + jj) & 3) >= 2) ? 1 : 0;
+    tcol = (uint32_t)(rank * 128);
+  }
+  const uint32_t trow = tmem_base + ((uint32_t)((tmem_quarter & 3) * 32) << 16) + tcol - (uint32_t)(it_lo * 32);
+  const int my_sp = (half < 2) ? half * 32 + lane : 0x7fff;   // species this lane loads, updates and writes back
   const int g_sp = gsp[half * 32 + lane];       // species whose source term this lane gathers (255 = none)
-  const uint4 *ge = (const uint4 *)(tbl + tb.o_gent) + (half ? tb.g_len4[0] * 32 : 0) + lane;
+  const uint4 *ge = (const uint4 *)(tbl + tb.o_gent) + tb.g_row0[half] * 32 + lane;
   const int g_len4 = tb.g_len4[half];
+  if (lane == 0) scal->t_star[half] = bits_to_double(0x7ff0000000000000ull);   // stays +inf for a warp without lists
 
   if (half == 0 && lane == 0) {
     cConc[0] = 1.0;
@@ -324,7 +340,7 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
       if (k < Rrev) cRof[k] = 1.0;                                                // Eq 11
     }
     tmem_wait_st();
-    double t = 0.0;
+    double t = 0.0, h_prev = 0.0, ictot_prev = 0.0;
     int steps = 0, slot = 0;
     cell_sync();
 
@@ -382,19 +398,33 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
         }
       }
       if (NW == 1) {
-        if (EST) pk_mlp(tb, tbl, cYp, cYwCp, cHOm, cHid, T, p, invT, lane);
-      } else if (half == 1) {
-        // warp 1 of the pair: all of the thermodynamics (its own ln T and 1/T: same operations, same bits)
+        if (EST) pk_mlp<4>(tb, tbl, cYp, cYwCp, cHOm, cHid, T, p, invT, lane, 0, tb.n_out);
+      } else if (NW >= 2 && half == 1) {
+        // warp 1 of the pair / quad: all of the thermodynamics (its own ln T and 1/T: same operations, same bits)
         const double invT1 = 1.0 / T;
         if (EST) {
           pk_nasa<false>(tb, tbl, cG, cYwCp, cHOm, T, invT1, ab_log(T), lane);
-          pk_mlp(tb, tbl, cYp, cYwCp, cHOm, cHid, T, p, invT1, lane);
+          pk_mlp<4>(tb, tbl, cYp, cYwCp, cHOm, cHid, T, p, invT1, lane, 0, tb.n_out);
         } else {
           pk_nasa<true>(tb, tbl, cG, cYwCp, cHOm, T, invT1, ab_log(T), lane);
         }
+      } else if (NW == 4 && half >= 2) {
+        // warps 2 and 3 of the quad: the ringing filter of the PREVIOUS step (it only feeds rOF, which phase B reads),
+        // concurrently with the scalars and the thermodynamics of this step on warps 0 and 1
+        if (steps > 0 && sc.dft_enable) {
+          switch (sc.nhf) {
+            case 1: pk_dft<1, false>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h_prev, ictot_prev, lane); break;
+            case 2: pk_dft<2, false>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h_prev, ictot_prev, lane); break;
+            case 3: pk_dft<3, false>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h_prev, ictot_prev, lane); break;
+            case 4: pk_dft<4, false>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h_prev, ictot_prev, lane); break;
+            case 5: pk_dft<5, false>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h_prev, ictot_prev, lane); break;
+            default: pk_dft<6, false>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h_prev, ictot_prev, lane); break;
+          }
+          slot = (slot + 1 == kWindow) ? 0 : slot + 1;
+        }
       }
       cell_sync();
-      if (NW == 2 && half) {
+      if (NW >= 2 && half) {
         lnT = scal->lnT;
         ln_c0 = scal->ln_c0;
         invT = scal->invT;
@@ -407,21 +437,22 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
       // warp and are evaluated four (small mechanisms: two) at a time, i.e. eight independent exp chains and one trip
       // through the load -> exp -> load -> store latency chain.  The stored multiples +q, -q, +2q, -2q (all exact) turn the sum
       // omega_i = sum_j nu_ij q_j into plain additions in the contract's order.
-      if (n_it > 2 * NW) {
+      if (NW < 4 && n_it > 2 * NW) {
         for (int b0 = half; b0 < n_it; b0 += 4 * NW)
           pk_rev_batch<4>(cell, rkA, rkB, rfac, rdg, cRof, cQ, Rp, Rrev, has2, invT, lnT, ln_c0, b0, NW, lane);
       } else {
         for (int b0 = half; b0 < n_it; b0 += 2 * NW)
           pk_rev_batch<2>(cell, rkA, rkB, rfac, rdg, cRof, cQ, Rp, Rrev, has2, invT, lnT, ln_c0, b0, NW, lane);
       }
-      // irreversible reactions [Rrev, R): 32-blocks c = half (mod 2), two at a time
-      for (int k0 = Rrev + half * 32; k0 < R; k0 += 64 * NW) {
-        double lk[2], fw[2];
-        uint4 f[2];
-        int kk[2];
+      // irreversible reactions [Rrev, R): 32-blocks c = half (mod NW), two at a time (quad: one)
+      constexpr int IU = (NW == 4) ? 1 : 2;
+      for (int k0 = Rrev + half * 32; k0 < R; k0 += 32 * IU * NW) {
+        double lk[IU], fw[IU];
+        uint4 f[IU];
+        int kk[IU];
         bool oor = false;
 #pragma unroll
-        for (int u = 0; u < 2; ++u) {
+        for (int u = 0; u < IU; ++u) {
           kk[u] = k0 + 32 * NW * u + lane;
           const int k = (kk[u] < R) ? kk[u] : R - 1;
           const double2 p0 = rkA[k];
@@ -432,17 +463,17 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
         }
         if (__any_sync(0xffffffffu, oor)) {
 #pragma unroll
-          for (int u = 0; u < 2; ++u) fw[u] = cexp(lk[u]);
+          for (int u = 0; u < IU; ++u) fw[u] = cexp(lk[u]);
         } else {
 #pragma unroll
-          for (int u = 0; u < 2; ++u) fw[u] = ab_exp_core(lk[u]);
+          for (int u = 0; u < IU; ++u) fw[u] = ab_exp_core(lk[u]);
         }
 #pragma unroll
-        for (int u = 0; u < 2; ++u) fw[u] = fw[u] * lds_f64(cell, f[u].x);
+        for (int u = 0; u < IU; ++u) fw[u] = fw[u] * lds_f64(cell, f[u].x);
 #pragma unroll
-        for (int u = 0; u < 2; ++u) fw[u] = fw[u] * lds_f64(cell, f[u].y);
+        for (int u = 0; u < IU; ++u) fw[u] = fw[u] * lds_f64(cell, f[u].y);
 #pragma unroll
-        for (int u = 0; u < 2; ++u) {
+        for (int u = 0; u < IU; ++u) {
           if (kk[u] < R) {
             const int k = kk[u];
             cQ[k] = fw[u];
@@ -460,7 +491,7 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
       // ================= phase C: source terms and the limiter (Eqs 1-3) =================
       // One species per lane; the entry lists hold the byte offsets of the stored multiples in the caller's reaction
       // order and are padded with the 0.0 slot to the longest list of the warp, so the loop is warp-uniform.
-      {
+      if (NW < 4 || g_len4 > 0) {
         const double inv_rho = 1.0 / rho;
         double om = 0.0;
         // Two rows of four entries per trip: the eight loads of a trip are independent and the offsets of the next
@@ -506,7 +537,9 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
 
       // ================= phase D =================
       // -- a3: step size (Eq 5) and landing on t_f (R5)
-      const double t_star = (NW == 2) ? pk_min_bits(scal->t_star[0], scal->t_star[1]) : scal->t_star[0];
+      double t_star = scal->t_star[0];
+      if (NW >= 2) t_star = pk_min_bits(t_star, scal->t_star[1]);
+      if (NW == 4) t_star = pk_min_bits(t_star, pk_min_bits(scal->t_star[2], scal->t_star[3]));
       double h = (t_star < dt_max) ? t_star : dt_max;
       bool last = false;
       const double rem = a.t_f - t;
@@ -538,28 +571,30 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
         if (lane == 0) scal->T_new = T;
       }
       bad = __any_sync(0xffffffffu, bad);
-      if (lane == 0) scal->bad[half] = bad;
+      if (lane == 0 && half < 2) scal->bad[half] = bad;
       // -- a5: DFT ringing filter of this warp's blocks (skipped on the landing step: the cell retires)
-      if (!last && sc.dft_enable) {
+      if (NW != 4 && !last && sc.dft_enable) {
         switch (sc.nhf) {
-          case 1: pk_dft<1>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h, inv_ctot, lane); break;
-          case 2: pk_dft<2>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h, inv_ctot, lane); break;
-          case 3: pk_dft<3>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h, inv_ctot, lane); break;
-          case 4: pk_dft<4>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h, inv_ctot, lane); break;
-          case 5: pk_dft<5>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h, inv_ctot, lane); break;
-          default: pk_dft<6>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h, inv_ctot, lane); break;
+          case 1: pk_dft<1, NW != 4>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h, inv_ctot, lane); break;
+          case 2: pk_dft<2, NW != 4>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h, inv_ctot, lane); break;
+          case 3: pk_dft<3, NW != 4>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h, inv_ctot, lane); break;
+          case 4: pk_dft<4, NW != 4>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h, inv_ctot, lane); break;
+          case 5: pk_dft<5, NW != 4>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h, inv_ctot, lane); break;
+          default: pk_dft<6, NW != 4>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h, inv_ctot, lane); break;
         }
         slot = (slot + 1 == kWindow) ? 0 : slot + 1;
       }
       cell_sync();
-      if (NW == 2 && half) T = scal->T_new;
+      if (NW >= 2 && half) T = scal->T_new;
       t = last ? a.t_f : t + h;
       steps += 1;
+      h_prev = h;
+      ictot_prev = inv_ctot;
 
       // -- a6: retirement (R20)
       int st = -1;
       if (last) st = 0;
-      else if (scal->bad[0] | (NW == 2 ? scal->bad[1] : 0)) st = 2;
+      else if (scal->bad[0] | (NW >= 2 ? scal->bad[1] : 0)) st = 2;
       else if (steps >= sc.max_steps) st = 1;
       if (st >= 0) {
         if (my_sp < S) a.Y[(long long)my_sp * a.ld + cidx] = cYp[my_sp].x;
@@ -576,7 +611,7 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
 }
 
 template <int NW>
-__global__ void __launch_bounds__(kPkThreads, 1) stev_pk_kernel(const __grid_constant__ PkArgs a) {
+__global__ void __launch_bounds__((NW == 4) ? kPkThreads4 : kPkThreads, 1) stev_pk_kernel(const __grid_constant__ PkArgs a) {
   extern __shared__ __align__(128) unsigned char smem[];
   __shared__ unsigned long long mbar;
   __shared__ uint32_t tmem_base_s;
@@ -598,8 +633,10 @@ __global__ void __launch_bounds__(kPkThreads, 1) stev_pk_kernel(const __grid_con
   // NW = 1: warp j is cell slot j.  NW = 2: warps j and 8 + (j + 1) % 8 form the pair of cell slot j.  The two warps of a
   // pair run the same phase at the same time, so they are placed on DIFFERENT schedulers (warp id mod 4): a scheduler
   // then interleaves four cells in four different phases (fp64-bound DFT against latency-bound gather and rates).
-  const int half = (NW == 2) ? (warp >> 3) : 0;
-  const int j = (NW == 2) ? (half ? ((warp - 8 + 7) & 7) : warp) : warp;
+  // NW = 4: warps 4 j .. 4 j + 3 serve cell slot j, one per scheduler and TMEM lane quarter; the role rotates with j, so
+  // every scheduler holds two warps of each role (the scalar chains, NASA-7, the two estimator halves).
+  const int half = (NW == 4) ? (((warp & 3) + (warp >> 2)) & 3) : ((NW == 2) ? (warp >> 3) : 0);
+  const int j = (NW == 4) ? (warp >> 2) : ((NW == 2) ? (half ? ((warp - 8 + 7) & 7) : warp) : warp);
   if (j < a.cells_per_block) {
     unsigned char *cell = smem + a.tb.bytes + (size_t)j * a.cl.stride;
     if (a.tb.has_est) pk_worker<true, NW>(a, smem, cell, j, half, warp & 3, tmem_base, lane);
@@ -609,7 +646,7 @@ __global__ void __launch_bounds__(kPkThreads, 1) stev_pk_kernel(const __grid_con
   if (lane == 0) atomicAdd(&done_warps, 1);
   if (warp == 0) {
     if (lane == 0) {
-      while (atomicAdd(&done_warps, 0) < kPkThreads / 32) __nanosleep(200);
+      while (atomicAdd(&done_warps, 0) < (int)(blockDim.x >> 5)) __nanosleep(200);
     }
     __syncwarp();
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem_base) : "memory");
