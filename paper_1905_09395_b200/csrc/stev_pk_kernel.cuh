@@ -270,6 +270,18 @@ __device__ __forceinline__ double pk_min_bits(double a, double b) {
 // One warp of the NW (1 or 2) warps that serve a cell.  `half` (0 .. NW-1) is warp-uniform.  With NW = 1 the pair
 // barriers degenerate to __syncwarp and the warp walks both halves of every phase (mid-size mechanisms: 16 cells per SM).
 // ---------------------------------------------------------------------------------------------------------
+#ifdef PK_TIMING
+__shared__ long long pk_tacc[32][8];
+#define PKT(i)                                                        \
+  if (lane == 0) {                                                    \
+    const long long now_ = clock64();                                 \
+    pk_tacc[threadIdx.x >> 5][i] += now_ - tlast_;                    \
+    tlast_ = now_;                                                    \
+  }
+#else
+#define PKT(i)
+#endif
+
 template <bool EST, int NW>
 __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *tbl, unsigned char *cell, int j, int half,
                                           int tmem_quarter, uint32_t tmem_base, int lane) {
@@ -322,6 +334,20 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
     cConc[0] = 1.0;
     cG[0] = 0.0;
   }
+  // a5 for this warp's blocks: h_s and ictot_s are the step size and 1/C_tot of the step whose progress is stored
+  auto run_dft = [&](int slot_s, double h_s, double ictot_s) {
+    switch (sc.nhf) {
+      case 1: pk_dft<1, NW != 4>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot_s, h_s, ictot_s, lane); break;
+      case 2: pk_dft<2, NW != 4>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot_s, h_s, ictot_s, lane); break;
+      case 3: pk_dft<3, NW != 4>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot_s, h_s, ictot_s, lane); break;
+      case 4: pk_dft<4, NW != 4>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot_s, h_s, ictot_s, lane); break;
+      case 5: pk_dft<5, NW != 4>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot_s, h_s, ictot_s, lane); break;
+      default: pk_dft<6, NW != 4>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot_s, h_s, ictot_s, lane); break;
+    }
+  };
+  // Pair: second named barrier of the cell (ids 9..15, and 0 -- free after the block-wide start-up -- for cell 7).
+  // Warp 0 arrives when the new T and Y are in shared memory, warp 1 waits for that before the thermodynamics.
+  const int xbar = (j < 7) ? 9 + j : 0;
 
   for (;;) {
     // ---- a6: variable load.  A pair whose cell retired pulls the next active cell from the global queue.
@@ -343,6 +369,11 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
     double t = 0.0, h_prev = 0.0, ictot_prev = 0.0;
     int steps = 0, slot = 0;
     cell_sync();
+#ifdef PK_TIMING
+    long long tlast_ = clock64();
+    if (lane == 0)
+      for (int i_ = 0; i_ < 8; ++i_) pk_tacc[threadIdx.x >> 5][i_] = 0;
+#endif
 
     for (;;) {
       // ================= phase A =================
@@ -397,6 +428,12 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
           }
         }
       }
+      if (NW == 2 && half == 0 && steps > 0 && sc.dft_enable) {
+        // warp 0 of the pair: its share of the ringing filter of the PREVIOUS step (it only feeds rOF, which phase B
+        // reads), after the scalars of this step, so that no barrier separates the update from phase A
+        run_dft(slot, h_prev, ictot_prev);
+        slot = (slot + 1 == kWindow) ? 0 : slot + 1;
+      }
       if (NW == 1) {
         if (EST) pk_mlp<4>(tb, tbl, cYp, cYwCp, cHOm, cHid, T, p, invT, lane, 0, tb.n_out);
       } else if (NW >= 2 && half == 1) {
@@ -412,18 +449,13 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
         // warps 2 and 3 of the quad: the ringing filter of the PREVIOUS step (it only feeds rOF, which phase B reads),
         // concurrently with the scalars and the thermodynamics of this step on warps 0 and 1
         if (steps > 0 && sc.dft_enable) {
-          switch (sc.nhf) {
-            case 1: pk_dft<1, false>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h_prev, ictot_prev, lane); break;
-            case 2: pk_dft<2, false>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h_prev, ictot_prev, lane); break;
-            case 3: pk_dft<3, false>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h_prev, ictot_prev, lane); break;
-            case 4: pk_dft<4, false>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h_prev, ictot_prev, lane); break;
-            case 5: pk_dft<5, false>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h_prev, ictot_prev, lane); break;
-            default: pk_dft<6, false>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h_prev, ictot_prev, lane); break;
-          }
+          run_dft(slot, h_prev, ictot_prev);
           slot = (slot + 1 == kWindow) ? 0 : slot + 1;
         }
       }
+      PKT(0)
       cell_sync();
+      PKT(1)
       if (NW >= 2 && half) {
         lnT = scal->lnT;
         ln_c0 = scal->ln_c0;
@@ -486,7 +518,9 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
           }
         }
       }
+      PKT(2)
       cell_sync();
+      PKT(3)
 
       // ================= phase C: source terms and the limiter (Eqs 1-3) =================
       // One species per lane; the entry lists hold the byte offsets of the stored multiples in the caller's reaction
@@ -533,7 +567,9 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
         const unsigned mlo = __reduce_min_sync(0xffffffffu, (hi == mhi) ? lo : 0xffffffffu);
         if (lane == 0) scal->t_star[half] = bits_to_double(((unsigned long long)mhi << 32) | mlo);
       }
+      PKT(4)
       cell_sync();
+      PKT(5)
 
       // ================= phase D =================
       // -- a3: step size (Eq 5) and landing on t_f (R5)
@@ -547,9 +583,22 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
         h = rem;
         last = true;
       }
-      // -- a4: forward Euler (Eq 18), one species per lane
+      // -- a4: forward Euler (Eq 18), one species per lane (pair: warp 0 updates all species, two per lane,
+      //    so that it depends on nothing of warp 1 between here and the end of phase A)
       int bad = 0;
-      if (my_sp < S) {
+      if (NW == 2) {
+        if (half == 0) {
+#pragma unroll
+          for (int u = 0; u < 2; ++u) {
+            const int i = lane + 32 * u;
+            if (i < S) {
+              const double y = fma_rn(h, cConc[1 + i], cYp[i].x);
+              cYp[i].x = y;
+              bad |= !(y - y == 0.0);
+            }
+          }
+        }
+      } else if (my_sp < S) {
         const double y = fma_rn(h, cConc[1 + my_sp], cYp[my_sp].x);
         cYp[my_sp].x = y;
         bad |= !(y - y == 0.0);
@@ -572,20 +621,32 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
       }
       bad = __any_sync(0xffffffffu, bad);
       if (lane == 0 && half < 2) scal->bad[half] = bad;
-      // -- a5: DFT ringing filter of this warp's blocks (skipped on the landing step: the cell retires)
-      if (NW != 4 && !last && sc.dft_enable) {
-        switch (sc.nhf) {
-          case 1: pk_dft<1, NW != 4>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h, inv_ctot, lane); break;
-          case 2: pk_dft<2, NW != 4>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h, inv_ctot, lane); break;
-          case 3: pk_dft<3, NW != 4>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h, inv_ctot, lane); break;
-          case 4: pk_dft<4, NW != 4>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h, inv_ctot, lane); break;
-          case 5: pk_dft<5, NW != 4>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h, inv_ctot, lane); break;
-          default: pk_dft<6, NW != 4>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot, h, inv_ctot, lane); break;
+      PKT(6)
+      if (NW == 2) {
+        // -- a5 on warp 1 now (skipped on the landing step: the cell retires); warp 0 runs its share after the scalars of
+        //    the next step.  Warp 0 announces the new T and Y (bar.arrive), warp 1 waits for them (bar.sync).
+        if (half == 0) {
+          __threadfence_block();
+          asm volatile("bar.arrive %0, 64;" ::"r"(xbar) : "memory");
+        } else {
+          if (!last && sc.dft_enable) {
+            run_dft(slot, h, inv_ctot);
+            slot = (slot + 1 == kWindow) ? 0 : slot + 1;
+          }
+          asm volatile("bar.sync %0, 64;" ::"r"(xbar) : "memory");
+          T = scal->T_new;
         }
-        slot = (slot + 1 == kWindow) ? 0 : slot + 1;
+      } else {
+        // -- a5: DFT ringing filter of this warp's blocks (skipped on the landing step: the cell retires; quad: it runs
+        //    at the start of the next step)
+        if (NW != 4 && !last && sc.dft_enable) {
+          run_dft(slot, h, inv_ctot);
+          slot = (slot + 1 == kWindow) ? 0 : slot + 1;
+        }
+        cell_sync();
+        if (NW >= 2 && half) T = scal->T_new;
       }
-      cell_sync();
-      if (NW >= 2 && half) T = scal->T_new;
+      PKT(7)
       t = last ? a.t_f : t + h;
       steps += 1;
       h_prev = h;
@@ -594,9 +655,16 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
       // -- a6: retirement (R20)
       int st = -1;
       if (last) st = 0;
-      else if (scal->bad[0] | (NW >= 2 ? scal->bad[1] : 0)) st = 2;
+      else if (scal->bad[0] | (NW == 4 ? scal->bad[1] : 0)) st = 2;
       else if (steps >= sc.max_steps) st = 1;
       if (st >= 0) {
+#ifdef PK_TIMING
+        if (blockIdx.x == 0 && j == 0 && lane == 0)
+          printf("PKT half %d steps %d per step: A %lld w %lld | B %lld w %lld | C %lld w %lld | D %lld w %lld\n", half, steps,
+                 pk_tacc[threadIdx.x >> 5][0] / steps, pk_tacc[threadIdx.x >> 5][1] / steps, pk_tacc[threadIdx.x >> 5][2] / steps,
+                 pk_tacc[threadIdx.x >> 5][3] / steps, pk_tacc[threadIdx.x >> 5][4] / steps, pk_tacc[threadIdx.x >> 5][5] / steps,
+                 pk_tacc[threadIdx.x >> 5][6] / steps, pk_tacc[threadIdx.x >> 5][7] / steps);
+#endif
         if (my_sp < S) a.Y[(long long)my_sp * a.ld + cidx] = cYp[my_sp].x;
         if (half == 0 && lane == 0) {
           a.T[cidx] = T;
