@@ -340,6 +340,7 @@ def main():
     kernel_name = {33: "stev_pk_kernel<1> (one warp per cell, DFT history in tensor memory)",
                    64: "stev_pk_kernel<2> (warp pair per cell, DFT history in tensor memory)",
                    66: "stev_ab_kernel (rate warp + DFT warp per cell)",
+                   96: "stev_pk_kernel<3> (warp triple per cell, DFT history in tensor memory)",
                    128: "stev_pk_kernel<4> (warp quad per cell, DFT history in tensor memory)"}.get(st["lanes_per_cell"],
                                                                              f"stev_integrate_kernel<{st['lanes_per_cell']}>")
     roofline = {"bound": "alu", "kernel": kernel_name,

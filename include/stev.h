@@ -116,6 +116,7 @@ typedef struct {
                              64 = a warp pair per cell, 8 cells per SM, both warps split every phase of a step
                                   (<= 64 species, 1..256 reversible reactions; the default for >= 128 reactions);
                              66 = warp-specialised variant of 64 (a rate warp + a DFT warp; also needs dft_enable);
+                             96 = a warp triple per cell, 8 cells per SM, 24 warps of 80 registers per SM (same limits as 64);
                              128 = a warp quad per cell, 8 cells per SM, 32 warps of 64 registers per SM (same limits as 64) */
 } stev_params;
 

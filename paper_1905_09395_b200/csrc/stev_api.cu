@@ -351,11 +351,11 @@ int stev_mechanism_create(const stev_mechanism_desc *d, stev_mechanism **out) {
       if (e == cudaSuccess) e = cudaMemcpy(m->d_ab_table, ab.data(), ab.size(), cudaMemcpyHostToDevice);
     }
   }
-  for (int n = 0; n < 3 && e == cudaSuccess; ++n) {   // the pair image first: it chooses the reaction order
-    static const int order[3] = {1, 2, 0};
+  for (int n = 0; n < 4 && e == cudaSuccess; ++n) {   // the pair image first: it chooses the reaction order
+    static const int order[4] = {1, 2, 3, 0}, nw_of[4] = {1, 2, 4, 3};
     const int w = order[n];
     std::vector<unsigned char> pk;
-    m->pk_ok[w] = build_pk_image(h, nullptr, 1 << w, pk, m->pk_tb[w], m->pk_cl[w]);
+    m->pk_ok[w] = build_pk_image(h, nullptr, nw_of[w], pk, m->pk_tb[w], m->pk_cl[w]);
     if (m->pk_ok[w]) {
       e = cudaMalloc(&m->d_pk_table[w], pk.size());
       if (e == cudaSuccess) e = cudaMemcpy(m->d_pk_table[w], pk.data(), pk.size(), cudaMemcpyHostToDevice);
@@ -373,7 +373,7 @@ void stev_mechanism_destroy(stev_mechanism *m) {
   if (!m) return;
   if (m->d_table) cudaFree(m->d_table);
   if (m->d_ab_table) cudaFree(m->d_ab_table);
-  for (int w = 0; w < 3; ++w)
+  for (int w = 0; w < 4; ++w)
     if (m->d_pk_table[w]) cudaFree(m->d_pk_table[w]);
   delete m;
 }
@@ -430,11 +430,11 @@ int stev_estimator_load(const stev_mechanism *m, const stev_estimator_desc *d, s
         if (ce == cudaSuccess) ce = cudaMemcpy(e->d_ab_table, ab.data(), ab.size(), cudaMemcpyHostToDevice);
       }
     }
-    for (int n = 0; n < 3 && ce == cudaSuccess; ++n) {
-      static const int order[3] = {1, 2, 0};
+    for (int n = 0; n < 4 && ce == cudaSuccess; ++n) {
+      static const int order[4] = {1, 2, 3, 0}, nw_of[4] = {1, 2, 4, 3};
       const int w = order[n];
       std::vector<unsigned char> pk;
-      e->pk_ok[w] = build_pk_image(m->host, &h, 1 << w, pk, e->pk_tb[w], e->pk_cl[w]);
+      e->pk_ok[w] = build_pk_image(m->host, &h, nw_of[w], pk, e->pk_tb[w], e->pk_cl[w]);
       if (e->pk_ok[w]) {
         ce = cudaMalloc(&e->d_pk_table[w], pk.size());
         if (ce == cudaSuccess) ce = cudaMemcpy(e->d_pk_table[w], pk.data(), pk.size(), cudaMemcpyHostToDevice);
@@ -472,7 +472,7 @@ void stev_estimator_destroy(stev_estimator *e) {
   if (!e) return;
   if (e->d_table) cudaFree(e->d_table);
   if (e->d_ab_table) cudaFree(e->d_ab_table);
-  for (int w = 0; w < 3; ++w)
+  for (int w = 0; w < 4; ++w)
     if (e->d_pk_table[w]) cudaFree(e->d_pk_table[w]);
   if (e->d_params) cudaFree(e->d_params);
   for (int k = 0; k < 2; ++k)
@@ -643,21 +643,25 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
   //   lanes_per_cell = 64: warp pair per cell, 8 cells per SM (both warps split every phase; the default for >= 128 reactions)
   //   lanes_per_cell = 66: warp-specialised kernel (a rate warp and a DFT warp per cell)
   //   lanes_per_cell = 128: warp quad per cell, 8 cells per SM, 32 warps of 64 registers per SM
+  //   lanes_per_cell = 96: warp triple per cell, 8 cells per SM, 24 warps of 80 registers per SM
   {
     const bool tm_common = p->chunk_steps == 0;
     const bool pk1_ok = (est ? est->pk_ok[0] : m->pk_ok[0]) && tm_common;
     const bool pk2_ok = (est ? est->pk_ok[1] : m->pk_ok[1]) && tm_common;
     const bool pk4_ok = (est ? est->pk_ok[2] : m->pk_ok[2]) && tm_common;
+    const bool pk3_ok = (est ? est->pk_ok[3] : m->pk_ok[3]) && tm_common;
     const bool ab_ok = (est ? est->ab_ok : m->ab_ok) && p->dft_enable && tm_common;
-    int kind = 0;   // 1: one warp per cell, 2: warp pair, 3: warp-specialised, 4: warp quad
+    int kind = 0;   // 1: one warp per cell, 2: warp pair, 3: warp-specialised, 4: warp quad, 5: warp triple
     if (p->lanes_per_cell == 33) kind = 1;
     else if (p->lanes_per_cell == 64) kind = 2;
     else if (p->lanes_per_cell == 66) kind = 3;
     else if (p->lanes_per_cell == 128) kind = 4;
+    else if (p->lanes_per_cell == 96) kind = 5;
     else if (p->lanes_per_cell == 0) kind = (tb->R >= 128 && pk2_ok) ? 2 : (pk1_ok ? 1 : (pk2_ok && tb->R >= 64 ? 2 : 0));
-    if ((kind == 1 && !pk1_ok) || (kind == 2 && !pk2_ok) || (kind == 3 && !ab_ok) || (kind == 4 && !pk4_ok)) {
-      set_error("stev_integrate: lanes_per_cell = 33 / 64 / 66 / 128 (tensor-memory kernels) need chunk_steps = 0, at most two factors "
-                "per reaction side, 1..128 (33) or 1..256 (64, 66, 128) reversible reactions, at most 32 (33) or 64 species "
+    if ((kind == 1 && !pk1_ok) || (kind == 2 && !pk2_ok) || (kind == 3 && !ab_ok) || (kind == 4 && !pk4_ok) ||
+        (kind == 5 && !pk3_ok)) {
+      set_error("stev_integrate: lanes_per_cell = 33 / 64 / 66 / 96 / 128 (tensor-memory kernels) need chunk_steps = 0, at most two factors "
+                "per reaction side, 1..128 (33) or 1..256 (64, 66, 96, 128) reversible reactions, at most 32 (33) or 64 species "
                 "(66 also dft_enable = 1)");
       return STEV_EINVAL;
     }
@@ -670,7 +674,7 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
                                  make_consts(p), dt_cfd, n, ld, T, pressure, Y, steps_out, status_out, w.counters, s, &blocks, &cpb,
                                  &smem);
       } else {
-        const int wi = (kind == 4) ? 2 : kind - 1;
+        const int wi = (kind == 4) ? 2 : (kind == 5 ? 3 : kind - 1);
         rc = integrate_pk_launch(est ? est->pk_tb[wi] : m->pk_tb[wi], est ? est->pk_cl[wi] : m->pk_cl[wi],
                                  est ? est->d_pk_table[wi] : m->d_pk_table[wi], make_consts(p), dt_cfd, n, ld, T, pressure, Y,
                                  steps_out, status_out, w.counters, s, &blocks, &cpb, &smem);
@@ -683,8 +687,8 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
       g_stats.passes = 1;
       g_stats.kernel_launches = 1;
       g_stats.blocks = blocks;
-      g_stats.lanes_per_cell = kind == 1 ? 33 : (kind == 2 ? 64 : (kind == 3 ? 66 : 128));
-      g_stats.threads_per_block = kind == 3 ? kAbThreads : (kind == 4 ? kPkThreads4 : kPkThreads);
+      g_stats.lanes_per_cell = kind == 1 ? 33 : (kind == 2 ? 64 : (kind == 3 ? 66 : (kind == 4 ? 128 : 96)));
+      g_stats.threads_per_block = kind == 3 ? kAbThreads : (kind == 4 ? kPkThreads4 : (kind == 5 ? kPkThreads3 : kPkThreads));
       g_stats.cells_per_block = cpb;
       g_stats.smem_bytes = (int64_t)smem;
       if (worst == 2) { set_error("some cells produced non-finite values (status 2)"); return STEV_WNONFINITE; }

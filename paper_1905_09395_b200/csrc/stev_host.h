@@ -81,10 +81,10 @@ struct stev_mechanism {
   stev::AbTables ab_tb{};
   stev::AbCell ab_cl{};
   unsigned char *d_ab_table = nullptr;
-  bool pk_ok[3] = {false, false, false}; // images of the tensor-memory kernel: [0] one warp per cell, [1] warp pair, [2] warp quad (NASA-7 thermo)
-  stev::PkTables pk_tb[3]{};
-  stev::PkCell pk_cl[3]{};
-  unsigned char *d_pk_table[3] = {nullptr, nullptr, nullptr};
+  bool pk_ok[4] = {false, false, false, false};   // images of the tensor-memory kernel: [0] one warp per cell, [1] pair, [2] quad, [3] triple (NASA-7 thermo)
+  stev::PkTables pk_tb[4]{};
+  stev::PkCell pk_cl[4]{};
+  unsigned char *d_pk_table[4] = {nullptr, nullptr, nullptr, nullptr};
 };
 
 struct stev_estimator {
@@ -96,10 +96,10 @@ struct stev_estimator {
   stev::AbTables ab_tb{};
   stev::AbCell ab_cl{};
   unsigned char *d_ab_table = nullptr;
-  bool pk_ok[3] = {false, false, false}; // images of the tensor-memory kernel (MLP thermo)
-  stev::PkTables pk_tb[3]{};
-  stev::PkCell pk_cl[3]{};
-  unsigned char *d_pk_table[3] = {nullptr, nullptr, nullptr};
+  bool pk_ok[4] = {false, false, false, false};   // images of the tensor-memory kernel (MLP thermo)
+  stev::PkTables pk_tb[4]{};
+  stev::PkCell pk_cl[4]{};
+  unsigned char *d_pk_table[4] = {nullptr, nullptr, nullptr, nullptr};
   // standalone evaluation (stev_estimator_eval): device copies in kernel-friendly layouts
   float *d_params = nullptr;             // in_shift, in_scale, W1T [n_in][H], b1, W2T [H][n_out], b2
   size_t params_floats = 0;

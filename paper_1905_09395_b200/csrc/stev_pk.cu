@@ -49,7 +49,7 @@ static void pk_layout(const PkTables &tb, PkCell &cl) {
 
 bool build_pk_image(const HostMechanism &m, const HostEstimator *e, int nw, std::vector<unsigned char> &image, PkTables &tb,
                     PkCell &cl) {
-  if ((nw != 1 && nw != 2 && nw != 4) || !pk_mechanism_ok(m, nw)) return false;
+  if (nw < 1 || nw > 4 || !pk_mechanism_ok(m, nw)) return false;
   const int S = m.S, R = m.R, Rrev = m.Rrev;
   tb = PkTables{};
   tb.S = S;
@@ -66,7 +66,10 @@ bool build_pk_image(const HostMechanism &m, const HostEstimator *e, int nw, std:
     int cnt = 0;
     if (nw == 1) cnt = (h == 0) ? tb.n_it : 0;
     else if (nw == 2) cnt = (h == 0) ? tb.n_it / 2 : (h == 1 ? tb.n_it - tb.n_it / 2 : 0);
-    else cnt = (h == 2) ? tb.n_it / 2 : (h == 3 ? tb.n_it - tb.n_it / 2 : 0);   // the filter runs on warps 2 and 3
+    else if (nw == 3) {   // warp 2 only filters (the larger half); warp 0 also has the update and the scalars: smallest share
+      const int k2 = (tb.n_it + 1) / 2, k0 = (tb.n_it - k2) / 3;
+      cnt = (h == 2) ? k2 : (h == 0 ? k0 : (h == 1 ? tb.n_it - k2 - k0 : 0));
+    } else cnt = (h == 2) ? tb.n_it / 2 : (h == 3 ? tb.n_it - tb.n_it / 2 : 0);   // the filter runs on warps 2 and 3
     tb.it_split[h + 1] = tb.it_split[h] + cnt;
   }
   if (e) {
@@ -118,7 +121,7 @@ bool build_pk_image(const HostMechanism &m, const HostEstimator *e, int nw, std:
   std::memset(gsp, 255, sizeof(gsp));
   std::memset(glen, 0, sizeof(glen));
   int g_len[kPkMaxNw] = {0, 0, 0, 0};
-  const int g_short = (nw == 4) ? 2 : 0, g_long = (nw == 4) ? 3 : 1;
+  const int g_short = (nw == 4) ? 2 : (nw == 3 ? 2 : 0), g_long = (nw == 4) ? 3 : 1;
   for (int n = 0; n < S; ++n) {
     const int group = n / 16;
     const int half = (nw >= 2) ? (group < 2 ? g_long : g_short) : 0, lane = (nw >= 2) ? (group & 1) * 16 + n % 16 : n;
@@ -366,8 +369,10 @@ int integrate_pk_launch(const PkTables &tb, const PkCell &cl, const unsigned cha
   a.cells_per_block = pk_cells_per_block(tb, cl);
   if (a.cells_per_block < 1) { set_error("pair kernel: shared memory too small"); return STEV_EINVAL; }
   const size_t smem = (size_t)tb.bytes + (size_t)a.cells_per_block * cl.stride;
-  void *fn = (tb.nw == 4) ? (void *)stev_pk_kernel<4> : ((tb.nw == 2) ? (void *)stev_pk_kernel<2> : (void *)stev_pk_kernel<1>);
-  const int threads = (tb.nw == 4) ? kPkThreads4 : kPkThreads;
+  void *fn = (tb.nw == 4) ? (void *)stev_pk_kernel<4>
+             : (tb.nw == 3) ? (void *)stev_pk_kernel<3>
+             : (tb.nw == 2) ? (void *)stev_pk_kernel<2> : (void *)stev_pk_kernel<1>;
+  const int threads = (tb.nw == 4) ? kPkThreads4 : (tb.nw == 3 ? kPkThreads3 : kPkThreads);
   STEV_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   const long long blocks = std::min<long long>(device_sm_count(), (n + a.cells_per_block - 1) / a.cells_per_block);
   void *args[] = {&a};

@@ -323,6 +323,14 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
     for (int jj = 0; jj < j; ++jj) rank += (((tmem_quarter + jj) & 3) >= 2) ? 1 : 0;
     tcol = (uint32_t)(rank * 128);
   }
+  if (NW == 3) {
+    // Triple: warp 3 j + h; the warps of one quarter hold every role twice, so the quarter's 512 columns are exactly
+    // the sum of their shares.  Columns start after the shares of the earlier warps of the same quarter.
+    const int w_me = 3 * j + half;
+    int cols = 0;
+    for (int w = (w_me & 3); w < w_me; w += 4) cols += 32 * (tb.it_split[w % 3 + 1] - tb.it_split[w % 3]);
+    tcol = (uint32_t)cols;
+  }
   const uint32_t trow = tmem_base + ((uint32_t)((tmem_quarter & 3) * 32) << 16) + tcol - (uint32_t)(it_lo * 32);
   const int my_sp = (half < 2) ? half * 32 + lane : 0x7fff;   // species this lane loads, updates and writes back
   const int g_sp = gsp[half * 32 + lane];       // species whose source term this lane gathers (255 = none)
@@ -335,14 +343,15 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
     cG[0] = 0.0;
   }
   // a5 for this warp's blocks: h_s and ictot_s are the step size and 1/C_tot of the step whose progress is stored
-  auto run_dft = [&](int slot_s, double h_s, double ictot_s) {
+  constexpr bool kPairWin = (NW <= 2);   // two windows side by side need ~125 registers
+  auto run_dft = [&](int slot_s, double h_s, double ictot_s) __attribute__((always_inline)) {
     switch (sc.nhf) {
-      case 1: pk_dft<1, NW != 4>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot_s, h_s, ictot_s, lane); break;
-      case 2: pk_dft<2, NW != 4>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot_s, h_s, ictot_s, lane); break;
-      case 3: pk_dft<3, NW != 4>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot_s, h_s, ictot_s, lane); break;
-      case 4: pk_dft<4, NW != 4>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot_s, h_s, ictot_s, lane); break;
-      case 5: pk_dft<5, NW != 4>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot_s, h_s, ictot_s, lane); break;
-      default: pk_dft<6, NW != 4>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot_s, h_s, ictot_s, lane); break;
+      case 1: pk_dft<1, kPairWin>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot_s, h_s, ictot_s, lane); break;
+      case 2: pk_dft<2, kPairWin>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot_s, h_s, ictot_s, lane); break;
+      case 3: pk_dft<3, kPairWin>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot_s, h_s, ictot_s, lane); break;
+      case 4: pk_dft<4, kPairWin>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot_s, h_s, ictot_s, lane); break;
+      case 5: pk_dft<5, kPairWin>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot_s, h_s, ictot_s, lane); break;
+      default: pk_dft<6, kPairWin>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot_s, h_s, ictot_s, lane); break;
     }
   };
   // Pair: second named barrier of the cell (ids 9..15, and 0 -- free after the block-wide start-up -- for cell 7).
@@ -428,7 +437,7 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
           }
         }
       }
-      if (NW == 2 && half == 0 && steps > 0 && sc.dft_enable) {
+      if ((NW == 2 || NW == 3) && half == 0 && steps > 0 && sc.dft_enable) {
         // warp 0 of the pair: its share of the ringing filter of the PREVIOUS step (it only feeds rOF, which phase B
         // reads), after the scalars of this step, so that no barrier separates the update from phase A
         run_dft(slot, h_prev, ictot_prev);
@@ -445,7 +454,7 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
         } else {
           pk_nasa<true>(tb, tbl, cG, cYwCp, cHOm, T, invT1, ab_log(T), lane);
         }
-      } else if (NW == 4 && half >= 2) {
+      } else if ((NW == 4 || NW == 3) && half >= 2) {
         // warps 2 and 3 of the quad: the ringing filter of the PREVIOUS step (it only feeds rOF, which phase B reads),
         // concurrently with the scalars and the thermodynamics of this step on warps 0 and 1
         if (steps > 0 && sc.dft_enable) {
@@ -472,12 +481,18 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
       if (NW < 4 && n_it > 2 * NW) {
         for (int b0 = half; b0 < n_it; b0 += 4 * NW)
           pk_rev_batch<4>(cell, rkA, rkB, rfac, rdg, cRof, cQ, Rp, Rrev, has2, invT, lnT, ln_c0, b0, NW, lane);
+      } else if (NW == 3) {
+        int b0 = half;
+        for (; b0 + NW < n_it; b0 += 2 * NW)
+          pk_rev_batch<2>(cell, rkA, rkB, rfac, rdg, cRof, cQ, Rp, Rrev, has2, invT, lnT, ln_c0, b0, NW, lane);
+        for (; b0 < n_it; b0 += NW)
+          pk_rev_batch<1>(cell, rkA, rkB, rfac, rdg, cRof, cQ, Rp, Rrev, has2, invT, lnT, ln_c0, b0, NW, lane);
       } else {
         for (int b0 = half; b0 < n_it; b0 += 2 * NW)
           pk_rev_batch<2>(cell, rkA, rkB, rfac, rdg, cRof, cQ, Rp, Rrev, has2, invT, lnT, ln_c0, b0, NW, lane);
       }
       // irreversible reactions [Rrev, R): 32-blocks c = half (mod NW), two at a time (quad: one)
-      constexpr int IU = (NW == 4) ? 1 : 2;
+      constexpr int IU = (NW >= 3) ? 1 : 2;
       for (int k0 = Rrev + half * 32; k0 < R; k0 += 32 * IU * NW) {
         double lk[IU], fw[IU];
         uint4 f[IU];
@@ -525,7 +540,7 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
       // ================= phase C: source terms and the limiter (Eqs 1-3) =================
       // One species per lane; the entry lists hold the byte offsets of the stored multiples in the caller's reaction
       // order and are padded with the 0.0 slot to the longest list of the warp, so the loop is warp-uniform.
-      if (NW < 4 || g_len4 > 0) {
+      if (NW < 3 || g_len4 > 0) {
         const double inv_rho = 1.0 / rho;
         double om = 0.0;
         // Two rows of four entries per trip: the eight loads of a trip are independent and the offsets of the next
@@ -575,6 +590,7 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
       // -- a3: step size (Eq 5) and landing on t_f (R5)
       double t_star = scal->t_star[0];
       if (NW >= 2) t_star = pk_min_bits(t_star, scal->t_star[1]);
+      if (NW == 3) t_star = pk_min_bits(t_star, scal->t_star[2]);
       if (NW == 4) t_star = pk_min_bits(t_star, pk_min_bits(scal->t_star[2], scal->t_star[3]));
       double h = (t_star < dt_max) ? t_star : dt_max;
       bool last = false;
@@ -586,7 +602,7 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
       // -- a4: forward Euler (Eq 18), one species per lane (pair: warp 0 updates all species, two per lane,
       //    so that it depends on nothing of warp 1 between here and the end of phase A)
       int bad = 0;
-      if (NW == 2) {
+      if (NW == 2 || NW == 3) {
         if (half == 0) {
 #pragma unroll
           for (int u = 0; u < 2; ++u) {
@@ -622,18 +638,21 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
       bad = __any_sync(0xffffffffu, bad);
       if (lane == 0 && half < 2) scal->bad[half] = bad;
       PKT(6)
-      if (NW == 2) {
+      if (NW == 2 || NW == 3) {
         // -- a5 on warp 1 now (skipped on the landing step: the cell retires); warp 0 runs its share after the scalars of
         //    the next step.  Warp 0 announces the new T and Y (bar.arrive), warp 1 waits for them (bar.sync).
+        //    (triple: warp 2 waits first and filters at the top of the next step, like warps 2-3 of the quad)
         if (half == 0) {
           __threadfence_block();
-          asm volatile("bar.arrive %0, 64;" ::"r"(xbar) : "memory");
+          if (NW == 3) asm volatile("bar.arrive %0, 96;" ::"r"(xbar) : "memory");
+          else asm volatile("bar.arrive %0, 64;" ::"r"(xbar) : "memory");
         } else {
-          if (!last && sc.dft_enable) {
+          if ((NW == 2 || half == 1) && !last && sc.dft_enable) {
             run_dft(slot, h, inv_ctot);
             slot = (slot + 1 == kWindow) ? 0 : slot + 1;
           }
-          asm volatile("bar.sync %0, 64;" ::"r"(xbar) : "memory");
+          if (NW == 3) asm volatile("bar.sync %0, 96;" ::"r"(xbar) : "memory");
+          else asm volatile("bar.sync %0, 64;" ::"r"(xbar) : "memory");
           T = scal->T_new;
         }
       } else {
@@ -679,7 +698,7 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
 }
 
 template <int NW>
-__global__ void __launch_bounds__((NW == 4) ? kPkThreads4 : kPkThreads, 1) stev_pk_kernel(const __grid_constant__ PkArgs a) {
+__global__ void __launch_bounds__((NW == 4) ? kPkThreads4 : (NW == 3 ? kPkThreads3 : kPkThreads), 1) stev_pk_kernel(const __grid_constant__ PkArgs a) {
   extern __shared__ __align__(128) unsigned char smem[];
   __shared__ unsigned long long mbar;
   __shared__ uint32_t tmem_base_s;
@@ -703,8 +722,9 @@ __global__ void __launch_bounds__((NW == 4) ? kPkThreads4 : kPkThreads, 1) stev_
   // then interleaves four cells in four different phases (fp64-bound DFT against latency-bound gather and rates).
   // NW = 4: warps 4 j .. 4 j + 3 serve cell slot j, one per scheduler and TMEM lane quarter; the role rotates with j, so
   // every scheduler holds two warps of each role (the scalar chains, NASA-7, the two estimator halves).
-  const int half = (NW == 4) ? (((warp & 3) + (warp >> 2)) & 3) : ((NW == 2) ? (warp >> 3) : 0);
-  const int j = (NW == 4) ? (warp >> 2) : ((NW == 2) ? (half ? ((warp - 8 + 7) & 7) : warp) : warp);
+  // NW = 3: warps 3 j .. 3 j + 2 serve cell slot j (consecutive warps: three different schedulers).
+  const int half = (NW == 4) ? (((warp & 3) + (warp >> 2)) & 3) : (NW == 3 ? warp % 3 : ((NW == 2) ? (warp >> 3) : 0));
+  const int j = (NW == 4) ? (warp >> 2) : (NW == 3 ? warp / 3 : ((NW == 2) ? (half ? ((warp - 8 + 7) & 7) : warp) : warp));
   if (j < a.cells_per_block) {
     unsigned char *cell = smem + a.tb.bytes + (size_t)j * a.cl.stride;
     if (a.tb.has_est) pk_worker<true, NW>(a, smem, cell, j, half, warp & 3, tmem_base, lane);

@@ -188,11 +188,12 @@ def test_result_does_not_depend_on_lanes_per_cell(stev, oracle, config, n, lanes
                                            (1, 100, dict(max_steps=150)), (2, 100, dict(alpha=0.0, dft_first_high_bin=1)),
                                            (2, 100, dict(energy_mode=1, delta_max=0.002, y_step_max=0.05)),
                                            (1, 100, dict(dft_enable=0, max_steps=3000))])
-@pytest.mark.parametrize("kernel", [33, 64, 66, 128])
+@pytest.mark.parametrize("kernel", [33, 64, 66, 96, 128])
 def test_tensor_memory_kernels_parity(stev, oracle, kernel, config, n, over):
     """lanes_per_cell = 33: one warp per cell (stev_pk_kernel.cuh, NW = 1), the default for small and mid-size mechanisms;
     lanes_per_cell = 64: the warp-pair kernel (stev_pk_kernel.cuh, NW = 2), the default for large mechanisms (config 3);
     lanes_per_cell = 66: the rate-warp / DFT-warp kernel (stev_ab_kernel.cuh);
+    lanes_per_cell = 96: the warp-triple kernel (stev_pk_kernel.cuh, NW = 3, 24 warps of 80 registers per SM);
     lanes_per_cell = 128: the warp-quad kernel (stev_pk_kernel.cuh, NW = 4, 32 warps of 64 registers per SM).  All keep the DFT history in tensor
     memory and are bit-exact against the oracle on every config they accept."""
     over = dict(over)
@@ -219,6 +220,8 @@ def test_tensor_memory_kernels_parity(stev, oracle, kernel, config, n, over):
                                                  (3, 64, 128), (3, 64, 129), (3, 64, 193), (3, 64, 224), (3, 66, 33),
                                                  (3, 128, 1), (3, 128, 33), (3, 128, 64), (3, 128, 97), (3, 128, 129), (3, 128, 161),
                                                  (3, 128, 193), (3, 128, 224), (2, 128, 33),
+                                                 (3, 96, 1), (3, 96, 33), (3, 96, 64), (3, 96, 97), (3, 96, 129), (3, 96, 161),
+                                                 (3, 96, 193), (3, 96, 224), (2, 96, 33),
                                                  (2, 33, 1), (2, 33, 31), (2, 33, 32), (2, 33, 33), (2, 64, 33), (1, 33, 1)])
 def test_tensor_memory_kernels_block_boundaries(stev, oracle, config, kernel, n_rev):
     """The tensor-memory kernels walk the reversible reactions in 32-blocks split over the warps of a cell; this runs
