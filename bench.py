@@ -338,6 +338,7 @@ def main():
     peak_instr = workmodel.fp64_peak_instr_per_s(sm_max)
     peak_tflops = 2.0 * peak_instr / 1e12
     kernel_name = {33: "stev_pk_kernel<1> (one warp per cell, DFT history in tensor memory)",
+                   34: "stev_pk_kernel<1, dense> (one warp per cell, 32 cells per SM, DFT history in tensor memory)",
                    64: "stev_pk_kernel<2> (warp pair per cell, DFT history in tensor memory)",
                    66: "stev_ab_kernel (rate warp + DFT warp per cell)",
                    96: "stev_pk_kernel<3> (warp triple per cell, DFT history in tensor memory)",

@@ -113,6 +113,7 @@ typedef struct {
                              shared memory (any mechanism, any chunk_steps).  Kernels that keep the DFT history in tensor
                              memory (need chunk_steps = 0, at most two factors per reaction side):
                              33 = one warp per cell, 16 cells per SM (<= 32 species, 1..128 reversible reactions);
+                             34 = the same at 64 registers, 32 cells per SM (<= 32 species, 1..64 reversible reactions);
                              64 = a warp pair per cell, 8 cells per SM, both warps split every phase of a step
                                   (<= 64 species, 1..256 reversible reactions; the default for >= 128 reactions);
                              66 = warp-specialised variant of 64 (a rate warp + a DFT warp; also needs dft_enable);

@@ -644,6 +644,7 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
   //   lanes_per_cell = 66: warp-specialised kernel (a rate warp and a DFT warp per cell)
   //   lanes_per_cell = 128: warp quad per cell, 8 cells per SM, 32 warps of 64 registers per SM
   //   lanes_per_cell = 96: warp triple per cell, 8 cells per SM, 24 warps of 80 registers per SM
+  int g_request = p->lanes_per_cell;   // group width handed to the shared-memory-history kernel (0: its own heuristic)
   {
     const bool tm_common = p->chunk_steps == 0;
     const bool pk1_ok = (est ? est->pk_ok[0] : m->pk_ok[0]) && tm_common;
@@ -651,15 +652,29 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
     const bool pk4_ok = (est ? est->pk_ok[2] : m->pk_ok[2]) && tm_common;
     const bool pk3_ok = (est ? est->pk_ok[3] : m->pk_ok[3]) && tm_common;
     const bool ab_ok = (est ? est->ab_ok : m->ab_ok) && p->dft_enable && tm_common;
-    int kind = 0;   // 1: one warp per cell, 2: warp pair, 3: warp-specialised, 4: warp quad, 5: warp triple
+    int kind = 0;   // 0: sub-warp groups (history in shared memory), 1: one warp per cell, 2: warp pair, 3: warp-specialised, 4: warp quad, 5: warp triple
     if (p->lanes_per_cell == 33) kind = 1;
     else if (p->lanes_per_cell == 64) kind = 2;
     else if (p->lanes_per_cell == 66) kind = 3;
     else if (p->lanes_per_cell == 128) kind = 4;
     else if (p->lanes_per_cell == 96) kind = 5;
-    else if (p->lanes_per_cell == 0) kind = (tb->R >= 128 && pk2_ok) ? 2 : (pk1_ok ? 1 : (pk2_ok && tb->R >= 64 ? 2 : 0));
+    else if (p->lanes_per_cell == 34) kind = 6;   // one warp per cell, dense (32 cells per SM at 64 registers)
+    else if (p->lanes_per_cell == 0) {
+      // Measured on B200: large mechanisms -> warp pair; tiny ones (a step is a few hundred
+      // instructions, most lanes of a warp idle) -> sub-warp groups with the history in shared memory; mid-size -> one
+      // warp per cell, 32 cells per SM when the reversible reactions fit two 32-blocks, else 16.
+      const bool dense_ok = pk1_ok && pk_dense_ok(est ? est->pk_tb[0] : m->pk_tb[0]);
+      if (tb->R >= 128 && pk2_ok) kind = 2;
+      else if (tb->S <= 16 && tb->R <= 32) {
+        kind = 0;
+        g_request = 4;
+        while (g_request < tb->S) g_request *= 2;
+      } else if (dense_ok) kind = 6;
+      else if (pk1_ok) kind = 1;
+      else if (pk2_ok && tb->R >= 64) kind = 2;
+    }
     if ((kind == 1 && !pk1_ok) || (kind == 2 && !pk2_ok) || (kind == 3 && !ab_ok) || (kind == 4 && !pk4_ok) ||
-        (kind == 5 && !pk3_ok)) {
+        (kind == 5 && !pk3_ok) || (kind == 6 && !(pk1_ok && pk_dense_ok(est ? est->pk_tb[0] : m->pk_tb[0])))) {
       set_error("stev_integrate: lanes_per_cell = 33 / 64 / 66 / 96 / 128 (tensor-memory kernels) need chunk_steps = 0, at most two factors "
                 "per reaction side, 1..128 (33) or 1..256 (64, 66, 96, 128) reversible reactions, at most 32 (33) or 64 species "
                 "(66 also dft_enable = 1)");
@@ -674,10 +689,10 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
                                  make_consts(p), dt_cfd, n, ld, T, pressure, Y, steps_out, status_out, w.counters, s, &blocks, &cpb,
                                  &smem);
       } else {
-        const int wi = (kind == 4) ? 2 : (kind == 5 ? 3 : kind - 1);
+        const int wi = (kind == 4) ? 2 : (kind == 5 ? 3 : (kind == 6 ? 0 : kind - 1));
         rc = integrate_pk_launch(est ? est->pk_tb[wi] : m->pk_tb[wi], est ? est->pk_cl[wi] : m->pk_cl[wi],
                                  est ? est->d_pk_table[wi] : m->d_pk_table[wi], make_consts(p), dt_cfd, n, ld, T, pressure, Y,
-                                 steps_out, status_out, w.counters, s, &blocks, &cpb, &smem);
+                                 steps_out, status_out, w.counters, s, &blocks, &cpb, &smem, kind == 6);
       }
       if (rc) return rc;
       int worst = 0;
@@ -687,8 +702,9 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
       g_stats.passes = 1;
       g_stats.kernel_launches = 1;
       g_stats.blocks = blocks;
-      g_stats.lanes_per_cell = kind == 1 ? 33 : (kind == 2 ? 64 : (kind == 3 ? 66 : (kind == 4 ? 128 : 96)));
-      g_stats.threads_per_block = kind == 3 ? kAbThreads : (kind == 4 ? kPkThreads4 : (kind == 5 ? kPkThreads3 : kPkThreads));
+      g_stats.lanes_per_cell = kind == 1 ? 33 : (kind == 2 ? 64 : (kind == 3 ? 66 : (kind == 4 ? 128 : (kind == 5 ? 96 : 34))));
+      g_stats.threads_per_block =
+          kind == 3 ? kAbThreads : ((kind == 4 || kind == 6) ? kPkThreads4 : (kind == 5 ? kPkThreads3 : kPkThreads));
       g_stats.cells_per_block = cpb;
       g_stats.smem_bytes = (int64_t)smem;
       if (worst == 2) { set_error("some cells produced non-finite values (status 2)"); return STEV_WNONFINITE; }
@@ -698,7 +714,7 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
   }
 
   LaunchConfig cfg;
-  if (!choose_config(*tb, p->lanes_per_cell, cfg)) {
+  if (!choose_config(*tb, g_request, cfg) && !(p->lanes_per_cell == 0 && choose_config(*tb, 0, cfg))) {
     set_error("stev_integrate: no launch configuration fits shared memory for this mechanism / lanes_per_cell");
     return STEV_EINVAL;
   }

@@ -69,7 +69,9 @@ bool build_pk_image(const HostMechanism &m, const HostEstimator *e, int nw, std:
                     PkCell &cl);
 int integrate_pk_launch(const PkTables &tb, const PkCell &cl, const unsigned char *d_table, const SolverConsts &sc, double t_f,
                         long long n, long long ld, double *T, const double *p, double *Y, int *steps, unsigned char *status,
-                        int *counters, cudaStream_t s, int *blocks_out, int *cells_per_block_out, size_t *smem_out);
+                        int *counters, cudaStream_t s, int *blocks_out, int *cells_per_block_out, size_t *smem_out,
+                        bool dense = false);
+bool pk_dense_ok(const PkTables &tb);
 
 }  // namespace stev
 

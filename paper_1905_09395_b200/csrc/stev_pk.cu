@@ -342,14 +342,19 @@ bool build_pk_image(const HostMechanism &m, const HostEstimator *e, int nw, std:
   return true;
 }
 
-int pk_cells_per_block(const PkTables &tb, const PkCell &cl) {
+// dense (one warp per cell only): 32 cells per block at 64 registers; needs at most two 32-blocks of reversible reactions
+bool pk_dense_ok(const PkTables &tb) { return tb.nw == 1 && tb.n_it <= 2; }
+
+int pk_cells_per_block(const PkTables &tb, const PkCell &cl, bool dense) {
   const size_t avail = kSmemMax - (size_t)tb.bytes - 256;
-  return (int)std::min<size_t>(tb.nw == 1 ? 2 * kPkMaxCells : kPkMaxCells, avail / (size_t)cl.stride);
+  const int cap = dense ? 4 * kPkMaxCells : (tb.nw == 1 ? 2 * kPkMaxCells : kPkMaxCells);
+  return (int)std::min<size_t>(cap, avail / (size_t)cl.stride);
 }
 
 int integrate_pk_launch(const PkTables &tb, const PkCell &cl, const unsigned char *d_table, const SolverConsts &sc, double t_f,
                         long long n, long long ld, double *T, const double *p, double *Y, int *steps, unsigned char *status,
-                        int *counters, cudaStream_t s, int *blocks_out, int *cells_per_block_out, size_t *smem_out) {
+                        int *counters, cudaStream_t s, int *blocks_out, int *cells_per_block_out, size_t *smem_out, bool dense) {
+  if (dense && !pk_dense_ok(tb)) { set_error("dense tensor-memory kernel: more than 64 reversible reactions"); return STEV_EINVAL; }
   PkArgs a{};
   a.tb = tb;
   a.table = d_table;
@@ -366,13 +371,14 @@ int integrate_pk_launch(const PkTables &tb, const PkCell &cl, const unsigned cha
   a.status = status;
   a.queue_head = counters;
   a.worst_status = counters + 1;
-  a.cells_per_block = pk_cells_per_block(tb, cl);
+  a.cells_per_block = pk_cells_per_block(tb, cl, dense);
   if (a.cells_per_block < 1) { set_error("pair kernel: shared memory too small"); return STEV_EINVAL; }
   const size_t smem = (size_t)tb.bytes + (size_t)a.cells_per_block * cl.stride;
-  void *fn = (tb.nw == 4) ? (void *)stev_pk_kernel<4>
+  void *fn = dense ? (void *)stev_pk_kernel<1, true>
+             : (tb.nw == 4) ? (void *)stev_pk_kernel<4>
              : (tb.nw == 3) ? (void *)stev_pk_kernel<3>
              : (tb.nw == 2) ? (void *)stev_pk_kernel<2> : (void *)stev_pk_kernel<1>;
-  const int threads = (tb.nw == 4) ? kPkThreads4 : (tb.nw == 3 ? kPkThreads3 : kPkThreads);
+  const int threads = (tb.nw == 4 || dense) ? kPkThreads4 : (tb.nw == 3 ? kPkThreads3 : kPkThreads);
   STEV_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   const long long blocks = std::min<long long>(device_sm_count(), (n + a.cells_per_block - 1) / a.cells_per_block);
   void *args[] = {&a};

@@ -282,7 +282,7 @@ __shared__ long long pk_tacc[32][8];
 #define PKT(i)
 #endif
 
-template <bool EST, int NW>
+template <bool EST, int NW, bool DENSE>
 __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *tbl, unsigned char *cell, int j, int half,
                                           int tmem_quarter, uint32_t tmem_base, int lane) {
   const PkTables &tb = a.tb;
@@ -317,7 +317,8 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
   // Quad: the four warps of cell j sit in the four quarters; warps 2 and 3 keep four blocks each, and since the role
   // rotates with j every quarter holds four such warps: columns [128 rank, +128), rank = earlier cells with a filter
   // warp in this quarter.
-  uint32_t tcol = (uint32_t)((j >> 2) * 128 + half * 256);
+  // (one warp per cell, dense: 32 cells per block, at most two blocks = 64 columns per cell)
+  uint32_t tcol = DENSE ? (uint32_t)((j >> 2) * 64) : (uint32_t)((j >> 2) * 128 + half * 256);
   if (NW == 4) {
     int rank = 0;
     for (int jj = 0; jj < j; ++jj) rank += (((tmem_quarter + jj) & 3) >= 2) ? 1 : 0;
@@ -343,7 +344,7 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
     cG[0] = 0.0;
   }
   // a5 for this warp's blocks: h_s and ictot_s are the step size and 1/C_tot of the step whose progress is stored
-  constexpr bool kPairWin = (NW <= 2);   // two windows side by side need ~125 registers
+  constexpr bool kPairWin = (NW <= 2) && !DENSE;   // two windows side by side need ~125 registers
   auto run_dft = [&](int slot_s, double h_s, double ictot_s) __attribute__((always_inline)) {
     switch (sc.nhf) {
       case 1: pk_dft<1, kPairWin>(sc, cQ, cRof, Rrev, it_lo, it_hi, trow, slot_s, h_s, ictot_s, lane); break;
@@ -478,7 +479,7 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
       // warp and are evaluated four (small mechanisms: two) at a time, i.e. eight independent exp chains and one trip
       // through the load -> exp -> load -> store latency chain.  The stored multiples +q, -q, +2q, -2q (all exact) turn the sum
       // omega_i = sum_j nu_ij q_j into plain additions in the contract's order.
-      if (NW < 4 && n_it > 2 * NW) {
+      if (NW < 3 && !DENSE && n_it > 2 * NW) {
         for (int b0 = half; b0 < n_it; b0 += 4 * NW)
           pk_rev_batch<4>(cell, rkA, rkB, rfac, rdg, cRof, cQ, Rp, Rrev, has2, invT, lnT, ln_c0, b0, NW, lane);
       } else if (NW == 3) {
@@ -697,8 +698,8 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
   }
 }
 
-template <int NW>
-__global__ void __launch_bounds__((NW == 4) ? kPkThreads4 : (NW == 3 ? kPkThreads3 : kPkThreads), 1) stev_pk_kernel(const __grid_constant__ PkArgs a) {
+template <int NW, bool DENSE = false>
+__global__ void __launch_bounds__((NW == 4 || DENSE) ? kPkThreads4 : (NW == 3 ? kPkThreads3 : kPkThreads), 1) stev_pk_kernel(const __grid_constant__ PkArgs a) {
   extern __shared__ __align__(128) unsigned char smem[];
   __shared__ unsigned long long mbar;
   __shared__ uint32_t tmem_base_s;
@@ -727,8 +728,8 @@ __global__ void __launch_bounds__((NW == 4) ? kPkThreads4 : (NW == 3 ? kPkThread
   const int j = (NW == 4) ? (warp >> 2) : (NW == 3 ? warp / 3 : ((NW == 2) ? (half ? ((warp - 8 + 7) & 7) : warp) : warp));
   if (j < a.cells_per_block) {
     unsigned char *cell = smem + a.tb.bytes + (size_t)j * a.cl.stride;
-    if (a.tb.has_est) pk_worker<true, NW>(a, smem, cell, j, half, warp & 3, tmem_base, lane);
-    else pk_worker<false, NW>(a, smem, cell, j, half, warp & 3, tmem_base, lane);
+    if (a.tb.has_est) pk_worker<true, NW, DENSE>(a, smem, cell, j, half, warp & 3, tmem_base, lane);
+    else pk_worker<false, NW, DENSE>(a, smem, cell, j, half, warp & 3, tmem_base, lane);
   }
   __syncwarp();
   if (lane == 0) atomicAdd(&done_warps, 1);
