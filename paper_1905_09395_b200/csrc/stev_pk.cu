@@ -40,7 +40,7 @@ static void pk_layout(const PkTables &tb, PkCell &cl) {
   cl.oG = take(8 * (1 + 2 * tb.S));
   cl.oQ = take(8 * tb.n_var * tb.Rp);
   cl.oRof = take(8 * tb.Rrev);
-  cl.oHid = take(4 * (tb.has_est ? tb.H : 0));
+  cl.oHid = take(4 * (tb.has_est ? tb.H + align_up(tb.n_in, 4) : 0));   // hidden activations, then the normalised inputs
   cl.oSc = take((int)sizeof(PkScal));
   // an odd multiple of 16 bytes keeps the cells of different pairs on different bank groups for the broadcast loads
   cl.stride = align_up(o, 16);

@@ -75,18 +75,34 @@ __device__ __forceinline__ void pk_mlp(const PkTables &tb, const unsigned char *
   const float *W1T = (const float *)(tbl + tb.o_W1T), *b1 = (const float *)(tbl + tb.o_b1);
   const float *W2p = (const float *)(tbl + tb.o_W2p), *b2 = (const float *)(tbl + tb.o_b2);
   const int H = tb.H, Hpad = tb.Hpad, n_in = tb.n_in;
-  for (int jh = lane; jh < H; jh += 32) {
-    float z = b1[jh];
-    for (int k = 0; k < n_in; ++k) {
-      const double raw = (k == 0) ? T : ((k == 1) ? p : cYp[k - 2].x);
-      const float xk = ((float)raw - eshift[k]) * escale[k];
-      z = __fmaf_rn(W1T[k * H + jh], xk, z);
-    }
+  // normalised inputs once (lane k: input k), then two hidden units per lane per pass; per unit the operations and
+  // their order are the contract's (fmaf over the inputs in index order)
+  float *cXn = cHid + H;
+  for (int k = lane; k < n_in; k += 32) {
+    const double raw = (k == 0) ? T : ((k == 1) ? p : cYp[k - 2].x);
+    cXn[k] = ((float)raw - eshift[k]) * escale[k];
+  }
+  __syncwarp();
+  auto activate = [&](float z) {
     const double zd = (double)z;
-    float act;
-    if (tb.act == 0) act = (float)(1.0 - 2.0 / (1.0 + ab_exp(2.0 * zd)));
-    else act = (float)(1.0 / (1.0 + ab_exp(-zd)));
-    cHid[jh] = act;
+    if (tb.act == 0) return (float)(1.0 - 2.0 / (1.0 + ab_exp(2.0 * zd)));
+    return (float)(1.0 / (1.0 + ab_exp(-zd)));
+  };
+  for (int jh0 = lane; jh0 < H; jh0 += 64) {
+    const int jh1_ = jh0 + 32;
+    const int jh1 = (jh1_ < H) ? jh1_ : jh0;
+    float z0 = b1[jh0], z1 = b1[jh1];
+    if (jh0 - lane + 32 < H) {   // warp-uniform: a second row of units exists
+      for (int k = 0; k < n_in; ++k) {
+        const float xk = cXn[k];
+        z0 = __fmaf_rn(W1T[k * H + jh0], xk, z0);
+        z1 = __fmaf_rn(W1T[k * H + jh1], xk, z1);
+      }
+    } else {
+      for (int k = 0; k < n_in; ++k) z0 = __fmaf_rn(W1T[k * H + jh0], cXn[k], z0);
+    }
+    cHid[jh0] = activate(z0);
+    if (jh1_ < H) cHid[jh1] = activate(z1);
   }
   __syncwarp();
   const float4 *hid4 = (const float4 *)cHid;
@@ -445,7 +461,11 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
         slot = (slot + 1 == kWindow) ? 0 : slot + 1;
       }
       if (NW == 1) {
-        if (EST) pk_mlp<4>(tb, tbl, cYp, cYwCp, cHOm, cHid, T, p, invT, lane, 0, tb.n_out);
+        if (EST) {
+          // outputs per lane per pass sized to the output layer (config 4 has 40 outputs: two per lane, not four)
+          if (tb.n_out <= 64) pk_mlp<2>(tb, tbl, cYp, cYwCp, cHOm, cHid, T, p, invT, lane, 0, tb.n_out);
+          else pk_mlp<4>(tb, tbl, cYp, cYwCp, cHOm, cHid, T, p, invT, lane, 0, tb.n_out);
+        }
       } else if (NW >= 2 && half == 1) {
         // warp 1 of the pair / quad: all of the thermodynamics (its own ln T and 1/T: same operations, same bits)
         const double invT1 = 1.0 / T;
