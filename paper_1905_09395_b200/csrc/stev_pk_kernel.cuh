@@ -64,6 +64,29 @@ __device__ __forceinline__ void pk_nasa(const PkTables &tb, const unsigned char 
   }
 }
 
+// The same with one species per lane (one warp per cell: at most 32 species, so the second slot would be idle).
+template <bool CPH>
+__device__ __forceinline__ void pk_nasa1(const PkTables &tb, const unsigned char *tbl, double *cG, double2 *cYwCp, double2 *cHOm,
+                                         double T, double invT, double lnT, int lane) {
+  const int S = tb.S;
+  const double *tmid = (const double *)(tbl + tb.o_tmid), *nasa = (const double *)(tbl + tb.o_nasa);
+  for (int ia = lane; ia < S; ia += 32) {
+    const double *ca = nasa + ((T < tmid[ia]) ? 0 : kNasaRows * S) + ia;
+    const double a1a = ca[0], a2a = ca[S];
+    const double hpa = fma_rn(fma_rn(fma_rn(fma_rn(ca[8 * S], T, ca[7 * S]), T, ca[6 * S]), T, ca[5 * S]), T, a1a);
+    const double hRTa = fma_rn(ca[9 * S], invT, hpa);
+    const double spa = fma_rn(fma_rn(fma_rn(ca[12 * S], T, ca[11 * S]), T, ca[10 * S]), T, a2a);
+    const double sRa = fma_rn(a1a, lnT, fma_rn(spa, T, ca[13 * S]));
+    const double ga = hRTa - sRa;
+    cG[1 + ia] = ga;
+    cG[1 + S + ia] = ga + ga;
+    if (CPH) {
+      cYwCp[ia].y = fma_rn(fma_rn(fma_rn(fma_rn(ca[4 * S], T, ca[3 * S]), T, ca[2 * S]), T, a2a), T, a1a);
+      cHOm[ia].x = hRTa;
+    }
+  }
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // a7 in the integrator (fp32 CUDA cores, R18): cp_i/R and h_i/(R T_ref) from the shallow MLP, by one warp.
 // ---------------------------------------------------------------------------------------------------------
@@ -276,6 +299,51 @@ __device__ __forceinline__ void pk_rev_batch(const unsigned char *cell, const do
   }
 }
 
+// a2 for IU irreversible reactions per lane side by side (reactions k0 + lane, k0 + ks + lane, ..): rate constants, progress
+// rates and their stored multiples.  Lanes past the end recompute the last reaction and store nothing.
+template <int IU>
+__device__ __forceinline__ void pk_irr_batch(const unsigned char *cell, const double2 *rkA, const double2 *rkB, const uint4 *rfac,
+                                             double *cQ, int Rp, int R, bool has2, double invT, double lnT, int k0, int ks, int lane) {
+  double lk[IU], fw[IU];
+  uint4 f[IU];
+  int kk[IU];
+  bool oor = false;
+#pragma unroll
+  for (int u = 0; u < IU; ++u) {
+    kk[u] = k0 + ks * u + lane;
+    const int k = (kk[u] < R) ? kk[u] : R - 1;
+    const double2 p0 = rkA[k];
+    const double ta = rkB[k].x;
+    f[u] = rfac[k];
+    lk[u] = fma_rn(-ta, invT, fma_rn(p0.y, lnT, p0.x));
+    oor = oor || ab_exp_out_of_range(lk[u]);
+  }
+  if (__any_sync(0xffffffffu, oor)) {
+#pragma unroll
+    for (int u = 0; u < IU; ++u) fw[u] = cexp(lk[u]);
+  } else {
+#pragma unroll
+    for (int u = 0; u < IU; ++u) fw[u] = ab_exp_core(lk[u]);
+  }
+#pragma unroll
+  for (int u = 0; u < IU; ++u) fw[u] = fw[u] * lds_f64(cell, f[u].x);
+#pragma unroll
+  for (int u = 0; u < IU; ++u) fw[u] = fw[u] * lds_f64(cell, f[u].y);
+#pragma unroll
+  for (int u = 0; u < IU; ++u) {
+    if (kk[u] < R) {
+      const int k = kk[u];
+      cQ[k] = fw[u];
+      cQ[Rp + k] = -fw[u];
+      if (has2) {
+        const double f2 = fw[u] + fw[u];
+        cQ[2 * Rp + k] = f2;
+        cQ[3 * Rp + k] = -f2;
+      }
+    }
+  }
+}
+
 // unsigned-bit-pattern minimum of positive doubles (NaN patterns sort above +inf and are thereby ignored, like the
 // contract's plain comparison `lim < t_star` ignores them)
 __device__ __forceinline__ double pk_min_bits(double a, double b) {
@@ -415,8 +483,8 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
         ln_c0 = __shfl_sync(0xffffffffu, lval, 16);
         inv_ctot = 1.0 / c_tot;
         if (NW == 1) {
-          if (EST) pk_nasa<false>(tb, tbl, cG, cYwCp, cHOm, T, invT, lnT, lane);
-          else pk_nasa<true>(tb, tbl, cG, cYwCp, cHOm, T, invT, lnT, lane);
+          if (EST) pk_nasa1<false>(tb, tbl, cG, cYwCp, cHOm, T, invT, lnT, lane);
+          else pk_nasa1<true>(tb, tbl, cG, cYwCp, cHOm, T, invT, lnT, lane);
         }
         // -- 1/Wbar = sum Y_i/W_i, sequential in species order (contract 5.4)
         double inv_wbar = 0.0;
@@ -435,6 +503,16 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
         }
         // -- Y_i/W_i (for the cp sum) and the small-species stabilisation (Eqs 6-7, R7):
         //    C** = gamma(y) rho y / W
+        if (NW == 1) {
+          for (int ia = lane; ia < S; ia += 32) {
+            const double2 va = cYp[ia];
+            const double ypa = (va.x > 0.0) ? va.x : 0.0;
+            double ca = (rho * ypa) * va.y;
+            if (sc.alpha > 0.0) ca = (ypa / (sc.alpha + ypa)) * ca;
+            cYwCp[ia].x = va.x * va.y;
+            cConc[1 + ia] = ca;
+          }
+        } else
         for (int ia = lane; ia < S; ia += 64) {
           const int ib_ = ia + 32;
           const int ib = (ib_ < S) ? ib_ : S - 1;
@@ -502,57 +580,19 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
       if (NW < 3 && !DENSE && n_it > 2 * NW) {
         for (int b0 = half; b0 < n_it; b0 += 4 * NW)
           pk_rev_batch<4>(cell, rkA, rkB, rfac, rdg, cRof, cQ, Rp, Rrev, has2, invT, lnT, ln_c0, b0, NW, lane);
-      } else if (NW == 3) {
+      } else {
         int b0 = half;
         for (; b0 + NW < n_it; b0 += 2 * NW)
           pk_rev_batch<2>(cell, rkA, rkB, rfac, rdg, cRof, cQ, Rp, Rrev, has2, invT, lnT, ln_c0, b0, NW, lane);
         for (; b0 < n_it; b0 += NW)
           pk_rev_batch<1>(cell, rkA, rkB, rfac, rdg, cRof, cQ, Rp, Rrev, has2, invT, lnT, ln_c0, b0, NW, lane);
-      } else {
-        for (int b0 = half; b0 < n_it; b0 += 2 * NW)
-          pk_rev_batch<2>(cell, rkA, rkB, rfac, rdg, cRof, cQ, Rp, Rrev, has2, invT, lnT, ln_c0, b0, NW, lane);
       }
-      // irreversible reactions [Rrev, R): 32-blocks c = half (mod NW), two at a time (quad: one)
-      constexpr int IU = (NW >= 3) ? 1 : 2;
-      for (int k0 = Rrev + half * 32; k0 < R; k0 += 32 * IU * NW) {
-        double lk[IU], fw[IU];
-        uint4 f[IU];
-        int kk[IU];
-        bool oor = false;
-#pragma unroll
-        for (int u = 0; u < IU; ++u) {
-          kk[u] = k0 + 32 * NW * u + lane;
-          const int k = (kk[u] < R) ? kk[u] : R - 1;
-          const double2 p0 = rkA[k];
-          const double ta = rkB[k].x;
-          f[u] = rfac[k];
-          lk[u] = fma_rn(-ta, invT, fma_rn(p0.y, lnT, p0.x));
-          oor = oor || ab_exp_out_of_range(lk[u]);
-        }
-        if (__any_sync(0xffffffffu, oor)) {
-#pragma unroll
-          for (int u = 0; u < IU; ++u) fw[u] = cexp(lk[u]);
-        } else {
-#pragma unroll
-          for (int u = 0; u < IU; ++u) fw[u] = ab_exp_core(lk[u]);
-        }
-#pragma unroll
-        for (int u = 0; u < IU; ++u) fw[u] = fw[u] * lds_f64(cell, f[u].x);
-#pragma unroll
-        for (int u = 0; u < IU; ++u) fw[u] = fw[u] * lds_f64(cell, f[u].y);
-#pragma unroll
-        for (int u = 0; u < IU; ++u) {
-          if (kk[u] < R) {
-            const int k = kk[u];
-            cQ[k] = fw[u];
-            cQ[Rp + k] = -fw[u];
-            if (has2) {
-              const double f2 = fw[u] + fw[u];
-              cQ[2 * Rp + k] = f2;
-              cQ[3 * Rp + k] = -f2;
-            }
-          }
-        }
+      // irreversible reactions [Rrev, R): 32-blocks c = half (mod NW), two at a time while two are left (triple, quad: one)
+      {
+        int k0 = Rrev + half * 32;
+        if (NW < 3)
+          for (; k0 + 32 * NW < R; k0 += 64 * NW) pk_irr_batch<2>(cell, rkA, rkB, rfac, cQ, Rp, R, has2, invT, lnT, k0, 32 * NW, lane);
+        for (; k0 < R; k0 += 32 * NW) pk_irr_batch<1>(cell, rkA, rkB, rfac, cQ, Rp, R, has2, invT, lnT, k0, 32 * NW, lane);
       }
       PKT(2)
       cell_sync();
