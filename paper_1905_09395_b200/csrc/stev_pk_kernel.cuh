@@ -25,6 +25,22 @@
 
 namespace stev {
 
+// 8-byte load at a 32-bit shared-memory address (warp-uniform base + per-lane table offset: one LDS with a
+// register + uniform-register address, no separate add).  Volatile, no memory clobber: it keeps its order with the cell
+// barriers (volatile asm / __syncwarp), which is all that is needed -- every value read this way was written in an
+// earlier phase -- and leaves the compiler free to schedule the surrounding table loads and arithmetic.
+__device__ __forceinline__ double lds_f64s(uint32_t base_s, unsigned off) {
+  double v;
+  asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(base_s + off));
+  return v;
+}
+// SA selects it; otherwise the plain C++ load, which the compiler may interleave freely (the large-mechanism kernels
+// run four reactions per lane side by side and lose more to the fixed order than they gain from the saved adds)
+template <bool SA>
+__device__ __forceinline__ double lds_sel(const unsigned char *cell, uint32_t cell_s, unsigned off) {
+  return SA ? lds_f64s(cell_s, off) : lds_f64(cell, off);
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // a1: NASA-7 (Eqs 15-16, R17) by one warp: g/RT (and 2 g/RT) always, cp/R and h/RT if CPH.
 // Two species per lane side by side; lanes past the end recompute the last species and store nothing.
@@ -234,8 +250,8 @@ __device__ __forceinline__ void pk_dft(const SolverConsts &sc, const double *cQ,
 // table load -> g loads -> exponentials -> concentration loads -> stores, with 2 U independent exp chains in flight.
 // Lanes past the end recompute the last reaction and store nothing.
 // ---------------------------------------------------------------------------------------------------------
-template <int U>
-__device__ __forceinline__ void pk_rev_batch(const unsigned char *cell, const double2 *rkA, const double2 *rkB, const uint4 *rfac,
+template <int U, bool SA>
+__device__ __forceinline__ void pk_rev_batch(const unsigned char *cell, uint32_t cell_s, const double2 *rkA, const double2 *rkB, const uint4 *rfac,
                                              const uint4 *rdg, const double *cRof, double *cQ, int Rp, int Rrev, bool has2,
                                              double invT, double lnT, double ln_c0, int b0, int bs, int lane) {
   int k_[U], k[U];
@@ -253,10 +269,10 @@ __device__ __forceinline__ void pk_rev_batch(const unsigned char *cell, const do
     const uint4 d = rdg[k[u]];
     f[u] = rfac[k[u]];
     lkf[u] = fma_rn(-p1.x, invT, fma_rn(p0.y, lnT, p0.x));
-    double dg = 0.0 - lds_f64(cell, d.x);
-    dg = dg - lds_f64(cell, d.y);
-    dg = dg + lds_f64(cell, d.z);
-    dg = dg + lds_f64(cell, d.w);
+    double dg = 0.0 - lds_sel<SA>(cell, cell_s, d.x);
+    dg = dg - lds_sel<SA>(cell, cell_s, d.y);
+    dg = dg + lds_sel<SA>(cell, cell_s, d.z);
+    dg = dg + lds_sel<SA>(cell, cell_s, d.w);
     lkr[u] = lkf[u] - fma_rn(p1.y, ln_c0, -dg);
     oor = oor || ab_exp_out_of_range(lkf[u]) || ab_exp_out_of_range(lkr[u]);
   }
@@ -276,13 +292,13 @@ __device__ __forceinline__ void pk_rev_batch(const unsigned char *cell, const do
   }
 #pragma unroll
   for (int u = 0; u < U; ++u) {
-    fwd[u] = fwd[u] * lds_f64(cell, f[u].x);
-    rev[u] = rev[u] * lds_f64(cell, f[u].z);
+    fwd[u] = fwd[u] * lds_sel<SA>(cell, cell_s, f[u].x);
+    rev[u] = rev[u] * lds_sel<SA>(cell, cell_s, f[u].z);
   }
 #pragma unroll
   for (int u = 0; u < U; ++u) {
-    fwd[u] = fwd[u] * lds_f64(cell, f[u].y);
-    rev[u] = rev[u] * lds_f64(cell, f[u].w);
+    fwd[u] = fwd[u] * lds_sel<SA>(cell, cell_s, f[u].y);
+    rev[u] = rev[u] * lds_sel<SA>(cell, cell_s, f[u].w);
   }
 #pragma unroll
   for (int u = 0; u < U; ++u) {
@@ -301,8 +317,8 @@ __device__ __forceinline__ void pk_rev_batch(const unsigned char *cell, const do
 
 // a2 for IU irreversible reactions per lane side by side (reactions k0 + lane, k0 + ks + lane, ..): rate constants, progress
 // rates and their stored multiples.  Lanes past the end recompute the last reaction and store nothing.
-template <int IU>
-__device__ __forceinline__ void pk_irr_batch(const unsigned char *cell, const double2 *rkA, const double2 *rkB, const uint4 *rfac,
+template <int IU, bool SA>
+__device__ __forceinline__ void pk_irr_batch(const unsigned char *cell, uint32_t cell_s, const double2 *rkA, const double2 *rkB, const uint4 *rfac,
                                              double *cQ, int Rp, int R, bool has2, double invT, double lnT, int k0, int ks, int lane) {
   double lk[IU], fw[IU];
   uint4 f[IU];
@@ -326,9 +342,9 @@ __device__ __forceinline__ void pk_irr_batch(const unsigned char *cell, const do
     for (int u = 0; u < IU; ++u) fw[u] = ab_exp_core(lk[u]);
   }
 #pragma unroll
-  for (int u = 0; u < IU; ++u) fw[u] = fw[u] * lds_f64(cell, f[u].x);
+  for (int u = 0; u < IU; ++u) fw[u] = fw[u] * lds_sel<SA>(cell, cell_s, f[u].x);
 #pragma unroll
-  for (int u = 0; u < IU; ++u) fw[u] = fw[u] * lds_f64(cell, f[u].y);
+  for (int u = 0; u < IU; ++u) fw[u] = fw[u] * lds_sel<SA>(cell, cell_s, f[u].y);
 #pragma unroll
   for (int u = 0; u < IU; ++u) {
     if (kk[u] < R) {
@@ -381,6 +397,8 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
   double *cRof = (double *)(cell + a.cl.oRof);
   float *cHid = (float *)(cell + a.cl.oHid);
   volatile PkScal *scal = (volatile PkScal *)(cell + a.cl.oSc);
+  const uint32_t cell_s = (uint32_t)__cvta_generic_to_shared(cell);   // table-driven loads address shared memory directly
+  constexpr bool kSA = (NW == 1), kGA = (NW == 1);
 
   const double *W = (const double *)(tbl + tb.o_W), *invW = (const double *)(tbl + tb.o_invW);
   const double2 *rkA = (const double2 *)(tbl + tb.o_rkA), *rkB = (const double2 *)(tbl + tb.o_rkB);
@@ -579,20 +597,20 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
       // omega_i = sum_j nu_ij q_j into plain additions in the contract's order.
       if (NW < 3 && !DENSE && n_it > 2 * NW) {
         for (int b0 = half; b0 < n_it; b0 += 4 * NW)
-          pk_rev_batch<4>(cell, rkA, rkB, rfac, rdg, cRof, cQ, Rp, Rrev, has2, invT, lnT, ln_c0, b0, NW, lane);
+          pk_rev_batch<4, kSA>(cell, cell_s, rkA, rkB, rfac, rdg, cRof, cQ, Rp, Rrev, has2, invT, lnT, ln_c0, b0, NW, lane);
       } else {
         int b0 = half;
         for (; b0 + NW < n_it; b0 += 2 * NW)
-          pk_rev_batch<2>(cell, rkA, rkB, rfac, rdg, cRof, cQ, Rp, Rrev, has2, invT, lnT, ln_c0, b0, NW, lane);
+          pk_rev_batch<2, kSA>(cell, cell_s, rkA, rkB, rfac, rdg, cRof, cQ, Rp, Rrev, has2, invT, lnT, ln_c0, b0, NW, lane);
         for (; b0 < n_it; b0 += NW)
-          pk_rev_batch<1>(cell, rkA, rkB, rfac, rdg, cRof, cQ, Rp, Rrev, has2, invT, lnT, ln_c0, b0, NW, lane);
+          pk_rev_batch<1, kSA>(cell, cell_s, rkA, rkB, rfac, rdg, cRof, cQ, Rp, Rrev, has2, invT, lnT, ln_c0, b0, NW, lane);
       }
       // irreversible reactions [Rrev, R): 32-blocks c = half (mod NW), two at a time while two are left (triple, quad: one)
       {
         int k0 = Rrev + half * 32;
         if (NW < 3)
-          for (; k0 + 32 * NW < R; k0 += 64 * NW) pk_irr_batch<2>(cell, rkA, rkB, rfac, cQ, Rp, R, has2, invT, lnT, k0, 32 * NW, lane);
-        for (; k0 < R; k0 += 32 * NW) pk_irr_batch<1>(cell, rkA, rkB, rfac, cQ, Rp, R, has2, invT, lnT, k0, 32 * NW, lane);
+          for (; k0 + 32 * NW < R; k0 += 64 * NW) pk_irr_batch<2, kSA>(cell, cell_s, rkA, rkB, rfac, cQ, Rp, R, has2, invT, lnT, k0, 32 * NW, lane);
+        for (; k0 < R; k0 += 32 * NW) pk_irr_batch<1, kSA>(cell, cell_s, rkA, rkB, rfac, cQ, Rp, R, has2, invT, lnT, k0, 32 * NW, lane);
       }
       PKT(2)
       cell_sync();
@@ -609,8 +627,8 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
         // length over the lanes; padding entries read the 0.0 slot, and adding +0.0 changes nothing (om is never -0.0).
         uint4 o0 = ge[0], o1 = ge[32];
         for (int e4 = 0; e4 < g_len4; e4 += 2) {
-          const double v0 = lds_f64(cell, o0.x), v1 = lds_f64(cell, o0.y), v2 = lds_f64(cell, o0.z), v3 = lds_f64(cell, o0.w);
-          const double v4 = lds_f64(cell, o1.x), v5 = lds_f64(cell, o1.y), v6 = lds_f64(cell, o1.z), v7 = lds_f64(cell, o1.w);
+          const double v0 = lds_sel<kGA>(cell, cell_s, o0.x), v1 = lds_sel<kGA>(cell, cell_s, o0.y), v2 = lds_sel<kGA>(cell, cell_s, o0.z), v3 = lds_sel<kGA>(cell, cell_s, o0.w);
+          const double v4 = lds_sel<kGA>(cell, cell_s, o1.x), v5 = lds_sel<kGA>(cell, cell_s, o1.y), v6 = lds_sel<kGA>(cell, cell_s, o1.z), v7 = lds_sel<kGA>(cell, cell_s, o1.w);
           o0 = ge[(e4 + 2) * 32];
           o1 = ge[(e4 + 3) * 32];
           om = om + v0;
