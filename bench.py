@@ -48,6 +48,9 @@ def parse_args():
     ap.add_argument("--cells", type=int, default=None, help="cells per GPU (default: the config's full size)")
     ap.add_argument("--impl", default="stev", choices=["stev", "reference"])
     ap.add_argument("--chunk-steps", type=int, default=0)
+    ap.add_argument("--max-steps", type=int, default=None,
+                    help="override the per-cell step cap (profiling runs only: cuts the 200000-step tail cells short; the "
+                         "line then reports finished_fraction < 1)")
     ap.add_argument("--lanes", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -245,7 +248,10 @@ def main():
     S = w.mech.n_species
     mech = stev.Mechanism(w.mech)
     est = stev.Estimator(mech, w.estimator) if w.estimator is not None else None
-    prm = stev.stev_params_default(chunk_steps=args.chunk_steps, lanes_per_cell=args.lanes, **w.params)
+    params = dict(w.params)
+    if args.max_steps is not None:
+        params["max_steps"] = args.max_steps
+    prm = stev.stev_params_default(chunk_steps=args.chunk_steps, lanes_per_cell=args.lanes, **params)
 
     T0 = torch.tensor(w.T, dtype=torch.float64, device=dev)
     p = torch.tensor(w.p, dtype=torch.float64, device=dev)
@@ -374,7 +380,7 @@ def main():
                        "estimator": None if w.estimator is None else f"mlp {w.estimator.n_in}-{w.estimator.n_hidden}-{w.estimator.n_out} fp32",
                        "parallelism": f"cells sharded over {world} GPU(s), no collective",
                        "l2": f"inputs larger than L2 ({(8 * n * (2 + S)) >> 20} MiB of state per GPU, restored between steps)",
-                       "chunk_steps": args.chunk_steps, "lanes_per_cell": st["lanes_per_cell"],
+                       "chunk_steps": args.chunk_steps, "max_steps": params["max_steps"], "lanes_per_cell": st["lanes_per_cell"],
                        "threads_per_block": st["threads_per_block"], "blocks": st["blocks"], "smem_bytes": st["smem_bytes"]},
             "cell_steps_per_s": cell_steps_all / (ms_per_step * 1e-3), "mean_steps_per_cell": cell_steps_all / (world * n),
             "finished_fraction": finished_all / (world * n), "return_code": rc,

@@ -132,13 +132,17 @@ __device__ __forceinline__ void pk_mlp(const PkTables &tb, const unsigned char *
     const int jh1 = (jh1_ < H) ? jh1_ : jh0;
     float z0 = b1[jh0], z1 = b1[jh1];
     if (jh0 - lane + 32 < H) {   // warp-uniform: a second row of units exists
-      for (int k = 0; k < n_in; ++k) {
+      const float *w = W1T + jh0;   // unit jh0 and, 32 floats on, unit jh0 + 32; one row of H floats per input
+#pragma unroll 4
+      for (int k = 0; k < n_in; ++k, w += H) {
         const float xk = cXn[k];
-        z0 = __fmaf_rn(W1T[k * H + jh0], xk, z0);
-        z1 = __fmaf_rn(W1T[k * H + jh1], xk, z1);
+        z0 = __fmaf_rn(w[0], xk, z0);
+        z1 = __fmaf_rn(w[32], xk, z1);
       }
     } else {
-      for (int k = 0; k < n_in; ++k) z0 = __fmaf_rn(W1T[k * H + jh0], cXn[k], z0);
+      const float *w = W1T + jh0;
+#pragma unroll 4
+      for (int k = 0; k < n_in; ++k, w += H) z0 = __fmaf_rn(w[0], cXn[k], z0);
     }
     cHid[jh0] = activate(z0);
     if (jh1_ < H) cHid[jh1] = activate(z1);
