@@ -119,6 +119,10 @@ typedef struct {
                              66 = warp-specialised variant of 64 (a rate warp + a DFT warp; also needs dft_enable);
                              96 = a warp triple per cell, 8 cells per SM, 24 warps of 80 registers per SM (same limits as 64);
                              128 = a warp quad per cell, 8 cells per SM, 32 warps of 64 registers per SM (same limits as 64) */
+  int32_t order_cells;    /* 1 (default): the persistent kernels pull the cells in order of decreasing temperature
+                             (a counting sort on the device before the launch) -- step counts grow with temperature,
+                             so the long integrations start first and do not end up running alone;
+                             0: in index order */
 } stev_params;
 
 /* Counters of the last stev_integrate / stev_integrate_host call on this thread. */

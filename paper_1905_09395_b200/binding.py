@@ -35,7 +35,8 @@ class stev_params(C.Structure):
     _fields_ = [("y_step_max", C.c_double), ("delta_max", C.c_double), ("alpha", C.c_double), ("tol_ring", C.c_double),
                 ("tol_freq", C.c_double), ("r_fac", C.c_double), ("rof_min", C.c_double),
                 ("dft_first_high_bin", C.c_int32), ("dft_enable", C.c_int32), ("max_steps", C.c_int32),
-                ("energy_mode", C.c_int32), ("chunk_steps", C.c_int32), ("lanes_per_cell", C.c_int32)]
+                ("energy_mode", C.c_int32), ("chunk_steps", C.c_int32), ("lanes_per_cell", C.c_int32),
+                ("order_cells", C.c_int32)]
 
 
 class stev_stats(C.Structure):

@@ -257,6 +257,7 @@ void stev_params_default(stev_params *p) {
   p->energy_mode = STEV_ENERGY_ADIABATIC;
   p->chunk_steps = 0;
   p->lanes_per_cell = 0;
+  p->order_cells = 1;
 }
 
 void stev_last_stats(stev_stats *out) {
@@ -489,6 +490,8 @@ namespace {
 struct Workspace {
   int *counters;            // [0] queue head, [1] worst status, [2] active count
   int *list[2];
+  int *order;               // launch order (hottest cells first), order_hist: its counting-sort scratch
+  int *order_hist;
   unsigned char *flags;
   int *block_counts;
   double *spill;
@@ -506,6 +509,10 @@ Workspace carve(void *base, const DevTables &tb, const stev_params *p, int64_t n
     return base ? (unsigned char *)base + o : (unsigned char *)nullptr;
   };
   w.counters = (int *)take(256);
+  if (p->order_cells) {
+    w.order = (int *)take(4 * (size_t)n);
+    w.order_hist = (int *)take(4 * (size_t)(kOrderBuckets + 1));
+  }
   if (p->chunk_steps > 0) {
     w.list[0] = (int *)take(4 * (size_t)n);
     w.list[1] = (int *)take(4 * (size_t)n);
@@ -682,6 +689,12 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
     }
     if (kind) {
       STEV_CUDA(cudaMemsetAsync(w.counters, 0, 256, s));
+      const int *order = nullptr;
+      if (p->order_cells && kind != 3 && n > 1) {
+        rc = order_cells_launch(T, n, w.order, w.order_hist, s);
+        if (rc) return rc;
+        order = w.order;
+      }
       int blocks = 0, cpb = 0;
       size_t smem = 0;
       if (kind == 3) {
@@ -692,7 +705,7 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
         const int wi = (kind == 4) ? 2 : (kind == 5 ? 3 : (kind == 6 ? 0 : kind - 1));
         rc = integrate_pk_launch(est ? est->pk_tb[wi] : m->pk_tb[wi], est ? est->pk_cl[wi] : m->pk_cl[wi],
                                  est ? est->d_pk_table[wi] : m->d_pk_table[wi], make_consts(p), dt_cfd, n, ld, T, pressure, Y,
-                                 steps_out, status_out, w.counters, s, &blocks, &cpb, &smem, kind == 6);
+                                 steps_out, status_out, w.counters, s, &blocks, &cpb, &smem, kind == 6, order);
       }
       if (rc) return rc;
       int worst = 0;
@@ -744,9 +757,15 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
   long long n_active = n;
   int cur = 0;
   STEV_CUDA(cudaMemsetAsync(w.counters, 0, 256, s));
+  const int *order = nullptr;
+  if (p->order_cells && n > 1) {
+    rc = order_cells_launch(T, n, w.order, w.order_hist, s);
+    if (rc) return rc;
+    order = w.order;
+  }
   for (int pass = 0; n_active > 0; ++pass) {
     a.n_active = n_active;
-    a.list = (pass == 0) ? nullptr : w.list[cur];
+    a.list = (pass == 0) ? order : w.list[cur];
     a.restore = (pass > 0);
     long long blocks = std::min<long long>((long long)sms * cfg.blocks_per_sm, (n_active + cfg.cells_per_block - 1) / cfg.cells_per_block);
     if (pass > 0) STEV_CUDA(cudaMemsetAsync(w.counters, 0, 4, s));

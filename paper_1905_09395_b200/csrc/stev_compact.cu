@@ -1,6 +1,8 @@
 // stev_compact.cu -- variable-load retirement between passes (row a6): the cells still active after
 // a pass are gathered, order preserved, into the next pass's active list.  Warp ballot + popc inside a warp,
 // a shared-memory scan across the warps of a block, and a grid-level exclusive prefix sum of the block totals.
+#include <algorithm>
+
 #include "stev_host.h"
 
 namespace stev {
@@ -88,6 +90,47 @@ __global__ void __launch_bounds__(kCB) compact_scatter_kernel(const unsigned cha
     const int dst = block_offsets[blockIdx.x] + warp_off[warp] + __popc(b & ((1u << lane) - 1u));
     list_out[dst] = list_in ? list_in[i] : i;
   }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Launch order of the cells (scheduling only): cells finish after very different numbers of
+// steps and the step count grows with temperature, so the persistent kernels pull the hottest cells first -- the
+// long integrations start at once and the short ones fill in behind them, instead of a few long cells running alone at
+// the end.  Counting sort on a 4096-bucket temperature scale (descending), order within a bucket arbitrary: results
+// do not depend on the order, only the schedule does.
+// ---------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ int order_bucket(double T) {
+  double x = (T - 200.0) * (double)kOrderBuckets / 3800.0;   // 200 K .. 4000 K; everything else (NaN too) in the end buckets
+  int b = (x >= 0.0) ? ((x < (double)(kOrderBuckets - 1)) ? (int)x : kOrderBuckets - 1) : 0;
+  return kOrderBuckets - 1 - b;
+}
+
+__global__ void __launch_bounds__(256) order_hist_kernel(const double *__restrict__ T, long long n, int *__restrict__ hist) {
+  __shared__ int h[kOrderBuckets];
+  for (int i = threadIdx.x; i < kOrderBuckets; i += 256) h[i] = 0;
+  __syncthreads();
+  for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < n; i += (long long)gridDim.x * 256)
+    atomicAdd(&h[order_bucket(T[i])], 1);
+  __syncthreads();
+  for (int i = threadIdx.x; i < kOrderBuckets; i += 256)
+    if (h[i]) atomicAdd(&hist[i], h[i]);
+}
+
+__global__ void __launch_bounds__(256) order_scatter_kernel(const double *__restrict__ T, long long n, int *__restrict__ offsets,
+                                                            int *__restrict__ list) {
+  for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < n; i += (long long)gridDim.x * 256)
+    list[atomicAdd(&offsets[order_bucket(T[i])], 1)] = (int)i;
+}
+
+// hist: kOrderBuckets + 1 ints of scratch; list: n ints
+int order_cells_launch(const double *T, long long n, int *list, int *hist, cudaStream_t s) {
+  STEV_CUDA(cudaMemsetAsync(hist, 0, sizeof(int) * (kOrderBuckets + 1), s));
+  const int blocks = (int)std::min<long long>((n + 255) / 256, 4 * (long long)device_sm_count());
+  order_hist_kernel<<<blocks, 256, 0, s>>>(T, n, hist);
+  compact_scan_kernel<<<1, kCB, 0, s>>>(hist, kOrderBuckets, hist + kOrderBuckets);   // exclusive scan in place
+  order_scatter_kernel<<<blocks, 256, 0, s>>>(T, n, hist, list);
+  STEV_CUDA(cudaGetLastError());
+  return STEV_OK;
 }
 
 int compact_launch(const unsigned char *flags, const int *list_in, int n, int *list_out, int *count_out, int *block_counts,

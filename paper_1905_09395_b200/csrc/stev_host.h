@@ -70,8 +70,12 @@ bool build_pk_image(const HostMechanism &m, const HostEstimator *e, int nw, std:
 int integrate_pk_launch(const PkTables &tb, const PkCell &cl, const unsigned char *d_table, const SolverConsts &sc, double t_f,
                         long long n, long long ld, double *T, const double *p, double *Y, int *steps, unsigned char *status,
                         int *counters, cudaStream_t s, int *blocks_out, int *cells_per_block_out, size_t *smem_out,
-                        bool dense = false);
+                        bool dense = false, const int *list = nullptr);
 bool pk_dense_ok(const PkTables &tb);
+
+// Launch order of the cells, hottest first (stev_compact.cu).  hist: kOrderBuckets + 1 ints of scratch; list: n ints.
+constexpr int kOrderBuckets = 4096;
+int order_cells_launch(const double *T, long long n, int *list, int *hist, cudaStream_t s);
 
 }  // namespace stev
 

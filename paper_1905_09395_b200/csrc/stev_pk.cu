@@ -353,7 +353,7 @@ int pk_cells_per_block(const PkTables &tb, const PkCell &cl, bool dense) {
 
 int integrate_pk_launch(const PkTables &tb, const PkCell &cl, const unsigned char *d_table, const SolverConsts &sc, double t_f,
                         long long n, long long ld, double *T, const double *p, double *Y, int *steps, unsigned char *status,
-                        int *counters, cudaStream_t s, int *blocks_out, int *cells_per_block_out, size_t *smem_out, bool dense) {
+                        int *counters, cudaStream_t s, int *blocks_out, int *cells_per_block_out, size_t *smem_out, bool dense, const int *list) {
   if (dense && !pk_dense_ok(tb)) { set_error("dense tensor-memory kernel: more than 64 reversible reactions"); return STEV_EINVAL; }
   PkArgs a{};
   a.tb = tb;
@@ -362,7 +362,7 @@ int integrate_pk_launch(const PkTables &tb, const PkCell &cl, const unsigned cha
   a.sc = sc;
   a.t_f = t_f;
   a.n_active = n;
-  a.list = nullptr;
+  a.list = list;
   a.ld = ld;
   a.T = T;
   a.p = p;

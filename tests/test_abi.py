@@ -38,8 +38,8 @@ def test_params_default_and_struct_layout():
     assert p.y_step_max == 1e-2 and p.delta_max == 1e-2 and p.alpha == 1e-5
     assert p.tol_ring == 0.5 and p.tol_freq == 0.1 and p.r_fac == 2.0 and p.rof_min == 2.0 ** -100
     assert p.dft_first_high_bin == 4 and p.dft_enable == 1 and p.max_steps == 200000
-    assert p.chunk_steps == 0 and p.lanes_per_cell == 0
-    assert ctypes.sizeof(stev.stev_params) == 7 * 8 + 6 * 4
+    assert p.chunk_steps == 0 and p.lanes_per_cell == 0 and p.order_cells == 1
+    assert ctypes.sizeof(stev.stev_params) == 7 * 8 + 8 * 4   # seven int32 fields, padded to a multiple of 8
     assert stev.stev_version().startswith("stev-b200")
 
 

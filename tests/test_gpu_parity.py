@@ -258,6 +258,28 @@ def test_default_kernel_selection(stev):
     assert gpu["stats"]["lanes_per_cell"] <= 32
 
 
+@pytest.mark.parametrize("config,n,over", [(2, 3000, {}), (1, 2000, {}), (3, 300, {}), (4, 500, {}), (2, 700, dict(chunk_steps=400)),
+                                           (2, 900, dict(lanes_per_cell=33)), (0, 5000, {})])
+def test_launch_order_is_pure_scheduling(stev, config, n, over):
+    """stev_params.order_cells: the persistent kernels pull the hottest cells first (counting sort on the device);
+    nothing of the result may depend on it."""
+    w = make_workload(config, n)
+    case = GpuCase(stev, w)
+    a = case.integrate(order_cells=0, **over)
+    b = case.integrate(order_cells=1, **over)
+    for k in ("T", "Y", "steps", "status"):
+        np.testing.assert_array_equal(a[k], b[k])
+    # degenerate temperatures (all equal, out of the bucket range, NaN) still give a permutation
+    T = w.T.copy()
+    T[: n // 3] = 5000.0
+    T[n // 3: n // 2] = 150.0
+    c = case.integrate(T=T, order_cells=1, max_steps=50, **over)
+    d = case.integrate(T=T, order_cells=0, max_steps=50, **over)
+    assert (c["steps"] > 0).all()
+    for k in ("T", "Y", "steps", "status"):
+        np.testing.assert_array_equal(c[k], d[k])
+
+
 @pytest.mark.parametrize("config,n,chunk", [(0, 3000, 64), (1, 600, 100), (1, 600, 1000), (2, 300, 333), (3, 100, 150)])
 def test_chunked_passes_with_compaction_give_identical_results(stev, config, n, chunk):
     """Row a6: retiring / spilling / compacting is pure scheduling -- results cannot depend on chunk_steps."""
