@@ -713,7 +713,7 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
       STEV_CUDA(cudaStreamSynchronize(s));
       STEV_CUDA(cudaGetLastError());
       g_stats.passes = 1;
-      g_stats.kernel_launches = 1;
+      g_stats.kernel_launches = 1 + (order ? 3 : 0);   // integrator + histogram, scan, scatter of the launch order
       g_stats.blocks = blocks;
       g_stats.lanes_per_cell = kind == 1 ? 33 : (kind == 2 ? 64 : (kind == 3 ? 66 : (kind == 4 ? 128 : (kind == 5 ? 96 : 34))));
       g_stats.threads_per_block =
@@ -763,6 +763,7 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
     if (rc) return rc;
     order = w.order;
   }
+  if (order) g_stats.kernel_launches += 3;
   for (int pass = 0; n_active > 0; ++pass) {
     a.n_active = n_active;
     a.list = (pass == 0) ? order : w.list[cur];
