@@ -172,6 +172,38 @@ def test_integrate_parity(stev, oracle, config, n):
     assert np.max(np.abs(gpu["Y"].sum(axis=0) - 1.0)) < 1e-12
 
 
+# --------------------------------------------------------------------- full size, the launch configuration bench.py times
+@pytest.mark.parametrize("config", [0, 1, 2, 3, 4])
+def test_full_size_sampled_parity_and_invariants(stev, oracle, config):
+    """BASELINE.json's full cell counts with the default parameters and kernel selection (what `bench.py --config C` times).
+    Cells are independent, so the oracle integrates a seeded sample of them one by one; the whole field is
+    checked through what holds at any size: mass fractions sum to one, element mass fractions are conserved (pins P3/P4 on
+    the GPU result), Y >= 0 (Eq 3 caps consumption at 0.9 y), every cell took at least one step and reports a status."""
+    w = make_workload(config)
+    n = w.n_cells
+    gpu = GpuCase(stev, w).integrate()
+    assert gpu["rc"] in (0, stev.STEV_WMAXSTEPS)
+    assert np.isfinite(gpu["T"]).all() and np.isfinite(gpu["Y"]).all()
+    assert (gpu["steps"] >= 1).all() and np.isin(gpu["status"], (0, 1)).all()
+    assert (gpu["status"] == 0).mean() >= 0.995
+    assert gpu["Y"].min() >= 0.0
+    assert np.max(np.abs(gpu["Y"].sum(axis=0) - 1.0)) < 1e-12
+    zW = w.mech.elem_comp / w.mech.mol_weight[:, None]            # [S, E] moles of element per unit mass of species
+    drift = np.abs(zW.T @ gpu["Y"] - zW.T @ w.Y) / np.maximum(zW.T @ w.Y, 1e-300)
+    assert drift.max() < 1e-11, drift.max()
+    # sampled cells, one by one through the oracle: a seeded draw plus the cells that took the most steps
+    rng = np.random.default_rng(20260000 + config)
+    m = {0: 512, 1: 512, 2: 384, 3: 256, 4: 256}[config]
+    idx = np.unique(np.concatenate([rng.choice(n, size=min(m, n), replace=False), np.argsort(gpu["steps"])[-8:],
+                                    [0, n - 1]]))
+    ref = oracle.integrate(w.mech, w.estimator, w.params, w.T[idx], w.p[idx], np.ascontiguousarray(w.Y[:, idx]), w.dt_cfd)
+    sub = dict(T=gpu["T"][idx], Y=gpu["Y"][:, idx], steps=gpu["steps"][idx], status=gpu["status"][idx])
+    rep = assert_parity(sub, ref)
+    print(f"config {config} full size n={n}: sampled {idx.size} cells {rep} kernel lanes={gpu['stats']['lanes_per_cell']} "
+          f"mean steps {gpu['steps'].mean():.0f} finished {(gpu['status'] == 0).mean():.5f}")
+    assert rep["bit_exact"] == 1.0
+
+
 @pytest.mark.parametrize("config,n,lanes", [(0, 500, 1), (0, 500, 2), (0, 500, 32), (1, 300, 1), (1, 300, 8), (1, 300, 32),
                                             (2, 200, 4), (2, 200, 32), (3, 64, 16)])
 def test_result_does_not_depend_on_lanes_per_cell(stev, oracle, config, n, lanes):
