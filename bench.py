@@ -52,6 +52,8 @@ def parse_args():
                     help="override the per-cell step cap (profiling runs only: cuts the 200000-step tail cells short; the "
                          "line then reports finished_fraction < 1)")
     ap.add_argument("--lanes", type=int, default=0)
+    ap.add_argument("--order", type=int, default=1, help="stev_params.order_cells (include/stev.h): 1 default, 0 index order, "
+                                                          "2 hottest first cell by cell, 3 hottest first in groups of four")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--ref-cells", type=int, default=None, help="cells per step of the --impl reference arm")
@@ -251,7 +253,7 @@ def main():
     params = dict(w.params)
     if args.max_steps is not None:
         params["max_steps"] = args.max_steps
-    prm = stev.stev_params_default(chunk_steps=args.chunk_steps, lanes_per_cell=args.lanes, **params)
+    prm = stev.stev_params_default(chunk_steps=args.chunk_steps, lanes_per_cell=args.lanes, order_cells=args.order, **params)
 
     T0 = torch.tensor(w.T, dtype=torch.float64, device=dev)
     p = torch.tensor(w.p, dtype=torch.float64, device=dev)

@@ -121,8 +121,12 @@ typedef struct {
                              128 = a warp quad per cell, 8 cells per SM, 32 warps of 64 registers per SM (same limits as 64) */
   int32_t order_cells;    /* 1 (default): the persistent kernels pull the cells in order of decreasing temperature
                              (a counting sort on the device before the launch) -- step counts grow with temperature,
-                             so the long integrations start first and do not end up running alone;
-                             0: in index order */
+                             so the long integrations start first and do not end up running alone.
+                             While the state (n x (S + 2) doubles) is at most 64 MiB, i.e. stays in L2, the order is cell
+                             by cell; above that, aligned groups of four consecutive cells (one 32-byte sector of T, p
+                             and every row of Y) are keyed by their hottest cell and stay together, so each sector is
+                             fetched from HBM once instead of once per cell.  2: cell by cell at any size; 3: groups of
+                             four at any size; 0: index order.  Scheduling only: results do not depend on it. */
 } stev_params;
 
 /* Counters of the last stev_integrate / stev_integrate_host call on this thread. */

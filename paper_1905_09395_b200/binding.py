@@ -66,7 +66,10 @@ def load(build: bool = True):
         try:
             _build.build()
         except Exception:
-            if not os.path.exists(_build.LIB):
+            # a stale library must not stand in for sources that no longer compile: only a box without nvcc may go on
+            # with the library that travelled with the snapshot
+            import shutil
+            if shutil.which("nvcc") is not None or not os.path.exists(_build.LIB):
                 raise
     if not os.path.exists(_build.LIB):
         raise ImportError(f"{_build.LIB} is missing: run `python -m paper_1905_09395_b200._build` (no CPU fallback exists)")

@@ -691,7 +691,7 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
       STEV_CUDA(cudaMemsetAsync(w.counters, 0, 256, s));
       const int *order = nullptr;
       if (p->order_cells && kind != 3 && n > 1) {
-        rc = order_cells_launch(T, n, w.order, w.order_hist, s);
+        rc = order_cells_launch(T, n, order_group(p->order_cells, n, tb->S), w.order, w.order_hist, s);
         if (rc) return rc;
         order = w.order;
       }
@@ -759,7 +759,7 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
   STEV_CUDA(cudaMemsetAsync(w.counters, 0, 256, s));
   const int *order = nullptr;
   if (p->order_cells && n > 1) {
-    rc = order_cells_launch(T, n, w.order, w.order_hist, s);
+    rc = order_cells_launch(T, n, order_group(p->order_cells, n, tb->S), w.order, w.order_hist, s);
     if (rc) return rc;
     order = w.order;
   }

@@ -105,30 +105,50 @@ __device__ __forceinline__ int order_bucket(double T) {
   return kOrderBuckets - 1 - b;
 }
 
-__global__ void __launch_bounds__(256) order_hist_kernel(const double *__restrict__ T, long long n, int *__restrict__ hist) {
+// `group` consecutive cells (1, or 4 = one 32-byte sector of every fp64 row of the state) share one key, the
+// temperature of their hottest cell, and stay together in the list: the lanes that pull them touch the same sectors of
+// T, p and the S rows of Y at about the same time, so each sector is fetched from DRAM once instead of once per cell.
+__device__ __forceinline__ int order_group_bucket(const double *__restrict__ T, long long i0, int cnt) {
+  int b = kOrderBuckets - 1;
+  for (int k = 0; k < cnt; ++k) b = min(b, order_bucket(T[i0 + k]));   // smallest bucket = hottest cell
+  return b;
+}
+
+__global__ void __launch_bounds__(256) order_hist_kernel(const double *__restrict__ T, long long n, int group,
+                                                         int *__restrict__ hist) {
   __shared__ int h[kOrderBuckets];
   for (int i = threadIdx.x; i < kOrderBuckets; i += 256) h[i] = 0;
   __syncthreads();
-  for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < n; i += (long long)gridDim.x * 256)
-    atomicAdd(&h[order_bucket(T[i])], 1);
+  const long long n_groups = (n + group - 1) / group;
+  for (long long g = (long long)blockIdx.x * 256 + threadIdx.x; g < n_groups; g += (long long)gridDim.x * 256) {
+    const long long i0 = g * group;
+    const int cnt = (int)min((long long)group, n - i0);
+    atomicAdd(&h[order_group_bucket(T, i0, cnt)], cnt);
+  }
   __syncthreads();
   for (int i = threadIdx.x; i < kOrderBuckets; i += 256)
     if (h[i]) atomicAdd(&hist[i], h[i]);
 }
 
-__global__ void __launch_bounds__(256) order_scatter_kernel(const double *__restrict__ T, long long n, int *__restrict__ offsets,
-                                                            int *__restrict__ list) {
-  for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < n; i += (long long)gridDim.x * 256)
-    list[atomicAdd(&offsets[order_bucket(T[i])], 1)] = (int)i;
+__global__ void __launch_bounds__(256) order_scatter_kernel(const double *__restrict__ T, long long n, int group,
+                                                            int *__restrict__ offsets, int *__restrict__ list) {
+  const long long n_groups = (n + group - 1) / group;
+  for (long long g = (long long)blockIdx.x * 256 + threadIdx.x; g < n_groups; g += (long long)gridDim.x * 256) {
+    const long long i0 = g * group;
+    const int cnt = (int)min((long long)group, n - i0);
+    const int dst = atomicAdd(&offsets[order_group_bucket(T, i0, cnt)], cnt);
+    for (int k = 0; k < cnt; ++k) list[dst + k] = (int)(i0 + k);
+  }
 }
 
 // hist: kOrderBuckets + 1 ints of scratch; list: n ints
-int order_cells_launch(const double *T, long long n, int *list, int *hist, cudaStream_t s) {
+int order_cells_launch(const double *T, long long n, int group, int *list, int *hist, cudaStream_t s) {
   STEV_CUDA(cudaMemsetAsync(hist, 0, sizeof(int) * (kOrderBuckets + 1), s));
-  const int blocks = (int)std::min<long long>((n + 255) / 256, 4 * (long long)device_sm_count());
-  order_hist_kernel<<<blocks, 256, 0, s>>>(T, n, hist);
+  const long long n_groups = (n + group - 1) / group;
+  const int blocks = (int)std::min<long long>((n_groups + 255) / 256, 4 * (long long)device_sm_count());
+  order_hist_kernel<<<blocks, 256, 0, s>>>(T, n, group, hist);
   compact_scan_kernel<<<1, kCB, 0, s>>>(hist, kOrderBuckets, hist + kOrderBuckets);   // exclusive scan in place
-  order_scatter_kernel<<<blocks, 256, 0, s>>>(T, n, hist, list);
+  order_scatter_kernel<<<blocks, 256, 0, s>>>(T, n, group, hist, list);
   STEV_CUDA(cudaGetLastError());
   return STEV_OK;
 }

@@ -298,18 +298,24 @@ def test_launch_order_is_pure_scheduling(stev, config, n, over):
     w = make_workload(config, n)
     case = GpuCase(stev, w)
     a = case.integrate(order_cells=0, **over)
-    b = case.integrate(order_cells=1, **over)
-    for k in ("T", "Y", "steps", "status"):
-        np.testing.assert_array_equal(a[k], b[k])
+    for mode in (1, 2, 3):          # by state size (cell by cell here), cell by cell, aligned groups of four cells
+        b = case.integrate(order_cells=mode, **over)
+        for k in ("T", "Y", "steps", "status"):
+            np.testing.assert_array_equal(a[k], b[k])
+    b = case.integrate(T=w.T[:n - 3], p=w.p[:n - 3], Y=w.Y[:, :n - 3], order_cells=3, **over)   # ragged last group
+    for k in ("T", "steps", "status"):
+        np.testing.assert_array_equal(a[k][:n - 3], b[k])
+    np.testing.assert_array_equal(a["Y"][:, :n - 3], b["Y"])
     # degenerate temperatures (all equal, out of the bucket range, NaN) still give a permutation
     T = w.T.copy()
     T[: n // 3] = 5000.0
     T[n // 3: n // 2] = 150.0
-    c = case.integrate(T=T, order_cells=1, max_steps=50, **over)
     d = case.integrate(T=T, order_cells=0, max_steps=50, **over)
-    assert (c["steps"] > 0).all()
-    for k in ("T", "Y", "steps", "status"):
-        np.testing.assert_array_equal(c[k], d[k])
+    for mode in (1, 3):
+        c = case.integrate(T=T, order_cells=mode, max_steps=50, **over)
+        assert (c["steps"] > 0).all()
+        for k in ("T", "Y", "steps", "status"):
+            np.testing.assert_array_equal(c[k], d[k])
 
 
 @pytest.mark.parametrize("config,n,chunk", [(0, 3000, 64), (1, 600, 100), (1, 600, 1000), (2, 300, 333), (3, 100, 150)])
