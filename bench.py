@@ -352,9 +352,14 @@ def main():
                    96: "stev_pk_kernel<3> (warp triple per cell, DFT history in tensor memory)",
                    128: "stev_pk_kernel<4> (warp quad per cell, DFT history in tensor memory)"}.get(st["lanes_per_cell"],
                                                                              f"stev_integrate_kernel<{st['lanes_per_cell']}>")
+    # DRAM bytes of one launch from ncu (dram__bytes_read.sum + dram__bytes_write.sum), known only for the captured
+    # workloads: profiles/r1_groups_cfg3.md (config 3 at full size, default kernel, by launch order)
+    traffic = None
+    if args.config == 3 and n == 1048576 and st["lanes_per_cell"] == 64 and args.max_steps is None:
+        traffic = {1: 1865687552 + 811976960, 2: 5996999680 + 2048877312}.get(args.order)
     roofline = {"bound": "alu", "kernel": kernel_name,
                 "achieved": flop / kernel_s / 1e12, "peak": peak_tflops, "unit": "TFLOP/s",
-                "frac": flop / kernel_s / 1e12 / peak_tflops, "traffic": None,
+                "frac": flop / kernel_s / 1e12 / peak_tflops, "traffic": traffic,
                 "peak_source": f"derived: 148 SM x 64 DFMA/clk x 2 x {sm_max:.0f} MHz (DESIGN.md section 8); not in MEASURED_PEAKS.json",
                 "fp64_instr": {"achieved_per_s": instr / kernel_s, "peak_per_s": peak_instr,
                                "frac": instr / kernel_s / peak_instr, "measured_dfma_per_s": dfma_per_s,
