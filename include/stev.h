@@ -126,7 +126,7 @@ typedef struct {
                              by cell; above that, aligned groups of four consecutive cells (one 32-byte sector of T, p
                              and every row of Y) are keyed by their hottest cell and stay together, so each sector is
                              fetched from HBM once instead of once per cell.  2: cell by cell at any size; 3: groups of
-                             four at any size; 0: index order.  Scheduling only: results do not depend on it. */
+                             four at any size; 4: groups of eight (two sectors per row) at any size; 0: index order.  Scheduling only: results do not depend on it. */
 } stev_params;
 
 /* Counters of the last stev_integrate / stev_integrate_host call on this thread. */

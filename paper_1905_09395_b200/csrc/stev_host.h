@@ -76,10 +76,11 @@ bool pk_dense_ok(const PkTables &tb);
 // Launch order of the cells, hottest first (stev_compact.cu).  hist: kOrderBuckets + 1 ints of scratch; list: n ints.
 constexpr int kOrderBuckets = 4096;
 int order_cells_launch(const double *T, long long n, int group, int *list, int *hist, cudaStream_t s);
-// group size of the launch order for stev_params.order_cells (1: by the size of the state against L2; 2: 1; 3: 4)
+// group size of the launch order for stev_params.order_cells (1: by the size of the state against L2; 2: 1; 3: 4; 4: 8)
 inline int order_group(int order_cells, long long n, int S) {
   if (order_cells == 2) return 1;
   if (order_cells == 3) return 4;
+  if (order_cells == 4) return 8;
   return ((double)n * (double)(S + 2) * 8.0 > 64.0 * 1024.0 * 1024.0) ? 4 : 1;
 }
 

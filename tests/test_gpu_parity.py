@@ -298,7 +298,7 @@ def test_launch_order_is_pure_scheduling(stev, config, n, over):
     w = make_workload(config, n)
     case = GpuCase(stev, w)
     a = case.integrate(order_cells=0, **over)
-    for mode in (1, 2, 3):          # by state size (cell by cell here), cell by cell, aligned groups of four cells
+    for mode in (1, 2, 3, 4):       # by state size (cell by cell here), cell by cell, aligned groups of four / eight cells
         b = case.integrate(order_cells=mode, **over)
         for k in ("T", "Y", "steps", "status"):
             np.testing.assert_array_equal(a[k], b[k])
@@ -311,7 +311,7 @@ def test_launch_order_is_pure_scheduling(stev, config, n, over):
     T[: n // 3] = 5000.0
     T[n // 3: n // 2] = 150.0
     d = case.integrate(T=T, order_cells=0, max_steps=50, **over)
-    for mode in (1, 3):
+    for mode in (1, 3, 4):
         c = case.integrate(T=T, order_cells=mode, max_steps=50, **over)
         assert (c["steps"] > 0).all()
         for k in ("T", "Y", "steps", "status"):
