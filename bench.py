@@ -356,7 +356,7 @@ def main():
     # workloads: profiles/r1_groups_cfg3.md (config 3 at full size, default kernel, by launch order)
     traffic = None
     if args.config == 3 and n == 1048576 and st["lanes_per_cell"] == 64 and args.max_steps is None:
-        traffic = {1: 1865687552 + 811976960, 2: 5996999680 + 2048877312, 4: 1118324224 + 781168128}.get(args.order)
+        traffic = {1: 1118324224 + 781168128, 2: 5996999680 + 2048877312, 3: 1865687552 + 811976960, 4: 1118324224 + 781168128}.get(args.order)
     roofline = {"bound": "alu", "kernel": kernel_name,
                 "achieved": flop / kernel_s / 1e12, "peak": peak_tflops, "unit": "TFLOP/s",
                 "frac": flop / kernel_s / 1e12 / peak_tflops, "traffic": traffic,

@@ -123,9 +123,9 @@ typedef struct {
                              (a counting sort on the device before the launch) -- step counts grow with temperature,
                              so the long integrations start first and do not end up running alone.
                              While the state (n x (S + 2) doubles) is at most 64 MiB, i.e. stays in L2, the order is cell
-                             by cell; above that, aligned groups of four consecutive cells (one 32-byte sector of T, p
-                             and every row of Y) are keyed by their hottest cell and stay together, so each sector is
-                             fetched from HBM once instead of once per cell.  2: cell by cell at any size; 3: groups of
+                             by cell; above that, aligned groups of eight consecutive cells (one 64-byte DRAM access = two
+                             32-byte sectors of T, p and every row of Y) are keyed by their hottest cell and stay together,
+                             so each sector is fetched from HBM once instead of once per cell.  2: cell by cell at any size; 3: groups of
                              four at any size; 4: groups of eight (two sectors per row) at any size; 0: index order.  Scheduling only: results do not depend on it. */
 } stev_params;
 

@@ -81,7 +81,7 @@ inline int order_group(int order_cells, long long n, int S) {
   if (order_cells == 2) return 1;
   if (order_cells == 3) return 4;
   if (order_cells == 4) return 8;
-  return ((double)n * (double)(S + 2) * 8.0 > 64.0 * 1024.0 * 1024.0) ? 4 : 1;
+  return ((double)n * (double)(S + 2) * 8.0 > 64.0 * 1024.0 * 1024.0) ? 8 : 1;
 }
 
 }  // namespace stev
