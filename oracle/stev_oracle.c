@@ -111,6 +111,16 @@ double ora_exp(double x) {
   p = fma(p, r, 1.0);
   p = fma(p, r, 1.0);
   double two_k = ora_from_bits((uint64_t)(int64_t)(ki + 1023) << 52);
+#ifdef ORA_SENSITIVITY_ULP
+  /* Self-sensitivity variant (SURVEY.md section 8c "Arithmetic contract"): built ONLY into
+   * libstev_oracle_ulp.so by tests/test_oracle_sensitivity.py.  It moves the result by one unit in the last place,
+   * up or down by a hash of the argument's bits, i.e. it is another routine that is still within 2 ulp of libm. */
+  {
+    uint64_t hsh = ora_bits(x) * 0x9e3779b97f4a7c15ULL;
+    uint64_t rb = ora_bits(p * two_k);
+    if (rb > 0x0010000000000000ULL && rb < 0x7fe0000000000000ULL) return ora_from_bits((hsh >> 63) ? rb + 1 : rb - 1);
+  }
+#endif
   return p * two_k;
 }
 
@@ -428,7 +438,10 @@ static int ora_integrate_cell(const ora_mechanism *m, const ora_estimator *est, 
           if (d > d_hi) d_hi = d;
         }
         double f_ring = d0 / ((d_hi > 1.0e-300) ? d_hi : 1.0e-300);            /* Eq 10 */
-        int ringing = (f_ring < prm->tol_ring) && (d0 < prm->tol_freq);        /* Eq 12 */
+        /* Eq 12.  A window without any high-frequency content (d_hi at or below the guard: a dormant reaction whose
+         * stored changes are all zero) is not ringing: "rOF will not decline unless the reversible rate is both
+         * ringing and at equilibrium". */
+        int ringing = (d_hi > 1.0e-300) && (f_ring < prm->tol_ring) && (d0 < prm->tol_freq);
         double rof = rOF[j] * (ringing ? 1.0 / prm->r_fac : prm->r_fac);       /* Eq 13 */
         if (rof > 1.0) rof = 1.0;
         if (rof < prm->rof_min) rof = prm->rof_min;
@@ -446,10 +459,10 @@ static int ora_integrate_cell(const ora_mechanism *m, const ora_estimator *est, 
     }
 
     /* 9. retirement, PAPER.md:105 (section 2.4) + R20. */
-    if (last) { status = 0; break; }
     int finite = (T - T == 0.0);
     for (int i = 0; i < S; ++i) finite = finite && (Y[i * ldy] - Y[i * ldy] == 0.0);
-    if (!finite) { status = 2; break; }
+    if (!finite) { status = 2; break; }      /* checked first: a landing step that produced NaN is not "finished" */
+    if (last) { status = 0; break; }
     if (steps >= prm->max_steps) { status = 1; break; }
   }
   *T_io = T;

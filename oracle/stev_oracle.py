@@ -27,6 +27,22 @@ def build(force: bool = False) -> str:
     return _LIB
 
 
+_variants = {}
+
+
+def load_variant(define: str):
+    """A second build of the same source with -D<define> (libstev_oracle_<define>.so), e.g. ORA_SENSITIVITY_ULP: the
+    exp routine perturbed by one unit in the last place, for the self-sensitivity measurement of DESIGN.md section 5."""
+    if define not in _variants:
+        lib = os.path.join(_HERE, f"libstev_oracle_{define.lower()}.so")
+        if not os.path.exists(lib) or os.path.getmtime(lib) < os.path.getmtime(_SRC):
+            cmd = ["gcc", "-O2", "-std=c11", "-Wall", "-Wextra", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC",
+                   f"-D{define}", "-o", lib, _SRC, "-lm"]
+            subprocess.run(cmd, check=True)
+        _variants[define] = C.CDLL(lib)
+    return _variants[define]
+
+
 class _Mech(C.Structure):
     _fields_ = [("n_species", C.c_int32), ("n_reactions", C.c_int32),
                 ("mol_weight", C.c_void_p), ("nasa_lo", C.c_void_p), ("nasa_hi", C.c_void_p), ("t_mid", C.c_void_p),
@@ -156,9 +172,9 @@ def rates_eval(mech, est, params: dict, T, p, Y, rOF=None):
     return dY, dT, q
 
 
-def integrate(mech, est, params: dict, T, p, Y, dt_cfd: float, n_threads: int | None = None):
+def integrate(mech, est, params: dict, T, p, Y, dt_cfd: float, n_threads: int | None = None, variant: str | None = None):
     """Advance n cells over dt_cfd. Inputs are copied. Returns dict(T, Y, steps, status, rof_min, rc)."""
-    lib = _load()
+    lib = load_variant(variant) if variant else _load()
     mh, eh, pr = _mech(mech), _est(est), _params(params)
     T = np.array(T, np.float64, copy=True)
     p = np.ascontiguousarray(p, np.float64)
