@@ -136,6 +136,8 @@ typedef struct {
   int32_t lanes_per_cell, threads_per_block, cells_per_block, blocks;
   int64_t smem_bytes;        /* dynamic shared memory per block */
   int64_t total_steps;       /* sum of per-cell step counts (filled by stev_integrate_host only; else -1) */
+  int32_t specialised;       /* 1: the kernel instantiation with this mechanism's dimensions as compile-time constants ran */
+  int32_t reserved;
 } stev_stats;
 
 STEV_API void stev_params_default(stev_params *p);

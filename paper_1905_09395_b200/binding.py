@@ -42,7 +42,7 @@ class stev_params(C.Structure):
 class stev_stats(C.Structure):
     _fields_ = [("passes", C.c_int32), ("kernel_launches", C.c_int32), ("lanes_per_cell", C.c_int32),
                 ("threads_per_block", C.c_int32), ("cells_per_block", C.c_int32), ("blocks", C.c_int32),
-                ("smem_bytes", C.c_int64), ("total_steps", C.c_int64)]
+                ("smem_bytes", C.c_int64), ("total_steps", C.c_int64), ("specialised", C.c_int32), ("reserved", C.c_int32)]
 
 
 EXPORTS = ["stev_params_default", "stev_mechanism_create", "stev_mechanism_destroy", "stev_mechanism_sizes",

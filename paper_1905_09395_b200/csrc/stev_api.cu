@@ -13,6 +13,7 @@ namespace stev {
 
 static thread_local std::string g_error;
 static thread_local stev_stats g_stats{};
+static thread_local int g_specialised = 0;
 
 void set_error(const std::string &msg) { g_error = msg; }
 int cuda_fail(cudaError_t e, const char *what) {
@@ -344,14 +345,6 @@ int stev_mechanism_create(const stev_mechanism_desc *d, stev_mechanism **out) {
   build_table_image(h, nullptr, image, m->tb);
   cudaError_t e = cudaMalloc(&m->d_table, image.size());
   if (e == cudaSuccess) e = cudaMemcpy(m->d_table, image.data(), image.size(), cudaMemcpyHostToDevice);
-  if (e == cudaSuccess) {
-    std::vector<unsigned char> ab;
-    m->ab_ok = build_ab_image(h, nullptr, ab, m->ab_tb, m->ab_cl);
-    if (m->ab_ok) {
-      e = cudaMalloc(&m->d_ab_table, ab.size());
-      if (e == cudaSuccess) e = cudaMemcpy(m->d_ab_table, ab.data(), ab.size(), cudaMemcpyHostToDevice);
-    }
-  }
   for (int n = 0; n < 4 && e == cudaSuccess; ++n) {   // the pair image first: it chooses the reaction order
     static const int order[4] = {1, 2, 3, 0}, nw_of[4] = {1, 2, 4, 3};
     const int w = order[n];
@@ -360,6 +353,14 @@ int stev_mechanism_create(const stev_mechanism_desc *d, stev_mechanism **out) {
     if (m->pk_ok[w]) {
       e = cudaMalloc(&m->d_pk_table[w], pk.size());
       if (e == cudaSuccess) e = cudaMemcpy(m->d_pk_table[w], pk.data(), pk.size(), cudaMemcpyHostToDevice);
+    }
+  }
+  if (e == cudaSuccess) {
+    std::vector<unsigned char> ls;
+    m->ls_ok = build_ls_image(h, nullptr, ls, m->ls_tb);
+    if (m->ls_ok) {
+      e = cudaMalloc(&m->d_ls_table, ls.size());
+      if (e == cudaSuccess) e = cudaMemcpy(m->d_ls_table, ls.data(), ls.size(), cudaMemcpyHostToDevice);
     }
   }
   if (e != cudaSuccess) {
@@ -373,9 +374,9 @@ int stev_mechanism_create(const stev_mechanism_desc *d, stev_mechanism **out) {
 void stev_mechanism_destroy(stev_mechanism *m) {
   if (!m) return;
   if (m->d_table) cudaFree(m->d_table);
-  if (m->d_ab_table) cudaFree(m->d_ab_table);
   for (int w = 0; w < 4; ++w)
     if (m->d_pk_table[w]) cudaFree(m->d_pk_table[w]);
+  if (m->d_ls_table) cudaFree(m->d_ls_table);
   delete m;
 }
 
@@ -423,14 +424,6 @@ int stev_estimator_load(const stev_mechanism *m, const stev_estimator_desc *d, s
     build_table_image(m->host, &h, image, e->tb);
     ce = cudaMalloc(&e->d_table, image.size());
     if (ce == cudaSuccess) ce = cudaMemcpy(e->d_table, image.data(), image.size(), cudaMemcpyHostToDevice);
-    if (ce == cudaSuccess) {
-      std::vector<unsigned char> ab;
-      e->ab_ok = build_ab_image(m->host, &h, ab, e->ab_tb, e->ab_cl);
-      if (e->ab_ok) {
-        ce = cudaMalloc(&e->d_ab_table, ab.size());
-        if (ce == cudaSuccess) ce = cudaMemcpy(e->d_ab_table, ab.data(), ab.size(), cudaMemcpyHostToDevice);
-      }
-    }
     for (int n = 0; n < 4 && ce == cudaSuccess; ++n) {
       static const int order[4] = {1, 2, 3, 0}, nw_of[4] = {1, 2, 4, 3};
       const int w = order[n];
@@ -440,6 +433,14 @@ int stev_estimator_load(const stev_mechanism *m, const stev_estimator_desc *d, s
         ce = cudaMalloc(&e->d_pk_table[w], pk.size());
         if (ce == cudaSuccess) ce = cudaMemcpy(e->d_pk_table[w], pk.data(), pk.size(), cudaMemcpyHostToDevice);
       }
+    }
+  }
+  if (ce == cudaSuccess && m) {
+    std::vector<unsigned char> ls;
+    e->ls_ok = build_ls_image(m->host, &h, ls, e->ls_tb);
+    if (e->ls_ok) {
+      ce = cudaMalloc(&e->d_ls_table, ls.size());
+      if (ce == cudaSuccess) ce = cudaMemcpy(e->d_ls_table, ls.data(), ls.size(), cudaMemcpyHostToDevice);
     }
   }
   if (ce == cudaSuccess) {
@@ -472,9 +473,9 @@ int stev_estimator_load(const stev_mechanism *m, const stev_estimator_desc *d, s
 void stev_estimator_destroy(stev_estimator *e) {
   if (!e) return;
   if (e->d_table) cudaFree(e->d_table);
-  if (e->d_ab_table) cudaFree(e->d_ab_table);
   for (int w = 0; w < 4; ++w)
     if (e->d_pk_table[w]) cudaFree(e->d_pk_table[w]);
+  if (e->d_ls_table) cudaFree(e->d_ls_table);
   if (e->d_params) cudaFree(e->d_params);
   for (int k = 0; k < 2; ++k)
     if (e->d_tc_image[k]) cudaFree(e->d_tc_image[k]);
@@ -658,11 +659,11 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
     const bool pk2_ok = (est ? est->pk_ok[1] : m->pk_ok[1]) && tm_common;
     const bool pk4_ok = (est ? est->pk_ok[2] : m->pk_ok[2]) && tm_common;
     const bool pk3_ok = (est ? est->pk_ok[3] : m->pk_ok[3]) && tm_common;
-    const bool ab_ok = (est ? est->ab_ok : m->ab_ok) && p->dft_enable && tm_common;
+    const bool ls_ok = (est ? est->ls_ok : m->ls_ok) && tm_common;
     int kind = 0;   // 0: sub-warp groups (history in shared memory), 1: one warp per cell, 2: warp pair, 3: warp-specialised, 4: warp quad, 5: warp triple
     if (p->lanes_per_cell == 33) kind = 1;
     else if (p->lanes_per_cell == 64) kind = 2;
-    else if (p->lanes_per_cell == 66) kind = 3;
+    else if (p->lanes_per_cell == 512 || p->lanes_per_cell == 513) kind = 7;   // lock-step block (stev_ls_kernel.cuh); 513: run-time dimensions only
     else if (p->lanes_per_cell == 128) kind = 4;
     else if (p->lanes_per_cell == 96) kind = 5;
     else if (p->lanes_per_cell == 34) kind = 6;   // one warp per cell, dense (32 cells per SM at 64 registers)
@@ -680,7 +681,7 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
       else if (pk1_ok) kind = 1;
       else if (pk2_ok && tb->R >= 64) kind = 2;
     }
-    if ((kind == 1 && !pk1_ok) || (kind == 2 && !pk2_ok) || (kind == 3 && !ab_ok) || (kind == 4 && !pk4_ok) ||
+    if ((kind == 1 && !pk1_ok) || (kind == 2 && !pk2_ok) || (kind == 7 && !ls_ok) || (kind == 4 && !pk4_ok) ||
         (kind == 5 && !pk3_ok) || (kind == 6 && !(pk1_ok && pk_dense_ok(est ? est->pk_tb[0] : m->pk_tb[0])))) {
       set_error("stev_integrate: lanes_per_cell = 33 / 64 / 66 / 96 / 128 (tensor-memory kernels) need chunk_steps = 0, at most two factors "
                 "per reaction side, 1..128 (33) or 1..256 (64, 66, 96, 128) reversible reactions, at most 32 (33) or 64 species "
@@ -690,17 +691,20 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
     if (kind) {
       STEV_CUDA(cudaMemsetAsync(w.counters, 0, 256, s));
       const int *order = nullptr;
-      if (p->order_cells && kind != 3 && n > 1) {
+      if (p->order_cells && n > 1) {
         rc = order_cells_launch(T, n, order_group(p->order_cells, n, tb->S), w.order, w.order_hist, s);
         if (rc) return rc;
         order = w.order;
       }
       int blocks = 0, cpb = 0;
       size_t smem = 0;
-      if (kind == 3) {
-        rc = integrate_ab_launch(est ? est->ab_tb : m->ab_tb, est ? est->ab_cl : m->ab_cl, est ? est->d_ab_table : m->d_ab_table,
-                                 make_consts(p), dt_cfd, n, ld, T, pressure, Y, steps_out, status_out, w.counters, s, &blocks, &cpb,
-                                 &smem);
+      if (kind == 7) {
+        const stev::LsTables &ltb = est ? est->ls_tb : m->ls_tb;
+        bool is_static = false;
+        rc = integrate_ls_launch(ltb, est ? est->d_ls_table : m->d_ls_table, make_consts(p), dt_cfd, n, ld, T, pressure, Y,
+                                 steps_out, status_out, w.counters, s, &blocks, &smem, order, p->lanes_per_cell != 513, &is_static);
+        cpb = ltb.d.C;
+        g_specialised = is_static ? 1 : 0;
       } else {
         const int wi = (kind == 4) ? 2 : (kind == 5 ? 3 : (kind == 6 ? 0 : kind - 1));
         rc = integrate_pk_launch(est ? est->pk_tb[wi] : m->pk_tb[wi], est ? est->pk_cl[wi] : m->pk_cl[wi],
@@ -713,11 +717,12 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
       STEV_CUDA(cudaStreamSynchronize(s));
       STEV_CUDA(cudaGetLastError());
       g_stats.passes = 1;
+      g_stats.specialised = g_specialised;
       g_stats.kernel_launches = 1 + (order ? 3 : 0);   // integrator + histogram, scan, scatter of the launch order
       g_stats.blocks = blocks;
-      g_stats.lanes_per_cell = kind == 1 ? 33 : (kind == 2 ? 64 : (kind == 3 ? 66 : (kind == 4 ? 128 : (kind == 5 ? 96 : 34))));
+      g_stats.lanes_per_cell = kind == 1 ? 33 : (kind == 2 ? 64 : (kind == 7 ? p->lanes_per_cell : (kind == 4 ? 128 : (kind == 5 ? 96 : 34))));
       g_stats.threads_per_block =
-          kind == 3 ? kAbThreads : ((kind == 4 || kind == 6) ? kPkThreads4 : (kind == 5 ? kPkThreads3 : kPkThreads));
+          kind == 7 ? kLsThreads : ((kind == 4 || kind == 6) ? kPkThreads4 : (kind == 5 ? kPkThreads3 : kPkThreads));
       g_stats.cells_per_block = cpb;
       g_stats.smem_bytes = (int64_t)smem;
       if (worst == 2) { set_error("some cells produced non-finite values (status 2)"); return STEV_WNONFINITE; }

@@ -349,7 +349,7 @@ __device__ __forceinline__ bool dft_is_ringing(const double (&x)[kWindow], const
   { v = dft_bin_sq<6>(x); m2 = (v > m2) ? v : m2; }
   const double d_hi = sqrt(m2);
   const double f_ring = d0 / ((d_hi > 1.0e-300) ? d_hi : 1.0e-300);
-  return (f_ring < sc.tol_ring) && (d0 < sc.tol_freq);
+  return (d_hi > 1.0e-300) && (f_ring < sc.tol_ring) && (d0 < sc.tol_freq);   // no high-frequency content: not ringing
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -470,8 +470,8 @@ __global__ void __launch_bounds__(512) stev_integrate_kernel(const __grid_consta
     // ---- a6: retirement (R20)
     bad = group_or<G>(bad);
     int st = -1;
-    if (last) st = 0;
-    else if (bad) st = 2;
+    if (bad) st = 2;            // checked first: a landing step that produced a non-finite state is not "finished"
+    else if (last) st = 0;
     else if (steps >= sc.max_steps) st = 1;
     const bool pause = (st < 0) && a.chunk_steps > 0 && steps_in_pass >= a.chunk_steps;
     if (active && (st >= 0 || pause)) {

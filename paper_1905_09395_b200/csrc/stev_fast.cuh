@@ -152,7 +152,7 @@ __device__ __forceinline__ void ab_window_stats(const double (&x)[kWindow], doub
 __device__ __forceinline__ bool ab_ring_exact(double d0, double m2, const SolverConsts &sc) {
   const double d_hi = sqrt(m2);
   const double f_ring = d0 / ((d_hi > 1.0e-300) ? d_hi : 1.0e-300);
-  return (f_ring < sc.tol_ring) && (d0 < sc.tol_freq);
+  return (d_hi > 1.0e-300) && (f_ring < sc.tol_ring) && (d0 < sc.tol_freq);   // no high-frequency content: not ringing
 }
 // The same decision without the square root and the division whenever it is not close: with u = 2^-53,
 // fl(d0/fl(sqrt m2)) = (d0/sqrt m2)(1 + 2.1u) at worst, while d0^2 and Tol_ring^2 m2 are each formed with at most

@@ -7,8 +7,8 @@
 #include <cuda_runtime.h>
 
 #include "../../include/stev.h"
-#include "stev_ab.cuh"
 #include "stev_pk.cuh"
+#include "stev_ls.cuh"
 #include "stev_device.cuh"
 
 struct stev_estimator;
@@ -53,14 +53,6 @@ bool choose_config(const DevTables &tb, int lanes_per_cell_request, LaunchConfig
 
 int device_sm_count();
 
-// Warp-specialised integrator (stev_ab.cuh / stev_ab.cu).  build_ab_image returns false if the mechanism is outside
-// its limits (more than two factors per reaction side, more than 256 reversible reactions, tables too large).
-bool build_ab_image(const HostMechanism &m, const HostEstimator *e, std::vector<unsigned char> &image, AbTables &tb, AbCell &cl);
-int ab_cells_per_block(const AbTables &tb, const AbCell &cl);
-int integrate_ab_launch(const AbTables &tb, const AbCell &cl, const unsigned char *d_table, const SolverConsts &sc, double t_f,
-                        long long n, long long ld, double *T, const double *p, double *Y, int *steps, unsigned char *status,
-                        int *counters, cudaStream_t s, int *blocks_out, int *cells_per_block_out, size_t *smem_out);
-
 int estimator_tensor_prepare(stev_estimator *e);
 
 // Warp-pair integrator (stev_pk.cuh / stev_pk.cu): both warps of a cell split every phase.  Same limits as above
@@ -72,6 +64,14 @@ int integrate_pk_launch(const PkTables &tb, const PkCell &cl, const unsigned cha
                         int *counters, cudaStream_t s, int *blocks_out, int *cells_per_block_out, size_t *smem_out,
                         bool dense = false, const int *list = nullptr);
 bool pk_dense_ok(const PkTables &tb);
+
+// Lock-step integrator (stev_ls.cuh / stev_ls.cu): all cells of a block step together.  build_ls_image returns false if
+// the mechanism is outside its limits (more than two factors per reaction side, tables too large for shared memory).
+bool build_ls_image(const HostMechanism &m, const HostEstimator *e, std::vector<unsigned char> &image, LsTables &tb);
+// allow_static: use the instantiation with compile-time dimensions if the shape list has one (*is_static says which ran)
+int integrate_ls_launch(const LsTables &tb, const unsigned char *d_table, const SolverConsts &sc, double t_f, long long n,
+                        long long ld, double *T, const double *p, double *Y, int *steps, unsigned char *status, int *counters,
+                        cudaStream_t s, int *blocks_out, size_t *smem_out, const int *list, bool allow_static, bool *is_static);
 
 // Launch order of the cells, hottest first (stev_compact.cu).  hist: kOrderBuckets + 1 ints of scratch; list: n ints.
 constexpr int kOrderBuckets = 4096;
@@ -90,14 +90,13 @@ struct stev_mechanism {
   stev::HostMechanism host;
   stev::DevTables tb{};
   unsigned char *d_table = nullptr;
-  bool ab_ok = false;                    // image of the warp-specialised kernel (NASA-7 thermo)
-  stev::AbTables ab_tb{};
-  stev::AbCell ab_cl{};
-  unsigned char *d_ab_table = nullptr;
   bool pk_ok[4] = {false, false, false, false};   // images of the tensor-memory kernel: [0] one warp per cell, [1] pair, [2] quad, [3] triple (NASA-7 thermo)
   stev::PkTables pk_tb[4]{};
   stev::PkCell pk_cl[4]{};
   unsigned char *d_pk_table[4] = {nullptr, nullptr, nullptr, nullptr};
+  bool ls_ok = false;                    // image of the lock-step kernel (NASA-7 thermo)
+  stev::LsTables ls_tb{};
+  unsigned char *d_ls_table = nullptr;
 };
 
 struct stev_estimator {
@@ -105,14 +104,13 @@ struct stev_estimator {
   const stev_mechanism *mech = nullptr;  // the mechanism it was loaded against (may be null)
   stev::DevTables tb{};                  // mechanism + estimator image (only if mech != null)
   unsigned char *d_table = nullptr;
-  bool ab_ok = false;                    // image of the warp-specialised kernel (MLP thermo)
-  stev::AbTables ab_tb{};
-  stev::AbCell ab_cl{};
-  unsigned char *d_ab_table = nullptr;
   bool pk_ok[4] = {false, false, false, false};   // images of the tensor-memory kernel (MLP thermo)
   stev::PkTables pk_tb[4]{};
   stev::PkCell pk_cl[4]{};
   unsigned char *d_pk_table[4] = {nullptr, nullptr, nullptr, nullptr};
+  bool ls_ok = false;                    // image of the lock-step kernel (MLP thermo)
+  stev::LsTables ls_tb{};
+  unsigned char *d_ls_table = nullptr;
   // standalone evaluation (stev_estimator_eval): device copies in kernel-friendly layouts
   float *d_params = nullptr;             // in_shift, in_scale, W1T [n_in][H], b1, W2T [H][n_out], b2
   size_t params_floats = 0;

@@ -1,0 +1,241 @@
+// stev_ls.cu -- host side of the lock-step integrator (stev_ls.cuh): table image, per-cell layout, launch.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <numeric>
+
+#include "stev_host.h"
+#include "stev_ls_kernel.cuh"
+
+namespace stev {
+
+static int align_up(int x, int a) { return (x + a - 1) / a * a; }
+static constexpr size_t kSmemMax = 227 * 1024;
+
+static unsigned magic(int d) { return d <= 1 ? 0u : (unsigned)(((1ull << 32) + (unsigned)d - 1) / (unsigned)d); }
+
+// At most two concentration factors per reaction side (total nu per side <= 2, so nu*g is exact for the equilibrium sum
+// and the stored multiples +-q, +-2q cover every coefficient) and one byte per species index.
+static bool ls_mechanism_ok(const HostMechanism &m) {
+  if (m.S > 64 || m.R > STEV_MAX_REACTIONS) return false;
+  for (int j = 0; j < m.R; ++j) {
+    int nr = 0, np = 0;
+    for (int e = m.reac_ptr[j]; e < m.reac_ptr[j + 1]; ++e) nr += m.reac_nu[e];
+    for (int e = m.prod_ptr[j]; e < m.prod_ptr[j + 1]; ++e) np += m.prod_nu[e];
+    if (nr > 2 || np > 2) return false;
+  }
+  return true;
+}
+
+bool build_ls_image(const HostMechanism &m, const HostEstimator *e, std::vector<unsigned char> &image, LsTables &tb) {
+  if (!ls_mechanism_ok(m)) return false;
+  const int S = m.S, R = m.R, Rrev = m.Rrev;
+  tb = LsTables{};
+  LsDims &d = tb.d;
+  d.S = S;
+  d.R = R;
+  d.Rrev = Rrev;
+  if (e) {
+    d.has_est = 1;
+    d.H = e->H;
+    d.n_in = e->n_in;
+    d.n_out = e->n_out;
+    tb.act = e->act;
+    tb.input_map = e->input_map;
+    tb.h_ref_T = e->h_ref_T;
+  }
+  // per-species entry lists in the caller's reaction order, reactant entries before product entries: the order in
+  // which the plain definition omega_i = sum_j nu_ij q_j adds them (same as the oracle's scatter, per species)
+  struct Ent { int j, coef; };
+  std::vector<std::vector<Ent>> gl(S);
+  const int variants[4] = {1, -1, 2, -2};   // stored multiples of q, fixed order
+  bool has2 = false;
+  auto variant_of = [&](int coef) {
+    for (int v = 0; v < 4; ++v)
+      if (variants[v] == coef) return v;
+    return -1;
+  };
+  for (int j = 0; j < R; ++j) {
+    for (int en = m.reac_ptr[j]; en < m.reac_ptr[j + 1]; ++en) gl[m.reac_sp[en]].push_back({j, -m.reac_nu[en]});
+    for (int en = m.prod_ptr[j]; en < m.prod_ptr[j + 1]; ++en) gl[m.prod_sp[en]].push_back({j, m.prod_nu[en]});
+  }
+  for (auto &v : gl)
+    for (auto &en : v) {
+      if (variant_of(en.coef) < 0) return false;
+      has2 = has2 || en.coef == 2 || en.coef == -2;
+    }
+  d.n_var = has2 ? 4 : 2;
+  d.C = 1;
+  LsLayout L = ls_layout_of(d);   // cell and table offsets do not depend on C
+
+  // internal reaction order: reversible first; within each group the bank-conflict-aware order of the pair kernel if
+  // the mechanism has one (stev_pk.cu), else the caller's
+  std::vector<int> orig_of = (m.pk_order.size() == (size_t)R) ? m.pk_order : m.orig_of, internal_of(R);
+  for (int k = 0; k < R; ++k) internal_of[orig_of[k]] = k;
+
+  // species sorted by decreasing list length: a warp of phase 3 holds a few neighbouring ranks (times all cells), so its
+  // lanes walk lists of nearly equal length
+  std::vector<int> rank(S);
+  std::iota(rank.begin(), rank.end(), 0);
+  std::stable_sort(rank.begin(), rank.end(), [&](int x, int y) { return gl[x].size() > gl[y].size(); });
+  int g_rows = 0;
+  std::vector<int> row0(S), rows(S);
+  for (int r = 0; r < S; ++r) {
+    row0[r] = g_rows;
+    rows[r] = ((int)gl[rank[r]].size() + 3) / 4;
+    g_rows += rows[r];
+  }
+  if (g_rows + 1 > 65535) return false;
+  tb.g_zero_row = g_rows;
+
+  tb.bytes = align_up(L.o_gent + 16 * (g_rows + 1), 128);
+
+  // cell slots per block: one lane of the scalar warp each, 2048 DFT windows in tensor memory, shared memory
+  const size_t avail = kSmemMax > (size_t)tb.bytes + 1024 ? kSmemMax - (size_t)tb.bytes - 1024 : 0;
+  int C = (int)std::min<size_t>(kLsMaxCells, avail / (size_t)L.stride);
+  if (Rrev > 0) C = std::min(C, (32 * kLsMaxPasses) / Rrev);
+  if (C < 1) return false;
+  d.C = C;
+  L = ls_layout_of(d);
+
+  image.assign(tb.bytes, 0);
+  unsigned char *base = image.data();
+  double *tmid = (double *)(base + L.o_tmid), *W = (double *)(base + L.o_W), *invW = (double *)(base + L.o_invW);
+  double *nasa = (double *)(base + L.o_nasa);
+  for (int i = 0; i < S; ++i) {
+    tmid[i] = m.t_mid[i];
+    W[i] = m.W[i];
+    invW[i] = 1.0 / m.W[i];
+    for (int rg = 0; rg < 2; ++rg) {
+      const double *c = (rg == 0 ? m.nasa_lo.data() : m.nasa_hi.data()) + 7 * i;
+      double *row = nasa + rg * kNasaRows * S + i;
+      row[0 * S] = c[0]; row[1 * S] = c[1]; row[2 * S] = c[2]; row[3 * S] = c[3]; row[4 * S] = c[4];
+      row[5 * S] = c[1] / 2.0; row[6 * S] = c[2] / 3.0; row[7 * S] = c[3] / 4.0; row[8 * S] = c[4] / 5.0;
+      row[9 * S] = c[5];
+      row[10 * S] = c[2] / 2.0; row[11 * S] = c[3] / 3.0; row[12 * S] = c[4] / 4.0;
+      row[13 * S] = c[6];
+    }
+  }
+  const unsigned one_slot = (unsigned)L.oConc, zero_slot = (unsigned)L.oG;
+  double *rkA = (double *)(base + L.o_rkA), *rkB = (double *)(base + L.o_rkB);
+  unsigned *rfac = (unsigned *)(base + L.o_rfac), *rdg = (unsigned *)(base + L.o_rdg);
+  for (int k = 0; k < R; ++k) {
+    const int j = orig_of[k];
+    double dnu = 0.0;
+    unsigned fac[4] = {one_slot, one_slot, one_slot, one_slot};
+    unsigned dgo[4] = {zero_slot, zero_slot, zero_slot, zero_slot};
+    int nf = 0, ne = 0;
+    for (int en = m.reac_ptr[j]; en < m.reac_ptr[j + 1]; ++en, ++ne) {
+      for (int n = 0; n < m.reac_nu[en]; ++n) fac[nf++] = (unsigned)(L.oConc + 8 * (1 + m.reac_sp[en]));
+      dgo[ne] = (unsigned)(L.oG + 8 * (1 + (m.reac_nu[en] == 2 ? S : 0) + m.reac_sp[en]));
+      dnu = dnu - (double)m.reac_nu[en];
+    }
+    nf = 2;
+    ne = 2;
+    for (int en = m.prod_ptr[j]; en < m.prod_ptr[j + 1]; ++en, ++ne) {
+      for (int n = 0; n < m.prod_nu[en]; ++n) fac[nf++] = (unsigned)(L.oConc + 8 * (1 + m.prod_sp[en]));
+      dgo[ne] = (unsigned)(L.oG + 8 * (1 + (m.prod_nu[en] == 2 ? S : 0) + m.prod_sp[en]));
+      dnu = dnu + (double)m.prod_nu[en];
+    }
+    rkA[2 * k] = clog(m.A[j]);
+    rkA[2 * k + 1] = m.b[j];
+    rkB[2 * k] = m.Ea[j] / kRcal;
+    rkB[2 * k + 1] = dnu;
+    std::memcpy(rfac + 4 * k, fac, 16);
+    if (k < Rrev) std::memcpy(rdg + 4 * k, dgo, 16);
+  }
+  unsigned char *gsp = base + L.o_gsp;
+  unsigned short *grow = (unsigned short *)(base + L.o_grow), *glen = (unsigned short *)(base + L.o_glen);
+  unsigned *gent = (unsigned *)(base + L.o_gent);
+  for (int n = 0; n < 4 * (g_rows + 1); ++n) gent[n] = zero_slot;
+  for (int r = 0; r < S; ++r) {
+    const int i = rank[r];
+    gsp[r] = (unsigned char)i;
+    grow[r] = (unsigned short)row0[r];
+    glen[r] = (unsigned short)rows[r];
+    for (int en = 0; en < (int)gl[i].size(); ++en)
+      gent[4 * row0[r] + en] = (unsigned)(L.oQ + 8 * (variant_of(gl[i][en].coef) * L.Rp + internal_of[gl[i][en].j]));
+  }
+  if (e) {
+    float *sh = (float *)(base + L.o_eshift), *scl = (float *)(base + L.o_escale), *W1T = (float *)(base + L.o_W1T);
+    float *b1 = (float *)(base + L.o_b1), *W2p = (float *)(base + L.o_W2p), *b2 = (float *)(base + L.o_b2);
+    for (int k = 0; k < e->n_in; ++k) {
+      sh[k] = e->in_shift[k];
+      scl[k] = e->in_scale[k];
+      for (int jh = 0; jh < e->H; ++jh) W1T[k * e->H + jh] = e->W1[(size_t)jh * e->n_in + k];
+    }
+    for (int jh = 0; jh < e->H; ++jh) b1[jh] = e->b1[jh];
+    for (int o = 0; o < e->n_out; ++o) {
+      b2[o] = e->b2[o];
+      for (int jh = 0; jh < e->H; ++jh) W2p[(size_t)o * L.Hpad + jh] = e->W2[(size_t)o * e->H + jh];
+    }
+  }
+  return true;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Shape list: mechanisms whose dimensions match an entry run the instantiation with compile-time dimensions, every
+// other mechanism runs the same kernel with the dimensions read at run time.  The entries are the shapes of the five
+// benchmark configurations of BASELINE.json (S, R, R_rev, stored multiples, estimator, H, n_in, n_out, C).
+// ---------------------------------------------------------------------------------------------------------
+using LsShape0 = LsFix<3, 2, 1, 2, 0, 0, 0, 0, 32>;
+using LsShape1 = LsFix<9, 19, 11, 4, 0, 0, 0, 0, 32>;
+using LsShape2 = LsFix<20, 60, 42, 4, 0, 0, 0, 0, 32>;
+using LsShape3 = LsFix<53, 325, 225, 4, 1, 32, 1, 106, 9>;
+using LsShape4 = LsFix<20, 60, 42, 4, 1, 64, 22, 40, 32>;
+
+static bool same_dims(const LsDims &x, const LsDims &y) {
+  return x.S == y.S && x.R == y.R && x.Rrev == y.Rrev && x.n_var == y.n_var && x.has_est == y.has_est && x.H == y.H &&
+         x.n_in == y.n_in && x.n_out == y.n_out && x.C == y.C;
+}
+
+static void *ls_kernel_for(const LsDims &d, bool allow_static, bool *is_static) {
+  *is_static = true;
+  if (allow_static) {
+    if (same_dims(d, LsShape0::D)) return (void *)stev_ls_kernel<LsShape0, false>;
+    if (same_dims(d, LsShape1::D)) return (void *)stev_ls_kernel<LsShape1, false>;
+    if (same_dims(d, LsShape2::D)) return (void *)stev_ls_kernel<LsShape2, false>;
+    if (same_dims(d, LsShape3::D)) return (void *)stev_ls_kernel<LsShape3, true>;
+    if (same_dims(d, LsShape4::D)) return (void *)stev_ls_kernel<LsShape4, true>;
+  }
+  *is_static = false;
+  return d.has_est ? (void *)stev_ls_kernel<LsDyn, true> : (void *)stev_ls_kernel<LsDyn, false>;
+}
+
+int integrate_ls_launch(const LsTables &tb, const unsigned char *d_table, const SolverConsts &sc, double t_f, long long n,
+                        long long ld, double *T, const double *p, double *Y, int *steps, unsigned char *status, int *counters,
+                        cudaStream_t s, int *blocks_out, size_t *smem_out, const int *list, bool allow_static, bool *is_static) {
+  LsArgs a{};
+  a.tb = tb;
+  a.lay = ls_layout_of(tb.d);
+  a.mS = magic(tb.d.S);
+  a.mRrev = magic(tb.d.Rrev);
+  a.mRirr = magic(tb.d.R - tb.d.Rrev);
+  a.mH = magic(tb.d.H);
+  a.mNout = magic(tb.d.n_out);
+  a.mC = magic(tb.d.C);
+  a.table = d_table;
+  a.sc = sc;
+  a.t_f = t_f;
+  a.n_active = n;
+  a.list = list;
+  a.ld = ld;
+  a.T = T;
+  a.p = p;
+  a.Y = Y;
+  a.steps = steps;
+  a.status = status;
+  a.queue_head = counters;
+  a.worst_status = counters + 1;
+  const size_t smem = (size_t)tb.bytes + (size_t)tb.d.C * a.lay.stride;
+  void *fn = ls_kernel_for(tb.d, allow_static, is_static);
+  STEV_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  const long long blocks = std::min<long long>(device_sm_count(), (n + tb.d.C - 1) / tb.d.C);
+  void *args[] = {&a};
+  STEV_CUDA(cudaLaunchKernel(fn, dim3((unsigned)blocks), dim3(kLsThreads), args, smem, s));
+  *blocks_out = (int)blocks;
+  *smem_out = smem;
+  return STEV_OK;
+}
+
+}  // namespace stev

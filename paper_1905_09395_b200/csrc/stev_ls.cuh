@@ -1,0 +1,150 @@
+// stev_ls.cuh -- types shared by the host and device side of the lock-step integrator (stev_ls_kernel.cuh).
+//
+// One block per SM holds C cells that advance in LOCK STEP: every step of the method costs the same work whatever the
+// state (all reactions, all DFT windows), so cells that step together never diverge; what differs between cells is the
+// NUMBER of steps, and a slot whose cell has landed on t_f is refilled from the global queue.  Stepping
+// together lets the block flatten its work over (cell, reaction) and (cell, species) pairs, so no lane idles because a
+// mechanism does not fill a multiple of 32 lanes, and lets ONE warp evaluate the scalar chains (logarithms, divisions,
+// the sequential species sums of the arithmetic contract) of all C cells at once, one cell per lane.
+//
+// Every size and byte offset of the kernel follows from LsDims through ONE constexpr function (ls_layout_of) that the host
+// uses to build the table image and the kernel uses to address it.  The kernel is instantiated once with the dimensions
+// read at run time (any mechanism) and once per entry of the shape list in stev_ls.cu with the dimensions as compile-time
+// constants (offsets become immediates, item loops unroll, divisions by S / R_rev / C become multiplications).
+#pragma once
+#include <cstdint>
+
+#include "stev_device.cuh"
+
+namespace stev {
+
+constexpr int kLsThreads = 512;                 // 16 warps; warp w reaches TMEM lane quarter w % 4
+constexpr int kLsWarps = kLsThreads / 32;
+constexpr int kLsSlots = 4;                     // 32-column window slots per warp: 4 warps per quarter x 4 x 32 = 512 columns
+constexpr int kLsMaxPasses = kLsWarps * kLsSlots;   // 64 warp passes = 2048 DFT windows per block
+constexpr int kLsMaxCells = 32;                 // one lane of the scalar warp per cell
+
+// Scalars of one cell slot.  Written by the cell's lane of the scalar warp unless stated; every field has one writer
+// per phase and is read only after the block barrier that ends that phase.
+struct LsScal {
+  double T, p;                         // state of this step (published at the top of the step)
+  double lnT, ln_c0, invT, inv_ctot, rho;
+  double rem;                          // t_f - t before this step
+  double h_dft, ictot_dft;             // step size and 1/C_tot of the step whose progress the ringing filter stores next
+  unsigned long long tstar_bits;       // running minimum of the limiter (atomicMin of the bit patterns, phase 3)
+  int active;                          // 1: the slot integrates a cell; 0: it waits for a refill (or the queue is empty)
+  int fresh;                           // 1 during the first step of a new cell: window owners zero the history, rOF = 1
+  int dft_on;                          // the step just taken stores its progress (not on a landing step, not without a cell)
+  int bad;                             // non-finite mass fraction seen by the update (atomicOr, phase 4)
+};
+
+struct LsDims {
+  int S, R, Rrev;
+  int n_var;                           // stored multiples of q: 2 (+q, -q) or 4 (+q, -q, +2q, -2q)
+  int has_est, H, n_in, n_out;
+  int C;                               // cell slots per block
+};
+
+// Byte offsets.  Cell scratch (from the cell base, multiples of 16):
+//   oYp double2 [S] {Y_i, 1/W_i} | oYwCp double2 [S] {Y_i/W_i, cp_i/R} | oHOm double2 [S] {h_i/RT, omega_i}
+//   oConc double [1+S] ([0] = 1.0, then C_i**, later dY_i/dt) | oG double [1+2S] ([0] = 0.0, g_i/RT, 2 g_i/RT)
+//   oQ double [n_var][Rp] multiples of q_eff | oRof double [Rrev] | oHid float [H] then the normalised inputs [n_in] | oSc LsScal
+// Table image (from the image base):
+//   o_tmid, o_W, o_invW double [S] | o_nasa double [2][14][S] | o_rkA double2 [R] {ln A, b} | o_rkB double2 [R] {Ea/R_cal, dnu}
+//   o_rfac uint4 [R] offsets (from the cell base) of the two reactant and two product concentration factors (1.0 slot if absent)
+//   o_rdg uint4 [Rrev] offsets of nu*g of the <= 2 reactant / <= 2 product entries (0.0 slot if absent)
+//   o_gsp uint8 [S] species with the r-th longest source-term list | o_grow, o_glen uint16 [S] first row / rows of that list
+//   o_eshift, o_escale float [n_in] | o_W1T float [n_in][H] | o_b1 float [H] | o_W2p float [n_out][Hpad] | o_b2 float [n_out]
+//   o_gent uint4 [rows + 1] (LAST: its length depends on the mechanism's lists) offsets of the stored multiples coef*q_j in
+//          the caller's reaction order, padded with the 0.0 slot; the last row is all padding
+struct LsLayout {
+  int Rp, Hpad;
+  int oYp, oYwCp, oHOm, oConc, oG, oQ, oRof, oHid, oSc, stride;
+  int o_tmid, o_W, o_invW, o_nasa, o_rkA, o_rkB, o_rfac, o_rdg, o_gsp, o_grow, o_glen;
+  int o_eshift, o_escale, o_W1T, o_b1, o_W2p, o_b2, o_gent;
+  int n_rev_pass, n_irr_pass;          // warp passes over the flattened (cell, reversible) / (cell, irreversible) pairs
+};
+
+__host__ __device__ constexpr int ls_align(int x, int a) { return (x + a - 1) / a * a; }
+
+__host__ __device__ constexpr LsLayout ls_layout_of(const LsDims &d) {
+  LsLayout L{};
+  L.Rp = (d.R + 1) & ~1;
+  L.Hpad = d.H + 4;
+  int o = 0;
+  L.oYp = o; o = ls_align(o + 16 * d.S, 16);
+  L.oYwCp = o; o = ls_align(o + 16 * d.S, 16);
+  L.oHOm = o; o = ls_align(o + 16 * d.S, 16);
+  L.oConc = o; o = ls_align(o + 8 * (1 + d.S), 16);
+  L.oG = o; o = ls_align(o + 8 * (1 + 2 * d.S), 16);
+  L.oQ = o; o = ls_align(o + 8 * d.n_var * L.Rp, 16);
+  L.oRof = o; o = ls_align(o + 8 * (d.Rrev > 0 ? d.Rrev : 1), 16);
+  L.oHid = o; o = ls_align(o + 4 * (d.has_est ? d.H + ls_align(d.n_in, 4) : 0), 16);
+  L.oSc = o; o = ls_align(o + (int)sizeof(LsScal), 16);
+  // an odd multiple of 16 bytes: the cells of neighbouring lanes (the scalar warp reads one cell per lane, 16 bytes at a
+  // time) start in different bank groups
+  L.stride = ((o / 16) % 2 == 0) ? o + 16 : o;
+  int t = 0;
+  L.o_tmid = t; t = ls_align(t + 8 * d.S, 16);
+  L.o_W = t; t = ls_align(t + 8 * d.S, 16);
+  L.o_invW = t; t = ls_align(t + 8 * d.S, 16);
+  L.o_nasa = t; t = ls_align(t + 8 * 2 * kNasaRows * d.S, 16);
+  L.o_rkA = t; t = ls_align(t + 16 * d.R, 16);
+  L.o_rkB = t; t = ls_align(t + 16 * d.R, 16);
+  L.o_rfac = t; t = ls_align(t + 16 * d.R, 16);
+  L.o_rdg = t; t = ls_align(t + 16 * (d.Rrev > 0 ? d.Rrev : 1), 16);
+  L.o_gsp = t; t = ls_align(t + d.S, 16);
+  L.o_grow = t; t = ls_align(t + 2 * d.S, 16);
+  L.o_glen = t; t = ls_align(t + 2 * d.S, 16);
+  L.o_eshift = t; t = ls_align(t + 4 * d.n_in, 16);
+  L.o_escale = t; t = ls_align(t + 4 * d.n_in, 16);
+  L.o_W1T = t; t = ls_align(t + 4 * d.n_in * d.H, 16);
+  L.o_b1 = t; t = ls_align(t + 4 * d.H, 16);
+  L.o_W2p = t; t = ls_align(t + 4 * d.n_out * L.Hpad, 16);
+  L.o_b2 = t; t = ls_align(t + 4 * d.n_out, 16);
+  L.o_gent = t;
+  L.n_rev_pass = (d.C * d.Rrev + 31) / 32;
+  L.n_irr_pass = (d.C * (d.R - d.Rrev) + 31) / 32;
+  return L;
+}
+
+// What the host keeps per (mechanism, estimator): the dimensions, the image size and the few values that are not sizes.
+struct LsTables {
+  LsDims d;
+  int act, input_map;
+  float h_ref_T;
+  int g_zero_row;                      // index of the all-padding row of o_gent
+  int bytes;                           // image size
+};
+
+struct LsArgs {
+  LsTables tb;
+  LsLayout lay;                        // ls_layout_of(tb.d)
+  unsigned mS, mRrev, mRirr, mH, mNout, mC;   // ceil(2^32 / d) for the run-time shape: x / d = umulhi(x, m) (0 for d = 1)
+  const unsigned char *table;
+  SolverConsts sc;
+  double t_f;
+  long long n_active;
+  const int *list;
+  long long ld;
+  double *T;
+  const double *p;
+  double *Y;
+  int *steps;
+  unsigned char *status;
+  int *queue_head;
+  int *worst_status;
+};
+
+// Dimensions known at compile time (an entry of the shape list) or read from the arguments.
+struct LsDyn {
+  static constexpr bool kStatic = false;
+  static constexpr LsDims D{};
+};
+template <int S_, int R_, int RREV_, int NVAR_, int EST_, int H_, int NIN_, int NOUT_, int C_>
+struct LsFix {
+  static constexpr bool kStatic = true;
+  static constexpr LsDims D{S_, R_, RREV_, NVAR_, EST_, H_, NIN_, NOUT_, C_};
+};
+
+}  // namespace stev

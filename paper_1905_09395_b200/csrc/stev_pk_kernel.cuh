@@ -756,8 +756,8 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
 
       // -- a6: retirement (R20)
       int st = -1;
-      if (last) st = 0;
-      else if (scal->bad[0] | (NW == 4 ? scal->bad[1] : 0)) st = 2;
+      if (scal->bad[0] | (NW == 4 ? scal->bad[1] : 0)) st = 2;   // checked first: a non-finite landing step is not "finished"
+      else if (last) st = 0;
       else if (steps >= sc.max_steps) st = 1;
       if (st >= 0) {
 #ifdef PK_TIMING
