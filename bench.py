@@ -348,9 +348,8 @@ def main():
     kernel_name = {33: "stev_pk_kernel<1> (one warp per cell, DFT history in tensor memory)",
                    34: "stev_pk_kernel<1, dense> (one warp per cell, 32 cells per SM, DFT history in tensor memory)",
                    64: "stev_pk_kernel<2> (warp pair per cell, DFT history in tensor memory)",
-                   66: "stev_ab_kernel (rate warp + DFT warp per cell)",
-                   96: "stev_pk_kernel<3> (warp triple per cell, DFT history in tensor memory)",
-                   128: "stev_pk_kernel<4> (warp quad per cell, DFT history in tensor memory)"}.get(st["lanes_per_cell"],
+                   512: "stev_ls_kernel (lock-step block, DFT history in tensor memory)",
+                   513: "stev_ls_kernel<LsDyn> (lock-step block, run-time dimensions)"}.get(st["lanes_per_cell"],
                                                                              f"stev_integrate_kernel<{st['lanes_per_cell']}>")
     # DRAM bytes of one launch from ncu (dram__bytes_read.sum + dram__bytes_write.sum), known only for the captured
     # workloads: profiles/r1_groups_cfg3.md (config 3 at full size, default kernel, by launch order)

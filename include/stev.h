@@ -116,9 +116,9 @@ typedef struct {
                              34 = the same at 64 registers, 32 cells per SM (<= 32 species, 1..64 reversible reactions);
                              64 = a warp pair per cell, 8 cells per SM, both warps split every phase of a step
                                   (<= 64 species, 1..256 reversible reactions; the default for >= 128 reactions);
-                             66 = warp-specialised variant of 64 (a rate warp + a DFT warp; also needs dft_enable);
-                             96 = a warp triple per cell, 8 cells per SM, 24 warps of 80 registers per SM (same limits as 64);
-                             128 = a warp quad per cell, 8 cells per SM, 32 warps of 64 registers per SM (same limits as 64) */
+                             512 = lock-step block: up to 32 cells of a block step together, work flattened over (reaction,
+                                  cell) and (species, cell) pairs, one warp for the scalar chains (<= 64 species; the
+                                  default for tiny mechanisms); 513 = the same with run-time dimensions only */
   int32_t order_cells;    /* 1 (default): the persistent kernels pull the cells in order of decreasing temperature
                              (a counting sort on the device before the launch) -- step counts grow with temperature,
                              so the long integrations start first and do not end up running alone.

@@ -14,7 +14,7 @@ HEADERS = ["stev_math.cuh", "stev_device.cuh", "stev_fast.cuh", "stev_pk.cuh", "
 
 # --fmad=false: no implicit FMA contraction anywhere (arithmetic contract); FMAs are explicit.
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "--fmad=false",
-              "-Xcompiler", "-fPIC,-ffp-contract=off,-fvisibility=hidden", "-Xptxas", "-v"]
+              "-Xcompiler", "-fPIC,-ffp-contract=off,-fvisibility=hidden", "-Xptxas", "-v"] + os.environ.get("STEV_EXTRA_NVCC", "").split()
 
 
 def _stale() -> bool:

@@ -13,7 +13,6 @@ namespace stev {
 
 static thread_local std::string g_error;
 static thread_local stev_stats g_stats{};
-static thread_local int g_specialised = 0;
 
 void set_error(const std::string &msg) { g_error = msg; }
 int cuda_fail(cudaError_t e, const char *what) {
@@ -345,8 +344,8 @@ int stev_mechanism_create(const stev_mechanism_desc *d, stev_mechanism **out) {
   build_table_image(h, nullptr, image, m->tb);
   cudaError_t e = cudaMalloc(&m->d_table, image.size());
   if (e == cudaSuccess) e = cudaMemcpy(m->d_table, image.data(), image.size(), cudaMemcpyHostToDevice);
-  for (int n = 0; n < 4 && e == cudaSuccess; ++n) {   // the pair image first: it chooses the reaction order
-    static const int order[4] = {1, 2, 3, 0}, nw_of[4] = {1, 2, 4, 3};
+  for (int n = 0; n < 2 && e == cudaSuccess; ++n) {   // the pair image first: it chooses the reaction order
+    static const int order[2] = {1, 0}, nw_of[2] = {1, 2};
     const int w = order[n];
     std::vector<unsigned char> pk;
     m->pk_ok[w] = build_pk_image(h, nullptr, nw_of[w], pk, m->pk_tb[w], m->pk_cl[w]);
@@ -374,7 +373,7 @@ int stev_mechanism_create(const stev_mechanism_desc *d, stev_mechanism **out) {
 void stev_mechanism_destroy(stev_mechanism *m) {
   if (!m) return;
   if (m->d_table) cudaFree(m->d_table);
-  for (int w = 0; w < 4; ++w)
+  for (int w = 0; w < 2; ++w)
     if (m->d_pk_table[w]) cudaFree(m->d_pk_table[w]);
   if (m->d_ls_table) cudaFree(m->d_ls_table);
   delete m;
@@ -424,8 +423,8 @@ int stev_estimator_load(const stev_mechanism *m, const stev_estimator_desc *d, s
     build_table_image(m->host, &h, image, e->tb);
     ce = cudaMalloc(&e->d_table, image.size());
     if (ce == cudaSuccess) ce = cudaMemcpy(e->d_table, image.data(), image.size(), cudaMemcpyHostToDevice);
-    for (int n = 0; n < 4 && ce == cudaSuccess; ++n) {
-      static const int order[4] = {1, 2, 3, 0}, nw_of[4] = {1, 2, 4, 3};
+    for (int n = 0; n < 2 && ce == cudaSuccess; ++n) {
+      static const int order[2] = {1, 0}, nw_of[2] = {1, 2};
       const int w = order[n];
       std::vector<unsigned char> pk;
       e->pk_ok[w] = build_pk_image(m->host, &h, nw_of[w], pk, e->pk_tb[w], e->pk_cl[w]);
@@ -473,7 +472,7 @@ int stev_estimator_load(const stev_mechanism *m, const stev_estimator_desc *d, s
 void stev_estimator_destroy(stev_estimator *e) {
   if (!e) return;
   if (e->d_table) cudaFree(e->d_table);
-  for (int w = 0; w < 4; ++w)
+  for (int w = 0; w < 2; ++w)
     if (e->d_pk_table[w]) cudaFree(e->d_pk_table[w]);
   if (e->d_ls_table) cudaFree(e->d_ls_table);
   if (e->d_params) cudaFree(e->d_params);
@@ -612,6 +611,17 @@ size_t g_scratch_bytes = 0;
 cudaStream_t g_host_stream = nullptr;
 }  // namespace
 
+// Reads back the worst per-cell status (one int) after the stream has drained and turns it into the return code.
+static int finish_integrate(const int *counters, cudaStream_t s) {
+  int worst = 0;
+  STEV_CUDA(cudaMemcpyAsync(&worst, counters + 1, 4, cudaMemcpyDeviceToHost, s));
+  STEV_CUDA(cudaStreamSynchronize(s));
+  STEV_CUDA(cudaGetLastError());
+  if (worst == 2) { set_error("some cells produced non-finite values (status 2)"); return STEV_WNONFINITE; }
+  if (worst == 1) { set_error("some cells stopped at max_steps (status 1)"); return STEV_WMAXSTEPS; }
+  return STEV_OK;
+}
+
 extern "C" {
 
 size_t stev_workspace_bytes(const stev_mechanism *m, const stev_estimator *e, const stev_params *p, int64_t n_cells) {
@@ -645,34 +655,31 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
   cudaStream_t s = (cudaStream_t)cuda_stream;
   Workspace w = carve(workspace, *tb, p, n);
 
-  // The whole-cell-on-chip kernels with the DFT history in tensor memory.
-  //   lanes_per_cell = 33: one warp per cell, 16 cells per SM (the default when the mechanism fits: <= 32 species,
-  //                        <= 128 reversible reactions)
-  //   lanes_per_cell = 64: warp pair per cell, 8 cells per SM (both warps split every phase; the default for >= 128 reactions)
-  //   lanes_per_cell = 66: warp-specialised kernel (a rate warp and a DFT warp per cell)
-  //   lanes_per_cell = 128: warp quad per cell, 8 cells per SM, 32 warps of 64 registers per SM
-  //   lanes_per_cell = 96: warp triple per cell, 8 cells per SM, 24 warps of 80 registers per SM
+  // The whole-cell-on-chip kernels with the DFT history in tensor memory (all need chunk_steps = 0 and at most two
+  // concentration factors per reaction side):
+  //   lanes_per_cell = 33:  one warp per cell, 16 cells per SM (<= 32 species, <= 128 reversible reactions)
+  //   lanes_per_cell = 34:  the same at 64 registers, 32 cells per SM (<= 64 reversible reactions)
+  //   lanes_per_cell = 64:  warp pair per cell, 8 cells per SM (both warps split every phase; the default for >= 128 reactions)
+  //   lanes_per_cell = 512: lock-step block (all cells of a block step together; the default for tiny mechanisms);
+  //                   513:  the same with the dimensions read at run time even if the shape list has the mechanism
   int g_request = p->lanes_per_cell;   // group width handed to the shared-memory-history kernel (0: its own heuristic)
   {
     const bool tm_common = p->chunk_steps == 0;
     const bool pk1_ok = (est ? est->pk_ok[0] : m->pk_ok[0]) && tm_common;
     const bool pk2_ok = (est ? est->pk_ok[1] : m->pk_ok[1]) && tm_common;
-    const bool pk4_ok = (est ? est->pk_ok[2] : m->pk_ok[2]) && tm_common;
-    const bool pk3_ok = (est ? est->pk_ok[3] : m->pk_ok[3]) && tm_common;
     const bool ls_ok = (est ? est->ls_ok : m->ls_ok) && tm_common;
-    int kind = 0;   // 0: sub-warp groups (history in shared memory), 1: one warp per cell, 2: warp pair, 3: warp-specialised, 4: warp quad, 5: warp triple
+    const bool dense_ok = pk1_ok && pk_dense_ok(est ? est->pk_tb[0] : m->pk_tb[0]);
+    int kind = 0;   // 0: sub-warp groups (history in shared memory), 1: one warp per cell, 2: warp pair, 6: dense one warp per cell, 7: lock step
     if (p->lanes_per_cell == 33) kind = 1;
     else if (p->lanes_per_cell == 64) kind = 2;
-    else if (p->lanes_per_cell == 512 || p->lanes_per_cell == 513) kind = 7;   // lock-step block (stev_ls_kernel.cuh); 513: run-time dimensions only
-    else if (p->lanes_per_cell == 128) kind = 4;
-    else if (p->lanes_per_cell == 96) kind = 5;
-    else if (p->lanes_per_cell == 34) kind = 6;   // one warp per cell, dense (32 cells per SM at 64 registers)
+    else if (p->lanes_per_cell == 34) kind = 6;
+    else if (p->lanes_per_cell == 512 || p->lanes_per_cell == 513) kind = 7;
     else if (p->lanes_per_cell == 0) {
       // Measured on B200: large mechanisms -> warp pair; tiny ones (a step is a few hundred
-      // instructions, most lanes of a warp idle) -> sub-warp groups with the history in shared memory; mid-size -> one
-      // warp per cell, 32 cells per SM when the reversible reactions fit two 32-blocks, else 16.
-      const bool dense_ok = pk1_ok && pk_dense_ok(est ? est->pk_tb[0] : m->pk_tb[0]);
+      // instructions) -> lock-step block, which flattens (cell, reaction) pairs over the lanes; mid-size -> one warp per
+      // cell, 32 cells per SM when the reversible reactions fit two 32-blocks, else 16.
       if (tb->R >= 128 && pk2_ok) kind = 2;
+      else if (tb->S <= 16 && tb->R <= 32 && ls_ok) kind = 7;
       else if (tb->S <= 16 && tb->R <= 32) {
         kind = 0;
         g_request = 4;
@@ -680,12 +687,12 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
       } else if (dense_ok) kind = 6;
       else if (pk1_ok) kind = 1;
       else if (pk2_ok && tb->R >= 64) kind = 2;
+      else if (ls_ok) kind = 7;
     }
-    if ((kind == 1 && !pk1_ok) || (kind == 2 && !pk2_ok) || (kind == 7 && !ls_ok) || (kind == 4 && !pk4_ok) ||
-        (kind == 5 && !pk3_ok) || (kind == 6 && !(pk1_ok && pk_dense_ok(est ? est->pk_tb[0] : m->pk_tb[0])))) {
-      set_error("stev_integrate: lanes_per_cell = 33 / 64 / 66 / 96 / 128 (tensor-memory kernels) need chunk_steps = 0, at most two factors "
-                "per reaction side, 1..128 (33) or 1..256 (64, 66, 96, 128) reversible reactions, at most 32 (33) or 64 species "
-                "(66 also dft_enable = 1)");
+    if ((kind == 1 && !pk1_ok) || (kind == 2 && !pk2_ok) || (kind == 6 && !dense_ok) || (kind == 7 && !ls_ok)) {
+      set_error("stev_integrate: lanes_per_cell = 33 / 34 / 64 / 512 / 513 (tensor-memory kernels) need chunk_steps = 0, at most two "
+                "factors per reaction side, 1..128 (33), 1..64 (34) or 1..256 (64) reversible reactions, at most 32 (33, 34) or 64 "
+                "species");
       return STEV_EINVAL;
     }
     if (kind) {
@@ -696,7 +703,7 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
         if (rc) return rc;
         order = w.order;
       }
-      int blocks = 0, cpb = 0;
+      int blocks = 0, cpb = 0, threads = kPkThreads, specialised = 0;
       size_t smem = 0;
       if (kind == 7) {
         const stev::LsTables &ltb = est ? est->ls_tb : m->ls_tb;
@@ -704,30 +711,25 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
         rc = integrate_ls_launch(ltb, est ? est->d_ls_table : m->d_ls_table, make_consts(p), dt_cfd, n, ld, T, pressure, Y,
                                  steps_out, status_out, w.counters, s, &blocks, &smem, order, p->lanes_per_cell != 513, &is_static);
         cpb = ltb.d.C;
-        g_specialised = is_static ? 1 : 0;
+        threads = kLsThreads;
+        specialised = is_static ? 1 : 0;
       } else {
-        const int wi = (kind == 4) ? 2 : (kind == 5 ? 3 : (kind == 6 ? 0 : kind - 1));
+        const int wi = (kind == 2) ? 1 : 0;
         rc = integrate_pk_launch(est ? est->pk_tb[wi] : m->pk_tb[wi], est ? est->pk_cl[wi] : m->pk_cl[wi],
                                  est ? est->d_pk_table[wi] : m->d_pk_table[wi], make_consts(p), dt_cfd, n, ld, T, pressure, Y,
                                  steps_out, status_out, w.counters, s, &blocks, &cpb, &smem, kind == 6, order);
+        threads = (kind == 6) ? kPkThreads4 : kPkThreads;
       }
       if (rc) return rc;
-      int worst = 0;
-      STEV_CUDA(cudaMemcpyAsync(&worst, w.counters + 1, 4, cudaMemcpyDeviceToHost, s));
-      STEV_CUDA(cudaStreamSynchronize(s));
-      STEV_CUDA(cudaGetLastError());
       g_stats.passes = 1;
-      g_stats.specialised = g_specialised;
+      g_stats.specialised = specialised;
       g_stats.kernel_launches = 1 + (order ? 3 : 0);   // integrator + histogram, scan, scatter of the launch order
       g_stats.blocks = blocks;
-      g_stats.lanes_per_cell = kind == 1 ? 33 : (kind == 2 ? 64 : (kind == 7 ? p->lanes_per_cell : (kind == 4 ? 128 : (kind == 5 ? 96 : 34))));
-      g_stats.threads_per_block =
-          kind == 7 ? kLsThreads : ((kind == 4 || kind == 6) ? kPkThreads4 : (kind == 5 ? kPkThreads3 : kPkThreads));
+      g_stats.lanes_per_cell = kind == 1 ? 33 : (kind == 2 ? 64 : (kind == 6 ? 34 : (p->lanes_per_cell == 513 ? 513 : 512)));
+      g_stats.threads_per_block = threads;
       g_stats.cells_per_block = cpb;
       g_stats.smem_bytes = (int64_t)smem;
-      if (worst == 2) { set_error("some cells produced non-finite values (status 2)"); return STEV_WNONFINITE; }
-      if (worst == 1) { set_error("some cells stopped at max_steps (status 1)"); return STEV_WMAXSTEPS; }
-      return STEV_OK;
+      return finish_integrate(w.counters, s);
     }
   }
 
@@ -790,17 +792,11 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
     n_active = count;
     cur ^= 1;
   }
-  int worst = 0;
-  STEV_CUDA(cudaMemcpyAsync(&worst, w.counters + 1, 4, cudaMemcpyDeviceToHost, s));
-  STEV_CUDA(cudaStreamSynchronize(s));
-  STEV_CUDA(cudaGetLastError());
   g_stats.lanes_per_cell = cfg.G;
   g_stats.threads_per_block = cfg.threads;
   g_stats.cells_per_block = cfg.cells_per_block;
   g_stats.smem_bytes = (int64_t)cfg.smem;
-  if (worst == 2) { set_error("some cells produced non-finite values (status 2)"); return STEV_WNONFINITE; }
-  if (worst == 1) { set_error("some cells stopped at max_steps (status 1)"); return STEV_WMAXSTEPS; }
-  return STEV_OK;
+  return finish_integrate(w.counters, s);
 }
 
 // ---------------------------------------------------------------------------------------------------------

@@ -90,10 +90,10 @@ struct stev_mechanism {
   stev::HostMechanism host;
   stev::DevTables tb{};
   unsigned char *d_table = nullptr;
-  bool pk_ok[4] = {false, false, false, false};   // images of the tensor-memory kernel: [0] one warp per cell, [1] pair, [2] quad, [3] triple (NASA-7 thermo)
-  stev::PkTables pk_tb[4]{};
-  stev::PkCell pk_cl[4]{};
-  unsigned char *d_pk_table[4] = {nullptr, nullptr, nullptr, nullptr};
+  bool pk_ok[2] = {false, false};         // images of the tensor-memory kernel: [0] one warp per cell, [1] pair (NASA-7 thermo)
+  stev::PkTables pk_tb[2]{};
+  stev::PkCell pk_cl[2]{};
+  unsigned char *d_pk_table[2] = {nullptr, nullptr};
   bool ls_ok = false;                    // image of the lock-step kernel (NASA-7 thermo)
   stev::LsTables ls_tb{};
   unsigned char *d_ls_table = nullptr;
@@ -104,10 +104,10 @@ struct stev_estimator {
   const stev_mechanism *mech = nullptr;  // the mechanism it was loaded against (may be null)
   stev::DevTables tb{};                  // mechanism + estimator image (only if mech != null)
   unsigned char *d_table = nullptr;
-  bool pk_ok[4] = {false, false, false, false};   // images of the tensor-memory kernel (MLP thermo)
-  stev::PkTables pk_tb[4]{};
-  stev::PkCell pk_cl[4]{};
-  unsigned char *d_pk_table[4] = {nullptr, nullptr, nullptr, nullptr};
+  bool pk_ok[2] = {false, false};         // images of the tensor-memory kernel (MLP thermo)
+  stev::PkTables pk_tb[2]{};
+  stev::PkCell pk_cl[2]{};
+  unsigned char *d_pk_table[2] = {nullptr, nullptr};
   bool ls_ok = false;                    // image of the lock-step kernel (MLP thermo)
   stev::LsTables ls_tb{};
   unsigned char *d_ls_table = nullptr;

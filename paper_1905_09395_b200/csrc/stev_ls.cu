@@ -66,7 +66,7 @@ bool build_ls_image(const HostMechanism &m, const HostEstimator *e, std::vector<
     }
   d.n_var = has2 ? 4 : 2;
   d.C = 1;
-  LsLayout L = ls_layout_of(d);   // cell and table offsets do not depend on C
+  LsLayout L = ls_layout_of(d);   // table offsets do not depend on C
 
   // internal reaction order: reversible first; within each group the bank-conflict-aware order of the pair kernel if
   // the mechanism has one (stev_pk.cu), else the caller's
@@ -92,11 +92,14 @@ bool build_ls_image(const HostMechanism &m, const HostEstimator *e, std::vector<
 
   // cell slots per block: one lane of the scalar warp each, 2048 DFT windows in tensor memory, shared memory
   const size_t avail = kSmemMax > (size_t)tb.bytes + 1024 ? kSmemMax - (size_t)tb.bytes - 1024 : 0;
-  int C = (int)std::min<size_t>(kLsMaxCells, avail / (size_t)L.stride);
+  int C = kLsMaxCells;
   if (Rrev > 0) C = std::min(C, (32 * kLsMaxPasses) / Rrev);
+  for (; C >= 1; --C) {
+    d.C = C;
+    L = ls_layout_of(d);
+    if ((size_t)L.cell_bytes <= avail) break;
+  }
   if (C < 1) return false;
-  d.C = C;
-  L = ls_layout_of(d);
 
   image.assign(tb.bytes, 0);
   unsigned char *base = image.data();
@@ -126,15 +129,15 @@ bool build_ls_image(const HostMechanism &m, const HostEstimator *e, std::vector<
     unsigned dgo[4] = {zero_slot, zero_slot, zero_slot, zero_slot};
     int nf = 0, ne = 0;
     for (int en = m.reac_ptr[j]; en < m.reac_ptr[j + 1]; ++en, ++ne) {
-      for (int n = 0; n < m.reac_nu[en]; ++n) fac[nf++] = (unsigned)(L.oConc + 8 * (1 + m.reac_sp[en]));
-      dgo[ne] = (unsigned)(L.oG + 8 * (1 + (m.reac_nu[en] == 2 ? S : 0) + m.reac_sp[en]));
+      for (int n = 0; n < m.reac_nu[en]; ++n) fac[nf++] = (unsigned)(L.oConc + 8 * C * (1 + m.reac_sp[en]));
+      dgo[ne] = (unsigned)(L.oG + 8 * C * (1 + (m.reac_nu[en] == 2 ? S : 0) + m.reac_sp[en]));
       dnu = dnu - (double)m.reac_nu[en];
     }
     nf = 2;
     ne = 2;
     for (int en = m.prod_ptr[j]; en < m.prod_ptr[j + 1]; ++en, ++ne) {
-      for (int n = 0; n < m.prod_nu[en]; ++n) fac[nf++] = (unsigned)(L.oConc + 8 * (1 + m.prod_sp[en]));
-      dgo[ne] = (unsigned)(L.oG + 8 * (1 + (m.prod_nu[en] == 2 ? S : 0) + m.prod_sp[en]));
+      for (int n = 0; n < m.prod_nu[en]; ++n) fac[nf++] = (unsigned)(L.oConc + 8 * C * (1 + m.prod_sp[en]));
+      dgo[ne] = (unsigned)(L.oG + 8 * C * (1 + (m.prod_nu[en] == 2 ? S : 0) + m.prod_sp[en]));
       dnu = dnu + (double)m.prod_nu[en];
     }
     rkA[2 * k] = clog(m.A[j]);
@@ -154,7 +157,7 @@ bool build_ls_image(const HostMechanism &m, const HostEstimator *e, std::vector<
     grow[r] = (unsigned short)row0[r];
     glen[r] = (unsigned short)rows[r];
     for (int en = 0; en < (int)gl[i].size(); ++en)
-      gent[4 * row0[r] + en] = (unsigned)(L.oQ + 8 * (variant_of(gl[i][en].coef) * L.Rp + internal_of[gl[i][en].j]));
+      gent[4 * row0[r] + en] = (unsigned)(L.oQ + 8 * C * (variant_of(gl[i][en].coef) * L.Rp + internal_of[gl[i][en].j]));
   }
   if (e) {
     float *sh = (float *)(base + L.o_eshift), *scl = (float *)(base + L.o_escale), *W1T = (float *)(base + L.o_W1T);
@@ -208,11 +211,6 @@ int integrate_ls_launch(const LsTables &tb, const unsigned char *d_table, const 
   LsArgs a{};
   a.tb = tb;
   a.lay = ls_layout_of(tb.d);
-  a.mS = magic(tb.d.S);
-  a.mRrev = magic(tb.d.Rrev);
-  a.mRirr = magic(tb.d.R - tb.d.Rrev);
-  a.mH = magic(tb.d.H);
-  a.mNout = magic(tb.d.n_out);
   a.mC = magic(tb.d.C);
   a.table = d_table;
   a.sc = sc;
@@ -227,7 +225,7 @@ int integrate_ls_launch(const LsTables &tb, const unsigned char *d_table, const 
   a.status = status;
   a.queue_head = counters;
   a.worst_status = counters + 1;
-  const size_t smem = (size_t)tb.bytes + (size_t)tb.d.C * a.lay.stride;
+  const size_t smem = (size_t)tb.bytes + (size_t)a.lay.cell_bytes;
   void *fn = ls_kernel_for(tb.d, allow_static, is_static);
   STEV_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   const long long blocks = std::min<long long>(device_sm_count(), (n + tb.d.C - 1) / tb.d.C);

@@ -24,18 +24,20 @@ constexpr int kLsSlots = 4;                     // 32-column window slots per wa
 constexpr int kLsMaxPasses = kLsWarps * kLsSlots;   // 64 warp passes = 2048 DFT windows per block
 constexpr int kLsMaxCells = 32;                 // one lane of the scalar warp per cell
 
-// Scalars of one cell slot.  Written by the cell's lane of the scalar warp unless stated; every field has one writer
-// per phase and is read only after the block barrier that ends that phase.
-struct LsScal {
-  double T, p;                         // state of this step (published at the top of the step)
-  double lnT, ln_c0, invT, inv_ctot, rho;
-  double rem;                          // t_f - t before this step
-  double h_dft, ictot_dft;             // step size and 1/C_tot of the step whose progress the ringing filter stores next
-  unsigned long long tstar_bits;       // running minimum of the limiter (atomicMin of the bit patterns, phase 3)
-  int active;                          // 1: the slot integrates a cell; 0: it waits for a refill (or the queue is empty)
-  int fresh;                           // 1 during the first step of a new cell: window owners zero the history, rOF = 1
-  int dft_on;                          // the step just taken stores its progress (not on a landing step, not without a cell)
-  int bad;                             // non-finite mass fraction seen by the update (atomicOr, phase 4)
+// Scalars of the cell slots, one array of C eight-byte entries per field (entry (f, c) at oSc + (f C + c) 8).  Written by the
+// cell's lane of the scalar warp unless stated; every field has one writer per phase and is read only after the block
+// barrier that ends that phase.
+enum LsField {
+  kF_T, kF_P,                          // state of this step (published at the top of the step)
+  kF_LNT, kF_LNC0, kF_INVT, kF_ICTOT, kF_RHO,
+  kF_REM,                              // t_f - t before this step
+  kF_HDFT, kF_ICDFT,                   // step size and 1/C_tot of the step whose progress the ringing filter stores next
+  kF_TSTAR,                            // u64: running minimum of the limiter (atomicMin of the bit patterns, phase 3)
+  kF_ACTIVE,                           // int: 1 the slot integrates a cell; 0 it waits for a refill (or the queue is empty)
+  kF_FRESH,                            // int: 1 during the first step of a new cell: window owners zero the history, rOF = 1
+  kF_DFTON,                            // int: the step just taken stores its progress (not on a landing step, not without a cell)
+  kF_BAD,                              // int: non-finite mass fraction seen by the update (atomicOr, phase 4)
+  kF_COUNT
 };
 
 struct LsDims {
@@ -45,24 +47,28 @@ struct LsDims {
   int C;                               // cell slots per block
 };
 
-// Byte offsets.  Cell scratch (from the cell base, multiples of 16):
-//   oYp double2 [S] {Y_i, 1/W_i} | oYwCp double2 [S] {Y_i/W_i, cp_i/R} | oHOm double2 [S] {h_i/RT, omega_i}
-//   oConc double [1+S] ([0] = 1.0, then C_i**, later dY_i/dt) | oG double [1+2S] ([0] = 0.0, g_i/RT, 2 g_i/RT)
-//   oQ double [n_var][Rp] multiples of q_eff | oRof double [Rrev] | oHid float [H] then the normalised inputs [n_in] | oSc LsScal
+// Byte offsets.  The working set of the block's C cells is stored INDEX-MAJOR, CELL-MINOR: element (idx, c) of an array at
+// offset o sits at o + (idx C + c) 8, so that lanes holding consecutive cells of the same species / reaction read
+// consecutive addresses (and the per-reaction tables are read by broadcast).  From the start of the cell region:
+//   oY [S] | oYw [S] Y_i/W_i | oCp [S] cp_i/R | oH [S] h_i/RT | oOm [S] omega_i
+//   oConc [1+S] ([0] = 1.0, then C_i**, later dY_i/dt) | oG [1+2S] ([0] = 0.0, g_i/RT, 2 g_i/RT)
+//   oQ [n_var][Rp] multiples of q_eff | oRof [Rrev] | oSc [kF_COUNT] the scalars
+//   oHid float [C][Hs] hidden activations, cell-major with Hs = H + 4 | oXn float [n_in][C] normalised estimator inputs
 // Table image (from the image base):
 //   o_tmid, o_W, o_invW double [S] | o_nasa double [2][14][S] | o_rkA double2 [R] {ln A, b} | o_rkB double2 [R] {Ea/R_cal, dnu}
-//   o_rfac uint4 [R] offsets (from the cell base) of the two reactant and two product concentration factors (1.0 slot if absent)
+//   o_rfac uint4 [R] offsets (from the cell region, for cell 0) of the two reactant and two product concentration factors
+//          (the 1.0 slot if absent)
 //   o_rdg uint4 [Rrev] offsets of nu*g of the <= 2 reactant / <= 2 product entries (0.0 slot if absent)
 //   o_gsp uint8 [S] species with the r-th longest source-term list | o_grow, o_glen uint16 [S] first row / rows of that list
 //   o_eshift, o_escale float [n_in] | o_W1T float [n_in][H] | o_b1 float [H] | o_W2p float [n_out][Hpad] | o_b2 float [n_out]
 //   o_gent uint4 [rows + 1] (LAST: its length depends on the mechanism's lists) offsets of the stored multiples coef*q_j in
 //          the caller's reaction order, padded with the 0.0 slot; the last row is all padding
 struct LsLayout {
-  int Rp, Hpad;
-  int oYp, oYwCp, oHOm, oConc, oG, oQ, oRof, oHid, oSc, stride;
+  int Rp, Hpad, Hs;
+  int oY, oYw, oCp, oH, oOm, oConc, oG, oQ, oRof, oSc, oHid, oXn, cell_bytes;
   int o_tmid, o_W, o_invW, o_nasa, o_rkA, o_rkB, o_rfac, o_rdg, o_gsp, o_grow, o_glen;
   int o_eshift, o_escale, o_W1T, o_b1, o_W2p, o_b2, o_gent;
-  int n_rev_pass, n_irr_pass;          // warp passes over the flattened (cell, reversible) / (cell, irreversible) pairs
+  int n_rev_pass, n_irr_pass;          // warp passes over the flattened (reversible reaction, cell) / (irreversible, cell) pairs
 };
 
 __host__ __device__ constexpr int ls_align(int x, int a) { return (x + a - 1) / a * a; }
@@ -71,19 +77,22 @@ __host__ __device__ constexpr LsLayout ls_layout_of(const LsDims &d) {
   LsLayout L{};
   L.Rp = (d.R + 1) & ~1;
   L.Hpad = d.H + 4;
+  L.Hs = d.H + 4;
+  const int C = d.C;
   int o = 0;
-  L.oYp = o; o = ls_align(o + 16 * d.S, 16);
-  L.oYwCp = o; o = ls_align(o + 16 * d.S, 16);
-  L.oHOm = o; o = ls_align(o + 16 * d.S, 16);
-  L.oConc = o; o = ls_align(o + 8 * (1 + d.S), 16);
-  L.oG = o; o = ls_align(o + 8 * (1 + 2 * d.S), 16);
-  L.oQ = o; o = ls_align(o + 8 * d.n_var * L.Rp, 16);
-  L.oRof = o; o = ls_align(o + 8 * (d.Rrev > 0 ? d.Rrev : 1), 16);
-  L.oHid = o; o = ls_align(o + 4 * (d.has_est ? d.H + ls_align(d.n_in, 4) : 0), 16);
-  L.oSc = o; o = ls_align(o + (int)sizeof(LsScal), 16);
-  // an odd multiple of 16 bytes: the cells of neighbouring lanes (the scalar warp reads one cell per lane, 16 bytes at a
-  // time) start in different bank groups
-  L.stride = ((o / 16) % 2 == 0) ? o + 16 : o;
+  L.oY = o; o = ls_align(o + 8 * C * d.S, 16);
+  L.oYw = o; o = ls_align(o + 8 * C * d.S, 16);
+  L.oCp = o; o = ls_align(o + 8 * C * d.S, 16);
+  L.oH = o; o = ls_align(o + 8 * C * d.S, 16);
+  L.oOm = o; o = ls_align(o + 8 * C * d.S, 16);
+  L.oConc = o; o = ls_align(o + 8 * C * (1 + d.S), 16);
+  L.oG = o; o = ls_align(o + 8 * C * (1 + 2 * d.S), 16);
+  L.oQ = o; o = ls_align(o + 8 * C * d.n_var * L.Rp, 16);
+  L.oRof = o; o = ls_align(o + 8 * C * (d.Rrev > 0 ? d.Rrev : 1), 16);
+  L.oSc = o; o = ls_align(o + 8 * C * (int)kF_COUNT, 16);
+  L.oHid = o; o = ls_align(o + 4 * C * (d.has_est ? L.Hs : 0), 16);
+  L.oXn = o; o = ls_align(o + 4 * C * (d.has_est ? d.n_in : 0), 16);
+  L.cell_bytes = o;
   int t = 0;
   L.o_tmid = t; t = ls_align(t + 8 * d.S, 16);
   L.o_W = t; t = ls_align(t + 8 * d.S, 16);
@@ -103,8 +112,8 @@ __host__ __device__ constexpr LsLayout ls_layout_of(const LsDims &d) {
   L.o_W2p = t; t = ls_align(t + 4 * d.n_out * L.Hpad, 16);
   L.o_b2 = t; t = ls_align(t + 4 * d.n_out, 16);
   L.o_gent = t;
-  L.n_rev_pass = (d.C * d.Rrev + 31) / 32;
-  L.n_irr_pass = (d.C * (d.R - d.Rrev) + 31) / 32;
+  L.n_rev_pass = (C * d.Rrev + 31) / 32;
+  L.n_irr_pass = (C * (d.R - d.Rrev) + 31) / 32;
   return L;
 }
 
@@ -120,7 +129,7 @@ struct LsTables {
 struct LsArgs {
   LsTables tb;
   LsLayout lay;                        // ls_layout_of(tb.d)
-  unsigned mS, mRrev, mRirr, mH, mNout, mC;   // ceil(2^32 / d) for the run-time shape: x / d = umulhi(x, m) (0 for d = 1)
+  unsigned mC;                         // ceil(2^32 / C) for the run-time shape: x / C = umulhi(x, mC) (0 for C = 1)
   const unsigned char *table;
   SolverConsts sc;
   double t_f;

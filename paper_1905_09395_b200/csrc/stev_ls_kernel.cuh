@@ -2,21 +2,25 @@
 //
 // A step of the block (all C cell slots together) is five phases separated by block barriers:
 //   0  scalar warp, one cell per lane: retirement / refill from the queue (a6), T-dependent scalars, 1/Wbar (sequential
-//      sum), estimator inputs;  all warps: the ringing filter (a5) of the step just taken, over (cell, reversible
-//      reaction) pairs -- it only feeds rOF, which phase 2 reads
-//   1  (cell, species) pairs: NASA-7 g/RT (+ cp, h without estimator), stabilised concentrations;
-//      (cell, hidden unit) pairs: first estimator layer (a7)
-//   2  (cell, output) pairs: second estimator layer;  (cell, reaction) pairs: rates (a2), q_eff = q rOF, stored multiples
-//   3  (cell, species) pairs: source terms gathered in the caller's reaction order, limiter (a3), atomicMin per cell
-//   4  (cell, species) pairs: step size, Euler update (a4);  scalar warp: the two sequential sums of the temperature
+//      sum), estimator inputs
+//   1  (species, cell) pairs: NASA-7 g/RT (+ cp, h without estimator), stabilised concentrations;
+//      (hidden unit, cell) pairs: first estimator layer (a7)
+//   2  (reaction, cell) pairs: rates (a2), q_eff = q rOF, stored multiples
+//   3  (species, cell) pairs: source terms gathered in the caller's reaction order, limiter (a3), atomicMin per cell;
+//      (output, cell) pairs: second estimator layer (it only feeds the temperature equation)
+//   4  (species, cell) pairs: step size, Euler update (a4);  scalar warp: the two sequential sums of the temperature
 //      equation, T, t, step count
-// The 13-deep history of every reversible reaction lives in TENSOR MEMORY: pass p of 32 consecutive (cell, reaction)
+// The ringing filter (a5) of a step only feeds rOF, which the rates of the NEXT step read, and the thread that owns a
+// (reaction, cell) pair owns its DFT window, its rOF and its rate.  Its filter passes are therefore free to run anywhere
+// between phase 4 (the step size is known) and the pair's own rate evaluation in phase 2 of the next step: each warp runs
+// one of its (up to four) passes in phase 4, 0, 1 and 2, so the fp64-bound filter fills the phases that are bound by the
+// latency of the scalar chains or by shared-memory bandwidth.
+// The 13-deep history of every reversible reaction lives in TENSOR MEMORY: pass p of 32 consecutive (reaction, cell)
 // pairs belongs to warp p % 16 and sits in one 32-column slot of that warp's TMEM lane quarter.  tcgen05.st writes one
 // column pair for all 32 lanes at once, so all cells of a block share the ring position: a slot is refilled only when
 // the block's step counter is a multiple of 13 (the new cell then starts at physical slot 0, as the contract's R10 wants;
 // a landed cell waits at most 12 steps, < 1.5 % of the shortest integrations of the five configurations).
-// Arithmetic follows the contract of DESIGN.md section 5 exactly; the per-item arithmetic is the one of
-// stev_pk_kernel.cuh, operation for operation.
+// Arithmetic follows the contract of DESIGN.md section 5 exactly.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -28,13 +32,6 @@
 
 namespace stev {
 
-// x / d for the small item counts of this kernel (x * d < 2^32): by a compile-time divisor when the shape is static,
-// else through m = ceil(2^32 / d) (0 for d = 1)
-template <class SH>
-__device__ __forceinline__ unsigned ls_div(unsigned x, int d, unsigned m) {
-  if (SH::kStatic) return x / (unsigned)(d > 0 ? d : 1);
-  return m ? __umulhi(x, m) : x;
-}
 template <class SH>
 struct LsConst {
   static constexpr LsLayout L = ls_layout_of(SH::D);
@@ -42,8 +39,19 @@ struct LsConst {
 // dimension / layout field: a compile-time constant for a static shape, else read from the kernel arguments
 #define LS_D(f) (SH::kStatic ? SH::D.f : a.tb.d.f)
 #define LS_L(f) (SH::kStatic ? LsConst<SH>::L.f : a.lay.f)
+// element (idx, c) of the cell-region array at byte offset `off` (index-major, cell-minor)
+#define LS_AT(type, off, idx, c) (*(type *)(cells + (off) + ((unsigned)((idx) * C + (c)) << 3)))
+#define LS_SC(type, field, c) LS_AT(type, LS_L(oSc), (int)(field), c)
 
 constexpr unsigned kFull = 0xffffffffu;
+
+// x / C for the small item counts of this kernel (x * C < 2^32): by a compile-time divisor when the shape is static,
+// else through m = ceil(2^32 / C) (0 for C = 1)
+template <class SH>
+__device__ __forceinline__ unsigned ls_div_c(unsigned x, int C, unsigned m) {
+  if (SH::kStatic) return x / (unsigned)(C > 0 ? C : 1);
+  return m ? __umulhi(x, m) : x;
+}
 
 // 26 consecutive columns of this lane back to tensor memory (x16 + x8 + x2)
 __device__ __forceinline__ void tmem_st26(uint32_t taddr, const uint32_t (&r)[26]) {
@@ -59,148 +67,206 @@ __device__ __forceinline__ void tmem_st26(uint32_t taddr, const uint32_t (&r)[26
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// a5: the ringing filter (Eqs 8-13) of this warp's passes over the (cell, reversible reaction) pairs.
+// a5: the ringing filter (Eqs 8-13) of pass `s` of this warp over the (reversible reaction, cell) pairs.
 // slot13: ring position of the step whose applied change in progress is stored (the same for every cell of the block).
+// IN_P4: the pass runs in phase 4 of that very step: the step size follows from the limiter's minimum (as in the
+// update); otherwise it is read from the fields the scalar warp left in phase 4.
 // ---------------------------------------------------------------------------------------------------------
-template <class SH, int NHF>
-__device__ __forceinline__ void ls_dft_passes(const LsArgs &a, unsigned char *cells, uint32_t trow, int slot13, int warp, int lane) {
+template <class SH, int NHF, bool IN_P4>
+__device__ __forceinline__ void ls_dft_pass(const LsArgs &a, unsigned char *cells, uint32_t trow, int s, int slot13, int warp,
+                                            int lane, double dt_max, double t_tol) {
   const SolverConsts &sc = a.sc;
-  const int Rrev = LS_D(Rrev), n_rev_pass = LS_L(n_rev_pass);
-  const unsigned n_items = (unsigned)(LS_D(C) * Rrev);
-#pragma unroll
-  for (int s = 0; s < kLsSlots; ++s) {
-    const int p = warp + s * kLsWarps;
-    if (p >= n_rev_pass) break;
-    unsigned f = (unsigned)(p * 32 + lane);
-    const bool valid = f < n_items;
-    f = valid ? f : n_items - 1;
-    const unsigned c = ls_div<SH>(f, Rrev, a.mRrev), k = f - c * (unsigned)Rrev;
-    unsigned char *cell = cells + c * (unsigned)LS_L(stride);
-    const LsScal *scl = (const LsScal *)(cell + LS_L(oSc));
-    const bool on = valid && scl->dft_on;
-    if (!__any_sync(kFull, on)) continue;   // landing steps and empty slots store nothing
-    double *cRof = (double *)(cell + LS_L(oRof));
-    const double q = ((const double *)(cell + LS_L(oQ)))[k];
-    const uint32_t tw = trow + (uint32_t)(s * 32);
-    // Eq 8 with R8, R9: the applied change in progress / C_tot.  (Lanes whose cell is not `on` overwrite a window that is
-    // zeroed before its next use.)
-    tmem_st2(tw + 2 * slot13, (q * scl->h_dft) * scl->ictot_dft);
-    tmem_wait_st();
-    uint32_t ra[26];
-    tmem_ld26(tw, ra);
-    tmem_wait_ld();
-    double x[kWindow];
-    unpack_window(ra, x);
-    double d0, m2;
-    ab_window_stats<NHF>(x, d0, m2);
-    bool sure;
-    bool ringing = ab_ring_filter(d0, m2, sc, sure);
-    if (__any_sync(kFull, !sure && on)) ringing = ab_ring_exact(d0, m2, sc);
-    if (on) {
-      double rof = cRof[k] * (ringing ? sc.inv_r_fac : sc.r_fac);   // Eqs 12-13
-      if (rof > 1.0) rof = 1.0;
-      if (rof < sc.rof_min) rof = sc.rof_min;
-      cRof[k] = rof;
-    }
+  const int C = LS_D(C);
+  const int p = warp + s * kLsWarps;
+  if (p >= LS_L(n_rev_pass)) return;
+  const unsigned n_items = (unsigned)(C * LS_D(Rrev));
+  unsigned f = (unsigned)(p * 32 + lane);
+  const bool valid = f < n_items;
+  f = valid ? f : n_items - 1;
+  const unsigned k = ls_div_c<SH>(f, C, a.mC), c = f - k * (unsigned)C;
+  bool on;
+  double h, ic;
+  if (IN_P4) {
+    const double t_star = bits_to_double(LS_SC(unsigned long long, kF_TSTAR, c));
+    h = (t_star < dt_max) ? t_star : dt_max;
+    const double rem = LS_SC(double, kF_REM, c);
+    const bool lst = rem - h < t_tol;
+    h = lst ? rem : h;
+    ic = LS_SC(double, kF_ICTOT, c);
+    on = valid && LS_SC(int, kF_ACTIVE, c) && !lst;   // the landing step's change is never looked at: the cell retires
+  } else {
+    h = LS_SC(double, kF_HDFT, c);
+    ic = LS_SC(double, kF_ICDFT, c);
+    on = valid && LS_SC(int, kF_DFTON, c);
+  }
+  if (!__any_sync(kFull, on)) return;   // landing steps and empty slots store nothing
+  const double q = LS_AT(double, LS_L(oQ), k, c);
+  const uint32_t tw = trow + (uint32_t)(s * 32);
+  // Eq 8 with R8, R9: the applied change in progress / C_tot.  (Lanes whose cell is not `on` overwrite a window that is
+  // zeroed before its next use.)
+  tmem_st2(tw + 2 * slot13, (q * h) * ic);
+  tmem_wait_st();
+  uint32_t ra[26];
+  tmem_ld26(tw, ra);
+  tmem_wait_ld();
+  double x[kWindow];
+  unpack_window(ra, x);
+  double d0, m2;
+  ab_window_stats<NHF>(x, d0, m2);
+  bool sure;
+  bool ringing = ab_ring_filter(d0, m2, sc, sure);
+  if (__any_sync(kFull, !sure && on)) ringing = ab_ring_exact(d0, m2, sc);
+  if (on) {
+    double &rof_ref = LS_AT(double, LS_L(oRof), k, c);
+    double rof = rof_ref * (ringing ? sc.inv_r_fac : sc.r_fac);   // Eqs 12-13
+    if (rof > 1.0) rof = 1.0;
+    if (rof < sc.rof_min) rof = sc.rof_min;
+    rof_ref = rof;
+  }
+}
+
+template <class SH, bool IN_P4>
+__device__ __forceinline__ void ls_dft(const LsArgs &a, unsigned char *cells, uint32_t trow, int s, int slot13, int warp, int lane,
+                                       double dt_max, double t_tol) {
+  if (!a.sc.dft_enable) return;
+  switch (a.sc.nhf) {
+    case 1: ls_dft_pass<SH, 1, IN_P4>(a, cells, trow, s, slot13, warp, lane, dt_max, t_tol); break;
+    case 2: ls_dft_pass<SH, 2, IN_P4>(a, cells, trow, s, slot13, warp, lane, dt_max, t_tol); break;
+    case 3: ls_dft_pass<SH, 3, IN_P4>(a, cells, trow, s, slot13, warp, lane, dt_max, t_tol); break;
+    case 4: ls_dft_pass<SH, 4, IN_P4>(a, cells, trow, s, slot13, warp, lane, dt_max, t_tol); break;
+    case 5: ls_dft_pass<SH, 5, IN_P4>(a, cells, trow, s, slot13, warp, lane, dt_max, t_tol); break;
+    default: ls_dft_pass<SH, 6, IN_P4>(a, cells, trow, s, slot13, warp, lane, dt_max, t_tol); break;
   }
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// a2: rates of this warp's passes over the (cell, reversible reaction) and (cell, irreversible reaction) pairs.
-// The owner of a (cell, reaction) pair also owns its DFT window and its rOF: on the first step of a new cell it zeroes
-// the window (R10) and sets rOF = 1 (Eq 11).
+// a2: rates of passes s0 .. s0 + U - 1 of this warp over the (reversible reaction, cell) pairs, side by side (2 U
+// independent exponential chains in flight).  The owner of a pair also owns its DFT window and its rOF: on the first
+// step of a new cell it zeroes the window (R10) and sets rOF = 1 (Eq 11).
 // ---------------------------------------------------------------------------------------------------------
-template <class SH>
-__device__ __forceinline__ void ls_rate_passes(const LsArgs &a, const unsigned char *tbl, unsigned char *cells, uint32_t trow, int warp,
-                                               int lane) {
-  const int Rrev = LS_D(Rrev), Rp = LS_L(Rp), Rirr = LS_D(R) - LS_D(Rrev);
-  const int n_rev_pass = LS_L(n_rev_pass), n_irr_pass = LS_L(n_irr_pass);
+template <class SH, int U>
+__device__ __forceinline__ void ls_rev_batch(const LsArgs &a, const unsigned char *tbl, unsigned char *cells, uint32_t trow, int s0,
+                                             int warp, int lane) {
+  const int C = LS_D(C), Rrev = LS_D(Rrev), Rp = LS_L(Rp);
   const bool has2 = LS_D(n_var) > 2;
-  const double2 *rkA = (const double2 *)(tbl + LS_L(o_rkA)), *rkB = (const double2 *)(tbl + LS_L(o_rkB));
-  const uint4 *rfac = (const uint4 *)(tbl + LS_L(o_rfac)), *rdg = (const uint4 *)(tbl + LS_L(o_rdg));
-  const unsigned n_rev = (unsigned)(LS_D(C) * Rrev), n_irr = (unsigned)(LS_D(C) * Rirr);
+  const unsigned n_rev = (unsigned)(C * Rrev);
+  unsigned k[U], c[U];
+  bool valid[U];
+  double lkf[U], lkr[U];
+  uint4 fo[U];
+  bool oor = false;
 #pragma unroll
-  for (int s = 0; s < kLsSlots; ++s) {
-    const int p = warp + s * kLsWarps;
-    if (p >= n_rev_pass) break;
+  for (int u = 0; u < U; ++u) {
+    const int p = warp + (s0 + u) * kLsWarps;
     unsigned f = (unsigned)(p * 32 + lane);
-    const bool valid = f < n_rev;
-    f = valid ? f : n_rev - 1;
-    const unsigned c = ls_div<SH>(f, Rrev, a.mRrev), k = f - c * (unsigned)Rrev;
-    unsigned char *cell = cells + c * (unsigned)LS_L(stride);
-    const LsScal *scl = (const LsScal *)(cell + LS_L(oSc));
-    double *cRof = (double *)(cell + LS_L(oRof)), *cQ = (double *)(cell + LS_L(oQ));
-    const bool fresh = valid && scl->fresh;
+    valid[u] = f < n_rev;
+    f = valid[u] ? f : n_rev - 1;
+    k[u] = ls_div_c<SH>(f, C, a.mC);
+    c[u] = f - k[u] * (unsigned)C;
+    const bool fresh = valid[u] && LS_SC(int, kF_FRESH, c[u]);
     if (__any_sync(kFull, fresh)) {   // rare: once per cell
-      const uint32_t tw = trow + (uint32_t)(s * 32);
+      const uint32_t tw = trow + (uint32_t)((s0 + u) * 32);
       uint32_t ra[26];
       tmem_ld26(tw, ra);
       tmem_wait_ld();
       if (fresh) {
 #pragma unroll
         for (int n = 0; n < 26; ++n) ra[n] = 0u;
-        cRof[k] = 1.0;
+        LS_AT(double, LS_L(oRof), k[u], c[u]) = 1.0;
       }
       tmem_st26(tw, ra);
       tmem_wait_st();
     }
-    const double invT = scl->invT, lnT = scl->lnT, ln_c0 = scl->ln_c0;
-    const double2 p0 = rkA[k], p1 = rkB[k];
-    const uint4 d = rdg[k], fo = rfac[k];
-    const double lkf = fma_rn(-p1.x, invT, fma_rn(p0.y, lnT, p0.x));
-    double dg = 0.0 - lds_f64(cell, d.x);
-    dg = dg - lds_f64(cell, d.y);
-    dg = dg + lds_f64(cell, d.z);
-    dg = dg + lds_f64(cell, d.w);
-    const double lkr = lkf - fma_rn(p1.y, ln_c0, -dg);
-    double fwd, rev;
-    if (__any_sync(kFull, ab_exp_out_of_range(lkf) || ab_exp_out_of_range(lkr))) {
-      fwd = cexp(lkf);
-      rev = cexp(lkr);
-    } else {
-      fwd = ab_exp_core(lkf);
-      rev = ab_exp_core(lkr);
+  }
+#pragma unroll
+  for (int u = 0; u < U; ++u) {
+    const unsigned char *cc = cells + (c[u] << 3);   // this lane's cell column
+    const double invT = LS_SC(double, kF_INVT, c[u]), lnT = LS_SC(double, kF_LNT, c[u]), ln_c0 = LS_SC(double, kF_LNC0, c[u]);
+    const double2 p0 = ((const double2 *)(tbl + LS_L(o_rkA)))[k[u]], p1 = ((const double2 *)(tbl + LS_L(o_rkB)))[k[u]];
+    const uint4 d = ((const uint4 *)(tbl + LS_L(o_rdg)))[k[u]];
+    fo[u] = ((const uint4 *)(tbl + LS_L(o_rfac)))[k[u]];
+    lkf[u] = fma_rn(-p1.x, invT, fma_rn(p0.y, lnT, p0.x));
+    double dg = 0.0 - lds_f64(cc, d.x);
+    dg = dg - lds_f64(cc, d.y);
+    dg = dg + lds_f64(cc, d.z);
+    dg = dg + lds_f64(cc, d.w);
+    lkr[u] = lkf[u] - fma_rn(p1.y, ln_c0, -dg);
+    oor = oor || ab_exp_out_of_range(lkf[u]) || ab_exp_out_of_range(lkr[u]);
+  }
+  double fwd[U], rev[U];
+  if (__any_sync(kFull, oor)) {
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      fwd[u] = cexp(lkf[u]);
+      rev[u] = cexp(lkr[u]);
     }
-    fwd = fwd * lds_f64(cell, fo.x);
-    rev = rev * lds_f64(cell, fo.z);
-    fwd = fwd * lds_f64(cell, fo.y);
-    rev = rev * lds_f64(cell, fo.w);
-    const double q = (fwd - rev) * cRof[k];   // Eq 14
-    if (valid) {
-      cQ[k] = q;
-      cQ[Rp + k] = -q;
+  } else {
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      fwd[u] = ab_exp_core(lkf[u]);
+      rev[u] = ab_exp_core(lkr[u]);
+    }
+  }
+#pragma unroll
+  for (int u = 0; u < U; ++u) {
+    const unsigned char *cc = cells + (c[u] << 3);
+    fwd[u] = fwd[u] * lds_f64(cc, fo[u].x);
+    rev[u] = rev[u] * lds_f64(cc, fo[u].z);
+    fwd[u] = fwd[u] * lds_f64(cc, fo[u].y);
+    rev[u] = rev[u] * lds_f64(cc, fo[u].w);
+    const double q = (fwd[u] - rev[u]) * LS_AT(double, LS_L(oRof), k[u], c[u]);   // Eq 14
+    if (valid[u]) {
+      LS_AT(double, LS_L(oQ), k[u], c[u]) = q;
+      LS_AT(double, LS_L(oQ), Rp + k[u], c[u]) = -q;
       if (has2) {
         const double q2 = q + q;
-        cQ[2 * Rp + k] = q2;
-        cQ[3 * Rp + k] = -q2;
+        LS_AT(double, LS_L(oQ), 2 * Rp + k[u], c[u]) = q2;
+        LS_AT(double, LS_L(oQ), 3 * Rp + k[u], c[u]) = -q2;
       }
     }
   }
-  // irreversible reactions: passes continue round robin after the reversible ones, so the warps that had one pass less get these first
-  for (int p = (warp - n_rev_pass) & (kLsWarps - 1); p < n_irr_pass; p += kLsWarps) {
+}
+
+// passes [s0, s1) of this warp, two at a time while two are left
+template <class SH>
+__device__ __forceinline__ void ls_rev_range(const LsArgs &a, const unsigned char *tbl, unsigned char *cells, uint32_t trow, int s0, int s1,
+                                             int warp, int lane) {
+  const int n_mine = (LS_L(n_rev_pass) - warp + kLsWarps - 1) / kLsWarps;   // passes of this warp
+  s1 = (s1 < n_mine) ? s1 : n_mine;
+  int s = s0;
+  for (; s + 2 <= s1; s += 2) ls_rev_batch<SH, 2>(a, tbl, cells, trow, s, warp, lane);
+  if (s < s1) ls_rev_batch<SH, 1>(a, tbl, cells, trow, s, warp, lane);
+}
+
+// irreversible reactions: passes continue round robin after the reversible ones, so the warps that had one pass less get these first
+template <class SH>
+__device__ __forceinline__ void ls_irr_passes(const LsArgs &a, const unsigned char *tbl, unsigned char *cells, int warp, int lane) {
+  const int C = LS_D(C), Rrev = LS_D(Rrev), Rp = LS_L(Rp), Rirr = LS_D(R) - LS_D(Rrev);
+  const int n_irr_pass = LS_L(n_irr_pass);
+  const bool has2 = LS_D(n_var) > 2;
+  const unsigned n_irr = (unsigned)(C * Rirr);
+  for (int p = (warp - LS_L(n_rev_pass)) & (kLsWarps - 1); p < n_irr_pass; p += kLsWarps) {
     unsigned f = (unsigned)(p * 32 + lane);
     const bool valid = f < n_irr;
     f = valid ? f : n_irr - 1;
-    const unsigned c = ls_div<SH>(f, Rirr, a.mRirr), k = (unsigned)Rrev + f - c * (unsigned)Rirr;
-    unsigned char *cell = cells + c * (unsigned)LS_L(stride);
-    const LsScal *scl = (const LsScal *)(cell + LS_L(oSc));
-    double *cQ = (double *)(cell + LS_L(oQ));
-    const double2 p0 = rkA[k];
-    const double ta = rkB[k].x;
-    const uint4 fo = rfac[k];
-    const double lk = fma_rn(-ta, scl->invT, fma_rn(p0.y, scl->lnT, p0.x));
+    const unsigned kk = ls_div_c<SH>(f, C, a.mC), c = f - kk * (unsigned)C, k = (unsigned)Rrev + kk;
+    const unsigned char *cc = cells + (c << 3);
+    const double2 p0 = ((const double2 *)(tbl + LS_L(o_rkA)))[k];
+    const double ta = ((const double2 *)(tbl + LS_L(o_rkB)))[k].x;
+    const uint4 fo = ((const uint4 *)(tbl + LS_L(o_rfac)))[k];
+    const double lk = fma_rn(-ta, LS_SC(double, kF_INVT, c), fma_rn(p0.y, LS_SC(double, kF_LNT, c), p0.x));
     double fw;
     if (__any_sync(kFull, ab_exp_out_of_range(lk))) fw = cexp(lk);
     else fw = ab_exp_core(lk);
-    fw = fw * lds_f64(cell, fo.x);
-    fw = fw * lds_f64(cell, fo.y);
+    fw = fw * lds_f64(cc, fo.x);
+    fw = fw * lds_f64(cc, fo.y);
     if (valid) {
-      cQ[k] = fw;
-      cQ[Rp + k] = -fw;
+      LS_AT(double, LS_L(oQ), k, c) = fw;
+      LS_AT(double, LS_L(oQ), Rp + k, c) = -fw;
       if (has2) {
         const double f2 = fw + fw;
-        cQ[2 * Rp + k] = f2;
-        cQ[3 * Rp + k] = -f2;
+        LS_AT(double, LS_L(oQ), 2 * Rp + k, c) = f2;
+        LS_AT(double, LS_L(oQ), 3 * Rp + k, c) = -f2;
       }
     }
   }
@@ -245,34 +311,39 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
 
   // the scalar lane of cell slot `lane` keeps the cell's own scalars in registers for the whole integration
   const bool my_slot = (warp == SW) && lane < C;
-  unsigned char *my_cell = cells + (unsigned)(my_slot ? lane : 0) * (unsigned)LS_L(stride);
-  LsScal *my_sc = (LsScal *)(my_cell + LS_L(oSc));
+  const int mc = my_slot ? lane : 0;
   double T = 1000.0, p = kPatm, t = 0.0, inv_ctot = 0.0, rho = 1.0;
   int steps = 0, cidx = -1, pending_st = -1;
   bool active = false, exhausted = false, last = false, bad_T = false;
   if (my_slot) {
     // a slot without a cell computes on a harmless finite state and commits nothing
-    double2 *cYp = (double2 *)(my_cell + LS_L(oYp));
-    for (int i = 0; i < S; ++i) cYp[i] = make_double2(1.0 / (double)S, invW[i]);
-    ((double *)(my_cell + LS_L(oConc)))[0] = 1.0;
-    ((double *)(my_cell + LS_L(oG)))[0] = 0.0;
-    my_sc->active = 0;
-    my_sc->fresh = 0;
-    my_sc->dft_on = 0;
-    my_sc->bad = 0;
-    my_sc->h_dft = 0.0;
-    my_sc->ictot_dft = 0.0;
+    for (int i = 0; i < S; ++i) LS_AT(double, LS_L(oY), i, mc) = 1.0 / (double)S;
+    LS_AT(double, LS_L(oConc), 0, mc) = 1.0;
+    LS_AT(double, LS_L(oG), 0, mc) = 0.0;
+    LS_SC(int, kF_ACTIVE, mc) = 0;
+    LS_SC(int, kF_FRESH, mc) = 0;
+    LS_SC(int, kF_DFTON, mc) = 0;
+    LS_SC(int, kF_BAD, mc) = 0;
+    LS_SC(double, kF_HDFT, mc) = 0.0;
+    LS_SC(double, kF_ICDFT, mc) = 0.0;
   }
   __syncthreads();
 
+#ifdef LS_TIMING
+  long long tph[6] = {0, 0, 0, 0, 0, 0}, tl_ = clock64(), n_steps_ = 0;
+#define LST(i) { const long long now_ = clock64(); tph[i] += now_ - tl_; tl_ = now_; }
+#else
+#define LST(i)
+#endif
   int g13 = 0;   // ring position of the step about to be taken (block-uniform)
   for (;;) {
+    const int sl_prev = (g13 == 0) ? kWindow - 1 : g13 - 1;   // ring position of the step just taken
     // =========================== phase 0 ===========================
     if (warp == SW) {
       // ---- a6: retirement (R20) of the step just taken
       if (my_slot && active) {
         int st = -1;
-        if (bad_T || my_sc->bad) st = 2;            // checked first: a non-finite landing step is not "finished"
+        if (bad_T || LS_SC(int, kF_BAD, mc)) st = 2;   // checked first: a non-finite landing step is not "finished"
         else if (last) st = 0;
         else if (steps >= sc.max_steps) st = 1;
         if (st >= 0) {
@@ -283,8 +354,7 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
       if (g13 == 0) {
         // ---- results leave and new cells enter only at ring position 0 (see the header): write back ...
         if (my_slot && pending_st >= 0) {
-          const double2 *cYp = (const double2 *)(my_cell + LS_L(oYp));
-          for (int i = 0; i < S; ++i) a.Y[(long long)i * a.ld + cidx] = cYp[i].x;
+          for (int i = 0; i < S; ++i) a.Y[(long long)i * a.ld + cidx] = LS_AT(double, LS_L(oY), i, mc);
           a.T[cidx] = T;
           a.steps[cidx] = steps;
           if (a.status) a.status[cidx] = (unsigned char)pending_st;
@@ -305,12 +375,11 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
               cidx = a.list ? a.list[pos] : (int)pos;
               T = a.T[cidx];
               p = a.p[cidx];
-              double2 *cYp = (double2 *)(my_cell + LS_L(oYp));
-              for (int i = 0; i < S; ++i) cYp[i].x = a.Y[(long long)i * a.ld + cidx];
+              for (int i = 0; i < S; ++i) LS_AT(double, LS_L(oY), i, mc) = a.Y[(long long)i * a.ld + cidx];
               t = 0.0;
               steps = 0;
               active = true;
-              my_sc->fresh = 1;
+              LS_SC(int, kF_FRESH, mc) = 1;
             } else {
               exhausted = true;
             }
@@ -328,65 +397,49 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
         const double ln_c0 = ab_log(kPatm / RuT);
         inv_ctot = 1.0 / c_tot;
         // 1/Wbar = sum Y_i/W_i, sequential in species order (contract 5.4); estimator inputs on the way (R18)
-        const double2 *cYp = (const double2 *)(my_cell + LS_L(oYp));
         double inv_wbar = 0.0;
         if (EST && LS_D(n_in) > 1) {
-          float *cXn = (float *)(my_cell + LS_L(oHid)) + LS_D(H);
+          float *cXn = (float *)(cells + LS_L(oXn));
           const float *eshift = (const float *)(tbl + LS_L(o_eshift)), *escale = (const float *)(tbl + LS_L(o_escale));
-          cXn[1] = ((float)p - eshift[1]) * escale[1];
+          cXn[1 * C + mc] = ((float)p - eshift[1]) * escale[1];
           for (int i = 0; i < S; ++i) {
-            const double2 v = cYp[i];
-            inv_wbar = fma_rn(v.x, v.y, inv_wbar);
-            cXn[2 + i] = ((float)v.x - eshift[2 + i]) * escale[2 + i];
+            const double y = LS_AT(double, LS_L(oY), i, mc);
+            inv_wbar = fma_rn(y, invW[i], inv_wbar);
+            cXn[(2 + i) * C + mc] = ((float)y - eshift[2 + i]) * escale[2 + i];
           }
         } else {
 #pragma unroll 4
-          for (int i = 0; i < S; ++i) {
-            const double2 v = cYp[i];
-            inv_wbar = fma_rn(v.x, v.y, inv_wbar);
-          }
+          for (int i = 0; i < S; ++i) inv_wbar = fma_rn(LS_AT(double, LS_L(oY), i, mc), invW[i], inv_wbar);
         }
         if (EST) {
-          float *cXn = (float *)(my_cell + LS_L(oHid)) + LS_D(H);
-          cXn[0] = ((float)T - ((const float *)(tbl + LS_L(o_eshift)))[0]) * ((const float *)(tbl + LS_L(o_escale)))[0];
+          float *cXn = (float *)(cells + LS_L(oXn));
+          cXn[mc] = ((float)T - ((const float *)(tbl + LS_L(o_eshift)))[0]) * ((const float *)(tbl + LS_L(o_escale)))[0];
         }
         rho = c_tot / inv_wbar;
-        my_sc->T = T;
-        my_sc->p = p;
-        my_sc->lnT = lnT;
-        my_sc->ln_c0 = ln_c0;
-        my_sc->invT = invT;
-        my_sc->inv_ctot = inv_ctot;
-        my_sc->rho = rho;
-        my_sc->rem = a.t_f - t;
-        my_sc->tstar_bits = kInfBits;
-        my_sc->active = active ? 1 : 0;
-        my_sc->bad = 0;
+        LS_SC(double, kF_T, mc) = T;
+        LS_SC(double, kF_P, mc) = p;
+        LS_SC(double, kF_LNT, mc) = lnT;
+        LS_SC(double, kF_LNC0, mc) = ln_c0;
+        LS_SC(double, kF_INVT, mc) = invT;
+        LS_SC(double, kF_ICTOT, mc) = inv_ctot;
+        LS_SC(double, kF_RHO, mc) = rho;
+        LS_SC(double, kF_REM, mc) = a.t_f - t;
+        LS_SC(unsigned long long, kF_TSTAR, mc) = kInfBits;
+        LS_SC(int, kF_ACTIVE, mc) = active ? 1 : 0;
+        LS_SC(int, kF_BAD, mc) = 0;
       }
     }
-    // ---- a5 of the step just taken (its ring position is the one before g13)
-    if (sc.dft_enable) {
-      const int sl = (g13 == 0) ? kWindow - 1 : g13 - 1;
-      switch (sc.nhf) {
-        case 1: ls_dft_passes<SH, 1>(a, cells, trow, sl, warp, lane); break;
-        case 2: ls_dft_passes<SH, 2>(a, cells, trow, sl, warp, lane); break;
-        case 3: ls_dft_passes<SH, 3>(a, cells, trow, sl, warp, lane); break;
-        case 4: ls_dft_passes<SH, 4>(a, cells, trow, sl, warp, lane); break;
-        case 5: ls_dft_passes<SH, 5>(a, cells, trow, sl, warp, lane); break;
-        default: ls_dft_passes<SH, 6>(a, cells, trow, sl, warp, lane); break;
-      }
-    }
+    ls_dft<SH, false>(a, cells, trow, 1, sl_prev, warp, lane, dt_max, t_tol);
+    LST(0)
     __syncthreads();
+    LST(5)
     if (!s_go) break;
 
     // =========================== phase 1: a1 thermo, concentrations, first estimator layer ===========================
     for (unsigned it = (unsigned)tid; it < n_cs; it += kLsThreads) {
-      const unsigned c = ls_div<SH>(it, S, a.mS), i = it - c * (unsigned)S;
-      unsigned char *cell = cells + c * (unsigned)LS_L(stride);
-      const LsScal *scl = (const LsScal *)(cell + LS_L(oSc));
-      const double Tc = scl->T, invT = scl->invT, lnT = scl->lnT, rho_c = scl->rho;
-      double *cG = (double *)(cell + LS_L(oG)), *cConc = (double *)(cell + LS_L(oConc));
-      double2 *cYwCp = (double2 *)(cell + LS_L(oYwCp)), *cHOm = (double2 *)(cell + LS_L(oHOm));
+      const unsigned i = ls_div_c<SH>(it, C, a.mC), c = it - i * (unsigned)C;
+      const double Tc = LS_SC(double, kF_T, c), invT = LS_SC(double, kF_INVT, c), lnT = LS_SC(double, kF_LNT, c);
+      const double rho_c = LS_SC(double, kF_RHO, c);
       // NASA-7 (Eqs 15-16, R17): g/RT and 2 g/RT always, cp/R and h/RT without an estimator
       const double *ca = nasa + ((Tc < tmid[i]) ? 0 : kNasaRows * S) + i;
       const double a1a = ca[0], a2a = ca[S];
@@ -395,61 +448,66 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
       const double spa = fma_rn(fma_rn(fma_rn(ca[12 * S], Tc, ca[11 * S]), Tc, ca[10 * S]), Tc, a2a);
       const double sRa = fma_rn(a1a, lnT, fma_rn(spa, Tc, ca[13 * S]));
       const double ga = hRTa - sRa;
-      cG[1 + i] = ga;
-      cG[1 + S + i] = ga + ga;
+      LS_AT(double, LS_L(oG), 1 + i, c) = ga;
+      LS_AT(double, LS_L(oG), 1 + S + i, c) = ga + ga;
       if (!EST) {
-        cYwCp[i].y = fma_rn(fma_rn(fma_rn(fma_rn(ca[4 * S], Tc, ca[3 * S]), Tc, ca[2 * S]), Tc, a2a), Tc, a1a);
-        cHOm[i].x = hRTa;
+        LS_AT(double, LS_L(oCp), i, c) = fma_rn(fma_rn(fma_rn(fma_rn(ca[4 * S], Tc, ca[3 * S]), Tc, ca[2 * S]), Tc, a2a), Tc, a1a);
+        LS_AT(double, LS_L(oH), i, c) = hRTa;
       }
       // Y_i/W_i (for the cp sum) and the small-species stabilisation (Eqs 6-7, R7): C** = gamma(y) rho y / W
-      const double2 va = ((const double2 *)(cell + LS_L(oYp)))[i];
-      const double ypa = (va.x > 0.0) ? va.x : 0.0;
-      double cc = (rho_c * ypa) * va.y;
+      const double y = LS_AT(double, LS_L(oY), i, c), iw = invW[i];
+      const double ypa = (y > 0.0) ? y : 0.0;
+      double cc = (rho_c * ypa) * iw;
       if (sc.alpha > 0.0) cc = (ypa / (sc.alpha + ypa)) * cc;
-      cYwCp[i].x = va.x * va.y;
-      cConc[1 + i] = cc;
+      LS_AT(double, LS_L(oYw), i, c) = y * iw;
+      LS_AT(double, LS_L(oConc), 1 + i, c) = cc;
     }
     if (EST) {
       // hidden units, dealt from the last thread downwards (the first threads have the species above)
       const int H = LS_D(H), n_in = LS_D(n_in);
       const float *W1T = (const float *)(tbl + LS_L(o_W1T)), *b1 = (const float *)(tbl + LS_L(o_b1));
-      for (unsigned it = (unsigned)(kLsThreads - 1 - tid); it < (unsigned)(C * H); it += kLsThreads) {
-        const unsigned c = ls_div<SH>(it, H, a.mH), j = it - c * (unsigned)H;
-        float *cHid = (float *)(cells + c * (unsigned)LS_L(stride) + LS_L(oHid));
-        const float *cXn = cHid + H;
-        float z = b1[j];
-        const float *w = W1T + j;
-        for (int k = 0; k < n_in; ++k, w += H) z = __fmaf_rn(w[0], cXn[k], z);
-        const double zd = (double)z;
-        cHid[j] = (tb.act == 0) ? (float)(1.0 - 2.0 / (1.0 + ab_exp(2.0 * zd))) : (float)(1.0 / (1.0 + ab_exp(-zd)));
-      }
-    }
-    __syncthreads();
-
-    // =========================== phase 2: second estimator layer, a2 rates ===========================
-    if (EST) {
-      const int H = LS_D(H), n_out = LS_D(n_out);
-      const float *W2p = (const float *)(tbl + LS_L(o_W2p)), *b2 = (const float *)(tbl + LS_L(o_b2));
-      for (unsigned it = (unsigned)tid; it < (unsigned)(C * n_out); it += kLsThreads) {
-        const unsigned c = ls_div<SH>(it, n_out, a.mNout), o = it - c * (unsigned)n_out;
-        unsigned char *cell = cells + c * (unsigned)LS_L(stride);
-        const float4 *hid4 = (const float4 *)(cell + LS_L(oHid));
-        const float4 *wrow = (const float4 *)(W2p + (size_t)o * LS_L(Hpad));
-        float y = b2[o];
-#pragma unroll 4
-        for (int q4 = 0; q4 < H / 4; ++q4) {
-          const float4 hv = hid4[q4], wv = wrow[q4];
-          y = __fmaf_rn(wv.x, hv.x, y);
-          y = __fmaf_rn(wv.y, hv.y, y);
-          y = __fmaf_rn(wv.z, hv.z, y);
-          y = __fmaf_rn(wv.w, hv.w, y);
+      const float *cXn = (const float *)(cells + LS_L(oXn));
+      float *cHid = (float *)(cells + LS_L(oHid));
+      constexpr int HU = 4;   // units per thread side by side (independent fmaf chains)
+      for (unsigned it0 = (unsigned)(kLsThreads - 1 - tid); it0 < (unsigned)(C * H); it0 += HU * kLsThreads) {
+        unsigned jj[HU], cc[HU];
+        float z[HU];
+#pragma unroll
+        for (int u = 0; u < HU; ++u) {
+          unsigned it = it0 + (unsigned)(u * kLsThreads);
+          it = (it < (unsigned)(C * H)) ? it : it0;
+          jj[u] = ls_div_c<SH>(it, C, a.mC);
+          cc[u] = it - jj[u] * (unsigned)C;
+          z[u] = b1[jj[u]];
         }
-        if (o < (unsigned)S) ((double2 *)(cell + LS_L(oYwCp)))[o].y = (double)y;
-        else ((double2 *)(cell + LS_L(oHOm)))[o - S].x = ((double)y * (double)tb.h_ref_T) * ((const LsScal *)(cell + LS_L(oSc)))->invT;
+        const float *w = W1T;
+        for (int k = 0; k < n_in; ++k, w += H) {
+#pragma unroll
+          for (int u = 0; u < HU; ++u) z[u] = __fmaf_rn(w[jj[u]], cXn[k * C + cc[u]], z[u]);
+        }
+#pragma unroll
+        for (int u = 0; u < HU; ++u) {
+          if (u == 0 || it0 + (unsigned)(u * kLsThreads) < (unsigned)(C * H)) {
+            const double zd = (double)z[u];
+            cHid[cc[u] * LS_L(Hs) + jj[u]] =
+                (tb.act == 0) ? (float)(1.0 - 2.0 / (1.0 + ab_exp(2.0 * zd))) : (float)(1.0 / (1.0 + ab_exp(-zd)));
+          }
+        }
       }
     }
-    ls_rate_passes<SH>(a, tbl, cells, trow, warp, lane);
+    ls_dft<SH, false>(a, cells, trow, 2, sl_prev, warp, lane, dt_max, t_tol);
+    LST(1)
     __syncthreads();
+    LST(5)
+
+    // =========================== phase 2: a2 rates ===========================
+    ls_rev_range<SH>(a, tbl, cells, trow, 0, 2, warp, lane);
+    ls_dft<SH, false>(a, cells, trow, 3, sl_prev, warp, lane, dt_max, t_tol);
+    ls_rev_range<SH>(a, tbl, cells, trow, 2, 4, warp, lane);
+    ls_irr_passes<SH>(a, tbl, cells, warp, lane);
+    LST(2)
+    __syncthreads();
+    LST(5)
 
     // =========================== phase 3: source terms and the limiter (Eqs 1-3) ===========================
     {
@@ -460,58 +518,107 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
         unsigned it = base + (unsigned)lane;
         const bool valid = it < n_cs;
         it = valid ? it : n_cs - 1;
-        const unsigned r = ls_div<SH>(it, C, a.mC), c = it - r * (unsigned)C;   // lanes of one species (same list) side by side
-        unsigned char *cell = cells + c * (unsigned)LS_L(stride);
+        const unsigned r = ls_div_c<SH>(it, C, a.mC), c = it - r * (unsigned)C;   // lanes of one species (same list) side by side
+        const unsigned char *cc = cells + (c << 3);
         const int i = gsp[r];
         const int row0 = grow[r], rows = glen[r];
         const int max_rows = __reduce_max_sync(kFull, rows);
         double om = 0.0;
-        // entries in the caller's reaction order; a shorter list reads the all-padding row (the 0.0 slot; om is never -0.0)
+        // entries in the caller's reaction order; a shorter list reads the all-padding row (the 0.0 slot; om is never -0.0).
+        // The values of the next row are fetched before this row is added.
         uint4 o = gent[(0 < rows) ? row0 : tb.g_zero_row];
+        double v0 = lds_f64(cc, o.x), v1 = lds_f64(cc, o.y), v2 = lds_f64(cc, o.z), v3 = lds_f64(cc, o.w);
+        o = gent[(1 < rows) ? row0 + 1 : tb.g_zero_row];
         for (int e = 0; e < max_rows; ++e) {
-          const double v0 = lds_f64(cell, o.x), v1 = lds_f64(cell, o.y), v2 = lds_f64(cell, o.z), v3 = lds_f64(cell, o.w);
-          o = gent[(e + 1 < rows) ? row0 + e + 1 : tb.g_zero_row];
-          om = om + v0;
-          om = om + v1;
-          om = om + v2;
-          om = om + v3;
+          const double u0 = v0, u1 = v1, u2 = v2, u3 = v3;
+          v0 = lds_f64(cc, o.x);
+          v1 = lds_f64(cc, o.y);
+          v2 = lds_f64(cc, o.z);
+          v3 = lds_f64(cc, o.w);
+          o = gent[(e + 2 < rows) ? row0 + e + 2 : tb.g_zero_row];
+          om = om + u0;
+          om = om + u1;
+          om = om + u2;
+          om = om + u3;
         }
-        LsScal *scl = (LsScal *)(cell + LS_L(oSc));
-        const double inv_rho = 1.0 / scl->rho;
+        const double inv_rho = 1.0 / LS_SC(double, kF_RHO, c);
         const double r0 = (W[i] * om) * inv_rho;
-        const double y0 = ((const double2 *)(cell + LS_L(oYp)))[i].x;
+        const double y0 = LS_AT(double, LS_L(oY), i, c);
         const double rs0 = (-r0 > 1.0e-30) ? -r0 : 1.0e-30;                       // Eq 1
         const double ys0 = (y0 < 1.0e-20) ? 1.0 : 0.9 * y0;                       // Eq 2 (R2)
         const double lim0 = ((sc.y_step_max < ys0) ? sc.y_step_max : ys0) / rs0;  // Eq 3
         if (valid) {
-          ((double *)(cell + LS_L(oConc)))[1 + i] = r0;     // concentrations are dead: reuse for dY_i/dt
-          ((double2 *)(cell + LS_L(oHOm)))[i].y = om;
+          LS_AT(double, LS_L(oConc), 1 + i, c) = r0;     // concentrations are dead: reuse for dY_i/dt
+          LS_AT(double, LS_L(oOm), i, c) = om;
           // min over species: every lim is a positive double, for which the ordering of the bit patterns as unsigned
           // integers is the ordering of the values; NaN is ignored like the contract's plain comparison ignores it
-          if (lim0 < bits_to_double(kInfBits)) atomicMin(&scl->tstar_bits, double_to_bits(lim0));
+          if (lim0 < bits_to_double(kInfBits)) atomicMin(&LS_SC(unsigned long long, kF_TSTAR, c), double_to_bits(lim0));
         }
       }
     }
+    if (EST) {
+      // second estimator layer: a thread owns output o for a GROUP of CG cells, so a row of weights is read once per group
+      // (the hidden activations of a cell are read by broadcast); per output the fmaf chain runs in index order (R18).
+      // Dealt from the last thread downwards (the first warps hold the longest lists above).
+      constexpr int CG = 4;
+      const int H = LS_D(H), n_out = LS_D(n_out);
+      const int n_grp = (C + CG - 1) / CG;
+      const float *W2p = (const float *)(tbl + LS_L(o_W2p)), *b2 = (const float *)(tbl + LS_L(o_b2));
+      for (unsigned it = (unsigned)(kLsThreads - 1 - tid); it < (unsigned)(n_grp * n_out); it += kLsThreads) {
+        const unsigned g = it / (unsigned)n_out;
+        const unsigned o = it - g * (unsigned)n_out;
+        const int c0 = (int)g * CG;
+        const float4 *wrow = (const float4 *)(W2p + o * (unsigned)LS_L(Hpad));
+        const float bias = b2[o];
+        float y[CG];
+        const float4 *hid4[CG];
+#pragma unroll
+        for (int u = 0; u < CG; ++u) {
+          y[u] = bias;
+          const int cu = (c0 + u < C) ? c0 + u : C - 1;
+          hid4[u] = (const float4 *)(cells + LS_L(oHid) + (unsigned)cu * (unsigned)(4 * LS_L(Hs)));
+        }
+#pragma unroll 2
+        for (int q4 = 0; q4 < H / 4; ++q4) {
+          const float4 wv = wrow[q4];
+#pragma unroll
+          for (int u = 0; u < CG; ++u) {
+            const float4 hv = hid4[u][q4];
+            y[u] = __fmaf_rn(wv.x, hv.x, y[u]);
+            y[u] = __fmaf_rn(wv.y, hv.y, y[u]);
+            y[u] = __fmaf_rn(wv.z, hv.z, y[u]);
+            y[u] = __fmaf_rn(wv.w, hv.w, y[u]);
+          }
+        }
+#pragma unroll
+        for (int u = 0; u < CG; ++u) {
+          const int c = c0 + u;
+          if (c < C) {
+            if (o < (unsigned)S) LS_AT(double, LS_L(oCp), o, c) = (double)y[u];
+            else LS_AT(double, LS_L(oH), o - S, c) = ((double)y[u] * (double)tb.h_ref_T) * LS_SC(double, kF_INVT, c);
+          }
+        }
+      }
+    }
+    LST(3)
     __syncthreads();
+    LST(5)
 
     // =========================== phase 4: a3 step size, a4 update ===========================
     for (unsigned it = (unsigned)tid; it < n_cs; it += kLsThreads) {
-      const unsigned c = ls_div<SH>(it, S, a.mS), i = it - c * (unsigned)S;
-      unsigned char *cell = cells + c * (unsigned)LS_L(stride);
-      LsScal *scl = (LsScal *)(cell + LS_L(oSc));
-      const double t_star = bits_to_double(scl->tstar_bits);
+      const unsigned i = ls_div_c<SH>(it, C, a.mC), c = it - i * (unsigned)C;
+      const double t_star = bits_to_double(LS_SC(unsigned long long, kF_TSTAR, c));
       double h = (t_star < dt_max) ? t_star : dt_max;       // Eq 5
-      const double rem = scl->rem;
+      const double rem = LS_SC(double, kF_REM, c);
       if (rem - h < t_tol) h = rem;                          // landing on t_f (R5)
-      if (scl->active) {
-        double2 *cYp = (double2 *)(cell + LS_L(oYp));
-        const double y = fma_rn(h, ((const double *)(cell + LS_L(oConc)))[1 + i], cYp[i].x);   // Eq 18
-        cYp[i].x = y;
-        if (!(y - y == 0.0)) atomicOr(&scl->bad, 1);
+      if (LS_SC(int, kF_ACTIVE, c)) {
+        const double y = fma_rn(h, LS_AT(double, LS_L(oConc), 1 + i, c), LS_AT(double, LS_L(oY), i, c));   // Eq 18
+        LS_AT(double, LS_L(oY), i, c) = y;
+        if (!(y - y == 0.0)) atomicOr(&LS_SC(int, kF_BAD, c), 1);
       }
     }
     if (my_slot) {
-      const double t_star = bits_to_double(my_sc->tstar_bits);
+      const double t_star = bits_to_double(LS_SC(unsigned long long, kF_TSTAR, mc));
       double h = (t_star < dt_max) ? t_star : dt_max;
       const double rem = a.t_f - t;
       bool lst = false;
@@ -520,19 +627,17 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
         lst = true;
       }
       // temperature equation (R15): sum (Y_i/W_i) cp_i/R and sum (h_i/RT) omega_i, each sequential in species order
-      const double2 *cYwCp = (const double2 *)(my_cell + LS_L(oYwCp)), *cHOm = (const double2 *)(my_cell + LS_L(oHOm));
       double sum_cp = 0.0, sum_h = 0.0;
 #pragma unroll 4
       for (int i = 0; i < S; ++i) {
-        const double2 u = cYwCp[i], v = cHOm[i];
-        sum_cp = fma_rn(u.x, u.y, sum_cp);
-        sum_h = fma_rn(v.x, v.y, sum_h);
+        sum_cp = fma_rn(LS_AT(double, LS_L(oYw), i, mc), LS_AT(double, LS_L(oCp), i, mc), sum_cp);
+        sum_h = fma_rn(LS_AT(double, LS_L(oH), i, mc), LS_AT(double, LS_L(oOm), i, mc), sum_h);
       }
       const double dTdt = (sc.energy_mode == 0) ? -((sum_h * kRu) * T) / (rho * (kRu * sum_cp)) : 0.0;
-      my_sc->fresh = 0;
-      my_sc->h_dft = h;
-      my_sc->ictot_dft = inv_ctot;
-      my_sc->dft_on = (active && !lst) ? 1 : 0;   // the landing step's change is never looked at: the cell retires
+      LS_SC(int, kF_FRESH, mc) = 0;
+      LS_SC(double, kF_HDFT, mc) = h;
+      LS_SC(double, kF_ICDFT, mc) = inv_ctot;
+      LS_SC(int, kF_DFTON, mc) = (active && !lst) ? 1 : 0;   // the landing step's change is never looked at: the cell retires
       if (active) {
         T = fma_rn(h, dTdt, T);
         bad_T = !(T - T == 0.0);
@@ -541,9 +646,20 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
         last = lst;
       }
     }
+    ls_dft<SH, true>(a, cells, trow, 0, g13, warp, lane, dt_max, t_tol);
+    LST(4)
     __syncthreads();
+    LST(5)
     g13 = (g13 + 1 == kWindow) ? 0 : g13 + 1;
+#ifdef LS_TIMING
+    n_steps_ += 1;
+#endif
   }
+#ifdef LS_TIMING
+  if (blockIdx.x == 0 && lane == 0 && (warp == 0 || warp == 7 || warp == SW))
+    printf("LST warp %d steps %lld per step: P0 %lld P1 %lld P2 %lld P3 %lld P4 %lld barrier-wait %lld\n", warp, n_steps_, tph[0] / n_steps_,
+           tph[1] / n_steps_, tph[2] / n_steps_, tph[3] / n_steps_, tph[4] / n_steps_, tph[5] / n_steps_);
+#endif
 
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
   __syncthreads();

@@ -49,7 +49,7 @@ static void pk_layout(const PkTables &tb, PkCell &cl) {
 
 bool build_pk_image(const HostMechanism &m, const HostEstimator *e, int nw, std::vector<unsigned char> &image, PkTables &tb,
                     PkCell &cl) {
-  if (nw < 1 || nw > 4 || !pk_mechanism_ok(m, nw)) return false;
+  if (nw < 1 || nw > 2 || !pk_mechanism_ok(m, nw)) return false;
   const int S = m.S, R = m.R, Rrev = m.Rrev;
   tb = PkTables{};
   tb.S = S;
@@ -59,17 +59,12 @@ bool build_pk_image(const HostMechanism &m, const HostEstimator *e, int nw, std:
   tb.Rp = (R + 1) & ~1;
   // DFT blocks: each warp keeps at most four blocks (128 TMEM columns); warp 0 takes the smaller half because it also
   // walks the two sequential sums of the temperature equation
-  // (quad: warps 2 and 3 run the filter of the previous step while warps 0 and 1 run phase A of the next one)
   tb.nw = nw;
   tb.it_split[0] = 0;
   for (int h = 0; h < kPkMaxNw; ++h) {
     int cnt = 0;
     if (nw == 1) cnt = (h == 0) ? tb.n_it : 0;
-    else if (nw == 2) cnt = (h == 0) ? tb.n_it / 2 : (h == 1 ? tb.n_it - tb.n_it / 2 : 0);
-    else if (nw == 3) {   // warp 2 only filters (the larger half); warp 0 also has the update and the scalars: smallest share
-      const int k2 = (tb.n_it + 1) / 2, k0 = (tb.n_it - k2) / 3;
-      cnt = (h == 2) ? k2 : (h == 0 ? k0 : (h == 1 ? tb.n_it - k2 - k0 : 0));
-    } else cnt = (h == 2) ? tb.n_it / 2 : (h == 3 ? tb.n_it - tb.n_it / 2 : 0);   // the filter runs on warps 2 and 3
+    else cnt = (h == 0) ? tb.n_it / 2 : tb.n_it - tb.n_it / 2;
     tb.it_split[h + 1] = tb.it_split[h] + cnt;
   }
   if (e) {
@@ -114,14 +109,12 @@ bool build_pk_image(const HostMechanism &m, const HostEstimator *e, int nw, std:
   std::vector<int> order(S);
   std::iota(order.begin(), order.end(), 0);
   std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return gl[x].size() > gl[y].size(); });
-  // With four warps per cell the gather stays in two of them (warps 2 and 3; a sequential sum cannot be split, so more
-  // warps would add instructions without shortening the longest list); warps 0 and 1 skip phase C.
   unsigned char gsp[32 * kPkMaxNw];
   unsigned short glen[32 * kPkMaxNw];
   std::memset(gsp, 255, sizeof(gsp));
   std::memset(glen, 0, sizeof(glen));
-  int g_len[kPkMaxNw] = {0, 0, 0, 0};
-  const int g_short = (nw == 4) ? 2 : (nw == 3 ? 2 : 0), g_long = (nw == 4) ? 3 : 1;
+  int g_len[kPkMaxNw] = {0, 0};
+  const int g_short = 0, g_long = 1;
   for (int n = 0; n < S; ++n) {
     const int group = n / 16;
     const int half = (nw >= 2) ? (group < 2 ? g_long : g_short) : 0, lane = (nw >= 2) ? (group & 1) * 16 + n % 16 : n;
@@ -374,11 +367,8 @@ int integrate_pk_launch(const PkTables &tb, const PkCell &cl, const unsigned cha
   a.cells_per_block = pk_cells_per_block(tb, cl, dense);
   if (a.cells_per_block < 1) { set_error("pair kernel: shared memory too small"); return STEV_EINVAL; }
   const size_t smem = (size_t)tb.bytes + (size_t)a.cells_per_block * cl.stride;
-  void *fn = dense ? (void *)stev_pk_kernel<1, true>
-             : (tb.nw == 4) ? (void *)stev_pk_kernel<4>
-             : (tb.nw == 3) ? (void *)stev_pk_kernel<3>
-             : (tb.nw == 2) ? (void *)stev_pk_kernel<2> : (void *)stev_pk_kernel<1>;
-  const int threads = (tb.nw == 4 || dense) ? kPkThreads4 : (tb.nw == 3 ? kPkThreads3 : kPkThreads);
+  void *fn = dense ? (void *)stev_pk_kernel<1, true> : (tb.nw == 2) ? (void *)stev_pk_kernel<2> : (void *)stev_pk_kernel<1>;
+  const int threads = dense ? kPkThreads4 : kPkThreads;
   STEV_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   const long long blocks = std::min<long long>(device_sm_count(), (n + a.cells_per_block - 1) / a.cells_per_block);
   void *args[] = {&a};

@@ -11,13 +11,12 @@ constexpr int kPkMaxCells = 8;       // cells per block with two warps per cell:
 constexpr int kPkMaxIt = 8;          // 32-blocks of reversible reactions per cell with two warps per cell (32 TMEM columns
                                      // each, 256 columns per cell); 4 with one warp per cell
 constexpr int kPkThreads = 64 * kPkMaxCells;   // block size with one or two warps per cell
-constexpr int kPkThreads4 = 128 * kPkMaxCells;  // block size with four warps per cell (8 cells, 64 registers per thread)
-constexpr int kPkThreads3 = 96 * kPkMaxCells;   // block size with three warps per cell (8 cells, 80 registers per thread)
-constexpr int kPkMaxNw = 4;
+constexpr int kPkThreads4 = 128 * kPkMaxCells;  // block size of the dense one-warp-per-cell kernel (32 cells, 64 registers per thread)
+constexpr int kPkMaxNw = 2;
 
 // Table image of the pair kernel (one contiguous buffer, copied verbatim to shared memory).  Byte offsets.
 struct PkTables {
-  int nw;                              // warps per cell: 4 (quad), 3 (triple), 2 (pair): 8 cells per block; 1: 16 cells
+  int nw;                              // warps per cell: 2 (pair): 8 cells per block; 1: 16 cells (dense: 32)
   int S, R, Rrev, n_it, Rp;            // n_it: 32-blocks of reversible reactions; Rp: row length of the q-variant array
   int has_est, H, Hpad, n_in, n_out, act, input_map;
   float h_ref_T;

@@ -417,27 +417,11 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
   };
   const double dt_max = a.t_f * sc.delta_max;   // Eq 4
   const double t_tol = 1.0e-12 * a.t_f;         // R5
-  const int it_lo = (NW == 1 || half == 0) ? 0 : tb.it_split[half], it_hi = (NW == 1) ? n_it : tb.it_split[half + 1];   // DFT blocks of this warp (at most four; quad: two)
+  const int it_lo = (NW == 1 || half == 0) ? 0 : tb.it_split[half], it_hi = (NW == 1) ? n_it : tb.it_split[half + 1];   // DFT blocks of this warp (at most four)
   // TMEM: a warp reaches the lane quarter (warp id mod 4); it keeps the windows of its own blocks in 128 columns of
   // that quarter: columns [128 (j / 4), +128) for warp 0 of a cell (or the only warp), [256 + 128 (j / 4), +128) for warp 1.
-  // Quad: the four warps of cell j sit in the four quarters; warps 2 and 3 keep four blocks each, and since the role
-  // rotates with j every quarter holds four such warps: columns [128 rank, +128), rank = earlier cells with a filter
-  // warp in this quarter.
   // (one warp per cell, dense: 32 cells per block, at most two blocks = 64 columns per cell)
   uint32_t tcol = DENSE ? (uint32_t)((j >> 2) * 64) : (uint32_t)((j >> 2) * 128 + half * 256);
-  if (NW == 4) {
-    int rank = 0;
-    for (int jj = 0; jj < j; ++jj) rank += (((tmem_quarter + jj) & 3) >= 2) ? 1 : 0;
-    tcol = (uint32_t)(rank * 128);
-  }
-  if (NW == 3) {
-    // Triple: warp 3 j + h; the warps of one quarter hold every role twice, so the quarter's 512 columns are exactly
-    // the sum of their shares.  Columns start after the shares of the earlier warps of the same quarter.
-    const int w_me = 3 * j + half;
-    int cols = 0;
-    for (int w = (w_me & 3); w < w_me; w += 4) cols += 32 * (tb.it_split[w % 3 + 1] - tb.it_split[w % 3]);
-    tcol = (uint32_t)cols;
-  }
   const uint32_t trow = tmem_base + ((uint32_t)((tmem_quarter & 3) * 32) << 16) + tcol - (uint32_t)(it_lo * 32);
   const int my_sp = (half < 2) ? half * 32 + lane : 0x7fff;   // species this lane loads, updates and writes back
   const int g_sp = gsp[half * 32 + lane];       // species whose source term this lane gathers (255 = none)
@@ -554,7 +538,7 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
           }
         }
       }
-      if ((NW == 2 || NW == 3) && half == 0 && steps > 0 && sc.dft_enable) {
+      if (NW == 2 && half == 0 && steps > 0 && sc.dft_enable) {
         // warp 0 of the pair: its share of the ringing filter of the PREVIOUS step (it only feeds rOF, which phase B
         // reads), after the scalars of this step, so that no barrier separates the update from phase A
         run_dft(slot, h_prev, ictot_prev);
@@ -567,20 +551,13 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
           else pk_mlp<4>(tb, tbl, cYp, cYwCp, cHOm, cHid, T, p, invT, lane, 0, tb.n_out);
         }
       } else if (NW >= 2 && half == 1) {
-        // warp 1 of the pair / quad: all of the thermodynamics (its own ln T and 1/T: same operations, same bits)
+        // warp 1 of the pair: all of the thermodynamics (its own ln T and 1/T: same operations, same bits)
         const double invT1 = 1.0 / T;
         if (EST) {
           pk_nasa<false>(tb, tbl, cG, cYwCp, cHOm, T, invT1, ab_log(T), lane);
           pk_mlp<4>(tb, tbl, cYp, cYwCp, cHOm, cHid, T, p, invT1, lane, 0, tb.n_out);
         } else {
           pk_nasa<true>(tb, tbl, cG, cYwCp, cHOm, T, invT1, ab_log(T), lane);
-        }
-      } else if ((NW == 4 || NW == 3) && half >= 2) {
-        // warps 2 and 3 of the quad: the ringing filter of the PREVIOUS step (it only feeds rOF, which phase B reads),
-        // concurrently with the scalars and the thermodynamics of this step on warps 0 and 1
-        if (steps > 0 && sc.dft_enable) {
-          run_dft(slot, h_prev, ictot_prev);
-          slot = (slot + 1 == kWindow) ? 0 : slot + 1;
         }
       }
       PKT(0)
@@ -599,7 +576,7 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
       // warp and are evaluated four (small mechanisms: two) at a time, i.e. eight independent exp chains and one trip
       // through the load -> exp -> load -> store latency chain.  The stored multiples +q, -q, +2q, -2q (all exact) turn the sum
       // omega_i = sum_j nu_ij q_j into plain additions in the contract's order.
-      if (NW < 3 && !DENSE && n_it > 2 * NW) {
+      if (!DENSE && n_it > 2 * NW) {
         for (int b0 = half; b0 < n_it; b0 += 4 * NW)
           pk_rev_batch<4, kSA>(cell, cell_s, rkA, rkB, rfac, rdg, cRof, cQ, Rp, Rrev, has2, invT, lnT, ln_c0, b0, NW, lane);
       } else {
@@ -609,11 +586,10 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
         for (; b0 < n_it; b0 += NW)
           pk_rev_batch<1, kSA>(cell, cell_s, rkA, rkB, rfac, rdg, cRof, cQ, Rp, Rrev, has2, invT, lnT, ln_c0, b0, NW, lane);
       }
-      // irreversible reactions [Rrev, R): 32-blocks c = half (mod NW), two at a time while two are left (triple, quad: one)
+      // irreversible reactions [Rrev, R): 32-blocks c = half (mod NW), two at a time while two are left
       {
         int k0 = Rrev + half * 32;
-        if (NW < 3)
-          for (; k0 + 32 * NW < R; k0 += 64 * NW) pk_irr_batch<2, kSA>(cell, cell_s, rkA, rkB, rfac, cQ, Rp, R, has2, invT, lnT, k0, 32 * NW, lane);
+        for (; k0 + 32 * NW < R; k0 += 64 * NW) pk_irr_batch<2, kSA>(cell, cell_s, rkA, rkB, rfac, cQ, Rp, R, has2, invT, lnT, k0, 32 * NW, lane);
         for (; k0 < R; k0 += 32 * NW) pk_irr_batch<1, kSA>(cell, cell_s, rkA, rkB, rfac, cQ, Rp, R, has2, invT, lnT, k0, 32 * NW, lane);
       }
       PKT(2)
@@ -623,7 +599,7 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
       // ================= phase C: source terms and the limiter (Eqs 1-3) =================
       // One species per lane; the entry lists hold the byte offsets of the stored multiples in the caller's reaction
       // order and are padded with the 0.0 slot to the longest list of the warp, so the loop is warp-uniform.
-      if (NW < 3 || g_len4 > 0) {
+      {
         const double inv_rho = 1.0 / rho;
         double om = 0.0;
         // Two rows of four entries per trip: the eight loads of a trip are independent and the offsets of the next
@@ -673,8 +649,6 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
       // -- a3: step size (Eq 5) and landing on t_f (R5)
       double t_star = scal->t_star[0];
       if (NW >= 2) t_star = pk_min_bits(t_star, scal->t_star[1]);
-      if (NW == 3) t_star = pk_min_bits(t_star, scal->t_star[2]);
-      if (NW == 4) t_star = pk_min_bits(t_star, pk_min_bits(scal->t_star[2], scal->t_star[3]));
       double h = (t_star < dt_max) ? t_star : dt_max;
       bool last = false;
       const double rem = a.t_f - t;
@@ -685,7 +659,7 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
       // -- a4: forward Euler (Eq 18), one species per lane (pair: warp 0 updates all species, two per lane,
       //    so that it depends on nothing of warp 1 between here and the end of phase A)
       int bad = 0;
-      if (NW == 2 || NW == 3) {
+      if (NW == 2) {
         if (half == 0) {
 #pragma unroll
           for (int u = 0; u < 2; ++u) {
@@ -721,27 +695,23 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
       bad = __any_sync(0xffffffffu, bad);
       if (lane == 0 && half < 2) scal->bad[half] = bad;
       PKT(6)
-      if (NW == 2 || NW == 3) {
+      if (NW == 2) {
         // -- a5 on warp 1 now (skipped on the landing step: the cell retires); warp 0 runs its share after the scalars of
         //    the next step.  Warp 0 announces the new T and Y (bar.arrive), warp 1 waits for them (bar.sync).
-        //    (triple: warp 2 waits first and filters at the top of the next step, like warps 2-3 of the quad)
         if (half == 0) {
           __threadfence_block();
-          if (NW == 3) asm volatile("bar.arrive %0, 96;" ::"r"(xbar) : "memory");
-          else asm volatile("bar.arrive %0, 64;" ::"r"(xbar) : "memory");
+          asm volatile("bar.arrive %0, 64;" ::"r"(xbar) : "memory");
         } else {
-          if ((NW == 2 || half == 1) && !last && sc.dft_enable) {
+          if (!last && sc.dft_enable) {
             run_dft(slot, h, inv_ctot);
             slot = (slot + 1 == kWindow) ? 0 : slot + 1;
           }
-          if (NW == 3) asm volatile("bar.sync %0, 96;" ::"r"(xbar) : "memory");
-          else asm volatile("bar.sync %0, 64;" ::"r"(xbar) : "memory");
+          asm volatile("bar.sync %0, 64;" ::"r"(xbar) : "memory");
           T = scal->T_new;
         }
       } else {
-        // -- a5: DFT ringing filter of this warp's blocks (skipped on the landing step: the cell retires; quad: it runs
-        //    at the start of the next step)
-        if (NW != 4 && !last && sc.dft_enable) {
+        // -- a5: DFT ringing filter of this warp's blocks (skipped on the landing step: the cell retires)
+        if (!last && sc.dft_enable) {
           run_dft(slot, h, inv_ctot);
           slot = (slot + 1 == kWindow) ? 0 : slot + 1;
         }
@@ -756,7 +726,7 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
 
       // -- a6: retirement (R20)
       int st = -1;
-      if (scal->bad[0] | (NW == 4 ? scal->bad[1] : 0)) st = 2;   // checked first: a non-finite landing step is not "finished"
+      if (scal->bad[0]) st = 2;   // checked first: a non-finite landing step is not "finished"
       else if (last) st = 0;
       else if (steps >= sc.max_steps) st = 1;
       if (st >= 0) {
@@ -781,7 +751,7 @@ __device__ __forceinline__ void pk_worker(const PkArgs &a, const unsigned char *
 }
 
 template <int NW, bool DENSE = false>
-__global__ void __launch_bounds__((NW == 4 || DENSE) ? kPkThreads4 : (NW == 3 ? kPkThreads3 : kPkThreads), 1) stev_pk_kernel(const __grid_constant__ PkArgs a) {
+__global__ void __launch_bounds__(DENSE ? kPkThreads4 : kPkThreads, 1) stev_pk_kernel(const __grid_constant__ PkArgs a) {
   extern __shared__ __align__(128) unsigned char smem[];
   __shared__ unsigned long long mbar;
   __shared__ uint32_t tmem_base_s;
@@ -803,11 +773,8 @@ __global__ void __launch_bounds__((NW == 4 || DENSE) ? kPkThreads4 : (NW == 3 ? 
   // NW = 1: warp j is cell slot j.  NW = 2: warps j and 8 + (j + 1) % 8 form the pair of cell slot j.  The two warps of a
   // pair run the same phase at the same time, so they are placed on DIFFERENT schedulers (warp id mod 4): a scheduler
   // then interleaves four cells in four different phases (fp64-bound DFT against latency-bound gather and rates).
-  // NW = 4: warps 4 j .. 4 j + 3 serve cell slot j, one per scheduler and TMEM lane quarter; the role rotates with j, so
-  // every scheduler holds two warps of each role (the scalar chains, NASA-7, the two estimator halves).
-  // NW = 3: warps 3 j .. 3 j + 2 serve cell slot j (consecutive warps: three different schedulers).
-  const int half = (NW == 4) ? (((warp & 3) + (warp >> 2)) & 3) : (NW == 3 ? warp % 3 : ((NW == 2) ? (warp >> 3) : 0));
-  const int j = (NW == 4) ? (warp >> 2) : (NW == 3 ? warp / 3 : ((NW == 2) ? (half ? ((warp - 8 + 7) & 7) : warp) : warp));
+  const int half = (NW == 2) ? (warp >> 3) : 0;
+  const int j = (NW == 2) ? (half ? ((warp - 8 + 7) & 7) : warp) : warp;
   if (j < a.cells_per_block) {
     unsigned char *cell = smem + a.tb.bytes + (size_t)j * a.cl.stride;
     if (a.tb.has_est) pk_worker<true, NW, DENSE>(a, smem, cell, j, half, warp & 3, tmem_base, lane);

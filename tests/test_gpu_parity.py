@@ -220,18 +220,14 @@ def test_result_does_not_depend_on_lanes_per_cell(stev, oracle, config, n, lanes
                                            (1, 100, dict(max_steps=150)), (2, 100, dict(alpha=0.0, dft_first_high_bin=1)),
                                            (2, 100, dict(energy_mode=1, delta_max=0.002, y_step_max=0.05)),
                                            (1, 100, dict(dft_enable=0, max_steps=3000))])
-@pytest.mark.parametrize("kernel", [33, 34, 64, 66, 96, 128])
+@pytest.mark.parametrize("kernel", [33, 34, 64])
 def test_tensor_memory_kernels_parity(stev, oracle, kernel, config, n, over):
     """lanes_per_cell = 33: one warp per cell (stev_pk_kernel.cuh, NW = 1), the default for small and mid-size mechanisms;
     lanes_per_cell = 34: the same at 64 registers, 32 cells per SM (at most 64 reversible reactions);
     lanes_per_cell = 64: the warp-pair kernel (stev_pk_kernel.cuh, NW = 2), the default for large mechanisms (config 3);
-    lanes_per_cell = 66: the rate-warp / DFT-warp kernel (stev_ab_kernel.cuh);
-    lanes_per_cell = 96: the warp-triple kernel (stev_pk_kernel.cuh, NW = 3, 24 warps of 80 registers per SM);
-    lanes_per_cell = 128: the warp-quad kernel (stev_pk_kernel.cuh, NW = 4, 32 warps of 64 registers per SM).  All keep the DFT history in tensor
-    memory and are bit-exact against the oracle on every config they accept."""
+    All keep the DFT history in tensor memory and are bit-exact against the oracle on every config they accept
+    (the lock-step kernel, lanes_per_cell = 512 / 513, has its own file: test_gpu_lockstep.py)."""
     over = dict(over)
-    if kernel == 66 and over.get("dft_enable", 1) == 0:
-        pytest.skip("the warp-specialised kernel needs the DFT filter on")
     if kernel in (33, 34) and config == 3:
         pytest.skip("one warp per cell holds at most 32 species / 128 reversible reactions (dense: 64)")
     w = make_workload(config, n)
@@ -250,11 +246,7 @@ def test_tensor_memory_kernels_parity(stev, oracle, kernel, config, n, over):
 
 
 @pytest.mark.parametrize("config,kernel,n_rev", [(3, 64, 1), (3, 64, 31), (3, 64, 32), (3, 64, 33), (3, 64, 64), (3, 64, 65),
-                                                 (3, 64, 128), (3, 64, 129), (3, 64, 193), (3, 64, 224), (3, 66, 33),
-                                                 (3, 128, 1), (3, 128, 33), (3, 128, 64), (3, 128, 97), (3, 128, 129), (3, 128, 161),
-                                                 (3, 128, 193), (3, 128, 224), (2, 128, 33),
-                                                 (3, 96, 1), (3, 96, 33), (3, 96, 64), (3, 96, 97), (3, 96, 129), (3, 96, 161),
-                                                 (3, 96, 193), (3, 96, 224), (2, 96, 33),
+                                                 (3, 64, 128), (3, 64, 129), (3, 64, 193), (3, 64, 224),
                                                  (2, 33, 1), (2, 33, 31), (2, 33, 32), (2, 33, 33), (2, 64, 33), (1, 33, 1),
                                                  (2, 34, 1), (2, 34, 31), (2, 34, 32), (2, 34, 33), (1, 34, 1)])
 def test_tensor_memory_kernels_block_boundaries(stev, oracle, config, kernel, n_rev):
@@ -283,9 +275,9 @@ def test_default_kernel_selection(stev):
     gpu = GpuCase(stev, make_workload(2, 64)).integrate()
     assert gpu["stats"]["lanes_per_cell"] == 34 and gpu["stats"]["cells_per_block"] == 32   # dense: 42 reversible reactions
     gpu = GpuCase(stev, make_workload(1, 64)).integrate()
-    assert gpu["stats"]["lanes_per_cell"] == 16     # 9 species: sub-warp groups, history in shared memory
+    assert gpu["stats"]["lanes_per_cell"] == 512 and gpu["stats"]["specialised"] == 1   # tiny mechanism: lock-step block
     gpu = GpuCase(stev, make_workload(0, 64)).integrate()
-    assert gpu["stats"]["lanes_per_cell"] == 4
+    assert gpu["stats"]["lanes_per_cell"] == 512
     gpu = GpuCase(stev, make_workload(2, 64)).integrate(chunk_steps=50)
     assert gpu["stats"]["lanes_per_cell"] <= 32
 
