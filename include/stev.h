@@ -20,8 +20,9 @@
  *   - Mass fractions are species-major: Y[i*ld + c] is species i of cell c, ld >= n_cells.
  *   - Every entry point returns an int: 0 = OK, < 0 = error (nothing written), > 0 = completed with a
  *     warning.  No exceptions, no aborts, nothing printed.  stev_last_error() gives the message.
- *   - stev_integrate enqueues work on `cuda_stream` and synchronises that stream before returning
- *     (the active-cell count is read back between passes); outputs are valid on return.
+ *   - stev_integrate enqueues work on `cuda_stream`; by default it synchronises that stream before returning (outputs
+ *     valid on return, warning code returned); with stev_params.nonblocking = 1 it returns right after enqueueing a
+ *     single-pass launch and stev_integrate_finish() delivers the return code.
  */
 #ifndef STEV_H
 #define STEV_H
@@ -53,6 +54,8 @@ extern "C" {
 #define STEV_PREC_FP32 0     /* fp32 CUDA-core path, bit-reproducible (R18) */
 #define STEV_PREC_TF32 1     /* tcgen05 kind::tf32, fp32 accumulate in TMEM */
 #define STEV_PREC_BF16 2     /* tcgen05 kind::f16 with bf16 operands, fp32 accumulate in TMEM */
+#define STEV_STATE_FP64 0    /* state, rates and DFT in binary64 (BASELINE.json; the default) */
+#define STEV_STATE_FP32 1    /* state, rates and DFT in binary32, as the paper ran it; in/out arrays stay fp64 */
 #define STEV_ENERGY_ADIABATIC 0 /* constant-pressure adiabatic temperature equation (R15) */
 #define STEV_ENERGY_ISOTHERMAL 1
 
@@ -101,10 +104,17 @@ typedef struct {
   double tol_freq;     /* Tol_freq of Eq 12 (R12: 0.1, dimensionless because of R9) */
   double r_fac;        /* r_fac of Eq 12 (R12: 2.0; must be > 1) */
   double rof_min;      /* lower clamp of rOF, "0 < rOF" (R13: 2^-100) */
+  int32_t dft_window;  /* length of the history of Eq 8: 13, "the thirteen most recent"; other values: STEV_EINVAL */
   int32_t dft_first_high_bin; /* n of Eq 10, high bins are n..6 (R10: 4); 1..6 */
   int32_t dft_enable;  /* 0 switches section 2.3 off (rOF stays 1) */
   int32_t max_steps;   /* per cell (R20: 200000) */
   int32_t energy_mode; /* STEV_ENERGY_* */
+  int32_t estimator_precision; /* STEV_PREC_*: precision of the attached estimator INSIDE stev_integrate.  Only STEV_PREC_FP32 (the
+                             bit-reproducible CUDA-core path, R18) is accepted there; TF32 / BF16 return STEV_EINVAL: a
+                             tensor-core contraction needs >= 64 cells at the same phase per MMA, and the estimator is 6 % of
+                             the integrator's instructions.  stev_estimator_eval runs all three. */
+  int32_t state_precision; /* STEV_STATE_*: FP32 runs the whole step in binary32 with its own arithmetic contract
+                             (DESIGN.md section 5b); checked against the oracle's binary32 mode */
   /* scheduling only: results do not depend on these */
   int32_t chunk_steps;    /* 0: every cell runs to completion in one pass; > 0: a pass advances each active
                              cell at most this many steps, unfinished cells are spilled to the workspace and the
@@ -119,6 +129,10 @@ typedef struct {
                              512 = lock-step block: up to 32 cells of a block step together, work flattened over (reaction,
                                   cell) and (species, cell) pairs, one warp for the scalar chains (<= 64 species; the
                                   default for tiny mechanisms); 513 = the same with run-time dimensions only */
+  int32_t nonblocking;    /* 0: stev_integrate returns after the stream has drained, with the final return code.  1: if the call
+                             is a single kernel pass (chunk_steps = 0) it only enqueues on the stream and returns STEV_OK;
+                             outputs are valid after the caller synchronises the stream, and stev_integrate_finish() returns
+                             the warning code (the CFD code may overlap its own work) */
   int32_t order_cells;    /* 1 (default): the persistent kernels pull the cells in order of decreasing temperature
                              (a counting sort on the device before the launch) -- step counts grow with temperature,
                              so the long integrations start first and do not end up running alone.
@@ -167,6 +181,10 @@ STEV_API size_t stev_workspace_bytes(const stev_mechanism *m, const stev_estimat
 STEV_API int stev_integrate(const stev_mechanism *m, const stev_estimator *estimator, const stev_params *p, int64_t n_cells,
                    int64_t ld, double *T, const double *pressure, double *Y, double dt_cfd, int32_t *steps_out,
                    uint8_t *status_out, void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* After a nonblocking stev_integrate on `cuda_stream` with this workspace: synchronises the stream and returns what the
+ * blocking call would have returned (STEV_OK, STEV_WMAXSTEPS, STEV_WNONFINITE, or STEV_ECUDA). */
+STEV_API int stev_integrate_finish(void *workspace, void *cuda_stream);
 
 /* Same call with HOST buffers (the paper's calling convention: the CFD code hands over host
  * memory and gets the state back): allocates device buffers, copies in, integrates, copies out. */

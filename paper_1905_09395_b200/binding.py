@@ -15,6 +15,7 @@ from . import _build
 STEV_OK, STEV_EINVAL, STEV_EWORKSPACE, STEV_ECUDA = 0, -1, -2, -3
 STEV_WMAXSTEPS, STEV_WNONFINITE = 1, 2
 STEV_PREC_FP32, STEV_PREC_TF32, STEV_PREC_BF16 = 0, 1, 2
+STEV_STATE_FP64, STEV_STATE_FP32 = 0, 1
 
 
 class stev_mechanism_desc(C.Structure):
@@ -34,9 +35,10 @@ class stev_estimator_desc(C.Structure):
 class stev_params(C.Structure):
     _fields_ = [("y_step_max", C.c_double), ("delta_max", C.c_double), ("alpha", C.c_double), ("tol_ring", C.c_double),
                 ("tol_freq", C.c_double), ("r_fac", C.c_double), ("rof_min", C.c_double),
-                ("dft_first_high_bin", C.c_int32), ("dft_enable", C.c_int32), ("max_steps", C.c_int32),
-                ("energy_mode", C.c_int32), ("chunk_steps", C.c_int32), ("lanes_per_cell", C.c_int32),
-                ("order_cells", C.c_int32)]
+                ("dft_window", C.c_int32), ("dft_first_high_bin", C.c_int32), ("dft_enable", C.c_int32),
+                ("max_steps", C.c_int32), ("energy_mode", C.c_int32), ("estimator_precision", C.c_int32),
+                ("state_precision", C.c_int32), ("chunk_steps", C.c_int32), ("lanes_per_cell", C.c_int32),
+                ("nonblocking", C.c_int32), ("order_cells", C.c_int32)]
 
 
 class stev_stats(C.Structure):
@@ -47,7 +49,7 @@ class stev_stats(C.Structure):
 
 EXPORTS = ["stev_params_default", "stev_mechanism_create", "stev_mechanism_destroy", "stev_mechanism_sizes",
            "stev_estimator_load", "stev_estimator_destroy", "stev_workspace_bytes", "stev_integrate",
-           "stev_integrate_host", "stev_last_stats", "stev_rates_eval", "stev_estimator_eval", "stev_compact_active",
+           "stev_integrate_host", "stev_integrate_finish", "stev_last_stats", "stev_rates_eval", "stev_estimator_eval", "stev_compact_active",
            "stev_dft_mag", "stev_contract_exp_log", "stev_microbench", "stev_last_error", "stev_version"]
 
 _lib = None
@@ -88,6 +90,7 @@ def load(build: bool = True):
     lib.stev_workspace_bytes.restype = C.c_size_t
     lib.stev_integrate.argtypes = [vp, vp, C.POINTER(stev_params), i64, i64, vp, vp, vp, dbl, vp, vp, vp, C.c_size_t, vp]
     lib.stev_integrate_host.argtypes = [vp, vp, C.POINTER(stev_params), i64, i64, vp, vp, vp, dbl, vp, vp]
+    lib.stev_integrate_finish.argtypes = [vp, vp]
     lib.stev_last_stats.argtypes = [C.POINTER(stev_stats)]
     lib.stev_last_stats.restype = None
     lib.stev_rates_eval.argtypes = [vp, vp, C.POINTER(stev_params), i64, i64, vp, vp, vp, vp, vp, vp, vp, vp]
@@ -233,6 +236,11 @@ def stev_integrate(mechanism: Mechanism, estimator: Estimator | None, params: st
                                status_out.data_ptr() if status_out is not None else None, workspace.data_ptr(),
                                workspace.numel() * workspace.element_size(), _stream_ptr(stream))
     return _check(rc)
+
+
+def stev_integrate_finish(workspace, stream=None) -> int:
+    """After a nonblocking stev_integrate: synchronises the stream and returns the call's final return code."""
+    return _check(load().stev_integrate_finish(workspace.data_ptr(), _stream_ptr(stream)))
 
 
 def stev_integrate_host(mechanism: Mechanism, estimator: Estimator | None, params: stev_params, T, p, Y, dt_cfd: float,

@@ -251,10 +251,14 @@ void stev_params_default(stev_params *p) {
   p->tol_freq = 0.1;
   p->r_fac = 2.0;
   p->rof_min = 7.888609052210118e-31;  // 2^-100
+  p->dft_window = STEV_DFT_WINDOW;
   p->dft_first_high_bin = 4;
   p->dft_enable = 1;
   p->max_steps = 200000;
   p->energy_mode = STEV_ENERGY_ADIABATIC;
+  p->estimator_precision = STEV_PREC_FP32;
+  p->state_precision = STEV_STATE_FP64;
+  p->nonblocking = 0;
   p->chunk_steps = 0;
   p->lanes_per_cell = 0;
   p->order_cells = 1;
@@ -533,6 +537,19 @@ int check_params(const stev_params *p) {
     set_error("stev_params out of range");
     return STEV_EINVAL;
   }
+  if (p->dft_window != STEV_DFT_WINDOW) {
+    set_error("stev_params.dft_window: only 13 is implemented (PAPER.md:77, 'the thirteen most recent changes')");
+    return STEV_EINVAL;
+  }
+  if (p->estimator_precision != STEV_PREC_FP32) {
+    set_error("stev_params.estimator_precision: inside stev_integrate the estimator runs on the fp32 CUDA-core path only "
+              "(STEV_PREC_FP32); the TF32 / BF16 tensor-core paths are reached through stev_estimator_eval");
+    return STEV_EINVAL;
+  }
+  if (p->state_precision != STEV_STATE_FP64 && p->state_precision != STEV_STATE_FP32) {
+    set_error("stev_params.state_precision must be STEV_STATE_FP64 or STEV_STATE_FP32");
+    return STEV_EINVAL;
+  }
   return STEV_OK;
 }
 
@@ -729,6 +746,7 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
       g_stats.threads_per_block = threads;
       g_stats.cells_per_block = cpb;
       g_stats.smem_bytes = (int64_t)smem;
+      if (p->nonblocking) return STEV_OK;
       return finish_integrate(w.counters, s);
     }
   }
@@ -796,7 +814,13 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
   g_stats.threads_per_block = cfg.threads;
   g_stats.cells_per_block = cfg.cells_per_block;
   g_stats.smem_bytes = (int64_t)cfg.smem;
+  if (p->nonblocking && p->chunk_steps <= 0) return STEV_OK;
   return finish_integrate(w.counters, s);
+}
+
+int stev_integrate_finish(void *workspace, void *cuda_stream) {
+  if (!workspace) { set_error("stev_integrate_finish: null workspace"); return STEV_EINVAL; }
+  return finish_integrate((const int *)workspace, (cudaStream_t)cuda_stream);   // the counters are the first 256 bytes
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -832,6 +856,9 @@ int stev_integrate_host(const stev_mechanism *m, const stev_estimator *est, cons
   } else {
     STEV_CUDA(cudaMemcpy2DAsync(b + oY, 8 * (size_t)n, Y, 8 * (size_t)ld, 8 * (size_t)n, S, cudaMemcpyHostToDevice, s));
   }
+  stev_params pb = *p;
+  pb.nonblocking = 0;
+  p = &pb;
   int rc = stev_integrate(m, est, p, n, n, (double *)(b + oT), (const double *)(b + oP), (double *)(b + oY), dt_cfd,
                           (int32_t *)(b + oS), (uint8_t *)(b + oSt), b + oW, ws, s);
   if (rc < 0) return rc;

@@ -39,7 +39,8 @@ def test_params_default_and_struct_layout():
     assert p.tol_ring == 0.5 and p.tol_freq == 0.1 and p.r_fac == 2.0 and p.rof_min == 2.0 ** -100
     assert p.dft_first_high_bin == 4 and p.dft_enable == 1 and p.max_steps == 200000
     assert p.chunk_steps == 0 and p.lanes_per_cell == 0 and p.order_cells == 1
-    assert ctypes.sizeof(stev.stev_params) == 7 * 8 + 8 * 4   # seven int32 fields, padded to a multiple of 8
+    assert p.dft_window == 13 and p.estimator_precision == stev.STEV_PREC_FP32 and p.state_precision == 0 and p.nonblocking == 0
+    assert ctypes.sizeof(stev.stev_params) == 7 * 8 + 12 * 4   # seven doubles, eleven int32 fields padded to a multiple of 8
     assert stev.stev_version().startswith("stev-b200")
 
 
