@@ -57,6 +57,9 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--ref-cells", type=int, default=None, help="cells per step of the --impl reference arm")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the per_config object (the other BASELINE.json configs at full size)")
+    ap.add_argument("--per-config-budget", type=float, default=330.0,
+                    help="seconds since start after which config 4 at full size (one call of about two minutes) is skipped")
     ap.add_argument("--what", default="integrate", choices=["integrate", "estimator"],
                     help="estimator: time the standalone MLP forward pass (row a7) of config 3/4 on the fp32, TF32 and BF16 paths")
     return ap.parse_args()
@@ -227,7 +230,87 @@ def run_estimator(args):
     return 0
 
 
+def measure_config(stev, workmodel, config: int, n: int, dev, sm_max: float, warmup: int = 1, state_precision: int = 0,
+                   max_steps=None) -> dict:
+    """One BASELINE.json config at n cells with the default kernel selection: `warmup` untimed calls, one timed call
+    (CUDA events on the launching stream, state restored from a pristine copy outside the events)."""
+    import torch
+    from stev_inputs.configs import make_workload
+    w = make_workload(config, n)
+    mech = stev.Mechanism(w.mech)
+    est = stev.Estimator(mech, w.estimator) if w.estimator is not None else None
+    params = dict(w.params)
+    if max_steps is not None:
+        params["max_steps"] = max_steps
+    prm = stev.stev_params_default(state_precision=state_precision, **params)
+    T0 = torch.tensor(w.T, dtype=torch.float64, device=dev)
+    p = torch.tensor(w.p, dtype=torch.float64, device=dev)
+    Y0 = torch.tensor(w.Y, dtype=torch.float64, device=dev)
+    T, Y = torch.empty_like(T0), torch.empty_like(Y0)
+    steps = torch.zeros(n, dtype=torch.int32, device=dev)
+    status = torch.zeros(n, dtype=torch.uint8, device=dev)
+    ws = torch.empty(max(stev.stev_workspace_bytes(mech, est, prm, n), 256), dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+    ms = 0.0
+    for k in range(warmup + 1):
+        T.copy_(T0)
+        Y.copy_(Y0)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        rc = stev.stev_integrate(mech, est, prm, T, p, Y, w.dt_cfd, steps, status, workspace=ws, stream=stream)
+        e1.record(stream)
+        e1.synchronize()
+        ms = e0.elapsed_time(e1)
+    st = stev.stev_last_stats()
+    cell_steps = int(steps.cpu().numpy().astype(np.int64).sum())
+    work = workmodel.cell_step_work(w.mech, w.estimator, dft_enable=bool(w.params["dft_enable"]),
+                                    first_high_bin=w.params["dft_first_high_bin"], alpha_on=w.params["alpha"] > 0,
+                                    adiabatic=w.params["energy_mode"] == 0)
+    peak = 2.0 * workmodel.fp64_peak_instr_per_s(sm_max) * (2.0 if state_precision else 1.0)
+    return {"workload": w.name, "cells": n, "ms_per_call": ms, "cells_per_s": n / (ms * 1e-3),
+            "cell_steps_per_s": cell_steps / (ms * 1e-3), "mean_steps_per_cell": cell_steps / n,
+            "finished_fraction": float((status == 0).float().mean().item()), "return_code": rc,
+            "kernel_lanes_per_cell": st["lanes_per_cell"], "specialised": st["specialised"],
+            "dtype": "f32" if state_precision else "f64", "warmup_calls": warmup,
+            "frac": work.fp64_flop * cell_steps / (ms * 1e-3) / peak,
+            "frac_of": "fp32 FMA peak (2 x the fp64 rate)" if state_precision else "derived fp64 peak"}
+
+
+def measure_estimator_paths(stev, dev, hbm_peak: float) -> dict:
+    """Row a7 on its own (config 4's estimator over all 4,194,304 cells): fp32 CUDA cores, TF32 and BF16 tcgen05."""
+    import torch
+    from stev_inputs.configs import make_workload, FULL_CELLS
+    n = FULL_CELLS[4]
+    w = make_workload(4, 4096)
+    e = w.estimator
+    est = stev.Estimator(None, e)
+    g = torch.Generator(device=dev).manual_seed(4)
+    X = torch.rand((n, e.n_in), dtype=torch.float32, device=dev, generator=g)
+    X[:, 0] = 1000.0 + 1500.0 * X[:, 0]
+    X[:, 1] = 1.0e6 * (1.0 + 4.0 * X[:, 1])
+    bytes_per_call = 4 * n * (e.n_in + e.n_out)
+    stream = torch.cuda.current_stream()
+    out = {}
+    for name in ("FP32", "TF32", "BF16"):
+        prec = getattr(stev, "STEV_PREC_" + name)
+        for _ in range(3):
+            stev.stev_estimator_eval(est, X, prec)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(3):
+            stev.stev_estimator_eval(est, X, prec)
+        e1.record(stream)
+        e1.synchronize()
+        t = e0.elapsed_time(e1) / 3 * 1e-3
+        out[name.lower()] = {"ms": 1e3 * t, "cells_per_s": n / t, "hbm_gbs": bytes_per_call / t / 1e9,
+                             "hbm_frac": bytes_per_call / t / 1e9 / hbm_peak}
+    out["cells"] = n
+    out["shape"] = f"{e.n_in}-{e.n_hidden}-{e.n_out}"
+    return out
+
+
 def main():
+    t_start = time.perf_counter()
     args = parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -353,12 +436,12 @@ def main():
                                                                              f"stev_integrate_kernel<{st['lanes_per_cell']}>")
     # DRAM bytes of one launch from ncu (dram__bytes_read.sum + dram__bytes_write.sum), known only for the captured
     # workloads: profiles/r1_groups_cfg3.md (config 3 at full size, default kernel, by launch order)
+    # not measured by this run (ncu is not running): the DRAM bytes of the dominant kernel are in profiles/ per capture
     traffic = None
-    if args.config == 3 and n == 1048576 and st["lanes_per_cell"] == 64 and args.max_steps is None:
-        traffic = {1: 1118324224 + 781168128, 2: 5996999680 + 2048877312, 3: 1865687552 + 811976960, 4: 1118324224 + 781168128}.get(args.order)
     roofline = {"bound": "alu", "kernel": kernel_name,
                 "achieved": flop / kernel_s / 1e12, "peak": peak_tflops, "unit": "TFLOP/s",
                 "frac": flop / kernel_s / 1e12 / peak_tflops, "traffic": traffic,
+                "traffic_source": "null here; ncu captures of this kernel and workload: profiles/r2_traffic_cfg3.md",
                 "peak_source": f"derived: 148 SM x 64 DFMA/clk x 2 x {sm_max:.0f} MHz (DESIGN.md section 8); not in MEASURED_PEAKS.json",
                 "fp64_instr": {"achieved_per_s": instr / kernel_s, "peak_per_s": peak_instr,
                                "frac": instr / kernel_s / peak_instr, "measured_dfma_per_s": dfma_per_s,
@@ -378,6 +461,32 @@ def main():
         cpu_baseline = {"value": cps, "unit": UNIT, "cores": thr, "kind": "oracle",
                         "sample": f"first {n_s} cells of this rank's field, {dt:.1f} s", "cell_steps_per_s": cs / dt}
 
+    per_config = None
+    if world == 1 and not args.no_per_config and args.config == 3 and args.cells is None and args.lanes == 0 and args.max_steps is None:
+        # the other BASELINE.json configs at full size (1 warm-up + 1 timed call each; config 4 -- one call takes about two
+        # minutes -- last, without warm-up, and only inside the wall-clock budget), and row a7 on its own
+        per_config = {}
+        from stev_inputs.configs import FULL_CELLS as _FULL
+        for c in (0, 1, 2):
+            per_config[str(c)] = measure_config(stev, workmodel, c, _FULL[c], dev, sm_max)
+        per_config["3"] = {"workload": w.name, "cells": n, "ms_per_call": ms_per_step, "cells_per_s": value,
+                           "cell_steps_per_s": cell_steps_all / (ms_per_step * 1e-3), "finished_fraction": finished_all / (world * n),
+                           "frac": roofline["frac"], "dtype": "f64", "kernel_lanes_per_cell": st["lanes_per_cell"]}
+        try:
+            per_config["3_f32"] = measure_config(stev, workmodel, 3, 262144, dev, sm_max, state_precision=1)
+        except Exception as ex:   # the binary32 state path may refuse a mechanism
+            per_config["3_f32"] = {"unavailable": str(ex)[:200]}
+        peaks = {}
+        try:
+            peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        except Exception:
+            pass
+        per_config["estimator_a7"] = measure_estimator_paths(stev, dev, float(peaks.get("hbm_gbs", 6650.0)))
+        if time.perf_counter() - t_start < args.per_config_budget:
+            per_config["4"] = measure_config(stev, workmodel, 4, _FULL[4], dev, sm_max, warmup=0)
+        else:
+            per_config["4"] = {"skipped": f"wall-clock budget of {args.per_config_budget:.0f} s used up before config 4"}
+
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic",
@@ -391,7 +500,7 @@ def main():
             "cell_steps_per_s": cell_steps_all / (ms_per_step * 1e-3), "mean_steps_per_cell": cell_steps_all / (world * n),
             "finished_fraction": finished_all / (world * n), "return_code": rc,
             "wall_s_timed_region": t_wall, "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
-            "roofline": roofline, "cpu_baseline": cpu_baseline}
+            "roofline": roofline, "cpu_baseline": cpu_baseline, "per_config": per_config}
     print(json.dumps(line), flush=True)
     multi.finish(ctx)
     return 0

@@ -68,7 +68,7 @@ typedef struct stev_estimator stev_estimator; /* opaque, library-owned, immutabl
 
 /* Species, NASA-7 thermodynamics (Eqs 15-16) and Arrhenius mass-action reactions
  * (Eqs 28-30).  All pointers: host.  Each reaction has 1..2 reactant entries and 1..2
- * product entries (CSR), integer stoichiometric coefficients 1..3, no species on both sides. */
+ * product entries (CSR), integer stoichiometric coefficients 1..3 (or real ones, below), no species on both sides. */
 typedef struct {
   int32_t n_species, n_elements, n_reactions;
   const double *mol_weight;        /* [S] g/mol */
@@ -80,6 +80,14 @@ typedef struct {
   const uint8_t *reversible;       /* [R] 1: reverse rate from K_c (Eq 30), 0: irreversible */
   const int32_t *reac_ptr, *reac_species, *reac_nu; /* [R+1], [nnz], [nnz] */
   const int32_t *prod_ptr, *prod_species, *prod_nu;
+  /* Optional, host, one double per CSR entry, each may be NULL (Eqs 26-29: the BFER methane mechanism has
+   * CH4 + 1.5 O2 -> CO + 2 H2O with the rate k C_CH4^0.5 C_O2^0.65, and CO + 0.5 O2 <=> CO2):
+   *   reac_coef / prod_coef    real stoichiometric coefficients (> 0) used in the species source terms, the reaction's
+   *                            Gibbs energy and Delta-nu of Eq 30; default (double) reac_nu / prod_nu
+   *   reac_order / prod_order  exponent (>= 0) of the species' concentration in the forward / reverse rate law; default the
+   *                            coefficient.  Exponents 1, 2, 3 multiply; any other is exp(x log C), and 0 for C <= 0 (R22).
+   * A mechanism with any of these runs on the shared-memory-history kernel (lanes_per_cell 0 or 1..32) only. */
+  const double *reac_coef, *prod_coef, *reac_order, *prod_order;
 } stev_mechanism_desc;
 
 /* Shallow MLP property estimator (Fig 2): one hidden layer, linear output.

@@ -51,6 +51,11 @@ typedef struct {
   const uint8_t *reversible;          /* [R] */
   const int32_t *reac_ptr, *reac_species, *reac_nu; /* CSR, integer nu >= 1 */
   const int32_t *prod_ptr, *prod_species, *prod_nu;
+  /* Optional (NULL = absent), one value per CSR entry.  PAPER.md:205-229 (BFER): CH4 + 1.5 O2 -> CO + 2 H2O with the
+   * rate k C_CH4^0.5 C_O2^0.65 (Eqs 26, 28) and CO + 0.5 O2 <=> CO2 (Eqs 27, 29) need real stoichiometric coefficients
+   * and forward orders that differ from them.  coef: stoichiometric coefficient (default (double)nu); order: exponent
+   * of the concentration in the rate law (default coef). */
+  const double *reac_coef, *prod_coef, *reac_order, *prod_order;
 } ora_mechanism;
 
 typedef struct {
@@ -248,6 +253,24 @@ void ora_dft_mag(const double *ring, double *D /*[7]*/) {
   for (int m = 0; m <= 6; ++m) D[m] = ora_dft_bin(ring, m);
 }
 
+/* Stoichiometric coefficient and rate-law exponent of CSR entry e (Eqs 28-29; R22). */
+static inline double ora_coef(const double *coef, const int32_t *nu, int e) { return coef ? coef[e] : (double)nu[e]; }
+static inline double ora_order(const double *order, const double *coef, const int32_t *nu, int e) {
+  return order ? order[e] : ora_coef(coef, nu, e);
+}
+
+/* f * C^x.  x = 1, 2, 3 by repeated multiplication (contract 5.5, the mass-action case); x = 0 leaves f; any other
+ * exponent (Eq 28: C^0.5, C^0.65) as exp(x log C), with C^x = 0 for C <= 0 (R22: the stabilised concentration is
+ * never negative, and a vanished reactant stops the reaction). */
+ORA_CLONES
+static double ora_times_power(double f, double c, double x) {
+  if (x == 1.0) return f * c;
+  if (x == 2.0) return (f * c) * c;
+  if (x == 3.0) return ((f * c) * c) * c;
+  if (x == 0.0) return f;
+  return f * ((c > 0.0) ? ora_exp(x * ora_log(c)) : 0.0);
+}
+
 /* ------------------------------------------------------------------------------------------
  * One evaluation of the right-hand side for one cell: steps 1-5 of DESIGN.md section 2.
  * Scratch arrays are caller-provided (length S or R).
@@ -321,22 +344,22 @@ static void ora_rhs_eval(const ora_mechanism *m, const ora_estimator *est, const
     double ln_kf = fma(-w->T_a[j], invT, fma(m->b[j], lnT, w->ln_A[j]));
     double fwd = ora_exp(ln_kf);
     for (int e = m->reac_ptr[j]; e < m->reac_ptr[j + 1]; ++e)
-      for (int n = 0; n < m->reac_nu[e]; ++n) fwd = fwd * w->conc[m->reac_species[e]];
+      fwd = ora_times_power(fwd, w->conc[m->reac_species[e]], ora_order(m->reac_order, m->reac_coef, m->reac_nu, e));
     double qj = fwd;
     if (m->reversible[j]) {
       double dg = 0.0, dnu = 0.0;
       for (int e = m->reac_ptr[j]; e < m->reac_ptr[j + 1]; ++e) {
-        dg = dg - (double)m->reac_nu[e] * w->gRT[m->reac_species[e]];
-        dnu = dnu - (double)m->reac_nu[e];
+        dg = dg - ora_coef(m->reac_coef, m->reac_nu, e) * w->gRT[m->reac_species[e]];
+        dnu = dnu - ora_coef(m->reac_coef, m->reac_nu, e);
       }
       for (int e = m->prod_ptr[j]; e < m->prod_ptr[j + 1]; ++e) {
-        dg = dg + (double)m->prod_nu[e] * w->gRT[m->prod_species[e]];
-        dnu = dnu + (double)m->prod_nu[e];
+        dg = dg + ora_coef(m->prod_coef, m->prod_nu, e) * w->gRT[m->prod_species[e]];
+        dnu = dnu + ora_coef(m->prod_coef, m->prod_nu, e);
       }
       double ln_kc = fma(dnu, ln_c0, -dg);
       double rev = ora_exp(ln_kf - ln_kc);
       for (int e = m->prod_ptr[j]; e < m->prod_ptr[j + 1]; ++e)
-        for (int n = 0; n < m->prod_nu[e]; ++n) rev = rev * w->conc[m->prod_species[e]];
+        rev = ora_times_power(rev, w->conc[m->prod_species[e]], ora_order(m->prod_order, m->prod_coef, m->prod_nu, e));
       qj = (fwd - rev) * (rOF ? rOF[j] : 1.0);
     }
     w->q[j] = qj;
@@ -348,9 +371,9 @@ static void ora_rhs_eval(const ora_mechanism *m, const ora_estimator *est, const
   for (int i = 0; i < S; ++i) w->omega[i] = 0.0;
   for (int j = 0; j < R; ++j) {
     for (int e = m->reac_ptr[j]; e < m->reac_ptr[j + 1]; ++e)
-      w->omega[m->reac_species[e]] = w->omega[m->reac_species[e]] - (double)m->reac_nu[e] * w->q[j];
+      w->omega[m->reac_species[e]] = w->omega[m->reac_species[e]] - ora_coef(m->reac_coef, m->reac_nu, e) * w->q[j];
     for (int e = m->prod_ptr[j]; e < m->prod_ptr[j + 1]; ++e)
-      w->omega[m->prod_species[e]] = w->omega[m->prod_species[e]] + (double)m->prod_nu[e] * w->q[j];
+      w->omega[m->prod_species[e]] = w->omega[m->prod_species[e]] + ora_coef(m->prod_coef, m->prod_nu, e) * w->q[j];
   }
   double inv_rho = 1.0 / rho;
   double sum_h = 0.0, sum_cp = 0.0;

@@ -48,7 +48,8 @@ class _Mech(C.Structure):
                 ("mol_weight", C.c_void_p), ("nasa_lo", C.c_void_p), ("nasa_hi", C.c_void_p), ("t_mid", C.c_void_p),
                 ("A", C.c_void_p), ("b", C.c_void_p), ("Ea", C.c_void_p), ("reversible", C.c_void_p),
                 ("reac_ptr", C.c_void_p), ("reac_species", C.c_void_p), ("reac_nu", C.c_void_p),
-                ("prod_ptr", C.c_void_p), ("prod_species", C.c_void_p), ("prod_nu", C.c_void_p)]
+                ("prod_ptr", C.c_void_p), ("prod_species", C.c_void_p), ("prod_nu", C.c_void_p),
+                ("reac_coef", C.c_void_p), ("prod_coef", C.c_void_p), ("reac_order", C.c_void_p), ("prod_order", C.c_void_p)]
 
 
 class _Est(C.Structure):
@@ -99,6 +100,10 @@ def _mech(m) -> _Holder:
         reac_nu=np.ascontiguousarray(m.reac_nu, np.int32),
         prod_ptr=np.ascontiguousarray(m.prod_ptr, np.int32), prod_species=np.ascontiguousarray(m.prod_species, np.int32),
         prod_nu=np.ascontiguousarray(m.prod_nu, np.int32))
+    for k in ("reac_coef", "prod_coef", "reac_order", "prod_order"):
+        v = getattr(m, k, None)
+        if v is not None:
+            arrs[k] = np.ascontiguousarray(v, np.float64)
     s = _Mech(n_species=m.n_species, n_reactions=m.n_reactions, **{k: _ptr(v) for k, v in arrs.items()})
     return _Holder(s, arrs)
 

@@ -23,7 +23,8 @@ class stev_mechanism_desc(C.Structure):
                 ("mol_weight", C.c_void_p), ("elem_comp", C.c_void_p), ("nasa_lo", C.c_void_p), ("nasa_hi", C.c_void_p),
                 ("t_mid", C.c_void_p), ("A", C.c_void_p), ("b", C.c_void_p), ("Ea", C.c_void_p), ("reversible", C.c_void_p),
                 ("reac_ptr", C.c_void_p), ("reac_species", C.c_void_p), ("reac_nu", C.c_void_p),
-                ("prod_ptr", C.c_void_p), ("prod_species", C.c_void_p), ("prod_nu", C.c_void_p)]
+                ("prod_ptr", C.c_void_p), ("prod_species", C.c_void_p), ("prod_nu", C.c_void_p),
+                ("reac_coef", C.c_void_p), ("prod_coef", C.c_void_p), ("reac_order", C.c_void_p), ("prod_order", C.c_void_p)]
 
 
 class stev_estimator_desc(C.Structure):
@@ -146,6 +147,9 @@ class Mechanism:
                  reac_ptr=_np(mech.reac_ptr, np.int32), reac_species=_np(mech.reac_species, np.int32),
                  reac_nu=_np(mech.reac_nu, np.int32), prod_ptr=_np(mech.prod_ptr, np.int32),
                  prod_species=_np(mech.prod_species, np.int32), prod_nu=_np(mech.prod_nu, np.int32))
+        for k in ("reac_coef", "prod_coef", "reac_order", "prod_order"):
+            if getattr(mech, k, None) is not None:
+                a[k] = _np(getattr(mech, k), np.float64)
         ec = _np(mech.elem_comp, np.float64) if validate_elements and mech.elem_comp is not None else None
         d = stev_mechanism_desc(n_species=mech.n_species, n_elements=0 if ec is None else ec.shape[1],
                                 n_reactions=mech.n_reactions, elem_comp=_p(ec), **{k: _p(v) for k, v in a.items()})

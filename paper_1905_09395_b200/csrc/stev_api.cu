@@ -42,11 +42,16 @@ void build_table_image(const HostMechanism &m, const HostEstimator *e, std::vect
   // gather lists: for species i, every (reaction, signed coefficient) in the caller's reaction order, reactant
   // entries before product entries -- the order in which the plain definition omega_i = sum_j nu_ij q_j is summed.
   std::vector<std::vector<unsigned>> gl(S);
+  std::vector<std::vector<double>> glc(S);   // the same entries' signed real coefficients
   for (int j = 0; j < R; ++j) {
-    for (int en = m.reac_ptr[j]; en < m.reac_ptr[j + 1]; ++en)
+    for (int en = m.reac_ptr[j]; en < m.reac_ptr[j + 1]; ++en) {
       gl[m.reac_sp[en]].push_back((unsigned)m.internal_of[j] | ((unsigned)(uint8_t)(int8_t)(-m.reac_nu[en]) << 16));
-    for (int en = m.prod_ptr[j]; en < m.prod_ptr[j + 1]; ++en)
+      glc[m.reac_sp[en]].push_back(-m.reac_coef[en]);
+    }
+    for (int en = m.prod_ptr[j]; en < m.prod_ptr[j + 1]; ++en) {
       gl[m.prod_sp[en]].push_back((unsigned)m.internal_of[j] | ((unsigned)(uint8_t)(int8_t)(m.prod_nu[en]) << 16));
+      glc[m.prod_sp[en]].push_back(m.prod_coef[en]);
+    }
   }
   int n_gather = 0;
   for (auto &v : gl) n_gather += (int)v.size();
@@ -70,6 +75,12 @@ void build_table_image(const HostMechanism &m, const HostEstimator *e, std::vect
   tb.o_orig = take(2 * R);
   tb.o_gptr = take(2 * (S + 1));
   tb.o_gent = take(4 * n_gather);
+  tb.has_real = m.has_real ? 1 : 0;
+  if (m.has_real) {
+    tb.o_rcoef = take(8 * 4 * R);
+    tb.o_rord = take(8 * 4 * R);
+    tb.o_gcoef = take(8 * n_gather);
+  }
   if (e) {
     tb.has_est = 1;
     tb.H = e->H;
@@ -120,13 +131,21 @@ void build_table_image(const HostMechanism &m, const HostEstimator *e, std::vect
     for (int en = m.reac_ptr[j]; en < m.reac_ptr[j + 1]; ++en, ++slot) {
       pk |= (unsigned long long)(m.reac_sp[en] & 0xff) << (16 * slot);
       pk |= (unsigned long long)(m.reac_nu[en] & 0xff) << (16 * slot + 8);
-      d = d - (double)m.reac_nu[en];
+      d = d - m.reac_coef[en];
+      if (m.has_real) {
+        ((double *)(base + tb.o_rcoef))[4 * k + slot] = m.reac_coef[en];
+        ((double *)(base + tb.o_rord))[4 * k + slot] = m.reac_order[en];
+      }
     }
     slot = 0;
     for (int en = m.prod_ptr[j]; en < m.prod_ptr[j + 1]; ++en, ++slot) {
       pk |= (unsigned long long)(m.prod_sp[en] & 0xff) << (32 + 16 * slot);
       pk |= (unsigned long long)(m.prod_nu[en] & 0xff) << (32 + 16 * slot + 8);
-      d = d + (double)m.prod_nu[en];
+      d = d + m.prod_coef[en];
+      if (m.has_real) {
+        ((double *)(base + tb.o_rcoef))[4 * k + 2 + slot] = m.prod_coef[en];
+        ((double *)(base + tb.o_rord))[4 * k + 2 + slot] = m.prod_order[en];
+      }
     }
     part[k] = pk;
     dnu[k] = d;
@@ -136,7 +155,10 @@ void build_table_image(const HostMechanism &m, const HostEstimator *e, std::vect
   int pos = 0;
   for (int i = 0; i < S; ++i) {
     gptr[i] = (unsigned short)pos;
-    for (unsigned v : gl[i]) gent[pos++] = v;
+    for (size_t q = 0; q < gl[i].size(); ++q) {
+      if (m.has_real) ((double *)(base + tb.o_gcoef))[pos] = glc[i][q];
+      gent[pos++] = gl[i][q];
+    }
   }
   gptr[S] = (unsigned short)pos;
   if (e) {
@@ -313,6 +335,25 @@ int stev_mechanism_create(const stev_mechanism_desc *d, stev_mechanism **out) {
   h.reac_nu.assign(d->reac_nu, d->reac_nu + h.reac_ptr[R]);
   h.prod_sp.assign(d->prod_species, d->prod_species + h.prod_ptr[R]);
   h.prod_nu.assign(d->prod_nu, d->prod_nu + h.prod_ptr[R]);
+  h.has_real = d->reac_coef || d->prod_coef || d->reac_order || d->prod_order;
+  h.reac_coef.resize(h.reac_sp.size());
+  h.reac_order.resize(h.reac_sp.size());
+  h.prod_coef.resize(h.prod_sp.size());
+  h.prod_order.resize(h.prod_sp.size());
+  for (size_t en = 0; en < h.reac_sp.size(); ++en) {
+    h.reac_coef[en] = d->reac_coef ? d->reac_coef[en] : (double)h.reac_nu[en];
+    h.reac_order[en] = d->reac_order ? d->reac_order[en] : h.reac_coef[en];
+  }
+  for (size_t en = 0; en < h.prod_sp.size(); ++en) {
+    h.prod_coef[en] = d->prod_coef ? d->prod_coef[en] : (double)h.prod_nu[en];
+    h.prod_order[en] = d->prod_order ? d->prod_order[en] : h.prod_coef[en];
+  }
+  for (size_t en = 0; en < h.reac_sp.size(); ++en)
+    if (!(h.reac_coef[en] > 0.0) || !(h.reac_order[en] >= 0.0) || !std::isfinite(h.reac_coef[en]) || !std::isfinite(h.reac_order[en]))
+      return bad("reac_coef must be positive and reac_order non-negative");
+  for (size_t en = 0; en < h.prod_sp.size(); ++en)
+    if (!(h.prod_coef[en] > 0.0) || !(h.prod_order[en] >= 0.0) || !std::isfinite(h.prod_coef[en]) || !std::isfinite(h.prod_order[en]))
+      return bad("prod_coef must be positive and prod_order non-negative");
   for (int j = 0; j < R; ++j) {
     int seen[4], ns = 0;
     for (int side = 0; side < 2; ++side) {
@@ -329,8 +370,8 @@ int stev_mechanism_create(const stev_mechanism_desc *d, stev_mechanism **out) {
     if (d->elem_comp && E > 0) {
       for (int el = 0; el < E; ++el) {
         double bal = 0.0;
-        for (int en = h.reac_ptr[j]; en < h.reac_ptr[j + 1]; ++en) bal -= h.reac_nu[en] * d->elem_comp[h.reac_sp[en] * E + el];
-        for (int en = h.prod_ptr[j]; en < h.prod_ptr[j + 1]; ++en) bal += h.prod_nu[en] * d->elem_comp[h.prod_sp[en] * E + el];
+        for (int en = h.reac_ptr[j]; en < h.reac_ptr[j + 1]; ++en) bal -= h.reac_coef[en] * d->elem_comp[h.reac_sp[en] * E + el];
+        for (int en = h.prod_ptr[j]; en < h.prod_ptr[j + 1]; ++en) bal += h.prod_coef[en] * d->elem_comp[h.prod_sp[en] * E + el];
         if (std::fabs(bal) > 1e-9) return bad("reaction does not conserve elements");
       }
     }

@@ -32,6 +32,10 @@ struct DevTables {
   int o_orig;                             // uint16 [R]
   int o_gptr, o_gent;                     // uint16 [S+1]; uint32 [n_gather] = internal reaction | (int8 coef) << 16
   int o_eshift, o_escale, o_W1T, o_b1, o_W2T, o_b2;  // float [n_in],[n_in],[n_in][H],[H],[H][n_out],[n_out]
+  // real stoichiometric coefficients / rate-law exponents (Eqs 26-29; only if has_real):
+  int has_real;
+  int o_rcoef, o_rord;                    // double [R][4] each: coefficient / exponent of reactant entries 0, 1 and product entries 0, 1
+  int o_gcoef;                            // double [n_gather]: signed coefficient of each gather entry
   int bytes;                              // multiple of 16
 };
 
@@ -145,7 +149,11 @@ struct TableView {
   const unsigned short *orig, *gptr;
   const unsigned *gent;
   const float *eshift, *escale, *W1T, *b1, *W2T, *b2;
+  const double *rcoef, *rord, *gcoef;
   __device__ __forceinline__ TableView(const unsigned char *base, const DevTables &tb) {
+    rcoef = (const double *)(base + tb.o_rcoef);
+    rord = (const double *)(base + tb.o_rord);
+    gcoef = (const double *)(base + tb.o_gcoef);
     invW = (const double *)(base + tb.o_invW);
     W = (const double *)(base + tb.o_W);
     tmid = (const double *)(base + tb.o_tmid);
@@ -166,6 +174,16 @@ struct TableView {
     b2 = (const float *)(base + tb.o_b2);
   }
 };
+
+// f * C^x (Eq 28; R22): x = 1, 2, 3 by repeated multiplication (the mass-action case, contract 5.5), x = 0
+// leaves f, any other exponent as exp(x log C) through the contract routines, and C^x = 0 for C <= 0.
+__device__ __forceinline__ double times_power(double f, double c, double x) {
+  if (x == 1.0) return f * c;
+  if (x == 2.0) return (f * c) * c;
+  if (x == 3.0) return ((f * c) * c) * c;
+  if (x == 0.0) return f;
+  return f * ((c > 0.0) ? cexp(x * clog(c)) : 0.0);
+}
 
 // What one right-hand-side evaluation leaves in registers (identical in every lane of the group).
 struct RhsOut {
@@ -259,29 +277,49 @@ __device__ __forceinline__ RhsOut rhs_eval(const DevTables &tb, const TableView 
     const unsigned long long pt = tv.part[k];
     const int r0 = (int)(pt & 0xff), n0 = (int)((pt >> 8) & 0xff), r1 = (int)((pt >> 16) & 0xff), n1 = (int)((pt >> 24) & 0xff);
     const int p0 = (int)((pt >> 32) & 0xff), m0 = (int)((pt >> 40) & 0xff), p1 = (int)((pt >> 48) & 0xff), m1 = (int)((pt >> 56) & 0xff);
-    {
-      const double c0 = cConc[r0];
-      for (int n = 0; n < n0; ++n) fwd = fwd * c0;
-      if (n1) {
-        const double c1 = cConc[r1];
-        for (int n = 0; n < n1; ++n) fwd = fwd * c1;
+    double qk;
+    if (tb.has_real) {
+      // real coefficients and exponents (Eqs 26-29): same order of operations as the integer case below
+      const double *co = tv.rcoef + 4 * k, *od = tv.rord + 4 * k;
+      fwd = times_power(fwd, cConc[r0], od[0]);
+      if (n1) fwd = times_power(fwd, cConc[r1], od[1]);
+      qk = fwd;
+      if (k < Rrev) {
+        double dg = 0.0 - co[0] * cG[r0];
+        if (n1) dg = dg - co[1] * cG[r1];
+        dg = dg + co[2] * cG[p0];
+        if (m1) dg = dg + co[3] * cG[p1];
+        const double ln_kc = fma_rn(tv.dnu[k], ln_c0, -dg);
+        double rev = cexp(ln_kf - ln_kc);
+        rev = times_power(rev, cConc[p0], od[2]);
+        if (m1) rev = times_power(rev, cConc[p1], od[3]);
+        qk = (fwd - rev) * (use_rof ? cRof[k] : 1.0);
       }
-    }
-    double qk = fwd;
-    if (k < Rrev) {
-      double dg = 0.0 - (double)n0 * cG[r0];
-      if (n1) dg = dg - (double)n1 * cG[r1];
-      dg = dg + (double)m0 * cG[p0];
-      if (m1) dg = dg + (double)m1 * cG[p1];
-      const double ln_kc = fma_rn(tv.dnu[k], ln_c0, -dg);
-      double rev = cexp(ln_kf - ln_kc);
-      const double d0 = cConc[p0];
-      for (int n = 0; n < m0; ++n) rev = rev * d0;
-      if (m1) {
-        const double d1 = cConc[p1];
-        for (int n = 0; n < m1; ++n) rev = rev * d1;
+    } else {
+      {
+        const double c0 = cConc[r0];
+        for (int n = 0; n < n0; ++n) fwd = fwd * c0;
+        if (n1) {
+          const double c1 = cConc[r1];
+          for (int n = 0; n < n1; ++n) fwd = fwd * c1;
+        }
       }
-      qk = (fwd - rev) * (use_rof ? cRof[k] : 1.0);
+      qk = fwd;
+      if (k < Rrev) {
+        double dg = 0.0 - (double)n0 * cG[r0];
+        if (n1) dg = dg - (double)n1 * cG[r1];
+        dg = dg + (double)m0 * cG[p0];
+        if (m1) dg = dg + (double)m1 * cG[p1];
+        const double ln_kc = fma_rn(tv.dnu[k], ln_c0, -dg);
+        double rev = cexp(ln_kf - ln_kc);
+        const double d0 = cConc[p0];
+        for (int n = 0; n < m0; ++n) rev = rev * d0;
+        if (m1) {
+          const double d1 = cConc[p1];
+          for (int n = 0; n < m1; ++n) rev = rev * d1;
+        }
+        qk = (fwd - rev) * (use_rof ? cRof[k] : 1.0);
+      }
     }
     cQ[k] = qk;
   }
@@ -296,7 +334,7 @@ __device__ __forceinline__ RhsOut rhs_eval(const DevTables &tb, const TableView 
     const int e1 = tv.gptr[i + 1];
     for (int e = tv.gptr[i]; e < e1; ++e) {
       const unsigned ent = tv.gent[e];
-      const double coef = (double)(int)(signed char)(ent >> 16);
+      const double coef = tb.has_real ? tv.gcoef[e] : (double)(int)(signed char)(ent >> 16);
       om = om + coef * cQ[ent & 0xffffu];
     }
     const double r = (tv.W[i] * om) * inv_rho;

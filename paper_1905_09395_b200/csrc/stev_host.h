@@ -35,6 +35,8 @@ struct HostMechanism {
   std::vector<double> W, nasa_lo, nasa_hi, t_mid, A, b, Ea;
   std::vector<uint8_t> reversible;
   std::vector<int> reac_ptr, reac_sp, reac_nu, prod_ptr, prod_sp, prod_nu;
+  bool has_real = false;         // real stoichiometric coefficients / rate-law exponents given
+  std::vector<double> reac_coef, prod_coef, reac_order, prod_order;   // per CSR entry, always filled (defaults applied)
   std::vector<int> internal_of;  // caller reaction index -> internal index (reversible first)
   std::vector<int> orig_of;      // internal -> caller
   mutable std::vector<int> pk_order;     // internal -> caller of the warp-pair kernel (bank-conflict-aware, chosen once)

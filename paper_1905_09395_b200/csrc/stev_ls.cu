@@ -17,7 +17,7 @@ static unsigned magic(int d) { return d <= 1 ? 0u : (unsigned)(((1ull << 32) + (
 // At most two concentration factors per reaction side (total nu per side <= 2, so nu*g is exact for the equilibrium sum
 // and the stored multiples +-q, +-2q cover every coefficient) and one byte per species index.
 static bool ls_mechanism_ok(const HostMechanism &m) {
-  if (m.S > 64 || m.R > STEV_MAX_REACTIONS) return false;
+  if (m.has_real || m.S > 64 || m.R > STEV_MAX_REACTIONS) return false;
   for (int j = 0; j < m.R; ++j) {
     int nr = 0, np = 0;
     for (int e = m.reac_ptr[j]; e < m.reac_ptr[j + 1]; ++e) nr += m.reac_nu[e];

@@ -16,7 +16,7 @@ static constexpr size_t kSmemMax = 227 * 1024;
 // for the equilibrium sum), 8 reversible reactions per TMEM lane (Rrev <= 256) and one species per lane (S <= 64).
 static bool pk_mechanism_ok(const HostMechanism &m, int nw) {
   const int nw2 = std::min(nw, 2);   // species and gather lists live in at most two warps, histories in 256 TMEM columns
-  if (m.S > 32 * nw2 || m.Rrev < 1 || m.Rrev > 16 * nw2 * kPkMaxIt) return false;
+  if (m.has_real || m.S > 32 * nw2 || m.Rrev < 1 || m.Rrev > 16 * nw2 * kPkMaxIt) return false;
   for (int j = 0; j < m.R; ++j) {
     int nr = 0, np = 0;
     for (int e = m.reac_ptr[j]; e < m.reac_ptr[j + 1]; ++e) nr += m.reac_nu[e];

@@ -38,6 +38,12 @@ class Mechanism:
     prod_nu: np.ndarray
     seed: int = 0
     stiffness_scale: float = 1.0
+    # optional, one value per CSR entry (BFER): real stoichiometric coefficients (default nu) and
+    # rate-law exponents (default the coefficient)
+    reac_coef: np.ndarray | None = None
+    prod_coef: np.ndarray | None = None
+    reac_order: np.ndarray | None = None
+    prod_order: np.ndarray | None = None
 
     @property
     def n_species(self) -> int:
@@ -54,11 +60,13 @@ class Mechanism:
     def stoich_matrix(self) -> np.ndarray:
         """Net stoichiometric coefficients [R, S] (products minus reactants)."""
         nu = np.zeros((self.n_reactions, self.n_species))
+        rc = self.reac_nu if self.reac_coef is None else self.reac_coef
+        pc = self.prod_nu if self.prod_coef is None else self.prod_coef
         for j in range(self.n_reactions):
             for e in range(self.reac_ptr[j], self.reac_ptr[j + 1]):
-                nu[j, self.reac_species[e]] -= self.reac_nu[e]
+                nu[j, self.reac_species[e]] -= rc[e]
             for e in range(self.prod_ptr[j], self.prod_ptr[j + 1]):
-                nu[j, self.prod_species[e]] += self.prod_nu[e]
+                nu[j, self.prod_species[e]] += pc[e]
         return nu
 
 
@@ -212,3 +220,50 @@ def synthetic_mechanism(n_species: int, n_reactions: int, n_elements: int, seed:
         if ok:
             return mech
     raise RuntimeError("no acceptable mechanism found")
+
+
+def bfer_shaped_mechanism(seed: int = 190509395 + 70) -> Mechanism:
+    """A mechanism with the SHAPE of the paper's BFER methane case: six species with the element
+    compositions of CH4, O2, CO, H2O, CO2, N2 and two reactions,
+        MEPOX  CH4 + 1.5 O2 -> CO + 2 H2O,  rate k exp(-Ea/RT) C_CH4^0.5 C_O2^0.65      (Eqs 26, 28)
+        COROX  CO + 0.5 O2 <=> CO2,         rate k T^0.7 exp(-Ea/RT) (C_CO C_O2^0.5 - C_CO2 / K)   (Eqs 27, 29, 30)
+    with the constants the paper prints in Table 1 (k = 4.9e9 / 2.0e8, Ea = 35500 / 12000 cal/mol; cm, s, mol, cal).
+    The NASA-7 THERMODYNAMICS ARE SYNTHETIC (seeded, near-linear cp, like every other mechanism here): the real
+    coefficients are not in this repository, so temperatures and equilibria are not those of methane combustion."""
+    rng = np.random.default_rng([seed, 0])
+    comp = np.array([[4, 0, 1, 0], [0, 2, 0, 0], [0, 1, 1, 0], [2, 1, 0, 0], [0, 2, 1, 0], [0, 0, 0, 2]], dtype=np.float64)  # H O C N
+    n_atoms = comp.sum(axis=1)
+    W = comp @ ATOMIC_WEIGHTS
+    S = 6
+    lo = np.zeros((S, 7))
+    lo[:, 0] = 2.5 + (n_atoms - 1) * rng.uniform(0.6, 1.0, S)
+    lo[:, 1] = n_atoms * rng.uniform(0.2, 1.0, S) * 1e-3
+    lo[:, 2] = -n_atoms * rng.uniform(0.0, 1.0, S) * 1e-7
+    # enthalpy offsets (K) chosen so that both reactions release heat, moderately: fuel and oxidiser high, products low
+    lo[:, 5] = np.array([-9000.0, 0.0, -13000.0, -29000.0, -47000.0, 0.0]) * rng.uniform(0.9, 1.1, S)
+    lo[:, 6] = rng.uniform(2.0, 8.0, S)
+    hi = _finish_high_range(lo, rng.uniform(0.6, 1.0, (S, 2)))
+    i32 = lambda a: np.asarray(a, np.int32)
+    return Mechanism(mol_weight=W, elem_comp=comp, nasa_lo=lo, nasa_hi=hi, t_mid=np.full(S, T_SPLIT),
+                     A=np.array([4.9e9, 2.0e8]), b=np.array([0.0, 0.7]), Ea=np.array([35500.0, 12000.0]),
+                     reversible=np.array([0, 1], np.uint8),
+                     reac_ptr=i32([0, 2, 4]), reac_species=i32([0, 1, 2, 1]), reac_nu=i32([1, 2, 1, 1]),
+                     prod_ptr=i32([0, 2, 3]), prod_species=i32([2, 3, 4]), prod_nu=i32([1, 2, 1]),
+                     seed=seed,
+                     reac_coef=np.array([1.0, 1.5, 1.0, 0.5]), prod_coef=np.array([1.0, 2.0, 1.0]),
+                     reac_order=np.array([0.5, 0.65, 1.0, 0.5]), prod_order=np.array([1.0, 2.0, 1.0]))
+
+
+def bfer_shaped_field(n: int, seed: int = 190509395 + 71):
+    """Random fixed thermochemical states: T0 ~ U[1000, 2200] K, p = 1 atm, lean-to-rich mixtures of the
+    fuel and oxidiser species in the inert one, with traces of the products."""
+    rng = np.random.default_rng([seed, n])
+    T = rng.uniform(1000.0, 2200.0, n)
+    Y = np.zeros((6, n))
+    Y[0] = rng.uniform(0.0, 0.08, n)          # fuel
+    Y[1] = rng.uniform(0.05, 0.25, n)         # oxidiser
+    Y[2] = rng.uniform(0.0, 0.02, n)
+    Y[3] = rng.uniform(0.0, 0.05, n)
+    Y[4] = rng.uniform(0.0, 0.05, n)
+    Y[5] = 1.0 - Y[:5].sum(axis=0)
+    return T, np.full(n, P_ATM), np.ascontiguousarray(Y)

@@ -49,15 +49,29 @@ def nasa_numpy(mech, T):
     return cp, h, s
 
 
-def stoich(mech):
+def _entries(mech, which, ptr, sp, default):
     R, S = mech.n_reactions, mech.n_species
-    nu_r, nu_p = np.zeros((R, S)), np.zeros((R, S))
+    vals = getattr(mech, which, None)
+    vals = default if vals is None else vals
+    out = np.zeros((R, S))
     for j in range(R):
-        for e in range(mech.reac_ptr[j], mech.reac_ptr[j + 1]):
-            nu_r[j, mech.reac_species[e]] += mech.reac_nu[e]
-        for e in range(mech.prod_ptr[j], mech.prod_ptr[j + 1]):
-            nu_p[j, mech.prod_species[e]] += mech.prod_nu[e]
-    return nu_r, nu_p
+        for e in range(ptr[j], ptr[j + 1]):
+            out[j, sp[e]] += vals[e]
+    return out
+
+
+def stoich(mech):
+    """Stoichiometric coefficient matrices [R, S] of reactants and products (real ones if the mechanism has them)."""
+    return (_entries(mech, "reac_coef", mech.reac_ptr, mech.reac_species, mech.reac_nu),
+            _entries(mech, "prod_coef", mech.prod_ptr, mech.prod_species, mech.prod_nu))
+
+
+def orders(mech):
+    """Rate-law exponent matrices [R, S] (Eq 28): the orders if given, else the coefficients."""
+    nu_r, nu_p = stoich(mech)
+    o_r = nu_r if getattr(mech, "reac_order", None) is None else _entries(mech, "reac_order", mech.reac_ptr, mech.reac_species, None)
+    o_p = nu_p if getattr(mech, "prod_order", None) is None else _entries(mech, "prod_order", mech.prod_ptr, mech.prod_species, None)
+    return o_r, o_p
 
 
 def rate_constants_numpy(mech, T):
@@ -79,8 +93,9 @@ def numpy_rhs(mech, T, p, Y, isothermal=False):
     rho = p / (R_U * T) / np.sum(Y / W)
     C = np.maximum(rho * Y / W, 0.0)
     kf, Kc = rate_constants_numpy(mech, T)
-    fwd = kf * np.prod(C[None, :] ** nu_r, axis=1)
-    rev = np.where(mech.reversible == 1, kf / Kc * np.prod(C[None, :] ** nu_p, axis=1), 0.0)
+    o_r, o_p = orders(mech)
+    fwd = kf * np.prod(C[None, :] ** o_r, axis=1)
+    rev = np.where(mech.reversible == 1, kf / Kc * np.prod(C[None, :] ** o_p, axis=1), 0.0)
     q = fwd - rev
     omega = (nu_p - nu_r).T @ q
     dY = W * omega / rho

@@ -149,3 +149,40 @@ def test_nonblocking_return_overlaps_host_work(stev, oracle, config, lanes):
     print(f"config {config}: blocking call {tc_b * 1e3:.2f} ms; nonblocking call returned after {tc_n * 1e3:.2f} ms of "
           f"{ta_n * 1e3:.2f} ms, host spun {spins} times meanwhile")
     assert tc_n < 0.5 * ta_n and spins > 10     # the call came back well before the kernel finished
+
+
+# ------------------------------------------------------------------------------------------ real coefficients / orders
+@pytest.mark.parametrize("lanes,n", [(0, 3000), (1, 500), (2, 500), (8, 777), (32, 500)])
+def test_bfer_shaped_mechanism_parity(stev, oracle, lanes, n):
+    """Eqs 26-30 with Table 1's constants and synthetic thermodynamics: real stoichiometric coefficients (1.5, 0.5) and
+    rate-law exponents (0.5, 0.65), t_f = 1 ms.  Runs on the shared-memory-history kernel, bit for bit."""
+    from stev_inputs.mechanisms import bfer_shaped_field, bfer_shaped_mechanism
+    mech = bfer_shaped_mechanism()
+    T, p, Y = bfer_shaped_field(n)
+    prm = default_params()
+    ref = oracle.integrate(mech, None, prm, T, p, Y, 1e-3)
+    gpu = _run(stev, mech, None, prm, T, p, Y, 1e-3, lanes_per_cell=lanes)
+    assert gpu["stats"]["lanes_per_cell"] <= 32
+    rep = assert_parity(gpu, ref)
+    print(f"BFER-shaped, {n} cells, lanes {gpu['stats']['lanes_per_cell']}: {rep}, steps {ref['steps'].min()}..{ref['steps'].max()}")
+    assert gpu["rc"] == ref["rc"] and rep["bit_exact"] == 1.0, rep
+
+
+def test_real_coefficients_are_refused_by_the_tensor_memory_kernels_and_integers_as_reals_agree(stev, oracle):
+    import dataclasses
+    from stev_inputs.mechanisms import bfer_shaped_field, bfer_shaped_mechanism
+    mech = bfer_shaped_mechanism()
+    T, p, Y = bfer_shaped_field(64)
+    for kernel in (33, 64, 512):
+        with pytest.raises(stev.StevError) as err:
+            _run(stev, mech, None, default_params(), T, p, Y, 1e-3, lanes_per_cell=kernel)
+        assert err.value.code == stev.STEV_EINVAL
+    w = make_workload(1, 200)
+    m = w.mech
+    as_real = dataclasses.replace(m, reac_coef=m.reac_nu.astype(float), prod_coef=m.prod_nu.astype(float),
+                                  reac_order=m.reac_nu.astype(float), prod_order=m.prod_nu.astype(float))
+    a = _run(stev, m, None, w.params, w.T, w.p, w.Y, w.dt_cfd, lanes_per_cell=16)
+    b = _run(stev, as_real, None, w.params, w.T, w.p, w.Y, w.dt_cfd)
+    assert b["stats"]["lanes_per_cell"] <= 32
+    for k in ("T", "Y", "steps", "status"):
+        np.testing.assert_array_equal(a[k], b[k])
