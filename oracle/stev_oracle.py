@@ -14,15 +14,17 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "stev_oracle.c")
+_SRCS = [_SRC, os.path.join(_HERE, "stev_oracle_f32.c")]
+_DEPS = _SRCS + [os.path.join(_HERE, "stev_oracle_types.h")]
 _LIB = os.path.join(_HERE, "libstev_oracle.so")
 _lib = None
 
 
 def build(force: bool = False) -> str:
     """gcc -O2 -ffp-contract=off (no implicit FMA contraction: DESIGN.md section 5.1)."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(d) for d in _DEPS):
         cmd = ["gcc", "-O2", "-std=c11", "-Wall", "-Wextra", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC",
-               "-o", _LIB, _SRC, "-lm"]
+               "-o", _LIB, *_SRCS, "-lm"]
         subprocess.run(cmd, check=True)
     return _LIB
 
@@ -35,9 +37,9 @@ def load_variant(define: str):
     exp routine perturbed by one unit in the last place, for the self-sensitivity measurement of DESIGN.md section 5."""
     if define not in _variants:
         lib = os.path.join(_HERE, f"libstev_oracle_{define.lower()}.so")
-        if not os.path.exists(lib) or os.path.getmtime(lib) < os.path.getmtime(_SRC):
+        if not os.path.exists(lib) or os.path.getmtime(lib) < max(os.path.getmtime(d) for d in _DEPS):
             cmd = ["gcc", "-O2", "-std=c11", "-Wall", "-Wextra", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC",
-                   f"-D{define}", "-o", lib, _SRC, "-lm"]
+                   f"-D{define}", "-o", lib, *_SRCS, "-lm"]
             subprocess.run(cmd, check=True)
         _variants[define] = C.CDLL(lib)
     return _variants[define]
@@ -74,6 +76,11 @@ def _load():
         _lib.ora_exp.argtypes = [C.c_double]
         _lib.ora_log.restype = C.c_double
         _lib.ora_log.argtypes = [C.c_double]
+        for f in (_lib.ora_expf, _lib.ora_logf):
+            f.restype = C.c_float
+            f.argtypes = [C.c_float]
+        _lib.ora_dft_bin_f32.restype = C.c_float
+        _lib.ora_dft_bin_f32.argtypes = [C.c_void_p, C.c_int]
     return _lib
 
 
@@ -132,6 +139,21 @@ def log(x: float) -> float:
     return _load().ora_log(float(x))
 
 
+def expf(x: float) -> float:
+    return _load().ora_expf(float(x))
+
+
+def logf(x: float) -> float:
+    return _load().ora_logf(float(x))
+
+
+def dft_mag_f32(ring) -> np.ndarray:
+    lib = _load()
+    r = np.ascontiguousarray(ring, np.float32)
+    assert r.shape == (13,)
+    return np.array([lib.ora_dft_bin_f32(_ptr(r), m) for m in range(7)], np.float32)
+
+
 def thermo(mech, T: float):
     """cp/R, h/RT, s/R of every species at temperature T (NASA-7)."""
     lib = _load()
@@ -160,7 +182,7 @@ def estimator_eval(est, X) -> np.ndarray:
     return out
 
 
-def rates_eval(mech, est, params: dict, T, p, Y, rOF=None):
+def rates_eval(mech, est, params: dict, T, p, Y, rOF=None, precision: str = "f64"):
     """Right-hand side of n cells. Y is [S, n] species-major. Returns dYdt [S,n], dTdt [n], q [R,n]."""
     lib = _load()
     mh, eh, pr = _mech(mech), _est(est), _params(params)
@@ -172,12 +194,13 @@ def rates_eval(mech, est, params: dict, T, p, Y, rOF=None):
     assert Y.shape == (S, n)
     dY, dT, q = np.empty((S, n)), np.empty(n), np.empty((R, n))
     rof = None if rOF is None else np.ascontiguousarray(rOF, np.float64)
-    lib.ora_rates_eval(C.byref(mh.struct), C.byref(eh.struct) if eh else None, C.byref(pr), C.c_int64(n), C.c_int64(n),
+    (lib.ora_rates_eval if precision == "f64" else lib.ora_rates_eval_f32)(C.byref(mh.struct), C.byref(eh.struct) if eh else None, C.byref(pr), C.c_int64(n), C.c_int64(n),
                        _ptr(T), _ptr(p), _ptr(Y), _ptr(rof) if rof is not None else None, _ptr(dY), _ptr(dT), _ptr(q))
     return dY, dT, q
 
 
-def integrate(mech, est, params: dict, T, p, Y, dt_cfd: float, n_threads: int | None = None, variant: str | None = None):
+def integrate(mech, est, params: dict, T, p, Y, dt_cfd: float, n_threads: int | None = None, variant: str | None = None,
+              precision: str = "f64"):
     """Advance n cells over dt_cfd. Inputs are copied. Returns dict(T, Y, steps, status, rof_min, rc)."""
     lib = load_variant(variant) if variant else _load()
     mh, eh, pr = _mech(mech), _est(est), _params(params)
@@ -191,13 +214,14 @@ def integrate(mech, est, params: dict, T, p, Y, dt_cfd: float, n_threads: int | 
     rof_min = np.ones(n)
     if n_threads is None:
         n_threads = os.cpu_count() or 1
-    rc = lib.ora_integrate(C.byref(mh.struct), C.byref(eh.struct) if eh else None, C.byref(pr), C.c_int64(n),
+    rc = (lib.ora_integrate if precision == "f64" else lib.ora_integrate_f32)(C.byref(mh.struct), C.byref(eh.struct) if eh else None, C.byref(pr), C.c_int64(n),
                            C.c_int64(n), _ptr(T), _ptr(p), _ptr(Y), C.c_double(dt_cfd), _ptr(steps), _ptr(status),
                            _ptr(rof_min), C.c_int32(n_threads))
     return dict(T=T, Y=Y, steps=steps, status=status, rof_min=rof_min, rc=rc, n_threads=n_threads)
 
 
-def integrate_trace(mech, est, params: dict, T: float, p: float, Y, dt_cfd: float, trace_cap: int = 100000):
+def integrate_trace(mech, est, params: dict, T: float, p: float, Y, dt_cfd: float, trace_cap: int = 100000,
+                    precision: str = "f64"):
     """One cell with a per-step trace: rows (t, h, T, Y[0..S), rOF[0..R))."""
     lib = _load()
     mh, eh, pr = _mech(mech), _est(est), _params(params)
@@ -206,7 +230,7 @@ def integrate_trace(mech, est, params: dict, T: float, p: float, Y, dt_cfd: floa
     Tc = C.c_double(T)
     steps = C.c_int32(0)
     trace = np.zeros((trace_cap, 3 + S + R))
-    st = lib.ora_integrate_trace(C.byref(mh.struct), C.byref(eh.struct) if eh else None, C.byref(pr), C.byref(Tc),
+    st = (lib.ora_integrate_trace if precision == "f64" else lib.ora_integrate_trace_f32)(C.byref(mh.struct), C.byref(eh.struct) if eh else None, C.byref(pr), C.byref(Tc),
                                  C.c_double(p), _ptr(Yc), C.c_double(dt_cfd), C.byref(steps), _ptr(trace),
                                  C.c_int64(trace_cap))
     n = min(steps.value, trace_cap)
