@@ -33,7 +33,8 @@ int device_sm_count() {
 // ---------------------------------------------------------------------------------------------------------
 static int align_up(int x, int a) { return (x + a - 1) / a * a; }
 
-void build_table_image(const HostMechanism &m, const HostEstimator *e, std::vector<unsigned char> &image, DevTables &tb) {
+void build_table_image(const HostMechanism &m, const HostEstimator *e, std::vector<unsigned char> &image, DevTables &tb, bool f32) {
+  const int es = f32 ? 4 : 8;   // bytes per real: the binary32 image holds every real table rounded to float once
   const int S = m.S, R = m.R;
   tb = DevTables{};
   tb.S = S;
@@ -63,23 +64,23 @@ void build_table_image(const HostMechanism &m, const HostEstimator *e, std::vect
     off = align_up(off + bytes, 16);
     return o;
   };
-  tb.o_invW = take(8 * S);
-  tb.o_W = take(8 * S);
-  tb.o_tmid = take(8 * S);
-  tb.o_nasa = take(8 * 2 * kNasaRows * S);
-  tb.o_lnA = take(8 * R);
-  tb.o_b = take(8 * R);
-  tb.o_Ta = take(8 * R);
-  tb.o_dnu = take(8 * R);
+  tb.o_invW = take(es * S);
+  tb.o_W = take(es * S);
+  tb.o_tmid = take(es * S);
+  tb.o_nasa = take(es * 2 * kNasaRows * S);
+  tb.o_lnA = take(es * R);
+  tb.o_b = take(es * R);
+  tb.o_Ta = take(es * R);
+  tb.o_dnu = take(es * R);
   tb.o_part = take(8 * R);
   tb.o_orig = take(2 * R);
   tb.o_gptr = take(2 * (S + 1));
   tb.o_gent = take(4 * n_gather);
   tb.has_real = m.has_real ? 1 : 0;
   if (m.has_real) {
-    tb.o_rcoef = take(8 * 4 * R);
-    tb.o_rord = take(8 * 4 * R);
-    tb.o_gcoef = take(8 * n_gather);
+    tb.o_rcoef = take(es * 4 * R);
+    tb.o_rord = take(es * 4 * R);
+    tb.o_gcoef = take(es * n_gather);
   }
   if (e) {
     tb.has_est = 1;
@@ -99,42 +100,48 @@ void build_table_image(const HostMechanism &m, const HostEstimator *e, std::vect
   tb.bytes = align_up(off, 128);
   image.assign(tb.bytes, 0);
   unsigned char *base = image.data();
-  double *invW = (double *)(base + tb.o_invW), *W = (double *)(base + tb.o_W), *tmid = (double *)(base + tb.o_tmid);
-  double *nasa = (double *)(base + tb.o_nasa);
+  // every real table entry is formed in double (the same operations as the oracle's table set-up) and stored as double or,
+  // for the binary32 image, rounded to float
+  auto put = [&](int off0, int idx, double v) {
+    if (f32) ((float *)(base + off0))[idx] = (float)v;
+    else ((double *)(base + off0))[idx] = v;
+  };
   for (int i = 0; i < S; ++i) {
-    invW[i] = 1.0 / m.W[i];
-    W[i] = m.W[i];
-    tmid[i] = m.t_mid[i];
+    put(tb.o_invW, i, 1.0 / m.W[i]);
+    put(tb.o_W, i, m.W[i]);
+    put(tb.o_tmid, i, m.t_mid[i]);
     for (int rg = 0; rg < 2; ++rg) {
       const double *a = (rg == 0 ? m.nasa_lo.data() : m.nasa_hi.data()) + 7 * i;
-      double *row = nasa + rg * kNasaRows * S + i;
-      row[0 * S] = a[0]; row[1 * S] = a[1]; row[2 * S] = a[2]; row[3 * S] = a[3]; row[4 * S] = a[4];
-      row[5 * S] = a[1] / 2.0; row[6 * S] = a[2] / 3.0; row[7 * S] = a[3] / 4.0; row[8 * S] = a[4] / 5.0;
-      row[9 * S] = a[5];
-      row[10 * S] = a[2] / 2.0; row[11 * S] = a[3] / 3.0; row[12 * S] = a[4] / 4.0;
-      row[13 * S] = a[6];
+      const int r0 = rg * kNasaRows * S + i;
+      put(tb.o_nasa, r0 + 0 * S, a[0]); put(tb.o_nasa, r0 + 1 * S, a[1]); put(tb.o_nasa, r0 + 2 * S, a[2]);
+      put(tb.o_nasa, r0 + 3 * S, a[3]); put(tb.o_nasa, r0 + 4 * S, a[4]);
+      put(tb.o_nasa, r0 + 5 * S, a[1] / 2.0); put(tb.o_nasa, r0 + 6 * S, a[2] / 3.0); put(tb.o_nasa, r0 + 7 * S, a[3] / 4.0);
+      put(tb.o_nasa, r0 + 8 * S, a[4] / 5.0);
+      put(tb.o_nasa, r0 + 9 * S, a[5]);
+      put(tb.o_nasa, r0 + 10 * S, a[2] / 2.0); put(tb.o_nasa, r0 + 11 * S, a[3] / 3.0); put(tb.o_nasa, r0 + 12 * S, a[4] / 4.0);
+      put(tb.o_nasa, r0 + 13 * S, a[6]);
     }
   }
-  double *lnA = (double *)(base + tb.o_lnA), *bb = (double *)(base + tb.o_b), *Ta = (double *)(base + tb.o_Ta);
-  double *dnu = (double *)(base + tb.o_dnu);
   unsigned long long *part = (unsigned long long *)(base + tb.o_part);
   unsigned short *orig = (unsigned short *)(base + tb.o_orig);
   for (int k = 0; k < R; ++k) {
     const int j = m.orig_of[k];
-    lnA[k] = clog(m.A[j]);
-    bb[k] = m.b[j];
-    Ta[k] = m.Ea[j] / kRcal;
+    put(tb.o_lnA, k, clog(m.A[j]));
+    put(tb.o_b, k, m.b[j]);
+    put(tb.o_Ta, k, m.Ea[j] / kRcal);
     orig[k] = (unsigned short)j;
     unsigned long long pk = 0;
     double d = 0.0;
+    float d32 = 0.0f;   // Delta-nu summed in the precision of the image, in entry order (as the oracle sums it)
     int slot = 0;
     for (int en = m.reac_ptr[j]; en < m.reac_ptr[j + 1]; ++en, ++slot) {
       pk |= (unsigned long long)(m.reac_sp[en] & 0xff) << (16 * slot);
       pk |= (unsigned long long)(m.reac_nu[en] & 0xff) << (16 * slot + 8);
       d = d - m.reac_coef[en];
+      d32 = d32 - (float)m.reac_coef[en];
       if (m.has_real) {
-        ((double *)(base + tb.o_rcoef))[4 * k + slot] = m.reac_coef[en];
-        ((double *)(base + tb.o_rord))[4 * k + slot] = m.reac_order[en];
+        put(tb.o_rcoef, 4 * k + slot, m.reac_coef[en]);
+        put(tb.o_rord, 4 * k + slot, m.reac_order[en]);
       }
     }
     slot = 0;
@@ -142,13 +149,14 @@ void build_table_image(const HostMechanism &m, const HostEstimator *e, std::vect
       pk |= (unsigned long long)(m.prod_sp[en] & 0xff) << (32 + 16 * slot);
       pk |= (unsigned long long)(m.prod_nu[en] & 0xff) << (32 + 16 * slot + 8);
       d = d + m.prod_coef[en];
+      d32 = d32 + (float)m.prod_coef[en];
       if (m.has_real) {
-        ((double *)(base + tb.o_rcoef))[4 * k + 2 + slot] = m.prod_coef[en];
-        ((double *)(base + tb.o_rord))[4 * k + 2 + slot] = m.prod_order[en];
+        put(tb.o_rcoef, 4 * k + 2 + slot, m.prod_coef[en]);
+        put(tb.o_rord, 4 * k + 2 + slot, m.prod_order[en]);
       }
     }
     part[k] = pk;
-    dnu[k] = d;
+    put(tb.o_dnu, k, f32 ? (double)d32 : d);
   }
   unsigned short *gptr = (unsigned short *)(base + tb.o_gptr);
   unsigned *gent = (unsigned *)(base + tb.o_gent);
@@ -156,7 +164,7 @@ void build_table_image(const HostMechanism &m, const HostEstimator *e, std::vect
   for (int i = 0; i < S; ++i) {
     gptr[i] = (unsigned short)pos;
     for (size_t q = 0; q < gl[i].size(); ++q) {
-      if (m.has_real) ((double *)(base + tb.o_gcoef))[pos] = glc[i][q];
+      if (m.has_real) put(tb.o_gcoef, pos, glc[i][q]);
       gent[pos++] = gl[i][q];
     }
   }
@@ -181,7 +189,7 @@ void build_table_image(const HostMechanism &m, const HostEstimator *e, std::vect
 static constexpr size_t kSmemMax = 227 * 1024;   // opt-in dynamic shared memory per block on sm_100
 static constexpr size_t kSmemPerSM = 228 * 1024;
 
-static void make_layout(const DevTables &tb, int G, CellLayout &cl) {
+static void make_layout(const DevTables &tb, int G, CellLayout &cl, int es) {
   const int S = tb.S, R = tb.R, Rrev = tb.Rrev;
   int o = 0;
   auto take = [&](int n) {
@@ -198,7 +206,7 @@ static void make_layout(const DevTables &tb, int G, CellLayout &cl) {
   cl.oRof = take(Rrev);
   cl.rrev_pad = Rrev;
   cl.oRing = take(kWindow * Rrev);
-  cl.oHid = take(tb.has_est ? (tb.H + 1) / 2 : 0);
+  cl.oHid = take(tb.has_est ? (es == 8 ? (tb.H + 1) / 2 : tb.H) : 0);   // H floats
   // pad the stride so that the groups of a half-warp (one 128-byte shared-memory phase) start in distinct banks
   int stride = o;
   if (G < 16) {
@@ -207,10 +215,10 @@ static void make_layout(const DevTables &tb, int G, CellLayout &cl) {
   cl.stride = stride;
 }
 
-bool choose_config(const DevTables &tb, int request, LaunchConfig &cfg) {
+bool choose_config(const DevTables &tb, int request, LaunchConfig &cfg, int es) {
   auto fits = [&](int G, LaunchConfig &c) -> bool {
-    make_layout(tb, G, c.cl);
-    const size_t cell_bytes = (size_t)c.cl.stride * 8;
+    make_layout(tb, G, c.cl, es);
+    const size_t cell_bytes = (size_t)c.cl.stride * es;
     const size_t avail = kSmemMax - tb.bytes - 64;
     const int cells_sm = (int)std::min<size_t>(avail / cell_bytes, 2048 / G);
     const int per_warp = 32 / G;
@@ -389,6 +397,11 @@ int stev_mechanism_create(const stev_mechanism_desc *d, stev_mechanism **out) {
   build_table_image(h, nullptr, image, m->tb);
   cudaError_t e = cudaMalloc(&m->d_table, image.size());
   if (e == cudaSuccess) e = cudaMemcpy(m->d_table, image.data(), image.size(), cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) {
+    build_table_image(h, nullptr, image, m->tb32, true);
+    e = cudaMalloc(&m->d_table32, image.size());
+    if (e == cudaSuccess) e = cudaMemcpy(m->d_table32, image.data(), image.size(), cudaMemcpyHostToDevice);
+  }
   for (int n = 0; n < 2 && e == cudaSuccess; ++n) {   // the pair image first: it chooses the reaction order
     static const int order[2] = {1, 0}, nw_of[2] = {1, 2};
     const int w = order[n];
@@ -418,6 +431,7 @@ int stev_mechanism_create(const stev_mechanism_desc *d, stev_mechanism **out) {
 void stev_mechanism_destroy(stev_mechanism *m) {
   if (!m) return;
   if (m->d_table) cudaFree(m->d_table);
+  if (m->d_table32) cudaFree(m->d_table32);
   for (int w = 0; w < 2; ++w)
     if (m->d_pk_table[w]) cudaFree(m->d_pk_table[w]);
   if (m->d_ls_table) cudaFree(m->d_ls_table);
@@ -468,6 +482,11 @@ int stev_estimator_load(const stev_mechanism *m, const stev_estimator_desc *d, s
     build_table_image(m->host, &h, image, e->tb);
     ce = cudaMalloc(&e->d_table, image.size());
     if (ce == cudaSuccess) ce = cudaMemcpy(e->d_table, image.data(), image.size(), cudaMemcpyHostToDevice);
+    if (ce == cudaSuccess) {
+      build_table_image(m->host, &h, image, e->tb32, true);
+      ce = cudaMalloc(&e->d_table32, image.size());
+      if (ce == cudaSuccess) ce = cudaMemcpy(e->d_table32, image.data(), image.size(), cudaMemcpyHostToDevice);
+    }
     for (int n = 0; n < 2 && ce == cudaSuccess; ++n) {
       static const int order[2] = {1, 0}, nw_of[2] = {1, 2};
       const int w = order[n];
@@ -517,6 +536,7 @@ int stev_estimator_load(const stev_mechanism *m, const stev_estimator_desc *d, s
 void stev_estimator_destroy(stev_estimator *e) {
   if (!e) return;
   if (e->d_table) cudaFree(e->d_table);
+  if (e->d_table32) cudaFree(e->d_table32);
   for (int w = 0; w < 2; ++w)
     if (e->d_pk_table[w]) cudaFree(e->d_pk_table[w]);
   if (e->d_ls_table) cudaFree(e->d_ls_table);
@@ -615,15 +635,16 @@ SolverConsts make_consts(const stev_params *p) {
   return sc;
 }
 
-int pick_tables(const stev_mechanism *m, const stev_estimator *e, const DevTables **tb, const unsigned char **table) {
+int pick_tables(const stev_mechanism *m, const stev_estimator *e, const DevTables **tb, const unsigned char **table,
+                bool f32 = false) {
   if (!m) { set_error("null mechanism"); return STEV_EINVAL; }
   if (e) {
     if (e->mech != m || !e->d_table) { set_error("estimator was not loaded against this mechanism"); return STEV_EINVAL; }
-    *tb = &e->tb;
-    *table = e->d_table;
+    *tb = f32 ? &e->tb32 : &e->tb;
+    *table = f32 ? e->d_table32 : e->d_table;
   } else {
-    *tb = &m->tb;
-    *table = m->d_table;
+    *tb = f32 ? &m->tb32 : &m->tb;
+    *table = f32 ? m->d_table32 : m->d_table;
   }
   return STEV_OK;
 }
@@ -631,27 +652,27 @@ int pick_tables(const stev_mechanism *m, const stev_estimator *e, const DevTable
 template <typename Args>
 using KernelPtr = void (*)(const Args);
 
-template <int G> void *integrate_fn() { return (void *)stev_integrate_kernel<G>; }
-template <int G> void *rates_fn() { return (void *)stev_rates_kernel<G>; }
+template <int G> void *integrate_fn(bool f32) { return f32 ? (void *)stev_integrate_kernel<G, float> : (void *)stev_integrate_kernel<G, double>; }
+template <int G> void *rates_fn(bool f32) { return f32 ? (void *)stev_rates_kernel<G, float> : (void *)stev_rates_kernel<G, double>; }
 
-void *integrate_kernel_for(int G) {
+void *integrate_kernel_for(int G, bool f32) {
   switch (G) {
-    case 1: return integrate_fn<1>();
-    case 2: return integrate_fn<2>();
-    case 4: return integrate_fn<4>();
-    case 8: return integrate_fn<8>();
-    case 16: return integrate_fn<16>();
-    default: return integrate_fn<32>();
+    case 1: return integrate_fn<1>(f32);
+    case 2: return integrate_fn<2>(f32);
+    case 4: return integrate_fn<4>(f32);
+    case 8: return integrate_fn<8>(f32);
+    case 16: return integrate_fn<16>(f32);
+    default: return integrate_fn<32>(f32);
   }
 }
-void *rates_kernel_for(int G) {
+void *rates_kernel_for(int G, bool f32) {
   switch (G) {
-    case 1: return rates_fn<1>();
-    case 2: return rates_fn<2>();
-    case 4: return rates_fn<4>();
-    case 8: return rates_fn<8>();
-    case 16: return rates_fn<16>();
-    default: return rates_fn<32>();
+    case 1: return rates_fn<1>(f32);
+    case 2: return rates_fn<2>(f32);
+    case 4: return rates_fn<4>(f32);
+    case 8: return rates_fn<8>(f32);
+    case 16: return rates_fn<16>(f32);
+    default: return rates_fn<32>(f32);
   }
 }
 }  // namespace
@@ -694,9 +715,14 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
                    void *workspace, size_t workspace_bytes, void *cuda_stream) {
   const DevTables *tb;
   const unsigned char *table;
-  int rc = pick_tables(m, est, &tb, &table);
+  int rc = check_params(p);
   if (rc) return rc;
-  if ((rc = check_params(p))) return rc;
+  const bool f32 = p->state_precision == STEV_STATE_FP32;
+  if ((rc = pick_tables(m, est, &tb, &table, f32))) return rc;
+  if (f32 && p->lanes_per_cell > 32) {
+    set_error("stev_integrate: state_precision = STEV_STATE_FP32 runs on the shared-memory-history kernel (lanes_per_cell 0 or 1..32)");
+    return STEV_EINVAL;
+  }
   if (n < 0 || n > 0x7fffffff || ld < n || !(dt_cfd > 0.0) || !std::isfinite(dt_cfd)) {
     set_error("stev_integrate: need 0 <= n_cells <= 2^31-1, ld >= n_cells, dt_cfd > 0");
     return STEV_EINVAL;
@@ -732,7 +758,7 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
     else if (p->lanes_per_cell == 64) kind = 2;
     else if (p->lanes_per_cell == 34) kind = 6;
     else if (p->lanes_per_cell == 512 || p->lanes_per_cell == 513) kind = 7;
-    else if (p->lanes_per_cell == 0) {
+    else if (p->lanes_per_cell == 0 && !f32) {
       // Measured on B200: large mechanisms -> warp pair; tiny ones (a step is a few hundred
       // instructions) -> lock-step block, which flattens (cell, reaction) pairs over the lanes; mid-size -> one warp per
       // cell, 32 cells per SM when the reversible reactions fit two 32-blocks, else 16.
@@ -792,12 +818,13 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
     }
   }
 
+  const int es = f32 ? 4 : 8;
   LaunchConfig cfg;
-  if (!choose_config(*tb, g_request, cfg) && !(p->lanes_per_cell == 0 && choose_config(*tb, 0, cfg))) {
+  if (!choose_config(*tb, g_request, cfg, es) && !(p->lanes_per_cell == 0 && choose_config(*tb, 0, cfg, es))) {
     set_error("stev_integrate: no launch configuration fits shared memory for this mechanism / lanes_per_cell");
     return STEV_EINVAL;
   }
-  void *fn = integrate_kernel_for(cfg.G);
+  void *fn = integrate_kernel_for(cfg.G, f32);
   STEV_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem));
 
   IntegrateArgs a{};
@@ -925,15 +952,17 @@ int stev_rates_eval(const stev_mechanism *m, const stev_estimator *est, const st
                     double *q, void *cuda_stream) {
   const DevTables *tb;
   const unsigned char *table;
-  int rc = pick_tables(m, est, &tb, &table);
+  int rc = check_params(p);
   if (rc) return rc;
-  if ((rc = check_params(p))) return rc;
+  const bool f32 = p->state_precision == STEV_STATE_FP32;
+  if ((rc = pick_tables(m, est, &tb, &table, f32))) return rc;
   if (n < 0 || ld < n) { set_error("stev_rates_eval: bad sizes"); return STEV_EINVAL; }
   if (n == 0) return STEV_OK;
   if (!T || !pressure || !Y || !dYdt || !dTdt || !q) { set_error("stev_rates_eval: null pointer"); return STEV_EINVAL; }
   LaunchConfig cfg;
-  if (!choose_config(*tb, p->lanes_per_cell, cfg)) { set_error("no launch configuration fits"); return STEV_EINVAL; }
-  void *fn = rates_kernel_for(cfg.G);
+  // lanes_per_cell values above 32 name the tensor-memory kernels of stev_integrate: here they mean "choose"
+  if (!choose_config(*tb, p->lanes_per_cell > 32 ? 0 : p->lanes_per_cell, cfg, f32 ? 4 : 8)) { set_error("no launch configuration fits"); return STEV_EINVAL; }
+  void *fn = rates_kernel_for(cfg.G, f32);
   STEV_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem));
   RatesArgs a{};
   a.tb = *tb;

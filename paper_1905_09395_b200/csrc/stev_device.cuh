@@ -125,12 +125,49 @@ __device__ __forceinline__ void group_sync() {
   if (G > 1) __syncwarp();
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// The arithmetic of one precision (DESIGN.md section 5 for binary64, section 5b for binary32: stev_params.state_precision).
+// ---------------------------------------------------------------------------------------------------------
+template <typename RT> struct MathT;
+template <> struct MathT<double> {
+  static __device__ __forceinline__ double fma(double a, double b, double c) { return fma_rn(a, b, c); }
+  static __device__ __forceinline__ double exp(double x) { return cexp(x); }
+  static __device__ __forceinline__ double log(double x) { return clog(x); }
+  static __device__ __forceinline__ double sqrt(double x) { return ::sqrt(x); }
+  static __device__ __forceinline__ double abs(double x) { return fabs(x); }
+  static __device__ __forceinline__ double inf() { return bits_to_double(0x7ff0000000000000ull); }
+  static __device__ __forceinline__ double ru() { return kRu; }
+  static __device__ __forceinline__ double patm() { return kPatm; }
+  static __device__ __forceinline__ double r_floor() { return 1.0e-30; }     // Eq 1
+  static __device__ __forceinline__ double y_small() { return 1.0e-20; }     // Eq 2 (R2)
+  static __device__ __forceinline__ double ninety() { return 0.9; }          // Eq 2
+  static __device__ __forceinline__ double dft_guard() { return 1.0e-300; }  // Eq 10 (R10)
+  static __device__ __forceinline__ double land_tol() { return 1.0e-12; }    // R5
+  static __device__ __forceinline__ double inv_r_fac(const SolverConsts &sc) { return sc.inv_r_fac; }
+};
+template <> struct MathT<float> {
+  static __device__ __forceinline__ float fma(float a, float b, float c) { return __fmaf_rn(a, b, c); }
+  static __device__ __forceinline__ float exp(float x) { return cexpf32(x); }
+  static __device__ __forceinline__ float log(float x) { return clogf32(x); }
+  static __device__ __forceinline__ float sqrt(float x) { return __fsqrt_rn(x); }
+  static __device__ __forceinline__ float abs(float x) { return fabsf(x); }
+  static __device__ __forceinline__ float inf() { return __int_as_float(0x7f800000); }
+  static __device__ __forceinline__ float ru() { return 0x1.3d2becp+26f; }   // (float) 8.31446261815324e7
+  static __device__ __forceinline__ float patm() { return 0x1.eec04p+19f; }  // (float) 1.01325e6
+  static __device__ __forceinline__ float r_floor() { return 1.0e-30f; }
+  static __device__ __forceinline__ float y_small() { return 1.0e-20f; }
+  static __device__ __forceinline__ float ninety() { return 0.9f; }
+  static __device__ __forceinline__ float dft_guard() { return 1.0e-30f; }   // R26
+  static __device__ __forceinline__ float land_tol() { return 1.0e-6f; }     // R26
+  static __device__ __forceinline__ float inv_r_fac(const SolverConsts &sc) { return 1.0f / (float)sc.r_fac; }
+};
+
 // min / or across the G lanes of a group (exact: min and or are associative and commutative)
-template <int G>
-__device__ __forceinline__ double group_min(double v) {
+template <int G, typename RT>
+__device__ __forceinline__ RT group_min(RT v) {
 #pragma unroll
   for (int off = G / 2; off >= 1; off >>= 1) {
-    double o = __shfl_xor_sync(0xffffffffu, v, off);
+    RT o = __shfl_xor_sync(0xffffffffu, v, off);
     v = (o < v) ? o : v;
   }
   return v;
@@ -143,25 +180,26 @@ __device__ __forceinline__ int group_or(int v) {
 }
 
 // Views of the staged tables.
+template <typename RT>
 struct TableView {
-  const double *invW, *W, *tmid, *nasa, *lnA, *b, *Ta, *dnu;
+  const RT *invW, *W, *tmid, *nasa, *lnA, *b, *Ta, *dnu;
   const unsigned long long *part;
   const unsigned short *orig, *gptr;
   const unsigned *gent;
   const float *eshift, *escale, *W1T, *b1, *W2T, *b2;
-  const double *rcoef, *rord, *gcoef;
+  const RT *rcoef, *rord, *gcoef;
   __device__ __forceinline__ TableView(const unsigned char *base, const DevTables &tb) {
-    rcoef = (const double *)(base + tb.o_rcoef);
-    rord = (const double *)(base + tb.o_rord);
-    gcoef = (const double *)(base + tb.o_gcoef);
-    invW = (const double *)(base + tb.o_invW);
-    W = (const double *)(base + tb.o_W);
-    tmid = (const double *)(base + tb.o_tmid);
-    nasa = (const double *)(base + tb.o_nasa);
-    lnA = (const double *)(base + tb.o_lnA);
-    b = (const double *)(base + tb.o_b);
-    Ta = (const double *)(base + tb.o_Ta);
-    dnu = (const double *)(base + tb.o_dnu);
+    rcoef = (const RT *)(base + tb.o_rcoef);
+    rord = (const RT *)(base + tb.o_rord);
+    gcoef = (const RT *)(base + tb.o_gcoef);
+    invW = (const RT *)(base + tb.o_invW);
+    W = (const RT *)(base + tb.o_W);
+    tmid = (const RT *)(base + tb.o_tmid);
+    nasa = (const RT *)(base + tb.o_nasa);
+    lnA = (const RT *)(base + tb.o_lnA);
+    b = (const RT *)(base + tb.o_b);
+    Ta = (const RT *)(base + tb.o_Ta);
+    dnu = (const RT *)(base + tb.o_dnu);
     part = (const unsigned long long *)(base + tb.o_part);
     orig = (const unsigned short *)(base + tb.o_orig);
     gptr = (const unsigned short *)(base + tb.o_gptr);
@@ -177,17 +215,19 @@ struct TableView {
 
 // f * C^x (Eq 28; R22): x = 1, 2, 3 by repeated multiplication (the mass-action case, contract 5.5), x = 0
 // leaves f, any other exponent as exp(x log C) through the contract routines, and C^x = 0 for C <= 0.
-__device__ __forceinline__ double times_power(double f, double c, double x) {
-  if (x == 1.0) return f * c;
-  if (x == 2.0) return (f * c) * c;
-  if (x == 3.0) return ((f * c) * c) * c;
-  if (x == 0.0) return f;
-  return f * ((c > 0.0) ? cexp(x * clog(c)) : 0.0);
+template <typename RT>
+__device__ __forceinline__ RT times_power(RT f, RT c, RT x) {
+  if (x == RT(1)) return f * c;
+  if (x == RT(2)) return (f * c) * c;
+  if (x == RT(3)) return ((f * c) * c) * c;
+  if (x == RT(0)) return f;
+  return f * ((c > RT(0)) ? MathT<RT>::exp(x * MathT<RT>::log(c)) : RT(0));
 }
 
 // What one right-hand-side evaluation leaves in registers (identical in every lane of the group).
+template <typename RT>
 struct RhsOut {
-  double c_tot, rho, dTdt, t_star;
+  RT c_tot, rho, dTdt, t_star;
 };
 
 // ---------------------------------------------------------------------------------------------------------
@@ -196,28 +236,29 @@ struct RhsOut {
 //   out: cell[oQ][k] effective progress rates (internal order), cell[oConc][i] := r_i = dY_i/dt,
 //        cell[oG][i] := omega_i, RhsOut.  Ends with the group converged and all writes visible.
 // ---------------------------------------------------------------------------------------------------------
-template <int G>
-__device__ __forceinline__ RhsOut rhs_eval(const DevTables &tb, const TableView &tv, const CellLayout &cl,
-                                           const SolverConsts &sc, double *cell, int gl, double T, double p,
-                                           bool use_rof) {
+template <int G, typename RT>
+__device__ __forceinline__ RhsOut<RT> rhs_eval(const DevTables &tb, const TableView<RT> &tv, const CellLayout &cl,
+                                               const SolverConsts &sc, RT *cell, int gl, RT T, RT p, bool use_rof) {
+  using M = MathT<RT>;
+  const RT alpha = (RT)sc.alpha, y_step_max = (RT)sc.y_step_max;
   const int S = tb.S, R = tb.R, Rrev = tb.Rrev;
-  double *cY = cell + cl.oY, *cConc = cell + cl.oConc, *cG = cell + cl.oG, *cCp = cell + cl.oCp, *cH = cell + cl.oH;
-  double *cQ = cell + cl.oQ;
-  const double *cRof = cell + cl.oRof;
+  RT *cY = cell + cl.oY, *cConc = cell + cl.oConc, *cG = cell + cl.oG, *cCp = cell + cl.oCp, *cH = cell + cl.oH;
+  RT *cQ = cell + cl.oQ;
+  const RT *cRof = cell + cl.oRof;
 
   // -- a1: thermo (Eqs 15-16, R17).  g/RT always from NASA-7.
-  const double lnT = clog(T);
-  const double invT = 1.0 / T;
+  const RT lnT = M::log(T);
+  const RT invT = RT(1) / T;
   for (int i = gl; i < S; i += G) {
-    const double *c = tv.nasa + ((T < tv.tmid[i]) ? 0 : kNasaRows * S) + i;
-    const double a1 = c[0], a2 = c[S];
-    double hp = fma_rn(fma_rn(fma_rn(fma_rn(c[8 * S], T, c[7 * S]), T, c[6 * S]), T, c[5 * S]), T, a1);
-    double hRT = fma_rn(c[9 * S], invT, hp);
-    double sp = fma_rn(fma_rn(fma_rn(c[12 * S], T, c[11 * S]), T, c[10 * S]), T, a2);
-    double sR = fma_rn(a1, lnT, fma_rn(sp, T, c[13 * S]));
+    const RT *c = tv.nasa + ((T < tv.tmid[i]) ? 0 : kNasaRows * S) + i;
+    const RT a1 = c[0], a2 = c[S];
+    RT hp = M::fma(M::fma(M::fma(M::fma(c[8 * S], T, c[7 * S]), T, c[6 * S]), T, c[5 * S]), T, a1);
+    RT hRT = M::fma(c[9 * S], invT, hp);
+    RT sp = M::fma(M::fma(M::fma(c[12 * S], T, c[11 * S]), T, c[10 * S]), T, a2);
+    RT sR = M::fma(a1, lnT, M::fma(sp, T, c[13 * S]));
     cG[i] = hRT - sR;
     if (!tb.has_est) {
-      cCp[i] = fma_rn(fma_rn(fma_rn(fma_rn(c[4 * S], T, c[3 * S]), T, c[2 * S]), T, a2), T, a1);
+      cCp[i] = M::fma(M::fma(M::fma(M::fma(c[4 * S], T, c[3 * S]), T, c[2 * S]), T, a2), T, a1);
       cH[i] = hRT;
     }
   }
@@ -228,97 +269,97 @@ __device__ __forceinline__ RhsOut rhs_eval(const DevTables &tb, const TableView 
     for (int jh = gl; jh < H; jh += G) {
       float z = tv.b1[jh];
       for (int k = 0; k < n_in; ++k) {
-        double raw = (k == 0) ? T : ((k == 1) ? p : cY[k - 2]);
+        const RT raw = (k == 0) ? T : ((k == 1) ? p : cY[k - 2]);
         float x = ((float)raw - tv.eshift[k]) * tv.escale[k];
         z = __fmaf_rn(tv.W1T[k * H + jh], x, z);
       }
-      double zd = (double)z;
+      const RT zd = (RT)z;
       float a;
-      if (tb.act == 0) a = (float)(1.0 - 2.0 / (1.0 + cexp(2.0 * zd)));
-      else a = (float)(1.0 / (1.0 + cexp(-zd)));
+      if (tb.act == 0) a = (float)(RT(1) - RT(2) / (RT(1) + M::exp(RT(2) * zd)));
+      else a = (float)(RT(1) / (RT(1) + M::exp(-zd)));
       hid[jh] = a;
     }
     group_sync<G>();
     for (int o = gl; o < n_out; o += G) {
       float y = tv.b2[o];
       for (int jh = 0; jh < H; ++jh) y = __fmaf_rn(tv.W2T[jh * n_out + o], hid[jh], y);
-      if (o < S) cCp[o] = (double)y;
-      else cH[o - S] = ((double)y * (double)tb.h_ref_T) * invT;
+      if (o < S) cCp[o] = (RT)y;
+      else cH[o - S] = ((RT)y * (RT)tb.h_ref_T) * invT;
     }
   }
   group_sync<G>();
 
   // -- mixture sums, sequential in species order (contract 5.4); every lane computes them redundantly.
-  double inv_wbar = 0.0, sum_cp = 0.0;
+  RT inv_wbar = RT(0), sum_cp = RT(0);
   for (int i = 0; i < S; ++i) {
-    double y = cY[i], w = tv.invW[i];
-    inv_wbar = fma_rn(y, w, inv_wbar);
-    sum_cp = fma_rn(y * w, cCp[i], sum_cp);
+    RT y = cY[i], w = tv.invW[i];
+    inv_wbar = M::fma(y, w, inv_wbar);
+    sum_cp = M::fma(y * w, cCp[i], sum_cp);
   }
-  RhsOut out;
-  out.c_tot = p / (kRu * T);
+  RhsOut<RT> out;
+  out.c_tot = p / (M::ru() * T);
   out.rho = out.c_tot / inv_wbar;
   // -- small-species stabilisation (Eqs 6-7, R7): C** = gamma(y) rho y / W
   for (int i = gl; i < S; i += G) {
-    double y = cY[i];
-    double yp = (y > 0.0) ? y : 0.0;
-    double c = (out.rho * yp) * tv.invW[i];
-    if (sc.alpha > 0.0) c = (yp / (sc.alpha + yp)) * c;
+    RT y = cY[i];
+    RT yp = (y > RT(0)) ? y : RT(0);
+    RT c = (out.rho * yp) * tv.invW[i];
+    if (alpha > RT(0)) c = (yp / (alpha + yp)) * c;
     cConc[i] = c;
   }
   group_sync<G>();
 
   // -- a2: rate constants and progress rates (Eqs 28-30; Eq 14).  Internal order:
   //    k < Rrev reversible, k >= Rrev irreversible, so the branch below is uniform except at one boundary.
-  const double ln_c0 = clog(kPatm / (kRu * T));
+  const RT ln_c0 = M::log(M::patm() / (M::ru() * T));
   for (int k = gl; k < R; k += G) {
-    const double ln_kf = fma_rn(-tv.Ta[k], invT, fma_rn(tv.b[k], lnT, tv.lnA[k]));
-    double fwd = cexp(ln_kf);
+    const RT ln_kf = M::fma(-tv.Ta[k], invT, M::fma(tv.b[k], lnT, tv.lnA[k]));
+    RT fwd = M::exp(ln_kf);
     const unsigned long long pt = tv.part[k];
     const int r0 = (int)(pt & 0xff), n0 = (int)((pt >> 8) & 0xff), r1 = (int)((pt >> 16) & 0xff), n1 = (int)((pt >> 24) & 0xff);
     const int p0 = (int)((pt >> 32) & 0xff), m0 = (int)((pt >> 40) & 0xff), p1 = (int)((pt >> 48) & 0xff), m1 = (int)((pt >> 56) & 0xff);
-    double qk;
+    RT qk;
     if (tb.has_real) {
       // real coefficients and exponents (Eqs 26-29): same order of operations as the integer case below
-      const double *co = tv.rcoef + 4 * k, *od = tv.rord + 4 * k;
-      fwd = times_power(fwd, cConc[r0], od[0]);
-      if (n1) fwd = times_power(fwd, cConc[r1], od[1]);
+      const RT *co = tv.rcoef + 4 * k, *od = tv.rord + 4 * k;
+      fwd = times_power<RT>(fwd, cConc[r0], od[0]);
+      if (n1) fwd = times_power<RT>(fwd, cConc[r1], od[1]);
       qk = fwd;
       if (k < Rrev) {
-        double dg = 0.0 - co[0] * cG[r0];
+        RT dg = RT(0) - co[0] * cG[r0];
         if (n1) dg = dg - co[1] * cG[r1];
         dg = dg + co[2] * cG[p0];
         if (m1) dg = dg + co[3] * cG[p1];
-        const double ln_kc = fma_rn(tv.dnu[k], ln_c0, -dg);
-        double rev = cexp(ln_kf - ln_kc);
-        rev = times_power(rev, cConc[p0], od[2]);
-        if (m1) rev = times_power(rev, cConc[p1], od[3]);
-        qk = (fwd - rev) * (use_rof ? cRof[k] : 1.0);
+        const RT ln_kc = M::fma(tv.dnu[k], ln_c0, -dg);
+        RT rev = M::exp(ln_kf - ln_kc);
+        rev = times_power<RT>(rev, cConc[p0], od[2]);
+        if (m1) rev = times_power<RT>(rev, cConc[p1], od[3]);
+        qk = (fwd - rev) * (use_rof ? cRof[k] : RT(1));
       }
     } else {
       {
-        const double c0 = cConc[r0];
+        const RT c0 = cConc[r0];
         for (int n = 0; n < n0; ++n) fwd = fwd * c0;
         if (n1) {
-          const double c1 = cConc[r1];
+          const RT c1 = cConc[r1];
           for (int n = 0; n < n1; ++n) fwd = fwd * c1;
         }
       }
       qk = fwd;
       if (k < Rrev) {
-        double dg = 0.0 - (double)n0 * cG[r0];
-        if (n1) dg = dg - (double)n1 * cG[r1];
-        dg = dg + (double)m0 * cG[p0];
-        if (m1) dg = dg + (double)m1 * cG[p1];
-        const double ln_kc = fma_rn(tv.dnu[k], ln_c0, -dg);
-        double rev = cexp(ln_kf - ln_kc);
-        const double d0 = cConc[p0];
+        RT dg = RT(0) - (RT)n0 * cG[r0];
+        if (n1) dg = dg - (RT)n1 * cG[r1];
+        dg = dg + (RT)m0 * cG[p0];
+        if (m1) dg = dg + (RT)m1 * cG[p1];
+        const RT ln_kc = M::fma(tv.dnu[k], ln_c0, -dg);
+        RT rev = M::exp(ln_kf - ln_kc);
+        const RT d0 = cConc[p0];
         for (int n = 0; n < m0; ++n) rev = rev * d0;
         if (m1) {
-          const double d1 = cConc[p1];
+          const RT d1 = cConc[p1];
           for (int n = 0; n < m1; ++n) rev = rev * d1;
         }
-        qk = (fwd - rev) * (use_rof ? cRof[k] : 1.0);
+        qk = (fwd - rev) * (use_rof ? cRof[k] : RT(1));
       }
     }
     cQ[k] = qk;
@@ -327,32 +368,32 @@ __device__ __forceinline__ RhsOut rhs_eval(const DevTables &tb, const TableView 
 
   // -- source terms and the step limiter (Eqs 1-3): omega_i gathered in the caller's reaction
   //    order, r_i = W_i omega_i / rho, t* = min_i min(Y_step^max, y_i*) / r_i*.
-  const double inv_rho = 1.0 / out.rho;
-  double t_star = bits_to_double(0x7ff0000000000000ull);
+  const RT inv_rho = RT(1) / out.rho;
+  RT t_star = M::inf();
   for (int i = gl; i < S; i += G) {
-    double om = 0.0;
+    RT om = RT(0);
     const int e1 = tv.gptr[i + 1];
     for (int e = tv.gptr[i]; e < e1; ++e) {
       const unsigned ent = tv.gent[e];
-      const double coef = tb.has_real ? tv.gcoef[e] : (double)(int)(signed char)(ent >> 16);
+      const RT coef = tb.has_real ? tv.gcoef[e] : (RT)(int)(signed char)(ent >> 16);
       om = om + coef * cQ[ent & 0xffffu];
     }
-    const double r = (tv.W[i] * om) * inv_rho;
-    const double y = cY[i];
-    const double r_star = (-r > 1.0e-30) ? -r : 1.0e-30;
-    const double y_star = (y < 1.0e-20) ? 1.0 : 0.9 * y;
-    const double lim = ((sc.y_step_max < y_star) ? sc.y_step_max : y_star) / r_star;
+    const RT r = (tv.W[i] * om) * inv_rho;
+    const RT y = cY[i];
+    const RT r_star = (-r > M::r_floor()) ? -r : M::r_floor();
+    const RT y_star = (y < M::y_small()) ? RT(1) : M::ninety() * y;
+    const RT lim = ((y_step_max < y_star) ? y_step_max : y_star) / r_star;
     if (lim < t_star) t_star = lim;
     cConc[i] = r;   // concentrations are dead: reuse for dY_i/dt
     cG[i] = om;     // g/RT is dead: reuse for omega_i
   }
-  out.t_star = group_min<G>(t_star);
+  out.t_star = group_min<G, RT>(t_star);
   group_sync<G>();
 
   // -- temperature equation (R15), enthalpy sum sequential in species order.
-  double sum_h = 0.0;
-  for (int i = 0; i < S; ++i) sum_h = fma_rn(cH[i], cG[i], sum_h);
-  out.dTdt = (sc.energy_mode == 0) ? -((sum_h * kRu) * T) / (out.rho * (kRu * sum_cp)) : 0.0;
+  RT sum_h = RT(0);
+  for (int i = 0; i < S; ++i) sum_h = M::fma(cH[i], cG[i], sum_h);
+  out.dTdt = (sc.energy_mode == 0) ? -((sum_h * M::ru()) * T) / (out.rho * (M::ru() * sum_cp)) : RT(0);
   return out;
 }
 
@@ -361,61 +402,66 @@ __device__ __forceinline__ RhsOut rhs_eval(const DevTables &tb, const TableView 
 // physical slot order.  Direct sums with the contract's twiddle literals; the largest high-bin magnitude is
 // sqrt(max |.|^2), which equals max sqrt(|.|^2) bit for bit because IEEE sqrt is monotone.
 // ---------------------------------------------------------------------------------------------------------
-template <int M>
-__device__ __forceinline__ double dft_bin_sq(const double (&x)[kWindow]) {
-  double re = 0.0, im = 0.0;
+template <int M, typename RT>
+__device__ __forceinline__ RT dft_bin_sq(const RT (&x)[kWindow]) {
+  RT re = RT(0), im = RT(0);
 #pragma unroll
   for (int k = 0; k < kWindow; ++k) {
-    re = fma_rn(x[k], cos13((M * k) % kWindow), re);
-    im = fma_rn(x[k], -sin13((M * k) % kWindow), im);
+    re = MathT<RT>::fma(x[k], (RT)cos13((M * k) % kWindow), re);
+    im = MathT<RT>::fma(x[k], -(RT)sin13((M * k) % kWindow), im);
   }
-  return fma_rn(re, re, im * im);
+  return MathT<RT>::fma(re, re, im * im);
 }
 
-__device__ __forceinline__ bool dft_is_ringing(const double (&x)[kWindow], const SolverConsts &sc) {
-  double d0 = 0.0;
+template <typename RT>
+__device__ __forceinline__ bool dft_is_ringing(const RT (&x)[kWindow], const SolverConsts &sc) {
+  RT d0 = RT(0);
 #pragma unroll
   for (int k = 0; k < kWindow; ++k) d0 = d0 + x[k];
-  d0 = fabs(d0);
-  double m2 = 0.0, v;
+  d0 = MathT<RT>::abs(d0);
+  RT m2 = RT(0), v;
   const int nhf = sc.nhf;
-  if (nhf <= 1) { v = dft_bin_sq<1>(x); m2 = (v > m2) ? v : m2; }
-  if (nhf <= 2) { v = dft_bin_sq<2>(x); m2 = (v > m2) ? v : m2; }
-  if (nhf <= 3) { v = dft_bin_sq<3>(x); m2 = (v > m2) ? v : m2; }
-  if (nhf <= 4) { v = dft_bin_sq<4>(x); m2 = (v > m2) ? v : m2; }
-  if (nhf <= 5) { v = dft_bin_sq<5>(x); m2 = (v > m2) ? v : m2; }
-  { v = dft_bin_sq<6>(x); m2 = (v > m2) ? v : m2; }
-  const double d_hi = sqrt(m2);
-  const double f_ring = d0 / ((d_hi > 1.0e-300) ? d_hi : 1.0e-300);
-  return (d_hi > 1.0e-300) && (f_ring < sc.tol_ring) && (d0 < sc.tol_freq);   // no high-frequency content: not ringing
+  if (nhf <= 1) { v = dft_bin_sq<1, RT>(x); m2 = (v > m2) ? v : m2; }
+  if (nhf <= 2) { v = dft_bin_sq<2, RT>(x); m2 = (v > m2) ? v : m2; }
+  if (nhf <= 3) { v = dft_bin_sq<3, RT>(x); m2 = (v > m2) ? v : m2; }
+  if (nhf <= 4) { v = dft_bin_sq<4, RT>(x); m2 = (v > m2) ? v : m2; }
+  if (nhf <= 5) { v = dft_bin_sq<5, RT>(x); m2 = (v > m2) ? v : m2; }
+  { v = dft_bin_sq<6, RT>(x); m2 = (v > m2) ? v : m2; }
+  const RT d_hi = MathT<RT>::sqrt(m2);
+  const RT guard = MathT<RT>::dft_guard();
+  const RT f_ring = d0 / ((d_hi > guard) ? d_hi : guard);
+  return (d_hi > guard) && (f_ring < (RT)sc.tol_ring) && (d0 < (RT)sc.tol_freq);   // no high-frequency content: not ringing
 }
 
 // ---------------------------------------------------------------------------------------------------------
 // The integrator.  One launch = one pass over the active-cell list.
 // ---------------------------------------------------------------------------------------------------------
-template <int G>
+template <int G, typename RT>
 __global__ void __launch_bounds__(512) stev_integrate_kernel(const __grid_constant__ IntegrateArgs a) {
+  using M = MathT<RT>;
   extern __shared__ __align__(128) unsigned char smem[];
   __shared__ unsigned long long mbar;
   stage_tables(smem, a.table, a.tb.bytes, &mbar);
   const DevTables &tb = a.tb;
   const CellLayout &cl = a.cl;
   const SolverConsts &sc = a.sc;
-  const TableView tv(smem, tb);
+  const TableView<RT> tv(smem, tb);
   const int S = tb.S, Rrev = tb.Rrev;
 
   const int lane = threadIdx.x & 31;
   const int gl = lane % G;                    // lane within the group
   const int grp = lane / G;                   // group within the warp
-  double *cell = (double *)(smem + tb.bytes) + (size_t)(threadIdx.x / G) * cl.stride;
-  double *cY = cell + cl.oY, *cConc = cell + cl.oConc, *cQ = cell + cl.oQ, *cRof = cell + cl.oRof, *cRing = cell + cl.oRing;
+  RT *cell = (RT *)(smem + tb.bytes) + (size_t)(threadIdx.x / G) * cl.stride;
+  RT *cY = cell + cl.oY, *cConc = cell + cl.oConc, *cQ = cell + cl.oQ, *cRof = cell + cl.oRof, *cRing = cell + cl.oRing;
   const int rp = cl.rrev_pad;
 
-  const double dt_max = a.t_f * sc.delta_max;   // Eq 4
-  const double t_tol = 1.0e-12 * a.t_f;         // R5
+  const RT t_f = (RT)a.t_f;
+  const RT dt_max = t_f * (RT)sc.delta_max;     // Eq 4
+  const RT t_tol = M::land_tol() * t_f;         // R5 (R26 in binary32)
+  const RT r_fac = (RT)sc.r_fac, inv_r_fac = M::inv_r_fac(sc), rof_floor = (RT)sc.rof_min;
 
   // per-cell scalars, identical in all lanes of the group
-  double T = 1000.0, p = kPatm, t = 0.0;
+  RT T = RT(1000), p = M::patm(), t = RT(0);
   int steps = 0, steps_in_pass = 0, slot = 0, cell_idx = -1;
   long long pos = -1;
   bool need = true, active = false, exhausted = false;
@@ -432,25 +478,25 @@ __global__ void __launch_bounds__(512) stev_integrate_kernel(const __grid_consta
         pos = (long long)base + __popc(req & ((1u << (grp * G)) - 1u));
         if (pos < a.n_active) {
           cell_idx = a.list ? a.list[pos] : (int)pos;
-          T = a.T[cell_idx];
-          p = a.p[cell_idx];
-          for (int i = gl; i < S; i += G) cY[i] = a.Y[(long long)i * a.ld + cell_idx];
+          T = (RT)a.T[cell_idx];
+          p = (RT)a.p[cell_idx];
+          for (int i = gl; i < S; i += G) cY[i] = (RT)a.Y[(long long)i * a.ld + cell_idx];
           steps_in_pass = 0;
           if (a.restore) {
             const double *rec = a.spill + (long long)cell_idx * a.spill_stride;
-            t = rec[0];
+            t = (RT)rec[0];
             steps = (int)rec[1];
             slot = (int)rec[2];
-            for (int k = gl; k < Rrev; k += G) cRof[k] = rec[3 + k];
+            for (int k = gl; k < Rrev; k += G) cRof[k] = (RT)rec[3 + k];
             for (int s = 0; s < kWindow; ++s)
-              for (int k = gl; k < Rrev; k += G) cRing[s * rp + k] = rec[3 + Rrev + s * Rrev + k];
+              for (int k = gl; k < Rrev; k += G) cRing[s * rp + k] = (RT)rec[3 + Rrev + s * Rrev + k];
           } else {
-            t = 0.0;
+            t = RT(0);
             steps = 0;
             slot = 0;
-            for (int k = gl; k < Rrev; k += G) cRof[k] = 1.0;                       // Eq 11
+            for (int k = gl; k < Rrev; k += G) cRof[k] = RT(1);                     // Eq 11
             for (int s = 0; s < kWindow; ++s)
-              for (int k = gl; k < Rrev; k += G) cRing[s * rp + k] = 0.0;           // R10
+              for (int k = gl; k < Rrev; k += G) cRing[s * rp + k] = RT(0);         // R10
           }
           active = true;
         } else {
@@ -464,12 +510,12 @@ __global__ void __launch_bounds__(512) stev_integrate_kernel(const __grid_consta
     if (!__any_sync(0xffffffffu, active)) break;
 
     // ---- a1, a2, a3: right-hand side and limiter
-    const RhsOut rhs = rhs_eval<G>(tb, tv, cl, sc, cell, gl, T, p, true);
+    const RhsOut<RT> rhs = rhs_eval<G, RT>(tb, tv, cl, sc, cell, gl, T, p, true);
 
     // ---- a3: step size (Eq 5) and landing on t_f (R5)
-    double h = (rhs.t_star < dt_max) ? rhs.t_star : dt_max;
+    RT h = (rhs.t_star < dt_max) ? rhs.t_star : dt_max;
     bool last = false;
-    const double rem = a.t_f - t;
+    const RT rem = t_f - t;
     if (rem - h < t_tol) {
       h = rem;
       last = true;
@@ -478,28 +524,28 @@ __global__ void __launch_bounds__(512) stev_integrate_kernel(const __grid_consta
     // ---- a4: forward Euler (Eq 18)
     int bad = 0;
     for (int i = gl; i < S; i += G) {
-      const double y = fma_rn(h, cConc[i], cY[i]);
+      const RT y = M::fma(h, cConc[i], cY[i]);
       cY[i] = y;
-      bad |= !(y - y == 0.0);
+      bad |= !(y - y == RT(0));
     }
-    T = fma_rn(h, rhs.dTdt, T);
-    t = last ? a.t_f : t + h;
+    T = M::fma(h, rhs.dTdt, T);
+    t = last ? t_f : t + h;
     steps += 1;
     steps_in_pass += 1;
-    bad |= !(T - T == 0.0);
+    bad |= !(T - T == RT(0));
 
     // ---- a5: DFT stabilisation (Eqs 8-14): store the applied change in progress (R8, R9), test, update rOF
     if (sc.dft_enable) {
-      const double inv_ctot = 1.0 / rhs.c_tot;
+      const RT inv_ctot = RT(1) / rhs.c_tot;
       for (int k = gl; k < Rrev; k += G) {
         cRing[slot * rp + k] = (cQ[k] * h) * inv_ctot;
-        double x[kWindow];
+        RT x[kWindow];
 #pragma unroll
         for (int s = 0; s < kWindow; ++s) x[s] = cRing[s * rp + k];
-        const bool ringing = dft_is_ringing(x, sc);
-        double rof = cRof[k] * (ringing ? sc.inv_r_fac : sc.r_fac);
-        if (rof > 1.0) rof = 1.0;
-        if (rof < sc.rof_min) rof = sc.rof_min;
+        const bool ringing = dft_is_ringing<RT>(x, sc);
+        RT rof = cRof[k] * (ringing ? inv_r_fac : r_fac);
+        if (rof > RT(1)) rof = RT(1);
+        if (rof < rof_floor) rof = rof_floor;
         cRof[k] = rof;
       }
       slot = (slot + 1 == kWindow) ? 0 : slot + 1;
@@ -513,9 +559,9 @@ __global__ void __launch_bounds__(512) stev_integrate_kernel(const __grid_consta
     else if (steps >= sc.max_steps) st = 1;
     const bool pause = (st < 0) && a.chunk_steps > 0 && steps_in_pass >= a.chunk_steps;
     if (active && (st >= 0 || pause)) {
-      for (int i = gl; i < S; i += G) a.Y[(long long)i * a.ld + cell_idx] = cY[i];
+      for (int i = gl; i < S; i += G) a.Y[(long long)i * a.ld + cell_idx] = (double)cY[i];
       if (gl == 0) {
-        a.T[cell_idx] = T;
+        a.T[cell_idx] = (double)T;
         a.steps[cell_idx] = steps;
         if (st >= 0 && a.status) a.status[cell_idx] = (unsigned char)st;
         if (st > 0) atomicMax(a.worst_status, st);
@@ -524,13 +570,13 @@ __global__ void __launch_bounds__(512) stev_integrate_kernel(const __grid_consta
       if (pause) {
         double *rec = a.spill + (long long)cell_idx * a.spill_stride;
         if (gl == 0) {
-          rec[0] = t;
+          rec[0] = (double)t;
           rec[1] = (double)steps;
           rec[2] = (double)slot;
         }
-        for (int k = gl; k < Rrev; k += G) rec[3 + k] = cRof[k];
+        for (int k = gl; k < Rrev; k += G) rec[3 + k] = (double)cRof[k];
         for (int s = 0; s < kWindow; ++s)
-          for (int k = gl; k < Rrev; k += G) rec[3 + Rrev + s * Rrev + k] = cRing[s * rp + k];
+          for (int k = gl; k < Rrev; k += G) rec[3 + Rrev + s * Rrev + k] = (double)cRing[s * rp + k];
       }
       need = true;
       active = false;
@@ -542,31 +588,31 @@ __global__ void __launch_bounds__(512) stev_integrate_kernel(const __grid_consta
 // ---------------------------------------------------------------------------------------------------------
 // Test export: one right-hand-side evaluation per cell with the same device code.
 // ---------------------------------------------------------------------------------------------------------
-template <int G>
+template <int G, typename RT>
 __global__ void __launch_bounds__(512) stev_rates_kernel(const __grid_constant__ RatesArgs a) {
   extern __shared__ __align__(128) unsigned char smem[];
   __shared__ unsigned long long mbar;
   stage_tables(smem, a.table, a.tb.bytes, &mbar);
   const DevTables &tb = a.tb;
   const CellLayout &cl = a.cl;
-  const TableView tv(smem, tb);
+  const TableView<RT> tv(smem, tb);
   const int S = tb.S, R = tb.R, Rrev = tb.Rrev;
   const int gl = (threadIdx.x & 31) % G;
-  double *cell = (double *)(smem + tb.bytes) + (size_t)(threadIdx.x / G) * cl.stride;
+  RT *cell = (RT *)(smem + tb.bytes) + (size_t)(threadIdx.x / G) * cl.stride;
   const long long cells_per_block = blockDim.x / G;
   for (long long base = (long long)blockIdx.x * cells_per_block; base < a.n; base += (long long)gridDim.x * cells_per_block) {
     const long long c = base + threadIdx.x / G;
     const bool valid = c < a.n;
     const long long cc = valid ? c : a.n - 1;
-    const double T = a.T[cc], p = a.p[cc];
-    for (int i = gl; i < S; i += G) cell[cl.oY + i] = a.Y[(long long)i * a.ld + cc];
-    for (int k = gl; k < Rrev; k += G) cell[cl.oRof + k] = a.rOF ? a.rOF[(long long)tv.orig[k] * a.ld + cc] : 1.0;
+    const RT T = (RT)a.T[cc], p = (RT)a.p[cc];
+    for (int i = gl; i < S; i += G) cell[cl.oY + i] = (RT)a.Y[(long long)i * a.ld + cc];
+    for (int k = gl; k < Rrev; k += G) cell[cl.oRof + k] = a.rOF ? (RT)a.rOF[(long long)tv.orig[k] * a.ld + cc] : RT(1);
     group_sync<G>();
-    const RhsOut rhs = rhs_eval<G>(tb, tv, cl, a.sc, cell, gl, T, p, true);
+    const RhsOut<RT> rhs = rhs_eval<G, RT>(tb, tv, cl, a.sc, cell, gl, T, p, true);
     if (valid) {
-      for (int i = gl; i < S; i += G) a.dYdt[(long long)i * a.ld + c] = cell[cl.oConc + i];
-      for (int k = gl; k < R; k += G) a.q[(long long)tv.orig[k] * a.ld + c] = cell[cl.oQ + k];
-      if (gl == 0) a.dTdt[c] = rhs.dTdt;
+      for (int i = gl; i < S; i += G) a.dYdt[(long long)i * a.ld + c] = (double)cell[cl.oConc + i];
+      for (int k = gl; k < R; k += G) a.q[(long long)tv.orig[k] * a.ld + c] = (double)cell[cl.oQ + k];
+      if (gl == 0) a.dTdt[c] = (double)rhs.dTdt;
     }
     group_sync<G>();
   }

@@ -43,7 +43,8 @@ struct HostMechanism {
 };
 
 // Builds the table image for a mechanism and, optionally, an estimator.
-void build_table_image(const HostMechanism &m, const HostEstimator *e, std::vector<unsigned char> &image, DevTables &tb);
+void build_table_image(const HostMechanism &m, const HostEstimator *e, std::vector<unsigned char> &image, DevTables &tb,
+                       bool f32 = false);
 
 struct LaunchConfig {
   int G = 1, threads = 128, cells_per_block = 128, blocks_per_sm = 1;
@@ -51,7 +52,7 @@ struct LaunchConfig {
   CellLayout cl{};
 };
 // Chooses lanes per cell, block shape and the per-cell shared-memory layout.  Returns false if nothing fits.
-bool choose_config(const DevTables &tb, int lanes_per_cell_request, LaunchConfig &cfg);
+bool choose_config(const DevTables &tb, int lanes_per_cell_request, LaunchConfig &cfg, int bytes_per_real = 8);
 
 int device_sm_count();
 
@@ -92,6 +93,8 @@ struct stev_mechanism {
   stev::HostMechanism host;
   stev::DevTables tb{};
   unsigned char *d_table = nullptr;
+  stev::DevTables tb32{};                // the same image with every real table rounded to float (state_precision FP32)
+  unsigned char *d_table32 = nullptr;
   bool pk_ok[2] = {false, false};         // images of the tensor-memory kernel: [0] one warp per cell, [1] pair (NASA-7 thermo)
   stev::PkTables pk_tb[2]{};
   stev::PkCell pk_cl[2]{};
@@ -106,6 +109,8 @@ struct stev_estimator {
   const stev_mechanism *mech = nullptr;  // the mechanism it was loaded against (may be null)
   stev::DevTables tb{};                  // mechanism + estimator image (only if mech != null)
   unsigned char *d_table = nullptr;
+  stev::DevTables tb32{};
+  unsigned char *d_table32 = nullptr;
   bool pk_ok[2] = {false, false};         // images of the tensor-memory kernel (MLP thermo)
   stev::PkTables pk_tb[2]{};
   stev::PkCell pk_cl[2]{};

@@ -111,6 +111,72 @@ __host__ __device__ __forceinline__ double clog(double x) {
   return res;
 }
 
+// The binary32 contract (stev_params.state_precision = STEV_STATE_FP32).
+// exp: k = rint(x log2 e) through the 1.5 * 2^23 shift, Cody-Waite reduction with ln2_hi = 0x1.62e4p-1 (11 trailing zero
+// bits), Taylor polynomial of degree 7 (Horner, fmaf), 2^k through the exponent field; > 88 -> +inf, < -87 -> 0.
+__host__ __device__ __forceinline__ float fmaf_rn(float a, float b, float c) {
+#ifdef __CUDA_ARCH__
+  return __fmaf_rn(a, b, c);
+#else
+  return __builtin_fmaf(a, b, c);
+#endif
+}
+__host__ __device__ __forceinline__ unsigned float_to_bits(float f) {
+  unsigned u;
+  __builtin_memcpy(&u, &f, 4);
+  return u;
+}
+__host__ __device__ __forceinline__ float bits_to_float(unsigned u) {
+  float f;
+  __builtin_memcpy(&f, &u, 4);
+  return f;
+}
+__host__ __device__ __forceinline__ float cexpf32(float x) {
+  const float kShift = 12582912.0f;
+  float t = fmaf_rn(x, 0x1.715476p+0f, kShift);
+  float k = t - kShift;
+  int ki = (int)(float_to_bits(t) & 0x7fffffu) - 0x400000;
+  float r = fmaf_rn(-k, 0x1.62e4p-1f, x);
+  r = fmaf_rn(-k, 0x1.7f7d1cp-20f, r);
+  float p = 0x1.a01a02p-13f;
+  p = fmaf_rn(p, r, 0x1.6c16c2p-10f);
+  p = fmaf_rn(p, r, 0x1.111112p-7f);
+  p = fmaf_rn(p, r, 0x1.555556p-5f);
+  p = fmaf_rn(p, r, 0x1.555556p-3f);
+  p = fmaf_rn(p, r, 0.5f);
+  p = fmaf_rn(p, r, 1.0f);
+  p = fmaf_rn(p, r, 1.0f);
+  float res = p * bits_to_float((unsigned)(ki + 127) << 23);
+  if (x > 88.0f) res = bits_to_float(0x7f800000u);
+  if (x < -87.0f) res = 0.0f;
+  if (x != x) res = x;
+  return res;
+}
+// log for positive normal x: x = m 2^e, m in (sqrt(1/2), sqrt 2], f = (m-1)/(m+1), log m = 2f (1 + s/3 + s^2/5 + s^3/7 + s^4/9)
+__host__ __device__ __forceinline__ float clogf32(float x) {
+  unsigned u = float_to_bits(x);
+  int e = (int)(u >> 23) - 127;
+  float m = bits_to_float((u & 0x007fffffu) | 0x3f800000u);
+  if (m > 0x1.6a09e6p+0f) {
+    m = m * 0.5f;
+    e = e + 1;
+  }
+  float f = (m - 1.0f) / (m + 1.0f);
+  float s = f * f;
+  float P = 0x1.c71c72p-4f;
+  P = fmaf_rn(P, s, 0x1.24924ap-3f);
+  P = fmaf_rn(P, s, 0x1.99999ap-3f);
+  P = fmaf_rn(P, s, 0x1.555556p-2f);
+  float two_f = f + f;
+  float log_m = fmaf_rn(two_f, s * P, two_f);
+  float ed = (float)e;
+  float res = fmaf_rn(ed, 0x1.62e4p-1f, fmaf_rn(ed, 0x1.7f7d1cp-20f, log_m));
+  if (x == 0.0f) res = -bits_to_float(0x7f800000u);
+  if (x < 0.0f || x != x) res = bits_to_float(0x7fc00000u);
+  if (x == bits_to_float(0x7f800000u)) res = x;
+  return res;
+}
+
 // cos, sin of 2 pi n / 13, n = 0..12: the literal table of DESIGN.md 5.6.
 __device__ __constant__ const double kCos13[13] = {
     1.0, 0.8854560256532099, 0.5680647467311559, 0.120536680255323, -0.35460488704253545,
