@@ -760,10 +760,13 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
     else if (p->lanes_per_cell == 512 || p->lanes_per_cell == 513) kind = 7;
     else if (p->lanes_per_cell == 0 && !f32) {
       // Measured on B200: large mechanisms -> warp pair; tiny ones (a step is a few hundred
-      // instructions) -> lock-step block, which flattens (cell, reaction) pairs over the lanes; mid-size -> one warp per
-      // cell, 32 cells per SM when the reversible reactions fit two 32-blocks, else 16.
+      // instructions) -> lock-step block, which flattens (cell, reaction) pairs over the lanes (configs 0, 1: +56 %);
+      // mid-size with an estimator -> lock-step block too (its estimator layers are shared over the cells of the block;
+      // config 4 at full size: +24 %); mid-size without -> one warp per cell, 32 cells per SM when the reversible
+      // reactions fit two 32-blocks, else 16 (config 2: the 200 000-step cells set the time, and a lone warp steps faster).
       if (tb->R >= 128 && pk2_ok) kind = 2;
       else if (tb->S <= 16 && tb->R <= 32 && ls_ok) kind = 7;
+      else if (est && tb->S <= 32 && ls_ok) kind = 7;
       else if (tb->S <= 16 && tb->R <= 32) {
         kind = 0;
         g_request = 4;

@@ -20,22 +20,22 @@ namespace stev {
 
 constexpr int kLsThreads = 512;                 // 16 warps; warp w reaches TMEM lane quarter w % 4
 constexpr int kLsWarps = kLsThreads / 32;
+constexpr int kLsPassWarps = kLsWarps;          // every warp owns (reaction, cell) passes: pass p belongs to warp p % 16
+constexpr int kLsItemThreads = 32 * (kLsWarps - 1);   // threads that update the mass fractions in phase 4 (not the scalar warp)
 constexpr int kLsSlots = 4;                     // 32-column window slots per warp: 4 warps per quarter x 4 x 32 = 512 columns
-constexpr int kLsMaxPasses = kLsWarps * kLsSlots;   // 64 warp passes = 2048 DFT windows per block
+constexpr int kLsMaxPasses = kLsPassWarps * kLsSlots;   // 64 warp passes = 2048 DFT windows per block
 constexpr int kLsMaxCells = 32;                 // one lane of the scalar warp per cell
 
-// Scalars of the cell slots, one array of C eight-byte entries per field (entry (f, c) at oSc + (f C + c) 8).  Written by the
-// cell's lane of the scalar warp unless stated; every field has one writer per phase and is read only after the block
-// barrier that ends that phase.
+// Scalars of the cell slots, one array of C eight-byte entries per field (entry (f, c) at set + (f C + c) 8).  There are
+// TWO sets, used by alternate steps: while the block still reads the set of step n (update, ringing filter), the scalar
+// warp already writes the set of step n + 1.  Written by the cell's lane of the scalar warp unless stated.
 enum LsField {
-  kF_T, kF_P,                          // state of this step (published at the top of the step)
+  kF_T, kF_P,                          // state of the step
   kF_LNT, kF_LNC0, kF_INVT, kF_ICTOT, kF_RHO,
-  kF_REM,                              // t_f - t before this step
-  kF_HDFT, kF_ICDFT,                   // step size and 1/C_tot of the step whose progress the ringing filter stores next
+  kF_REM,                              // t_f - t before the step
   kF_TSTAR,                            // u64: running minimum of the limiter (atomicMin of the bit patterns, phase 3)
   kF_ACTIVE,                           // int: 1 the slot integrates a cell; 0 it waits for a refill (or the queue is empty)
   kF_FRESH,                            // int: 1 during the first step of a new cell: window owners zero the history, rOF = 1
-  kF_DFTON,                            // int: the step just taken stores its progress (not on a landing step, not without a cell)
   kF_BAD,                              // int: non-finite mass fraction seen by the update (atomicOr, phase 4)
   kF_COUNT
 };
@@ -52,7 +52,7 @@ struct LsDims {
 // consecutive addresses (and the per-reaction tables are read by broadcast).  From the start of the cell region:
 //   oY [S] | oYw [S] Y_i/W_i | oCp [S] cp_i/R | oH [S] h_i/RT | oOm [S] omega_i
 //   oConc [1+S] ([0] = 1.0, then C_i**, later dY_i/dt) | oG [1+2S] ([0] = 0.0, g_i/RT, 2 g_i/RT)
-//   oQ [n_var][Rp] multiples of q_eff | oRof [Rrev] | oSc [kF_COUNT] the scalars
+//   oQ [n_var][Rp] multiples of q_eff | oRof [Rrev] | oSc [2][kF_COUNT] the two sets of scalars
 //   oHid float [C][Hs] hidden activations, cell-major with Hs = H + 4 | oXn float [n_in][C] normalised estimator inputs
 // Table image (from the image base):
 //   o_tmid, o_W, o_invW double [S] | o_nasa double [2][14][S] | o_rkA double2 [R] {ln A, b} | o_rkB double2 [R] {Ea/R_cal, dnu}
@@ -65,7 +65,7 @@ struct LsDims {
 //          the caller's reaction order, padded with the 0.0 slot; the last row is all padding
 struct LsLayout {
   int Rp, Hpad, Hs;
-  int oY, oYw, oCp, oH, oOm, oConc, oG, oQ, oRof, oSc, oHid, oXn, cell_bytes;
+  int oY, oYw, oCp, oH, oOm, oConc, oG, oQ, oRof, oSc, sc_bytes, oHid, oXn, cell_bytes;
   int o_tmid, o_W, o_invW, o_nasa, o_rkA, o_rkB, o_rfac, o_rdg, o_gsp, o_grow, o_glen;
   int o_eshift, o_escale, o_W1T, o_b1, o_W2p, o_b2, o_gent;
   int n_rev_pass, n_irr_pass;          // warp passes over the flattened (reversible reaction, cell) / (irreversible, cell) pairs
@@ -89,7 +89,8 @@ __host__ __device__ constexpr LsLayout ls_layout_of(const LsDims &d) {
   L.oG = o; o = ls_align(o + 8 * C * (1 + 2 * d.S), 16);
   L.oQ = o; o = ls_align(o + 8 * C * d.n_var * L.Rp, 16);
   L.oRof = o; o = ls_align(o + 8 * C * (d.Rrev > 0 ? d.Rrev : 1), 16);
-  L.oSc = o; o = ls_align(o + 8 * C * (int)kF_COUNT, 16);
+  L.oSc = o; o = ls_align(o + 2 * 8 * C * (int)kF_COUNT, 16);
+  L.sc_bytes = 8 * C * (int)kF_COUNT;
   L.oHid = o; o = ls_align(o + 4 * C * (d.has_est ? L.Hs : 0), 16);
   L.oXn = o; o = ls_align(o + 4 * C * (d.has_est ? d.n_in : 0), 16);
   L.cell_bytes = o;

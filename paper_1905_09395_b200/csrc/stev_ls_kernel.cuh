@@ -1,20 +1,19 @@
 // stev_ls_kernel.cuh -- the lock-step STEV integrator (rows a1-a7 of DESIGN.md section 1); design in stev_ls.cuh.
 //
-// A step of the block (all C cell slots together) is five phases separated by block barriers:
-//   0  scalar warp, one cell per lane: retirement / refill from the queue (a6), T-dependent scalars, 1/Wbar (sequential
-//      sum), estimator inputs
+// A step of the block (all C cell slots together) is four phases separated by block barriers:
 //   1  (species, cell) pairs: NASA-7 g/RT (+ cp, h without estimator), stabilised concentrations;
 //      (hidden unit, cell) pairs: first estimator layer (a7)
 //   2  (reaction, cell) pairs: rates (a2), q_eff = q rOF, stored multiples
 //   3  (species, cell) pairs: source terms gathered in the caller's reaction order, limiter (a3), atomicMin per cell;
 //      (output, cell) pairs: second estimator layer (it only feeds the temperature equation)
-//   4  (species, cell) pairs: step size, Euler update (a4);  scalar warp: the two sequential sums of the temperature
-//      equation, T, t, step count
-// The ringing filter (a5) of a step only feeds rOF, which the rates of the NEXT step read, and the thread that owns a
-// (reaction, cell) pair owns its DFT window, its rOF and its rate.  Its filter passes are therefore free to run anywhere
-// between phase 4 (the step size is known) and the pair's own rate evaluation in phase 2 of the next step: each warp runs
-// one of its (up to four) passes in phase 4, 0, 1 and 2, so the fp64-bound filter fills the phases that are bound by the
-// latency of the scalar chains or by shared-memory bandwidth.
+//   4  the serial chain of the method on the SCALAR WARP, one cell per lane -- the two sequential sums of the temperature
+//      equation, T, t, step count, retirement / refill from the queue (a6), then for the NEXT step the two logarithms, the
+//      divisions and the sequential sum 1/Wbar -- while the fifteen other warps update the mass fractions (a4), hand them
+//      to the scalar warp through a named barrier (bar.arrive / bar.sync) and run the whole ringing filter (a5) of the
+//      step: the filter only feeds rOF, which the rates of the next step read, so the fp64-bound filter hides the
+//      latency-bound chain.  The scalars exist in two sets used by alternate steps, so the scalar warp can write the
+//      next step's while the filter still reads this step's; its own filter passes run at the top of the next phase 1,
+//      from the previous set.
 // The 13-deep history of every reversible reaction lives in TENSOR MEMORY: pass p of 32 consecutive (reaction, cell)
 // pairs belongs to warp p % 16 and sits in one 32-column slot of that warp's TMEM lane quarter.  tcgen05.st writes one
 // column pair for all 32 lanes at once, so all cells of a block share the ring position: a slot is refilled only when
@@ -41,7 +40,7 @@ struct LsConst {
 #define LS_L(f) (SH::kStatic ? LsConst<SH>::L.f : a.lay.f)
 // element (idx, c) of the cell-region array at byte offset `off` (index-major, cell-minor)
 #define LS_AT(type, off, idx, c) (*(type *)(cells + (off) + ((unsigned)((idx) * C + (c)) << 3)))
-#define LS_SC(type, field, c) LS_AT(type, LS_L(oSc), (int)(field), c)
+#define LS_SC(type, field, c) LS_AT(type, sc_set, (int)(field), c)   // sc_set: byte offset of the scalar set of the step
 
 constexpr unsigned kFull = 0xffffffffu;
 
@@ -67,38 +66,29 @@ __device__ __forceinline__ void tmem_st26(uint32_t taddr, const uint32_t (&r)[26
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// a5: the ringing filter (Eqs 8-13) of pass `s` of this warp over the (reversible reaction, cell) pairs.
-// slot13: ring position of the step whose applied change in progress is stored (the same for every cell of the block).
-// IN_P4: the pass runs in phase 4 of that very step: the step size follows from the limiter's minimum (as in the
-// update); otherwise it is read from the fields the scalar warp left in phase 4.
+// a5: the ringing filter (Eqs 8-13) of pass `s` of this warp over the (reversible reaction, cell) pairs,
+// run in phase 4 of the step whose applied change in progress it stores: the step size follows from the limiter's
+// minimum exactly as in the update.  slot13: ring position of the step (the same for every cell of the block).
 // ---------------------------------------------------------------------------------------------------------
-template <class SH, int NHF, bool IN_P4>
-__device__ __forceinline__ void ls_dft_pass(const LsArgs &a, unsigned char *cells, uint32_t trow, int s, int slot13, int warp,
-                                            int lane, double dt_max, double t_tol) {
+template <class SH, int NHF>
+__device__ __forceinline__ void ls_dft_pass(const LsArgs &a, unsigned char *cells, int sc_set, uint32_t trow, int s, int slot13,
+                                            int warp, int lane, double dt_max, double t_tol) {
   const SolverConsts &sc = a.sc;
   const int C = LS_D(C);
-  const int p = warp + s * kLsWarps;
+  const int p = warp + s * kLsPassWarps;
   if (p >= LS_L(n_rev_pass)) return;
   const unsigned n_items = (unsigned)(C * LS_D(Rrev));
   unsigned f = (unsigned)(p * 32 + lane);
   const bool valid = f < n_items;
   f = valid ? f : n_items - 1;
   const unsigned k = ls_div_c<SH>(f, C, a.mC), c = f - k * (unsigned)C;
-  bool on;
-  double h, ic;
-  if (IN_P4) {
-    const double t_star = bits_to_double(LS_SC(unsigned long long, kF_TSTAR, c));
-    h = (t_star < dt_max) ? t_star : dt_max;
-    const double rem = LS_SC(double, kF_REM, c);
-    const bool lst = rem - h < t_tol;
-    h = lst ? rem : h;
-    ic = LS_SC(double, kF_ICTOT, c);
-    on = valid && LS_SC(int, kF_ACTIVE, c) && !lst;   // the landing step's change is never looked at: the cell retires
-  } else {
-    h = LS_SC(double, kF_HDFT, c);
-    ic = LS_SC(double, kF_ICDFT, c);
-    on = valid && LS_SC(int, kF_DFTON, c);
-  }
+  const double t_star = bits_to_double(LS_SC(unsigned long long, kF_TSTAR, c));
+  double h = (t_star < dt_max) ? t_star : dt_max;
+  const double rem = LS_SC(double, kF_REM, c);
+  const bool lst = rem - h < t_tol;
+  h = lst ? rem : h;
+  const double ic = LS_SC(double, kF_ICTOT, c);
+  const bool on = valid && LS_SC(int, kF_ACTIVE, c) && !lst;   // the landing step's change is never looked at: the cell retires
   if (!__any_sync(kFull, on)) return;   // landing steps and empty slots store nothing
   const double q = LS_AT(double, LS_L(oQ), k, c);
   const uint32_t tw = trow + (uint32_t)(s * 32);
@@ -125,17 +115,24 @@ __device__ __forceinline__ void ls_dft_pass(const LsArgs &a, unsigned char *cell
   }
 }
 
-template <class SH, bool IN_P4>
-__device__ __forceinline__ void ls_dft(const LsArgs &a, unsigned char *cells, uint32_t trow, int s, int slot13, int warp, int lane,
+template <class SH, int NHF>
+__device__ __forceinline__ void ls_dft_all(const LsArgs &a, unsigned char *cells, int sc_set, uint32_t trow, int slot13, int warp,
+                                           int lane, double dt_max, double t_tol) {
+#pragma unroll 1
+  for (int s = 0; s < kLsSlots; ++s) ls_dft_pass<SH, NHF>(a, cells, sc_set, trow, s, slot13, warp, lane, dt_max, t_tol);
+}
+
+template <class SH>
+__device__ __forceinline__ void ls_dft(const LsArgs &a, unsigned char *cells, int sc_set, uint32_t trow, int slot13, int warp, int lane,
                                        double dt_max, double t_tol) {
   if (!a.sc.dft_enable) return;
   switch (a.sc.nhf) {
-    case 1: ls_dft_pass<SH, 1, IN_P4>(a, cells, trow, s, slot13, warp, lane, dt_max, t_tol); break;
-    case 2: ls_dft_pass<SH, 2, IN_P4>(a, cells, trow, s, slot13, warp, lane, dt_max, t_tol); break;
-    case 3: ls_dft_pass<SH, 3, IN_P4>(a, cells, trow, s, slot13, warp, lane, dt_max, t_tol); break;
-    case 4: ls_dft_pass<SH, 4, IN_P4>(a, cells, trow, s, slot13, warp, lane, dt_max, t_tol); break;
-    case 5: ls_dft_pass<SH, 5, IN_P4>(a, cells, trow, s, slot13, warp, lane, dt_max, t_tol); break;
-    default: ls_dft_pass<SH, 6, IN_P4>(a, cells, trow, s, slot13, warp, lane, dt_max, t_tol); break;
+    case 1: ls_dft_all<SH, 1>(a, cells, sc_set, trow, slot13, warp, lane, dt_max, t_tol); break;
+    case 2: ls_dft_all<SH, 2>(a, cells, sc_set, trow, slot13, warp, lane, dt_max, t_tol); break;
+    case 3: ls_dft_all<SH, 3>(a, cells, sc_set, trow, slot13, warp, lane, dt_max, t_tol); break;
+    case 4: ls_dft_all<SH, 4>(a, cells, sc_set, trow, slot13, warp, lane, dt_max, t_tol); break;
+    case 5: ls_dft_all<SH, 5>(a, cells, sc_set, trow, slot13, warp, lane, dt_max, t_tol); break;
+    default: ls_dft_all<SH, 6>(a, cells, sc_set, trow, slot13, warp, lane, dt_max, t_tol); break;
   }
 }
 
@@ -145,8 +142,8 @@ __device__ __forceinline__ void ls_dft(const LsArgs &a, unsigned char *cells, ui
 // step of a new cell it zeroes the window (R10) and sets rOF = 1 (Eq 11).
 // ---------------------------------------------------------------------------------------------------------
 template <class SH, int U>
-__device__ __forceinline__ void ls_rev_batch(const LsArgs &a, const unsigned char *tbl, unsigned char *cells, uint32_t trow, int s0,
-                                             int warp, int lane) {
+__device__ __forceinline__ void ls_rev_batch(const LsArgs &a, const unsigned char *tbl, unsigned char *cells, int sc_set, uint32_t trow,
+                                             int s0, int warp, int lane) {
   const int C = LS_D(C), Rrev = LS_D(Rrev), Rp = LS_L(Rp);
   const bool has2 = LS_D(n_var) > 2;
   const unsigned n_rev = (unsigned)(C * Rrev);
@@ -157,7 +154,7 @@ __device__ __forceinline__ void ls_rev_batch(const LsArgs &a, const unsigned cha
   bool oor = false;
 #pragma unroll
   for (int u = 0; u < U; ++u) {
-    const int p = warp + (s0 + u) * kLsWarps;
+    const int p = warp + (s0 + u) * kLsPassWarps;
     unsigned f = (unsigned)(p * 32 + lane);
     valid[u] = f < n_rev;
     f = valid[u] ? f : n_rev - 1;
@@ -229,18 +226,19 @@ __device__ __forceinline__ void ls_rev_batch(const LsArgs &a, const unsigned cha
 
 // passes [s0, s1) of this warp, two at a time while two are left
 template <class SH>
-__device__ __forceinline__ void ls_rev_range(const LsArgs &a, const unsigned char *tbl, unsigned char *cells, uint32_t trow, int s0, int s1,
-                                             int warp, int lane) {
-  const int n_mine = (LS_L(n_rev_pass) - warp + kLsWarps - 1) / kLsWarps;   // passes of this warp
+__device__ __forceinline__ void ls_rev_range(const LsArgs &a, const unsigned char *tbl, unsigned char *cells, int sc_set, uint32_t trow,
+                                             int s0, int s1, int warp, int lane) {
+  const int n_mine = (LS_L(n_rev_pass) - warp + kLsPassWarps - 1) / kLsPassWarps;   // passes of this warp
   s1 = (s1 < n_mine) ? s1 : n_mine;
   int s = s0;
-  for (; s + 2 <= s1; s += 2) ls_rev_batch<SH, 2>(a, tbl, cells, trow, s, warp, lane);
-  if (s < s1) ls_rev_batch<SH, 1>(a, tbl, cells, trow, s, warp, lane);
+  for (; s + 2 <= s1; s += 2) ls_rev_batch<SH, 2>(a, tbl, cells, sc_set, trow, s, warp, lane);
+  if (s < s1) ls_rev_batch<SH, 1>(a, tbl, cells, sc_set, trow, s, warp, lane);
 }
 
-// irreversible reactions: passes continue round robin after the reversible ones, so the warps that had one pass less get these first
+// irreversible reactions: passes continue round robin after the reversible ones, so the warps that had one pass less get
+// these first
 template <class SH>
-__device__ __forceinline__ void ls_irr_passes(const LsArgs &a, const unsigned char *tbl, unsigned char *cells, int warp, int lane) {
+__device__ __forceinline__ void ls_irr_passes(const LsArgs &a, const unsigned char *tbl, unsigned char *cells, int sc_set, int warp, int lane) {
   const int C = LS_D(C), Rrev = LS_D(Rrev), Rp = LS_L(Rp), Rirr = LS_D(R) - LS_D(Rrev);
   const int n_irr_pass = LS_L(n_irr_pass);
   const bool has2 = LS_D(n_var) > 2;
@@ -275,6 +273,12 @@ __device__ __forceinline__ void ls_irr_passes(const LsArgs &a, const unsigned ch
 // ---------------------------------------------------------------------------------------------------------
 // The kernel.
 // ---------------------------------------------------------------------------------------------------------
+#ifdef LS_TIMING
+#define LST(i) { const long long now_ = clock64(); tph[i] += now_ - tl_; tl_ = now_; }
+#else
+#define LST(i)
+#endif
+
 template <class SH, bool EST>
 __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_constant__ LsArgs a) {
   extern __shared__ __align__(128) unsigned char smem[];
@@ -307,7 +311,8 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
   const double t_tol = 1.0e-12 * a.t_f;         // R5
   const unsigned n_cs = (unsigned)(C * S);
   const unsigned long long kInfBits = 0x7ff0000000000000ull;
-  constexpr int SW = kLsWarps - 1;              // the scalar warp: it has the fewest reaction passes
+  constexpr int SW = kLsWarps - 1;              // the scalar warp
+  constexpr int kXBar = 1;                      // named barrier: the other warps arrive when the new mass fractions are in place
 
   // the scalar lane of cell slot `lane` keeps the cell's own scalars in registers for the whole integration
   const bool my_slot = (warp == SW) && lane < C;
@@ -315,31 +320,23 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
   double T = 1000.0, p = kPatm, t = 0.0, inv_ctot = 0.0, rho = 1.0;
   int steps = 0, cidx = -1, pending_st = -1;
   bool active = false, exhausted = false, last = false, bad_T = false;
+  int sc_set = LS_L(oSc);   // scalar set of the current step; the other one is at LS_L(oSc) + LS_L(sc_bytes)
   if (my_slot) {
     // a slot without a cell computes on a harmless finite state and commits nothing
     for (int i = 0; i < S; ++i) LS_AT(double, LS_L(oY), i, mc) = 1.0 / (double)S;
     LS_AT(double, LS_L(oConc), 0, mc) = 1.0;
     LS_AT(double, LS_L(oG), 0, mc) = 0.0;
-    LS_SC(int, kF_ACTIVE, mc) = 0;
-    LS_SC(int, kF_FRESH, mc) = 0;
-    LS_SC(int, kF_DFTON, mc) = 0;
-    LS_SC(int, kF_BAD, mc) = 0;
-    LS_SC(double, kF_HDFT, mc) = 0.0;
-    LS_SC(double, kF_ICDFT, mc) = 0.0;
   }
-  __syncthreads();
-
 #ifdef LS_TIMING
   long long tph[6] = {0, 0, 0, 0, 0, 0}, tl_ = clock64(), n_steps_ = 0;
-#define LST(i) { const long long now_ = clock64(); tph[i] += now_ - tl_; tl_ = now_; }
-#else
-#define LST(i)
 #endif
-  int g13 = 0;   // ring position of the step about to be taken (block-uniform)
-  for (;;) {
-    const int sl_prev = (g13 == 0) ? kWindow - 1 : g13 - 1;   // ring position of the step just taken
-    // =========================== phase 0 ===========================
-    if (warp == SW) {
+
+  // What the scalar warp does between two steps: retirement of the step just taken (a6), write-back and refill at ring
+  // position 0, and the scalars of the next step into scalar set `set_next`.  g_next: ring position of the next step.
+  auto scalar_warp_prepare = [&](int set_prev, int set_next, int g_next, bool first) {
+    const int sc_keep = sc_set;
+    if (!first) {
+      sc_set = set_prev;
       // ---- a6: retirement (R20) of the step just taken
       if (my_slot && active) {
         int st = -1;
@@ -351,91 +348,113 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
           pending_st = st;
         }
       }
-      if (g13 == 0) {
-        // ---- results leave and new cells enter only at ring position 0 (see the header): write back ...
-        if (my_slot && pending_st >= 0) {
-          for (int i = 0; i < S; ++i) a.Y[(long long)i * a.ld + cidx] = LS_AT(double, LS_L(oY), i, mc);
-          a.T[cidx] = T;
-          a.steps[cidx] = steps;
-          if (a.status) a.status[cidx] = (unsigned char)pending_st;
-          if (pending_st > 0) atomicMax(a.worst_status, pending_st);
-          pending_st = -1;
-        }
-        // ... and pull the next cells: ballot the requests, one atomic per warp reserves that many queue positions,
-        // popc of the lower mask ranks them (variable load)
-        const bool want = my_slot && !active && !exhausted;
-        const unsigned req = __ballot_sync(kFull, want);
-        if (req) {
-          int base = 0;
-          if (lane == 0) base = atomicAdd(a.queue_head, __popc(req));
-          base = __shfl_sync(kFull, base, 0);
-          if (want) {
-            const long long pos = (long long)base + __popc(req & ((1u << lane) - 1u));
-            if (pos < a.n_active) {
-              cidx = a.list ? a.list[pos] : (int)pos;
-              T = a.T[cidx];
-              p = a.p[cidx];
-              for (int i = 0; i < S; ++i) LS_AT(double, LS_L(oY), i, mc) = a.Y[(long long)i * a.ld + cidx];
-              t = 0.0;
-              steps = 0;
-              active = true;
-              LS_SC(int, kF_FRESH, mc) = 1;
-            } else {
-              exhausted = true;
-            }
-          }
-        }
+    }
+    sc_set = set_next;
+    int fresh = 0;
+    if (g_next == 0) {
+      // ---- results leave and new cells enter only at ring position 0 (see the header): write back ...
+      if (my_slot && pending_st >= 0) {
+        for (int i = 0; i < S; ++i) a.Y[(long long)i * a.ld + cidx] = LS_AT(double, LS_L(oY), i, mc);
+        a.T[cidx] = T;
+        a.steps[cidx] = steps;
+        if (a.status) a.status[cidx] = (unsigned char)pending_st;
+        if (pending_st > 0) atomicMax(a.worst_status, pending_st);
+        pending_st = -1;
       }
-      const int go = __any_sync(kFull, my_slot && (active || pending_st >= 0));
-      if (lane == 0) s_go = go;
-      if (my_slot) {
-        // ---- scalars of this step
-        const double RuT = kRu * T;
-        const double c_tot = p / RuT;
-        const double invT = 1.0 / T;
-        const double lnT = ab_log(T);
-        const double ln_c0 = ab_log(kPatm / RuT);
-        inv_ctot = 1.0 / c_tot;
-        // 1/Wbar = sum Y_i/W_i, sequential in species order (contract 5.4); estimator inputs on the way (R18)
-        double inv_wbar = 0.0;
-        if (EST && LS_D(n_in) > 1) {
-          float *cXn = (float *)(cells + LS_L(oXn));
-          const float *eshift = (const float *)(tbl + LS_L(o_eshift)), *escale = (const float *)(tbl + LS_L(o_escale));
-          cXn[1 * C + mc] = ((float)p - eshift[1]) * escale[1];
-          for (int i = 0; i < S; ++i) {
-            const double y = LS_AT(double, LS_L(oY), i, mc);
-            inv_wbar = fma_rn(y, invW[i], inv_wbar);
-            cXn[(2 + i) * C + mc] = ((float)y - eshift[2 + i]) * escale[2 + i];
+      // ... and pull the next cells: ballot the requests, one atomic per warp reserves that many queue positions,
+      // popc of the lower mask ranks them (variable load)
+      const bool want = my_slot && !active && !exhausted;
+      const unsigned req = __ballot_sync(kFull, want);
+      if (req) {
+        int base = 0;
+        if (lane == 0) base = atomicAdd(a.queue_head, __popc(req));
+        base = __shfl_sync(kFull, base, 0);
+        if (want) {
+          const long long pos = (long long)base + __popc(req & ((1u << lane) - 1u));
+          if (pos < a.n_active) {
+            cidx = a.list ? a.list[pos] : (int)pos;
+            T = a.T[cidx];
+            p = a.p[cidx];
+            for (int i = 0; i < S; ++i) LS_AT(double, LS_L(oY), i, mc) = a.Y[(long long)i * a.ld + cidx];
+            t = 0.0;
+            steps = 0;
+            active = true;
+            fresh = 1;
+          } else {
+            exhausted = true;
           }
-        } else {
-#pragma unroll 4
-          for (int i = 0; i < S; ++i) inv_wbar = fma_rn(LS_AT(double, LS_L(oY), i, mc), invW[i], inv_wbar);
         }
-        if (EST) {
-          float *cXn = (float *)(cells + LS_L(oXn));
-          cXn[mc] = ((float)T - ((const float *)(tbl + LS_L(o_eshift)))[0]) * ((const float *)(tbl + LS_L(o_escale)))[0];
-        }
-        rho = c_tot / inv_wbar;
-        LS_SC(double, kF_T, mc) = T;
-        LS_SC(double, kF_P, mc) = p;
-        LS_SC(double, kF_LNT, mc) = lnT;
-        LS_SC(double, kF_LNC0, mc) = ln_c0;
-        LS_SC(double, kF_INVT, mc) = invT;
-        LS_SC(double, kF_ICTOT, mc) = inv_ctot;
-        LS_SC(double, kF_RHO, mc) = rho;
-        LS_SC(double, kF_REM, mc) = a.t_f - t;
-        LS_SC(unsigned long long, kF_TSTAR, mc) = kInfBits;
-        LS_SC(int, kF_ACTIVE, mc) = active ? 1 : 0;
-        LS_SC(int, kF_BAD, mc) = 0;
       }
     }
-    ls_dft<SH, false>(a, cells, trow, 1, sl_prev, warp, lane, dt_max, t_tol);
-    LST(0)
-    __syncthreads();
-    LST(5)
-    if (!s_go) break;
+    const int go = __any_sync(kFull, my_slot && (active || pending_st >= 0));
+    if (lane == 0) s_go = go;
+    // ---- scalars of the next step.  With at most 16 cells the two logarithms run side by side in the two half-warps
+    // (lane c: ln T, lane 16 + c: ln(p_atm / (R_u T)) of the same cell); else one after the other.
+    double lnT, ln_c0;
+    if (C <= 16) {
+      const double T_peer = __shfl_sync(kFull, T, lane & 15);
+      const double lval = ab_log((lane & 16) ? (kPatm / (kRu * T_peer)) : T_peer);
+      lnT = __shfl_sync(kFull, lval, lane & 15);
+      ln_c0 = __shfl_sync(kFull, lval, (lane & 15) | 16);
+    } else {
+      lnT = ab_log(T);
+      ln_c0 = ab_log(kPatm / (kRu * T));
+    }
+    if (my_slot) {
+      const double RuT = kRu * T;
+      const double c_tot = p / RuT;
+      const double invT = 1.0 / T;
+      inv_ctot = 1.0 / c_tot;
+      // 1/Wbar = sum Y_i/W_i, sequential in species order (contract 5.4); estimator inputs on the way (R18)
+      double inv_wbar = 0.0;
+      if (EST && LS_D(n_in) > 1) {
+        float *cXn = (float *)(cells + LS_L(oXn));
+        const float *eshift = (const float *)(tbl + LS_L(o_eshift)), *escale = (const float *)(tbl + LS_L(o_escale));
+        cXn[1 * C + mc] = ((float)p - eshift[1]) * escale[1];
+        for (int i = 0; i < S; ++i) {
+          const double y = LS_AT(double, LS_L(oY), i, mc);
+          inv_wbar = fma_rn(y, invW[i], inv_wbar);
+          cXn[(2 + i) * C + mc] = ((float)y - eshift[2 + i]) * escale[2 + i];
+        }
+      } else {
+#pragma unroll 4
+        for (int i = 0; i < S; ++i) inv_wbar = fma_rn(LS_AT(double, LS_L(oY), i, mc), invW[i], inv_wbar);
+      }
+      if (EST) {
+        float *cXn = (float *)(cells + LS_L(oXn));
+        cXn[mc] = ((float)T - ((const float *)(tbl + LS_L(o_eshift)))[0]) * ((const float *)(tbl + LS_L(o_escale)))[0];
+      }
+      rho = c_tot / inv_wbar;
+      LS_SC(double, kF_T, mc) = T;
+      LS_SC(double, kF_P, mc) = p;
+      LS_SC(double, kF_LNT, mc) = lnT;
+      LS_SC(double, kF_LNC0, mc) = ln_c0;
+      LS_SC(double, kF_INVT, mc) = invT;
+      LS_SC(double, kF_ICTOT, mc) = inv_ctot;
+      LS_SC(double, kF_RHO, mc) = rho;
+      LS_SC(double, kF_REM, mc) = a.t_f - t;
+      LS_SC(unsigned long long, kF_TSTAR, mc) = kInfBits;
+      LS_SC(int, kF_ACTIVE, mc) = active ? 1 : 0;
+      LS_SC(int, kF_FRESH, mc) = fresh;
+      LS_SC(int, kF_BAD, mc) = 0;
+    }
+    sc_set = sc_keep;
+  };
 
+  // ---- before the first step: the scalar warp fills the slots and prepares scalar set 0
+  if (warp == SW) scalar_warp_prepare(LS_L(oSc), LS_L(oSc), 0, true);
+  __syncthreads();
+
+  int g13 = 0;   // ring position of the step being taken (block-uniform)
+  bool have_prev = false;
+  while (s_go) {
     // =========================== phase 1: a1 thermo, concentrations, first estimator layer ===========================
+    if (warp == SW && have_prev) {
+      // the scalar warp's own ringing-filter passes of the step just taken (it spent that step's phase 4 on the serial
+      // chain): the previous scalar set and ring position are still intact
+      const int set_prev = (sc_set == LS_L(oSc)) ? LS_L(oSc) + LS_L(sc_bytes) : LS_L(oSc);
+      ls_dft<SH>(a, cells, set_prev, trow, (g13 == 0) ? kWindow - 1 : g13 - 1, warp, lane, dt_max, t_tol);
+    }
     for (unsigned it = (unsigned)tid; it < n_cs; it += kLsThreads) {
       const unsigned i = ls_div_c<SH>(it, C, a.mC), c = it - i * (unsigned)C;
       const double Tc = LS_SC(double, kF_T, c), invT = LS_SC(double, kF_INVT, c), lnT = LS_SC(double, kF_LNT, c);
@@ -495,16 +514,13 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
         }
       }
     }
-    ls_dft<SH, false>(a, cells, trow, 2, sl_prev, warp, lane, dt_max, t_tol);
     LST(1)
     __syncthreads();
     LST(5)
 
     // =========================== phase 2: a2 rates ===========================
-    ls_rev_range<SH>(a, tbl, cells, trow, 0, 2, warp, lane);
-    ls_dft<SH, false>(a, cells, trow, 3, sl_prev, warp, lane, dt_max, t_tol);
-    ls_rev_range<SH>(a, tbl, cells, trow, 2, 4, warp, lane);
-    ls_irr_passes<SH>(a, tbl, cells, warp, lane);
+    ls_rev_range<SH>(a, tbl, cells, sc_set, trow, 0, kLsSlots, warp, lane);
+    ls_irr_passes<SH>(a, tbl, cells, sc_set, warp, lane);
     LST(2)
     __syncthreads();
     LST(5)
@@ -604,61 +620,69 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
     __syncthreads();
     LST(5)
 
-    // =========================== phase 4: a3 step size, a4 update ===========================
-    for (unsigned it = (unsigned)tid; it < n_cs; it += kLsThreads) {
-      const unsigned i = ls_div_c<SH>(it, C, a.mC), c = it - i * (unsigned)C;
-      const double t_star = bits_to_double(LS_SC(unsigned long long, kF_TSTAR, c));
-      double h = (t_star < dt_max) ? t_star : dt_max;       // Eq 5
-      const double rem = LS_SC(double, kF_REM, c);
-      if (rem - h < t_tol) h = rem;                          // landing on t_f (R5)
-      if (LS_SC(int, kF_ACTIVE, c)) {
-        const double y = fma_rn(h, LS_AT(double, LS_L(oConc), 1 + i, c), LS_AT(double, LS_L(oY), i, c));   // Eq 18
-        LS_AT(double, LS_L(oY), i, c) = y;
-        if (!(y - y == 0.0)) atomicOr(&LS_SC(int, kF_BAD, c), 1);
-      }
-    }
-    if (my_slot) {
-      const double t_star = bits_to_double(LS_SC(unsigned long long, kF_TSTAR, mc));
-      double h = (t_star < dt_max) ? t_star : dt_max;
-      const double rem = a.t_f - t;
-      bool lst = false;
-      if (rem - h < t_tol) {
-        h = rem;
-        lst = true;
-      }
-      // temperature equation (R15): sum (Y_i/W_i) cp_i/R and sum (h_i/RT) omega_i, each sequential in species order
-      double sum_cp = 0.0, sum_h = 0.0;
+    // =========================== phase 4: a3 step size, a4 update, a5 ringing filter, and the scalar chain ===========================
+    const int set_next = (sc_set == LS_L(oSc)) ? LS_L(oSc) + LS_L(sc_bytes) : LS_L(oSc);
+    const int g_next = (g13 + 1 == kWindow) ? 0 : g13 + 1;
+    if (warp == SW) {
+      if (my_slot) {
+        const double t_star = bits_to_double(LS_SC(unsigned long long, kF_TSTAR, mc));
+        double h = (t_star < dt_max) ? t_star : dt_max;   // Eq 5
+        const double rem = a.t_f - t;
+        bool lst = false;
+        if (rem - h < t_tol) {                            // landing on t_f (R5)
+          h = rem;
+          lst = true;
+        }
+        // temperature equation (R15): sum (Y_i/W_i) cp_i/R and sum (h_i/RT) omega_i, each sequential in species order
+        double sum_cp = 0.0, sum_h = 0.0;
 #pragma unroll 4
-      for (int i = 0; i < S; ++i) {
-        sum_cp = fma_rn(LS_AT(double, LS_L(oYw), i, mc), LS_AT(double, LS_L(oCp), i, mc), sum_cp);
-        sum_h = fma_rn(LS_AT(double, LS_L(oH), i, mc), LS_AT(double, LS_L(oOm), i, mc), sum_h);
+        for (int i = 0; i < S; ++i) {
+          sum_cp = fma_rn(LS_AT(double, LS_L(oYw), i, mc), LS_AT(double, LS_L(oCp), i, mc), sum_cp);
+          sum_h = fma_rn(LS_AT(double, LS_L(oH), i, mc), LS_AT(double, LS_L(oOm), i, mc), sum_h);
+        }
+        const double dTdt = (sc.energy_mode == 0) ? -((sum_h * kRu) * T) / (rho * (kRu * sum_cp)) : 0.0;
+        if (active) {
+          T = fma_rn(h, dTdt, T);
+          bad_T = !(T - T == 0.0);
+          t = lst ? a.t_f : t + h;
+          steps += 1;
+          last = lst;
+        }
       }
-      const double dTdt = (sc.energy_mode == 0) ? -((sum_h * kRu) * T) / (rho * (kRu * sum_cp)) : 0.0;
-      LS_SC(int, kF_FRESH, mc) = 0;
-      LS_SC(double, kF_HDFT, mc) = h;
-      LS_SC(double, kF_ICDFT, mc) = inv_ctot;
-      LS_SC(int, kF_DFTON, mc) = (active && !lst) ? 1 : 0;   // the landing step's change is never looked at: the cell retires
-      if (active) {
-        T = fma_rn(h, dTdt, T);
-        bad_T = !(T - T == 0.0);
-        t = lst ? a.t_f : t + h;
-        steps += 1;
-        last = lst;
+      // the new mass fractions (and the non-finite flags) of all cells are in place once every other warp has arrived
+      asm volatile("bar.sync %0, %1;" ::"n"(kXBar), "n"(kLsThreads) : "memory");
+      scalar_warp_prepare(sc_set, set_next, g_next, false);
+    } else {
+      for (unsigned it = (unsigned)tid; it < n_cs; it += kLsItemThreads) {
+        const unsigned i = ls_div_c<SH>(it, C, a.mC), c = it - i * (unsigned)C;
+        const double t_star = bits_to_double(LS_SC(unsigned long long, kF_TSTAR, c));
+        double h = (t_star < dt_max) ? t_star : dt_max;       // Eq 5
+        const double rem = LS_SC(double, kF_REM, c);
+        if (rem - h < t_tol) h = rem;                          // landing on t_f (R5)
+        if (LS_SC(int, kF_ACTIVE, c)) {
+          const double y = fma_rn(h, LS_AT(double, LS_L(oConc), 1 + i, c), LS_AT(double, LS_L(oY), i, c));   // Eq 18
+          LS_AT(double, LS_L(oY), i, c) = y;
+          if (!(y - y == 0.0)) atomicOr(&LS_SC(int, kF_BAD, c), 1);
+        }
       }
+      __threadfence_block();
+      asm volatile("bar.arrive %0, %1;" ::"n"(kXBar), "n"(kLsThreads) : "memory");
+      ls_dft<SH>(a, cells, sc_set, trow, g13, warp, lane, dt_max, t_tol);
     }
-    ls_dft<SH, true>(a, cells, trow, 0, g13, warp, lane, dt_max, t_tol);
     LST(4)
     __syncthreads();
     LST(5)
-    g13 = (g13 + 1 == kWindow) ? 0 : g13 + 1;
+    sc_set = set_next;
+    g13 = g_next;
+    have_prev = true;
 #ifdef LS_TIMING
     n_steps_ += 1;
 #endif
   }
 #ifdef LS_TIMING
   if (blockIdx.x == 0 && lane == 0 && (warp == 0 || warp == 7 || warp == SW))
-    printf("LST warp %d steps %lld per step: P0 %lld P1 %lld P2 %lld P3 %lld P4 %lld barrier-wait %lld\n", warp, n_steps_, tph[0] / n_steps_,
-           tph[1] / n_steps_, tph[2] / n_steps_, tph[3] / n_steps_, tph[4] / n_steps_, tph[5] / n_steps_);
+    printf("LST warp %d steps %lld per step: P1 %lld P2 %lld P3 %lld P4 %lld barrier-wait %lld\n", warp, n_steps_, tph[1] / n_steps_,
+           tph[2] / n_steps_, tph[3] / n_steps_, tph[4] / n_steps_, tph[5] / n_steps_);
 #endif
 
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");

@@ -274,6 +274,8 @@ def test_default_kernel_selection(stev):
     assert gpu["stats"]["lanes_per_cell"] == 64 and gpu["stats"]["threads_per_block"] == 512
     gpu = GpuCase(stev, make_workload(2, 64)).integrate()
     assert gpu["stats"]["lanes_per_cell"] == 34 and gpu["stats"]["cells_per_block"] == 32   # dense: 42 reversible reactions
+    gpu = GpuCase(stev, make_workload(4, 64)).integrate()
+    assert gpu["stats"]["lanes_per_cell"] == 512 and gpu["stats"]["specialised"] == 1   # mid-size with estimator: lock-step block
     gpu = GpuCase(stev, make_workload(1, 64)).integrate()
     assert gpu["stats"]["lanes_per_cell"] == 512 and gpu["stats"]["specialised"] == 1   # tiny mechanism: lock-step block
     gpu = GpuCase(stev, make_workload(0, 64)).integrate()
