@@ -57,6 +57,8 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--ref-cells", type=int, default=None, help="cells per step of the --impl reference arm")
+    ap.add_argument("--state-precision", default="f64", choices=["f64", "f32"],
+                    help="f32: stev_params.state_precision = STEV_STATE_FP32 (PAPER.md:428); reported with dtype f32, beside the f64 headline")
     ap.add_argument("--no-per-config", action="store_true", help="skip the per_config object (the other BASELINE.json configs at full size)")
     ap.add_argument("--per-config-budget", type=float, default=330.0,
                     help="seconds since start after which config 4 at full size (one call of about two minutes) is skipped")
@@ -336,7 +338,9 @@ def main():
     params = dict(w.params)
     if args.max_steps is not None:
         params["max_steps"] = args.max_steps
-    prm = stev.stev_params_default(chunk_steps=args.chunk_steps, lanes_per_cell=args.lanes, order_cells=args.order, **params)
+    f32 = args.state_precision == "f32"
+    prm = stev.stev_params_default(chunk_steps=args.chunk_steps, lanes_per_cell=args.lanes, order_cells=args.order,
+                                   state_precision=1 if f32 else 0, **params)
 
     T0 = torch.tensor(w.T, dtype=torch.float64, device=dev)
     p = torch.tensor(w.p, dtype=torch.float64, device=dev)
@@ -453,7 +457,7 @@ def main():
                 "hbm_bytes_per_launch": n * (8 * (2 + S) + 8 * (1 + S) + 5)}
 
     cpu_baseline = None
-    if not args.no_cpu_baseline:
+    if not args.no_cpu_baseline and not f32:
         cores = os.cpu_count() or 1
         n_s = {0: 4096, 1: 4096, 2: 2048, 3: 768 * cores, 4: 1024}[args.config]   # about 10-30 s of oracle time
         n_s = min(n_s, n)
@@ -462,7 +466,7 @@ def main():
                         "sample": f"first {n_s} cells of this rank's field, {dt:.1f} s", "cell_steps_per_s": cs / dt}
 
     per_config = None
-    if world == 1 and not args.no_per_config and args.config == 3 and args.cells is None and args.lanes == 0 and args.max_steps is None:
+    if world == 1 and not args.no_per_config and args.config == 3 and args.cells is None and args.lanes == 0 and args.max_steps is None and not f32:
         # the other BASELINE.json configs at full size (1 warm-up + 1 timed call each; config 4 -- one call takes about two
         # minutes -- last, without warm-up, and only inside the wall-clock budget), and row a7 on its own
         per_config = {}
@@ -488,7 +492,7 @@ def main():
             per_config["4"] = {"skipped": f"wall-clock budget of {args.per_config_budget:.0f} s used up before config 4"}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32" if f32 else "f64",
             "data": "synthetic",
             "config": {"workload": w.name, "cells_per_gpu": n, "species": S, "reactions": w.mech.n_reactions,
                        "reversible": w.mech.n_reversible, "dt_cfd": w.dt_cfd,

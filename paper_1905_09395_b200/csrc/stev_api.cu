@@ -419,6 +419,11 @@ int stev_mechanism_create(const stev_mechanism_desc *d, stev_mechanism **out) {
       e = cudaMalloc(&m->d_ls_table, ls.size());
       if (e == cudaSuccess) e = cudaMemcpy(m->d_ls_table, ls.data(), ls.size(), cudaMemcpyHostToDevice);
     }
+    m->ls32_ok = e == cudaSuccess && build_ls_image(h, nullptr, ls, m->ls_tb32, true);
+    if (m->ls32_ok) {
+      e = cudaMalloc(&m->d_ls_table32, ls.size());
+      if (e == cudaSuccess) e = cudaMemcpy(m->d_ls_table32, ls.data(), ls.size(), cudaMemcpyHostToDevice);
+    }
   }
   if (e != cudaSuccess) {
     stev_mechanism_destroy(m);
@@ -435,6 +440,7 @@ void stev_mechanism_destroy(stev_mechanism *m) {
   for (int w = 0; w < 2; ++w)
     if (m->d_pk_table[w]) cudaFree(m->d_pk_table[w]);
   if (m->d_ls_table) cudaFree(m->d_ls_table);
+  if (m->d_ls_table32) cudaFree(m->d_ls_table32);
   delete m;
 }
 
@@ -505,6 +511,11 @@ int stev_estimator_load(const stev_mechanism *m, const stev_estimator_desc *d, s
       ce = cudaMalloc(&e->d_ls_table, ls.size());
       if (ce == cudaSuccess) ce = cudaMemcpy(e->d_ls_table, ls.data(), ls.size(), cudaMemcpyHostToDevice);
     }
+    e->ls32_ok = ce == cudaSuccess && build_ls_image(m->host, &h, ls, e->ls_tb32, true);
+    if (e->ls32_ok) {
+      ce = cudaMalloc(&e->d_ls_table32, ls.size());
+      if (ce == cudaSuccess) ce = cudaMemcpy(e->d_ls_table32, ls.data(), ls.size(), cudaMemcpyHostToDevice);
+    }
   }
   if (ce == cudaSuccess) {
     // standalone parameter block: in_shift, in_scale, W1T [n_in][H], b1, W2T [H][n_out], b2
@@ -540,6 +551,7 @@ void stev_estimator_destroy(stev_estimator *e) {
   for (int w = 0; w < 2; ++w)
     if (e->d_pk_table[w]) cudaFree(e->d_pk_table[w]);
   if (e->d_ls_table) cudaFree(e->d_ls_table);
+  if (e->d_ls_table32) cudaFree(e->d_ls_table32);
   if (e->d_params) cudaFree(e->d_params);
   for (int k = 0; k < 2; ++k)
     if (e->d_tc_image[k]) cudaFree(e->d_tc_image[k]);
@@ -719,8 +731,9 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
   if (rc) return rc;
   const bool f32 = p->state_precision == STEV_STATE_FP32;
   if ((rc = pick_tables(m, est, &tb, &table, f32))) return rc;
-  if (f32 && p->lanes_per_cell > 32) {
-    set_error("stev_integrate: state_precision = STEV_STATE_FP32 runs on the shared-memory-history kernel (lanes_per_cell 0 or 1..32)");
+  if (f32 && p->lanes_per_cell > 32 && p->lanes_per_cell != 512 && p->lanes_per_cell != 513) {
+    set_error("stev_integrate: state_precision = STEV_STATE_FP32 runs on the lock-step kernel (lanes_per_cell 0, 512, 513) or the "
+              "shared-memory-history kernel (1..32)");
     return STEV_EINVAL;
   }
   if (n < 0 || n > 0x7fffffff || ld < n || !(dt_cfd > 0.0) || !std::isfinite(dt_cfd)) {
@@ -751,14 +764,16 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
     const bool tm_common = p->chunk_steps == 0;
     const bool pk1_ok = (est ? est->pk_ok[0] : m->pk_ok[0]) && tm_common;
     const bool pk2_ok = (est ? est->pk_ok[1] : m->pk_ok[1]) && tm_common;
-    const bool ls_ok = (est ? est->ls_ok : m->ls_ok) && tm_common;
+    const bool ls_ok = (f32 ? (est ? est->ls32_ok : m->ls32_ok) : (est ? est->ls_ok : m->ls_ok)) && tm_common;
     const bool dense_ok = pk1_ok && pk_dense_ok(est ? est->pk_tb[0] : m->pk_tb[0]);
     int kind = 0;   // 0: sub-warp groups (history in shared memory), 1: one warp per cell, 2: warp pair, 6: dense one warp per cell, 7: lock step
     if (p->lanes_per_cell == 33) kind = 1;
     else if (p->lanes_per_cell == 64) kind = 2;
     else if (p->lanes_per_cell == 34) kind = 6;
     else if (p->lanes_per_cell == 512 || p->lanes_per_cell == 513) kind = 7;
-    else if (p->lanes_per_cell == 0 && !f32) {
+    else if (p->lanes_per_cell == 0 && f32) {
+      if (ls_ok) kind = 7;   // binary32 state: the lock-step kernel where the mechanism fits it, else sub-warp groups
+    } else if (p->lanes_per_cell == 0) {
       // Measured on B200: large mechanisms -> warp pair; tiny ones (a step is a few hundred
       // instructions) -> lock-step block, which flattens (cell, reaction) pairs over the lanes (configs 0, 1: +56 %);
       // mid-size with an estimator -> lock-step block too (its estimator layers are shared over the cells of the block;
@@ -793,9 +808,10 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
       int blocks = 0, cpb = 0, threads = kPkThreads, specialised = 0;
       size_t smem = 0;
       if (kind == 7) {
-        const stev::LsTables &ltb = est ? est->ls_tb : m->ls_tb;
+        const stev::LsTables &ltb = f32 ? (est ? est->ls_tb32 : m->ls_tb32) : (est ? est->ls_tb : m->ls_tb);
+        const unsigned char *ltable = f32 ? (est ? est->d_ls_table32 : m->d_ls_table32) : (est ? est->d_ls_table : m->d_ls_table);
         bool is_static = false;
-        rc = integrate_ls_launch(ltb, est ? est->d_ls_table : m->d_ls_table, make_consts(p), dt_cfd, n, ld, T, pressure, Y,
+        rc = integrate_ls_launch(ltb, ltable, make_consts(p), dt_cfd, n, ld, T, pressure, Y,
                                  steps_out, status_out, w.counters, s, &blocks, &smem, order, p->lanes_per_cell != 513, &is_static);
         cpb = ltb.d.C;
         threads = kLsThreads;

@@ -70,7 +70,7 @@ bool pk_dense_ok(const PkTables &tb);
 
 // Lock-step integrator (stev_ls.cuh / stev_ls.cu): all cells of a block step together.  build_ls_image returns false if
 // the mechanism is outside its limits (more than two factors per reaction side, tables too large for shared memory).
-bool build_ls_image(const HostMechanism &m, const HostEstimator *e, std::vector<unsigned char> &image, LsTables &tb);
+bool build_ls_image(const HostMechanism &m, const HostEstimator *e, std::vector<unsigned char> &image, LsTables &tb, bool f32 = false);
 // allow_static: use the instantiation with compile-time dimensions if the shape list has one (*is_static says which ran)
 int integrate_ls_launch(const LsTables &tb, const unsigned char *d_table, const SolverConsts &sc, double t_f, long long n,
                         long long ld, double *T, const double *p, double *Y, int *steps, unsigned char *status, int *counters,
@@ -102,6 +102,9 @@ struct stev_mechanism {
   bool ls_ok = false;                    // image of the lock-step kernel (NASA-7 thermo)
   stev::LsTables ls_tb{};
   unsigned char *d_ls_table = nullptr;
+  bool ls32_ok = false;                  // the same for the binary32 state path
+  stev::LsTables ls_tb32{};
+  unsigned char *d_ls_table32 = nullptr;
 };
 
 struct stev_estimator {
@@ -118,6 +121,9 @@ struct stev_estimator {
   bool ls_ok = false;                    // image of the lock-step kernel (MLP thermo)
   stev::LsTables ls_tb{};
   unsigned char *d_ls_table = nullptr;
+  bool ls32_ok = false;
+  stev::LsTables ls_tb32{};
+  unsigned char *d_ls_table32 = nullptr;
   // standalone evaluation (stev_estimator_eval): device copies in kernel-friendly layouts
   float *d_params = nullptr;             // in_shift, in_scale, W1T [n_in][H], b1, W2T [H][n_out], b2
   size_t params_floats = 0;

@@ -27,14 +27,16 @@ static bool ls_mechanism_ok(const HostMechanism &m) {
   return true;
 }
 
-bool build_ls_image(const HostMechanism &m, const HostEstimator *e, std::vector<unsigned char> &image, LsTables &tb) {
+bool build_ls_image(const HostMechanism &m, const HostEstimator *e, std::vector<unsigned char> &image, LsTables &tb, bool f32) {
   if (!ls_mechanism_ok(m)) return false;
+  const int es = f32 ? 4 : 8;
   const int S = m.S, R = m.R, Rrev = m.Rrev;
   tb = LsTables{};
   LsDims &d = tb.d;
   d.S = S;
   d.R = R;
   d.Rrev = Rrev;
+  d.es = es;
   if (e) {
     d.has_est = 1;
     d.H = e->H;
@@ -93,7 +95,7 @@ bool build_ls_image(const HostMechanism &m, const HostEstimator *e, std::vector<
   // cell slots per block: one lane of the scalar warp each, 2048 DFT windows in tensor memory, shared memory
   const size_t avail = kSmemMax > (size_t)tb.bytes + 1024 ? kSmemMax - (size_t)tb.bytes - 1024 : 0;
   int C = kLsMaxCells;
-  if (Rrev > 0) C = std::min(C, (32 * kLsMaxPasses) / Rrev);
+  if (Rrev > 0) C = std::min(C, (32 * ls_max_passes(es)) / Rrev);
   for (; C >= 1; --C) {
     d.C = C;
     L = ls_layout_of(d);
@@ -103,47 +105,54 @@ bool build_ls_image(const HostMechanism &m, const HostEstimator *e, std::vector<
 
   image.assign(tb.bytes, 0);
   unsigned char *base = image.data();
-  double *tmid = (double *)(base + L.o_tmid), *W = (double *)(base + L.o_W), *invW = (double *)(base + L.o_invW);
-  double *nasa = (double *)(base + L.o_nasa);
+  // every real table entry is formed in double and stored as double or, for the binary32 image, rounded to float once
+  auto put = [&](int off0, int idx, double v) {
+    if (f32) ((float *)(base + off0))[idx] = (float)v;
+    else ((double *)(base + off0))[idx] = v;
+  };
   for (int i = 0; i < S; ++i) {
-    tmid[i] = m.t_mid[i];
-    W[i] = m.W[i];
-    invW[i] = 1.0 / m.W[i];
+    put(L.o_tmid, i, m.t_mid[i]);
+    put(L.o_W, i, m.W[i]);
+    put(L.o_invW, i, 1.0 / m.W[i]);
     for (int rg = 0; rg < 2; ++rg) {
       const double *c = (rg == 0 ? m.nasa_lo.data() : m.nasa_hi.data()) + 7 * i;
-      double *row = nasa + rg * kNasaRows * S + i;
-      row[0 * S] = c[0]; row[1 * S] = c[1]; row[2 * S] = c[2]; row[3 * S] = c[3]; row[4 * S] = c[4];
-      row[5 * S] = c[1] / 2.0; row[6 * S] = c[2] / 3.0; row[7 * S] = c[3] / 4.0; row[8 * S] = c[4] / 5.0;
-      row[9 * S] = c[5];
-      row[10 * S] = c[2] / 2.0; row[11 * S] = c[3] / 3.0; row[12 * S] = c[4] / 4.0;
-      row[13 * S] = c[6];
+      const int r0 = rg * kNasaRows * S + i;
+      put(L.o_nasa, r0 + 0 * S, c[0]); put(L.o_nasa, r0 + 1 * S, c[1]); put(L.o_nasa, r0 + 2 * S, c[2]);
+      put(L.o_nasa, r0 + 3 * S, c[3]); put(L.o_nasa, r0 + 4 * S, c[4]);
+      put(L.o_nasa, r0 + 5 * S, c[1] / 2.0); put(L.o_nasa, r0 + 6 * S, c[2] / 3.0); put(L.o_nasa, r0 + 7 * S, c[3] / 4.0);
+      put(L.o_nasa, r0 + 8 * S, c[4] / 5.0);
+      put(L.o_nasa, r0 + 9 * S, c[5]);
+      put(L.o_nasa, r0 + 10 * S, c[2] / 2.0); put(L.o_nasa, r0 + 11 * S, c[3] / 3.0); put(L.o_nasa, r0 + 12 * S, c[4] / 4.0);
+      put(L.o_nasa, r0 + 13 * S, c[6]);
     }
   }
   const unsigned one_slot = (unsigned)L.oConc, zero_slot = (unsigned)L.oG;
-  double *rkA = (double *)(base + L.o_rkA), *rkB = (double *)(base + L.o_rkB);
   unsigned *rfac = (unsigned *)(base + L.o_rfac), *rdg = (unsigned *)(base + L.o_rdg);
   for (int k = 0; k < R; ++k) {
     const int j = orig_of[k];
     double dnu = 0.0;
+    float dnu32 = 0.0f;   // Delta-nu summed in the precision of the image, in entry order (as the oracle sums it)
     unsigned fac[4] = {one_slot, one_slot, one_slot, one_slot};
     unsigned dgo[4] = {zero_slot, zero_slot, zero_slot, zero_slot};
     int nf = 0, ne = 0;
     for (int en = m.reac_ptr[j]; en < m.reac_ptr[j + 1]; ++en, ++ne) {
-      for (int n = 0; n < m.reac_nu[en]; ++n) fac[nf++] = (unsigned)(L.oConc + 8 * C * (1 + m.reac_sp[en]));
-      dgo[ne] = (unsigned)(L.oG + 8 * C * (1 + (m.reac_nu[en] == 2 ? S : 0) + m.reac_sp[en]));
+      for (int n = 0; n < m.reac_nu[en]; ++n) fac[nf++] = (unsigned)(L.oConc + es * C * (1 + m.reac_sp[en]));
+      dgo[ne] = (unsigned)(L.oG + es * C * (1 + (m.reac_nu[en] == 2 ? S : 0) + m.reac_sp[en]));
       dnu = dnu - (double)m.reac_nu[en];
+      dnu32 = dnu32 - (float)m.reac_nu[en];
     }
     nf = 2;
     ne = 2;
     for (int en = m.prod_ptr[j]; en < m.prod_ptr[j + 1]; ++en, ++ne) {
-      for (int n = 0; n < m.prod_nu[en]; ++n) fac[nf++] = (unsigned)(L.oConc + 8 * C * (1 + m.prod_sp[en]));
-      dgo[ne] = (unsigned)(L.oG + 8 * C * (1 + (m.prod_nu[en] == 2 ? S : 0) + m.prod_sp[en]));
+      for (int n = 0; n < m.prod_nu[en]; ++n) fac[nf++] = (unsigned)(L.oConc + es * C * (1 + m.prod_sp[en]));
+      dgo[ne] = (unsigned)(L.oG + es * C * (1 + (m.prod_nu[en] == 2 ? S : 0) + m.prod_sp[en]));
       dnu = dnu + (double)m.prod_nu[en];
+      dnu32 = dnu32 + (float)m.prod_nu[en];
     }
-    rkA[2 * k] = clog(m.A[j]);
-    rkA[2 * k + 1] = m.b[j];
-    rkB[2 * k] = m.Ea[j] / kRcal;
-    rkB[2 * k + 1] = dnu;
+    put(L.o_rkA, 2 * k, clog(m.A[j]));
+    put(L.o_rkA, 2 * k + 1, m.b[j]);
+    put(L.o_rkB, 2 * k, m.Ea[j] / kRcal);
+    put(L.o_rkB, 2 * k + 1, f32 ? (double)dnu32 : dnu);
     std::memcpy(rfac + 4 * k, fac, 16);
     if (k < Rrev) std::memcpy(rdg + 4 * k, dgo, 16);
   }
@@ -157,7 +166,7 @@ bool build_ls_image(const HostMechanism &m, const HostEstimator *e, std::vector<
     grow[r] = (unsigned short)row0[r];
     glen[r] = (unsigned short)rows[r];
     for (int en = 0; en < (int)gl[i].size(); ++en)
-      gent[4 * row0[r] + en] = (unsigned)(L.oQ + 8 * C * (variant_of(gl[i][en].coef) * L.Rp + internal_of[gl[i][en].j]));
+      gent[4 * row0[r] + en] = (unsigned)(L.oQ + es * C * (variant_of(gl[i][en].coef) * L.Rp + internal_of[gl[i][en].j]));
   }
   if (e) {
     float *sh = (float *)(base + L.o_eshift), *scl = (float *)(base + L.o_escale), *W1T = (float *)(base + L.o_W1T);
@@ -186,23 +195,28 @@ using LsShape1 = LsFix<9, 19, 11, 4, 0, 0, 0, 0, 32>;
 using LsShape2 = LsFix<20, 60, 42, 4, 0, 0, 0, 0, 32>;
 using LsShape3 = LsFix<53, 325, 225, 4, 1, 32, 1, 106, 9>;
 using LsShape4 = LsFix<20, 60, 42, 4, 1, 64, 22, 40, 32>;
+using LsShape3f = LsFix<53, 325, 225, 4, 1, 32, 1, 106, 18, 4>;   // config 3 with the binary32 state: 18 cells per block
+using LsShape4f = LsFix<20, 60, 42, 4, 1, 64, 22, 40, 32, 4>;
 
 static bool same_dims(const LsDims &x, const LsDims &y) {
   return x.S == y.S && x.R == y.R && x.Rrev == y.Rrev && x.n_var == y.n_var && x.has_est == y.has_est && x.H == y.H &&
-         x.n_in == y.n_in && x.n_out == y.n_out && x.C == y.C;
+         x.n_in == y.n_in && x.n_out == y.n_out && x.C == y.C && x.es == y.es;
 }
 
 static void *ls_kernel_for(const LsDims &d, bool allow_static, bool *is_static) {
   *is_static = true;
   if (allow_static) {
-    if (same_dims(d, LsShape0::D)) return (void *)stev_ls_kernel<LsShape0, false>;
-    if (same_dims(d, LsShape1::D)) return (void *)stev_ls_kernel<LsShape1, false>;
-    if (same_dims(d, LsShape2::D)) return (void *)stev_ls_kernel<LsShape2, false>;
-    if (same_dims(d, LsShape3::D)) return (void *)stev_ls_kernel<LsShape3, true>;
-    if (same_dims(d, LsShape4::D)) return (void *)stev_ls_kernel<LsShape4, true>;
+    if (same_dims(d, LsShape0::D)) return (void *)stev_ls_kernel<LsShape0, false, double>;
+    if (same_dims(d, LsShape1::D)) return (void *)stev_ls_kernel<LsShape1, false, double>;
+    if (same_dims(d, LsShape2::D)) return (void *)stev_ls_kernel<LsShape2, false, double>;
+    if (same_dims(d, LsShape3::D)) return (void *)stev_ls_kernel<LsShape3, true, double>;
+    if (same_dims(d, LsShape4::D)) return (void *)stev_ls_kernel<LsShape4, true, double>;
+    if (same_dims(d, LsShape3f::D)) return (void *)stev_ls_kernel<LsShape3f, true, float>;
+    if (same_dims(d, LsShape4f::D)) return (void *)stev_ls_kernel<LsShape4f, true, float>;
   }
   *is_static = false;
-  return d.has_est ? (void *)stev_ls_kernel<LsDyn, true> : (void *)stev_ls_kernel<LsDyn, false>;
+  if (d.es == 4) return d.has_est ? (void *)stev_ls_kernel<LsDyn, true, float> : (void *)stev_ls_kernel<LsDyn, false, float>;
+  return d.has_est ? (void *)stev_ls_kernel<LsDyn, true, double> : (void *)stev_ls_kernel<LsDyn, false, double>;
 }
 
 int integrate_ls_launch(const LsTables &tb, const unsigned char *d_table, const SolverConsts &sc, double t_f, long long n,

@@ -22,8 +22,11 @@ constexpr int kLsThreads = 512;                 // 16 warps; warp w reaches TMEM
 constexpr int kLsWarps = kLsThreads / 32;
 constexpr int kLsPassWarps = kLsWarps;          // every warp owns (reaction, cell) passes: pass p belongs to warp p % 16
 constexpr int kLsItemThreads = 32 * (kLsWarps - 1);   // threads that update the mass fractions in phase 4 (not the scalar warp)
-constexpr int kLsSlots = 4;                     // 32-column window slots per warp: 4 warps per quarter x 4 x 32 = 512 columns
-constexpr int kLsMaxPasses = kLsPassWarps * kLsSlots;   // 64 warp passes = 2048 DFT windows per block
+// A warp owns 128 tensor-memory columns of its lane quarter (4 warps per quarter x 128 = 512): four 32-column slots of
+// thirteen doubles, or eight 16-column slots of thirteen floats (stev_params.state_precision = STEV_STATE_FP32).
+__host__ __device__ constexpr int ls_slot_pitch(int es) { return es == 8 ? 32 : 16; }
+__host__ __device__ constexpr int ls_slots(int es) { return 128 / ls_slot_pitch(es); }
+__host__ __device__ constexpr int ls_max_passes(int es) { return kLsPassWarps * ls_slots(es); }   // 64 (2048 windows) / 128 (4096)
 constexpr int kLsMaxCells = 32;                 // one lane of the scalar warp per cell
 
 // Scalars of the cell slots, one array of C eight-byte entries per field (entry (f, c) at set + (f C + c) 8).  There are
@@ -45,17 +48,18 @@ struct LsDims {
   int n_var;                           // stored multiples of q: 2 (+q, -q) or 4 (+q, -q, +2q, -2q)
   int has_est, H, n_in, n_out;
   int C;                               // cell slots per block
+  int es;                              // bytes per real: 8 (binary64 state) or 4 (binary32 state)
 };
 
-// Byte offsets.  The working set of the block's C cells is stored INDEX-MAJOR, CELL-MINOR: element (idx, c) of an array at
-// offset o sits at o + (idx C + c) 8, so that lanes holding consecutive cells of the same species / reaction read
+// Byte offsets; "real" is double or float (LsDims.es bytes).  The working set of the block's C cells is stored INDEX-MAJOR,
+// CELL-MINOR: element (idx, c) of a real array at offset o sits at o + (idx C + c) es, so that lanes holding consecutive cells of the same species / reaction read
 // consecutive addresses (and the per-reaction tables are read by broadcast).  From the start of the cell region:
 //   oY [S] | oYw [S] Y_i/W_i | oCp [S] cp_i/R | oH [S] h_i/RT | oOm [S] omega_i
 //   oConc [1+S] ([0] = 1.0, then C_i**, later dY_i/dt) | oG [1+2S] ([0] = 0.0, g_i/RT, 2 g_i/RT)
 //   oQ [n_var][Rp] multiples of q_eff | oRof [Rrev] | oSc [2][kF_COUNT] the two sets of scalars
 //   oHid float [C][Hs] hidden activations, cell-major with Hs = H + 4 | oXn float [n_in][C] normalised estimator inputs
 // Table image (from the image base):
-//   o_tmid, o_W, o_invW double [S] | o_nasa double [2][14][S] | o_rkA double2 [R] {ln A, b} | o_rkB double2 [R] {Ea/R_cal, dnu}
+//   o_tmid, o_W, o_invW real [S] | o_nasa real [2][14][S] | o_rkA real2 [R] {ln A, b} | o_rkB real2 [R] {Ea/R_cal, dnu}
 //   o_rfac uint4 [R] offsets (from the cell region, for cell 0) of the two reactant and two product concentration factors
 //          (the 1.0 slot if absent)
 //   o_rdg uint4 [Rrev] offsets of nu*g of the <= 2 reactant / <= 2 product entries (0.0 slot if absent)
@@ -78,29 +82,29 @@ __host__ __device__ constexpr LsLayout ls_layout_of(const LsDims &d) {
   L.Rp = (d.R + 1) & ~1;
   L.Hpad = d.H + 4;
   L.Hs = d.H + 4;
-  const int C = d.C;
+  const int C = d.C, es = d.es;
   int o = 0;
-  L.oY = o; o = ls_align(o + 8 * C * d.S, 16);
-  L.oYw = o; o = ls_align(o + 8 * C * d.S, 16);
-  L.oCp = o; o = ls_align(o + 8 * C * d.S, 16);
-  L.oH = o; o = ls_align(o + 8 * C * d.S, 16);
-  L.oOm = o; o = ls_align(o + 8 * C * d.S, 16);
-  L.oConc = o; o = ls_align(o + 8 * C * (1 + d.S), 16);
-  L.oG = o; o = ls_align(o + 8 * C * (1 + 2 * d.S), 16);
-  L.oQ = o; o = ls_align(o + 8 * C * d.n_var * L.Rp, 16);
-  L.oRof = o; o = ls_align(o + 8 * C * (d.Rrev > 0 ? d.Rrev : 1), 16);
+  L.oY = o; o = ls_align(o + es * C * d.S, 16);
+  L.oYw = o; o = ls_align(o + es * C * d.S, 16);
+  L.oCp = o; o = ls_align(o + es * C * d.S, 16);
+  L.oH = o; o = ls_align(o + es * C * d.S, 16);
+  L.oOm = o; o = ls_align(o + es * C * d.S, 16);
+  L.oConc = o; o = ls_align(o + es * C * (1 + d.S), 16);
+  L.oG = o; o = ls_align(o + es * C * (1 + 2 * d.S), 16);
+  L.oQ = o; o = ls_align(o + es * C * d.n_var * L.Rp, 16);
+  L.oRof = o; o = ls_align(o + es * C * (d.Rrev > 0 ? d.Rrev : 1), 16);
   L.oSc = o; o = ls_align(o + 2 * 8 * C * (int)kF_COUNT, 16);
   L.sc_bytes = 8 * C * (int)kF_COUNT;
   L.oHid = o; o = ls_align(o + 4 * C * (d.has_est ? L.Hs : 0), 16);
   L.oXn = o; o = ls_align(o + 4 * C * (d.has_est ? d.n_in : 0), 16);
   L.cell_bytes = o;
   int t = 0;
-  L.o_tmid = t; t = ls_align(t + 8 * d.S, 16);
-  L.o_W = t; t = ls_align(t + 8 * d.S, 16);
-  L.o_invW = t; t = ls_align(t + 8 * d.S, 16);
-  L.o_nasa = t; t = ls_align(t + 8 * 2 * kNasaRows * d.S, 16);
-  L.o_rkA = t; t = ls_align(t + 16 * d.R, 16);
-  L.o_rkB = t; t = ls_align(t + 16 * d.R, 16);
+  L.o_tmid = t; t = ls_align(t + es * d.S, 16);
+  L.o_W = t; t = ls_align(t + es * d.S, 16);
+  L.o_invW = t; t = ls_align(t + es * d.S, 16);
+  L.o_nasa = t; t = ls_align(t + es * 2 * kNasaRows * d.S, 16);
+  L.o_rkA = t; t = ls_align(t + 2 * es * d.R, 16);
+  L.o_rkB = t; t = ls_align(t + 2 * es * d.R, 16);
   L.o_rfac = t; t = ls_align(t + 16 * d.R, 16);
   L.o_rdg = t; t = ls_align(t + 16 * (d.Rrev > 0 ? d.Rrev : 1), 16);
   L.o_gsp = t; t = ls_align(t + d.S, 16);
@@ -151,10 +155,10 @@ struct LsDyn {
   static constexpr bool kStatic = false;
   static constexpr LsDims D{};
 };
-template <int S_, int R_, int RREV_, int NVAR_, int EST_, int H_, int NIN_, int NOUT_, int C_>
+template <int S_, int R_, int RREV_, int NVAR_, int EST_, int H_, int NIN_, int NOUT_, int C_, int ES_ = 8>
 struct LsFix {
   static constexpr bool kStatic = true;
-  static constexpr LsDims D{S_, R_, RREV_, NVAR_, EST_, H_, NIN_, NOUT_, C_};
+  static constexpr LsDims D{S_, R_, RREV_, NVAR_, EST_, H_, NIN_, NOUT_, C_, ES_};
 };
 
 }  // namespace stev

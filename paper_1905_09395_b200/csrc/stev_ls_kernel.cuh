@@ -38,9 +38,10 @@ struct LsConst {
 // dimension / layout field: a compile-time constant for a static shape, else read from the kernel arguments
 #define LS_D(f) (SH::kStatic ? SH::D.f : a.tb.d.f)
 #define LS_L(f) (SH::kStatic ? LsConst<SH>::L.f : a.lay.f)
-// element (idx, c) of the cell-region array at byte offset `off` (index-major, cell-minor)
-#define LS_AT(type, off, idx, c) (*(type *)(cells + (off) + ((unsigned)((idx) * C + (c)) << 3)))
-#define LS_SC(type, field, c) LS_AT(type, sc_set, (int)(field), c)   // sc_set: byte offset of the scalar set of the step
+// element (idx, c) of the cell-region array of reals at byte offset `off` (index-major, cell-minor)
+#define LS_AT(type, off, idx, c) (*(type *)(cells + (off) + (unsigned)((idx) * C + (c)) * (unsigned)sizeof(type)))
+// scalar `field` of cell c in the scalar set at byte offset sc_set: eight-byte entries whatever the type
+#define LS_SC(type, field, c) (*(type *)(cells + sc_set + ((unsigned)((int)(field) * C + (c)) << 3)))
 
 constexpr unsigned kFull = 0xffffffffu;
 
@@ -65,14 +66,146 @@ __device__ __forceinline__ void tmem_st26(uint32_t taddr, const uint32_t (&r)[26
   asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1,%2};" ::"r"(taddr + 24), "r"(r[24]), "r"(r[25]) : "memory");
 }
 
+// the thirteen floats of a binary32 window: 13 consecutive columns of this lane (x8 + x4 + x1)
+__device__ __forceinline__ void tmem_ld13(uint32_t taddr, uint32_t (&r)[13]) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+               : "r"(taddr)
+               : "memory");
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11])
+               : "r"(taddr + 8)
+               : "memory");
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x1.b32 {%0}, [%1];" : "=r"(r[12]) : "r"(taddr + 12) : "memory");
+}
+__device__ __forceinline__ void tmem_st13(uint32_t taddr, const uint32_t (&r)[13]) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"r"(taddr), "r"(r[0]), "r"(r[1]),
+               "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7])
+               : "memory");
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1,%2,%3,%4};" ::"r"(taddr + 8), "r"(r[8]), "r"(r[9]), "r"(r[10]),
+               "r"(r[11])
+               : "memory");
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x1.b32 [%0], {%1};" ::"r"(taddr + 12), "r"(r[12]) : "memory");
+}
+__device__ __forceinline__ void tmem_st1(uint32_t taddr, float v) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x1.b32 [%0], {%1};" ::"r"(taddr), "r"(__float_as_uint(v)) : "memory");
+}
+
+// The pieces of a step that differ between the two precisions (DESIGN.md sections 5 and 5b).
+template <typename RT> struct LsReal;
+template <> struct LsReal<double> {
+  using bits_t = unsigned long long;
+  static __device__ __forceinline__ bits_t inf_bits() { return 0x7ff0000000000000ull; }
+  static __device__ __forceinline__ double from_bits(bits_t u) { return bits_to_double(u); }
+  static __device__ __forceinline__ bits_t to_bits(double v) { return double_to_bits(v); }
+  // forward and reverse exponentials of a batch: the generic routine only if any lane of the warp is out of range
+  template <int U>
+  static __device__ __forceinline__ void exp_pairs(const double (&lkf)[U], const double (&lkr)[U], double (&fwd)[U], double (&rev)[U]) {
+    bool oor = false;
+#pragma unroll
+    for (int u = 0; u < U; ++u) oor = oor || ab_exp_out_of_range(lkf[u]) || ab_exp_out_of_range(lkr[u]);
+    if (__any_sync(0xffffffffu, oor)) {
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        fwd[u] = cexp(lkf[u]);
+        rev[u] = cexp(lkr[u]);
+      }
+    } else {
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        fwd[u] = ab_exp_core(lkf[u]);
+        rev[u] = ab_exp_core(lkr[u]);
+      }
+    }
+  }
+  static __device__ __forceinline__ double exp1(double x) {
+    if (__any_sync(0xffffffffu, ab_exp_out_of_range(x))) return cexp(x);
+    return ab_exp_core(x);
+  }
+  static __device__ __forceinline__ float activation(float z, int act) {
+    const double zd = (double)z;
+    return (act == 0) ? (float)(1.0 - 2.0 / (1.0 + ab_exp(2.0 * zd))) : (float)(1.0 / (1.0 + ab_exp(-zd)));
+  }
+  // stores the new sample in column pair `slot13` of the window at tw, reads the window back, decides Eq 12
+  template <int NHF>
+  static __device__ __forceinline__ bool window_rings(uint32_t tw, int slot13, double v, bool on, const SolverConsts &sc) {
+    tmem_st2(tw + 2 * slot13, v);
+    tmem_wait_st();
+    uint32_t ra[26];
+    tmem_ld26(tw, ra);
+    tmem_wait_ld();
+    double x[kWindow];
+    unpack_window(ra, x);
+    double d0, m2;
+    ab_window_stats<NHF>(x, d0, m2);
+    bool sure;
+    bool ringing = ab_ring_filter(d0, m2, sc, sure);
+    if (__any_sync(0xffffffffu, !sure && on)) ringing = ab_ring_exact(d0, m2, sc);
+    return ringing;
+  }
+  static __device__ __forceinline__ void window_zero_if(uint32_t tw, bool fresh) {
+    uint32_t ra[26];
+    tmem_ld26(tw, ra);
+    tmem_wait_ld();
+    if (fresh) {
+#pragma unroll
+      for (int n = 0; n < 26; ++n) ra[n] = 0u;
+    }
+    tmem_st26(tw, ra);
+    tmem_wait_st();
+  }
+};
+template <> struct LsReal<float> {
+  using bits_t = unsigned int;
+  static __device__ __forceinline__ bits_t inf_bits() { return 0x7f800000u; }
+  static __device__ __forceinline__ float from_bits(bits_t u) { return __uint_as_float(u); }
+  static __device__ __forceinline__ bits_t to_bits(float v) { return __float_as_uint(v); }
+  template <int U>
+  static __device__ __forceinline__ void exp_pairs(const float (&lkf)[U], const float (&lkr)[U], float (&fwd)[U], float (&rev)[U]) {
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      fwd[u] = cexpf32(lkf[u]);
+      rev[u] = cexpf32(lkr[u]);
+    }
+  }
+  static __device__ __forceinline__ float exp1(float x) { return cexpf32(x); }
+  static __device__ __forceinline__ float activation(float z, int act) {
+    return (act == 0) ? 1.0f - 2.0f / (1.0f + cexpf32(2.0f * z)) : 1.0f / (1.0f + cexpf32(-z));
+  }
+  template <int NHF>
+  static __device__ __forceinline__ bool window_rings(uint32_t tw, int slot13, float v, bool on, const SolverConsts &sc) {
+    tmem_st1(tw + slot13, v);
+    tmem_wait_st();
+    uint32_t ra[13];
+    tmem_ld13(tw, ra);
+    tmem_wait_ld();
+    float x[kWindow];
+#pragma unroll
+    for (int n = 0; n < kWindow; ++n) x[n] = __uint_as_float(ra[n]);
+    return dft_is_ringing<float>(x, sc);   // Eqs 9-12 as written (float sqrt and division are cheap)
+  }
+  static __device__ __forceinline__ void window_zero_if(uint32_t tw, bool fresh) {
+    uint32_t ra[13];
+    tmem_ld13(tw, ra);
+    tmem_wait_ld();
+    if (fresh) {
+#pragma unroll
+      for (int n = 0; n < 13; ++n) ra[n] = 0u;
+    }
+    tmem_st13(tw, ra);
+    tmem_wait_st();
+  }
+};
+
 // ---------------------------------------------------------------------------------------------------------
 // a5: the ringing filter (Eqs 8-13) of pass `s` of this warp over the (reversible reaction, cell) pairs,
 // run in phase 4 of the step whose applied change in progress it stores: the step size follows from the limiter's
 // minimum exactly as in the update.  slot13: ring position of the step (the same for every cell of the block).
 // ---------------------------------------------------------------------------------------------------------
-template <class SH, int NHF>
+template <class SH, typename RT, int NHF>
 __device__ __forceinline__ void ls_dft_pass(const LsArgs &a, unsigned char *cells, int sc_set, uint32_t trow, int s, int slot13,
-                                            int warp, int lane, double dt_max, double t_tol) {
+                                            int warp, int lane, RT dt_max, RT t_tol) {
+  using LR = LsReal<RT>;
   const SolverConsts &sc = a.sc;
   const int C = LS_D(C);
   const int p = warp + s * kLsPassWarps;
@@ -82,76 +215,72 @@ __device__ __forceinline__ void ls_dft_pass(const LsArgs &a, unsigned char *cell
   const bool valid = f < n_items;
   f = valid ? f : n_items - 1;
   const unsigned k = ls_div_c<SH>(f, C, a.mC), c = f - k * (unsigned)C;
-  const double t_star = bits_to_double(LS_SC(unsigned long long, kF_TSTAR, c));
-  double h = (t_star < dt_max) ? t_star : dt_max;
-  const double rem = LS_SC(double, kF_REM, c);
+  const RT t_star = LR::from_bits(LS_SC(typename LR::bits_t, kF_TSTAR, c));
+  RT h = (t_star < dt_max) ? t_star : dt_max;
+  const RT rem = LS_SC(RT, kF_REM, c);
   const bool lst = rem - h < t_tol;
   h = lst ? rem : h;
-  const double ic = LS_SC(double, kF_ICTOT, c);
+  const RT ic = LS_SC(RT, kF_ICTOT, c);
   const bool on = valid && LS_SC(int, kF_ACTIVE, c) && !lst;   // the landing step's change is never looked at: the cell retires
   if (!__any_sync(kFull, on)) return;   // landing steps and empty slots store nothing
-  const double q = LS_AT(double, LS_L(oQ), k, c);
-  const uint32_t tw = trow + (uint32_t)(s * 32);
+  const RT q = LS_AT(RT, LS_L(oQ), k, c);
   // Eq 8 with R8, R9: the applied change in progress / C_tot.  (Lanes whose cell is not `on` overwrite a window that is
   // zeroed before its next use.)
-  tmem_st2(tw + 2 * slot13, (q * h) * ic);
-  tmem_wait_st();
-  uint32_t ra[26];
-  tmem_ld26(tw, ra);
-  tmem_wait_ld();
-  double x[kWindow];
-  unpack_window(ra, x);
-  double d0, m2;
-  ab_window_stats<NHF>(x, d0, m2);
-  bool sure;
-  bool ringing = ab_ring_filter(d0, m2, sc, sure);
-  if (__any_sync(kFull, !sure && on)) ringing = ab_ring_exact(d0, m2, sc);
+  const bool ringing = LR::template window_rings<NHF>(trow + (uint32_t)(s * ls_slot_pitch((int)sizeof(RT))), slot13, (q * h) * ic, on, sc);
   if (on) {
-    double &rof_ref = LS_AT(double, LS_L(oRof), k, c);
-    double rof = rof_ref * (ringing ? sc.inv_r_fac : sc.r_fac);   // Eqs 12-13
-    if (rof > 1.0) rof = 1.0;
-    if (rof < sc.rof_min) rof = sc.rof_min;
+    RT &rof_ref = LS_AT(RT, LS_L(oRof), k, c);
+    RT rof = rof_ref * (ringing ? MathT<RT>::inv_r_fac(sc) : (RT)sc.r_fac);   // Eqs 12-13
+    if (rof > RT(1)) rof = RT(1);
+    if (rof < (RT)sc.rof_min) rof = (RT)sc.rof_min;
     rof_ref = rof;
   }
 }
 
-template <class SH, int NHF>
+template <class SH, typename RT, int NHF>
 __device__ __forceinline__ void ls_dft_all(const LsArgs &a, unsigned char *cells, int sc_set, uint32_t trow, int slot13, int warp,
-                                           int lane, double dt_max, double t_tol) {
+                                           int lane, RT dt_max, RT t_tol) {
 #pragma unroll 1
-  for (int s = 0; s < kLsSlots; ++s) ls_dft_pass<SH, NHF>(a, cells, sc_set, trow, s, slot13, warp, lane, dt_max, t_tol);
+  for (int s = 0; s < ls_slots((int)sizeof(RT)); ++s) ls_dft_pass<SH, RT, NHF>(a, cells, sc_set, trow, s, slot13, warp, lane, dt_max, t_tol);
 }
 
-template <class SH>
+template <class SH, typename RT>
 __device__ __forceinline__ void ls_dft(const LsArgs &a, unsigned char *cells, int sc_set, uint32_t trow, int slot13, int warp, int lane,
-                                       double dt_max, double t_tol) {
+                                       RT dt_max, RT t_tol) {
   if (!a.sc.dft_enable) return;
+  if (sizeof(RT) == 4) {   // the binary32 filter reads the first high bin at run time
+    ls_dft_all<SH, RT, 0>(a, cells, sc_set, trow, slot13, warp, lane, dt_max, t_tol);
+    return;
+  }
   switch (a.sc.nhf) {
-    case 1: ls_dft_all<SH, 1>(a, cells, sc_set, trow, slot13, warp, lane, dt_max, t_tol); break;
-    case 2: ls_dft_all<SH, 2>(a, cells, sc_set, trow, slot13, warp, lane, dt_max, t_tol); break;
-    case 3: ls_dft_all<SH, 3>(a, cells, sc_set, trow, slot13, warp, lane, dt_max, t_tol); break;
-    case 4: ls_dft_all<SH, 4>(a, cells, sc_set, trow, slot13, warp, lane, dt_max, t_tol); break;
-    case 5: ls_dft_all<SH, 5>(a, cells, sc_set, trow, slot13, warp, lane, dt_max, t_tol); break;
-    default: ls_dft_all<SH, 6>(a, cells, sc_set, trow, slot13, warp, lane, dt_max, t_tol); break;
+    case 1: ls_dft_all<SH, RT, 1>(a, cells, sc_set, trow, slot13, warp, lane, dt_max, t_tol); break;
+    case 2: ls_dft_all<SH, RT, 2>(a, cells, sc_set, trow, slot13, warp, lane, dt_max, t_tol); break;
+    case 3: ls_dft_all<SH, RT, 3>(a, cells, sc_set, trow, slot13, warp, lane, dt_max, t_tol); break;
+    case 4: ls_dft_all<SH, RT, 4>(a, cells, sc_set, trow, slot13, warp, lane, dt_max, t_tol); break;
+    case 5: ls_dft_all<SH, RT, 5>(a, cells, sc_set, trow, slot13, warp, lane, dt_max, t_tol); break;
+    default: ls_dft_all<SH, RT, 6>(a, cells, sc_set, trow, slot13, warp, lane, dt_max, t_tol); break;
   }
 }
+
+// two reals / four table offsets of a reaction
+template <typename RT> struct alignas(2 * sizeof(RT)) LsPair { RT x, y; };
 
 // ---------------------------------------------------------------------------------------------------------
 // a2: rates of passes s0 .. s0 + U - 1 of this warp over the (reversible reaction, cell) pairs, side by side (2 U
 // independent exponential chains in flight).  The owner of a pair also owns its DFT window and its rOF: on the first
 // step of a new cell it zeroes the window (R10) and sets rOF = 1 (Eq 11).
 // ---------------------------------------------------------------------------------------------------------
-template <class SH, int U>
+template <class SH, typename RT, int U>
 __device__ __forceinline__ void ls_rev_batch(const LsArgs &a, const unsigned char *tbl, unsigned char *cells, int sc_set, uint32_t trow,
                                              int s0, int warp, int lane) {
+  using M = MathT<RT>;
+  using LR = LsReal<RT>;
   const int C = LS_D(C), Rrev = LS_D(Rrev), Rp = LS_L(Rp);
   const bool has2 = LS_D(n_var) > 2;
   const unsigned n_rev = (unsigned)(C * Rrev);
   unsigned k[U], c[U];
   bool valid[U];
-  double lkf[U], lkr[U];
+  RT lkf[U], lkr[U];
   uint4 fo[U];
-  bool oor = false;
 #pragma unroll
   for (int u = 0; u < U; ++u) {
     const int p = warp + (s0 + u) * kLsPassWarps;
@@ -162,83 +291,62 @@ __device__ __forceinline__ void ls_rev_batch(const LsArgs &a, const unsigned cha
     c[u] = f - k[u] * (unsigned)C;
     const bool fresh = valid[u] && LS_SC(int, kF_FRESH, c[u]);
     if (__any_sync(kFull, fresh)) {   // rare: once per cell
-      const uint32_t tw = trow + (uint32_t)((s0 + u) * 32);
-      uint32_t ra[26];
-      tmem_ld26(tw, ra);
-      tmem_wait_ld();
-      if (fresh) {
-#pragma unroll
-        for (int n = 0; n < 26; ++n) ra[n] = 0u;
-        LS_AT(double, LS_L(oRof), k[u], c[u]) = 1.0;
-      }
-      tmem_st26(tw, ra);
-      tmem_wait_st();
+      LR::window_zero_if(trow + (uint32_t)((s0 + u) * ls_slot_pitch((int)sizeof(RT))), fresh);
+      if (fresh) LS_AT(RT, LS_L(oRof), k[u], c[u]) = RT(1);
     }
   }
 #pragma unroll
   for (int u = 0; u < U; ++u) {
-    const unsigned char *cc = cells + (c[u] << 3);   // this lane's cell column
-    const double invT = LS_SC(double, kF_INVT, c[u]), lnT = LS_SC(double, kF_LNT, c[u]), ln_c0 = LS_SC(double, kF_LNC0, c[u]);
-    const double2 p0 = ((const double2 *)(tbl + LS_L(o_rkA)))[k[u]], p1 = ((const double2 *)(tbl + LS_L(o_rkB)))[k[u]];
+    const unsigned char *cc = cells + c[u] * (unsigned)sizeof(RT);   // this lane's cell column
+    const RT invT = LS_SC(RT, kF_INVT, c[u]), lnT = LS_SC(RT, kF_LNT, c[u]), ln_c0 = LS_SC(RT, kF_LNC0, c[u]);
+    const LsPair<RT> p0 = ((const LsPair<RT> *)(tbl + LS_L(o_rkA)))[k[u]], p1 = ((const LsPair<RT> *)(tbl + LS_L(o_rkB)))[k[u]];
     const uint4 d = ((const uint4 *)(tbl + LS_L(o_rdg)))[k[u]];
     fo[u] = ((const uint4 *)(tbl + LS_L(o_rfac)))[k[u]];
-    lkf[u] = fma_rn(-p1.x, invT, fma_rn(p0.y, lnT, p0.x));
-    double dg = 0.0 - lds_f64(cc, d.x);
-    dg = dg - lds_f64(cc, d.y);
-    dg = dg + lds_f64(cc, d.z);
-    dg = dg + lds_f64(cc, d.w);
-    lkr[u] = lkf[u] - fma_rn(p1.y, ln_c0, -dg);
-    oor = oor || ab_exp_out_of_range(lkf[u]) || ab_exp_out_of_range(lkr[u]);
+    lkf[u] = M::fma(-p1.x, invT, M::fma(p0.y, lnT, p0.x));
+    RT dg = RT(0) - *(const RT *)(cc + d.x);
+    dg = dg - *(const RT *)(cc + d.y);
+    dg = dg + *(const RT *)(cc + d.z);
+    dg = dg + *(const RT *)(cc + d.w);
+    lkr[u] = lkf[u] - M::fma(p1.y, ln_c0, -dg);
   }
-  double fwd[U], rev[U];
-  if (__any_sync(kFull, oor)) {
-#pragma unroll
-    for (int u = 0; u < U; ++u) {
-      fwd[u] = cexp(lkf[u]);
-      rev[u] = cexp(lkr[u]);
-    }
-  } else {
-#pragma unroll
-    for (int u = 0; u < U; ++u) {
-      fwd[u] = ab_exp_core(lkf[u]);
-      rev[u] = ab_exp_core(lkr[u]);
-    }
-  }
+  RT fwd[U], rev[U];
+  LR::template exp_pairs<U>(lkf, lkr, fwd, rev);
 #pragma unroll
   for (int u = 0; u < U; ++u) {
-    const unsigned char *cc = cells + (c[u] << 3);
-    fwd[u] = fwd[u] * lds_f64(cc, fo[u].x);
-    rev[u] = rev[u] * lds_f64(cc, fo[u].z);
-    fwd[u] = fwd[u] * lds_f64(cc, fo[u].y);
-    rev[u] = rev[u] * lds_f64(cc, fo[u].w);
-    const double q = (fwd[u] - rev[u]) * LS_AT(double, LS_L(oRof), k[u], c[u]);   // Eq 14
+    const unsigned char *cc = cells + c[u] * (unsigned)sizeof(RT);
+    fwd[u] = fwd[u] * *(const RT *)(cc + fo[u].x);
+    rev[u] = rev[u] * *(const RT *)(cc + fo[u].z);
+    fwd[u] = fwd[u] * *(const RT *)(cc + fo[u].y);
+    rev[u] = rev[u] * *(const RT *)(cc + fo[u].w);
+    const RT q = (fwd[u] - rev[u]) * LS_AT(RT, LS_L(oRof), k[u], c[u]);   // Eq 14
     if (valid[u]) {
-      LS_AT(double, LS_L(oQ), k[u], c[u]) = q;
-      LS_AT(double, LS_L(oQ), Rp + k[u], c[u]) = -q;
+      LS_AT(RT, LS_L(oQ), k[u], c[u]) = q;
+      LS_AT(RT, LS_L(oQ), Rp + k[u], c[u]) = -q;
       if (has2) {
-        const double q2 = q + q;
-        LS_AT(double, LS_L(oQ), 2 * Rp + k[u], c[u]) = q2;
-        LS_AT(double, LS_L(oQ), 3 * Rp + k[u], c[u]) = -q2;
+        const RT q2 = q + q;
+        LS_AT(RT, LS_L(oQ), 2 * Rp + k[u], c[u]) = q2;
+        LS_AT(RT, LS_L(oQ), 3 * Rp + k[u], c[u]) = -q2;
       }
     }
   }
 }
 
 // passes [s0, s1) of this warp, two at a time while two are left
-template <class SH>
+template <class SH, typename RT>
 __device__ __forceinline__ void ls_rev_range(const LsArgs &a, const unsigned char *tbl, unsigned char *cells, int sc_set, uint32_t trow,
                                              int s0, int s1, int warp, int lane) {
   const int n_mine = (LS_L(n_rev_pass) - warp + kLsPassWarps - 1) / kLsPassWarps;   // passes of this warp
   s1 = (s1 < n_mine) ? s1 : n_mine;
   int s = s0;
-  for (; s + 2 <= s1; s += 2) ls_rev_batch<SH, 2>(a, tbl, cells, sc_set, trow, s, warp, lane);
-  if (s < s1) ls_rev_batch<SH, 1>(a, tbl, cells, sc_set, trow, s, warp, lane);
+  for (; s + 2 <= s1; s += 2) ls_rev_batch<SH, RT, 2>(a, tbl, cells, sc_set, trow, s, warp, lane);
+  if (s < s1) ls_rev_batch<SH, RT, 1>(a, tbl, cells, sc_set, trow, s, warp, lane);
 }
 
 // irreversible reactions: passes continue round robin after the reversible ones, so the warps that had one pass less get
 // these first
-template <class SH>
+template <class SH, typename RT>
 __device__ __forceinline__ void ls_irr_passes(const LsArgs &a, const unsigned char *tbl, unsigned char *cells, int sc_set, int warp, int lane) {
+  using M = MathT<RT>;
   const int C = LS_D(C), Rrev = LS_D(Rrev), Rp = LS_L(Rp), Rirr = LS_D(R) - LS_D(Rrev);
   const int n_irr_pass = LS_L(n_irr_pass);
   const bool has2 = LS_D(n_var) > 2;
@@ -248,23 +356,21 @@ __device__ __forceinline__ void ls_irr_passes(const LsArgs &a, const unsigned ch
     const bool valid = f < n_irr;
     f = valid ? f : n_irr - 1;
     const unsigned kk = ls_div_c<SH>(f, C, a.mC), c = f - kk * (unsigned)C, k = (unsigned)Rrev + kk;
-    const unsigned char *cc = cells + (c << 3);
-    const double2 p0 = ((const double2 *)(tbl + LS_L(o_rkA)))[k];
-    const double ta = ((const double2 *)(tbl + LS_L(o_rkB)))[k].x;
+    const unsigned char *cc = cells + c * (unsigned)sizeof(RT);
+    const LsPair<RT> p0 = ((const LsPair<RT> *)(tbl + LS_L(o_rkA)))[k];
+    const RT ta = ((const LsPair<RT> *)(tbl + LS_L(o_rkB)))[k].x;
     const uint4 fo = ((const uint4 *)(tbl + LS_L(o_rfac)))[k];
-    const double lk = fma_rn(-ta, LS_SC(double, kF_INVT, c), fma_rn(p0.y, LS_SC(double, kF_LNT, c), p0.x));
-    double fw;
-    if (__any_sync(kFull, ab_exp_out_of_range(lk))) fw = cexp(lk);
-    else fw = ab_exp_core(lk);
-    fw = fw * lds_f64(cc, fo.x);
-    fw = fw * lds_f64(cc, fo.y);
+    const RT lk = M::fma(-ta, LS_SC(RT, kF_INVT, c), M::fma(p0.y, LS_SC(RT, kF_LNT, c), p0.x));
+    RT fw = LsReal<RT>::exp1(lk);
+    fw = fw * *(const RT *)(cc + fo.x);
+    fw = fw * *(const RT *)(cc + fo.y);
     if (valid) {
-      LS_AT(double, LS_L(oQ), k, c) = fw;
-      LS_AT(double, LS_L(oQ), Rp + k, c) = -fw;
+      LS_AT(RT, LS_L(oQ), k, c) = fw;
+      LS_AT(RT, LS_L(oQ), Rp + k, c) = -fw;
       if (has2) {
-        const double f2 = fw + fw;
-        LS_AT(double, LS_L(oQ), 2 * Rp + k, c) = f2;
-        LS_AT(double, LS_L(oQ), 3 * Rp + k, c) = -f2;
+        const RT f2 = fw + fw;
+        LS_AT(RT, LS_L(oQ), 2 * Rp + k, c) = f2;
+        LS_AT(RT, LS_L(oQ), 3 * Rp + k, c) = -f2;
       }
     }
   }
@@ -279,8 +385,11 @@ __device__ __forceinline__ void ls_irr_passes(const LsArgs &a, const unsigned ch
 #define LST(i)
 #endif
 
-template <class SH, bool EST>
+template <class SH, bool EST, typename RT>
 __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_constant__ LsArgs a) {
+  using M = MathT<RT>;
+  using LR = LsReal<RT>;
+  using bits_t = typename LR::bits_t;
   extern __shared__ __align__(128) unsigned char smem[];
   __shared__ unsigned long long mbar;
   __shared__ uint32_t tmem_base_s;
@@ -298,34 +407,36 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
   __syncthreads();
   asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
   const uint32_t tmem_base = tmem_base_s;
-  const uint32_t trow = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)((warp >> 2) * (32 * kLsSlots));
+  const uint32_t trow = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)((warp >> 2) * 128);
 
   const LsTables &tb = a.tb;
   const SolverConsts &sc = a.sc;
   const unsigned char *tbl = smem;
   unsigned char *cells = smem + tb.bytes;
   const int S = LS_D(S), C = LS_D(C);
-  const double *W = (const double *)(tbl + LS_L(o_W)), *invW = (const double *)(tbl + LS_L(o_invW));
-  const double *tmid = (const double *)(tbl + LS_L(o_tmid)), *nasa = (const double *)(tbl + LS_L(o_nasa));
-  const double dt_max = a.t_f * sc.delta_max;   // Eq 4
-  const double t_tol = 1.0e-12 * a.t_f;         // R5
+  const RT *W = (const RT *)(tbl + LS_L(o_W)), *invW = (const RT *)(tbl + LS_L(o_invW));
+  const RT *tmid = (const RT *)(tbl + LS_L(o_tmid)), *nasa = (const RT *)(tbl + LS_L(o_nasa));
+  const RT t_f = (RT)a.t_f;
+  const RT dt_max = t_f * (RT)sc.delta_max;     // Eq 4
+  const RT t_tol = M::land_tol() * t_f;         // R5 (R26 in binary32)
+  const RT alpha = (RT)sc.alpha, y_step_max = (RT)sc.y_step_max;
   const unsigned n_cs = (unsigned)(C * S);
-  const unsigned long long kInfBits = 0x7ff0000000000000ull;
+  const bits_t kInfBits = LR::inf_bits();
   constexpr int SW = kLsWarps - 1;              // the scalar warp
   constexpr int kXBar = 1;                      // named barrier: the other warps arrive when the new mass fractions are in place
 
   // the scalar lane of cell slot `lane` keeps the cell's own scalars in registers for the whole integration
   const bool my_slot = (warp == SW) && lane < C;
   const int mc = my_slot ? lane : 0;
-  double T = 1000.0, p = kPatm, t = 0.0, inv_ctot = 0.0, rho = 1.0;
+  RT T = RT(1000), p = M::patm(), t = RT(0), inv_ctot = RT(0), rho = RT(1);
   int steps = 0, cidx = -1, pending_st = -1;
   bool active = false, exhausted = false, last = false, bad_T = false;
   int sc_set = LS_L(oSc);   // scalar set of the current step; the other one is at LS_L(oSc) + LS_L(sc_bytes)
   if (my_slot) {
     // a slot without a cell computes on a harmless finite state and commits nothing
-    for (int i = 0; i < S; ++i) LS_AT(double, LS_L(oY), i, mc) = 1.0 / (double)S;
-    LS_AT(double, LS_L(oConc), 0, mc) = 1.0;
-    LS_AT(double, LS_L(oG), 0, mc) = 0.0;
+    for (int i = 0; i < S; ++i) LS_AT(RT, LS_L(oY), i, mc) = RT(1) / (RT)S;
+    LS_AT(RT, LS_L(oConc), 0, mc) = RT(1);
+    LS_AT(RT, LS_L(oG), 0, mc) = RT(0);
   }
 #ifdef LS_TIMING
   long long tph[6] = {0, 0, 0, 0, 0, 0}, tl_ = clock64(), n_steps_ = 0;
@@ -354,8 +465,8 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
     if (g_next == 0) {
       // ---- results leave and new cells enter only at ring position 0 (see the header): write back ...
       if (my_slot && pending_st >= 0) {
-        for (int i = 0; i < S; ++i) a.Y[(long long)i * a.ld + cidx] = LS_AT(double, LS_L(oY), i, mc);
-        a.T[cidx] = T;
+        for (int i = 0; i < S; ++i) a.Y[(long long)i * a.ld + cidx] = (double)LS_AT(RT, LS_L(oY), i, mc);
+        a.T[cidx] = (double)T;
         a.steps[cidx] = steps;
         if (a.status) a.status[cidx] = (unsigned char)pending_st;
         if (pending_st > 0) atomicMax(a.worst_status, pending_st);
@@ -373,10 +484,10 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
           const long long pos = (long long)base + __popc(req & ((1u << lane) - 1u));
           if (pos < a.n_active) {
             cidx = a.list ? a.list[pos] : (int)pos;
-            T = a.T[cidx];
-            p = a.p[cidx];
-            for (int i = 0; i < S; ++i) LS_AT(double, LS_L(oY), i, mc) = a.Y[(long long)i * a.ld + cidx];
-            t = 0.0;
+            T = (RT)a.T[cidx];
+            p = (RT)a.p[cidx];
+            for (int i = 0; i < S; ++i) LS_AT(RT, LS_L(oY), i, mc) = (RT)a.Y[(long long)i * a.ld + cidx];
+            t = RT(0);
             steps = 0;
             active = true;
             fresh = 1;
@@ -390,50 +501,50 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
     if (lane == 0) s_go = go;
     // ---- scalars of the next step.  With at most 16 cells the two logarithms run side by side in the two half-warps
     // (lane c: ln T, lane 16 + c: ln(p_atm / (R_u T)) of the same cell); else one after the other.
-    double lnT, ln_c0;
+    RT lnT, ln_c0;
     if (C <= 16) {
-      const double T_peer = __shfl_sync(kFull, T, lane & 15);
-      const double lval = ab_log((lane & 16) ? (kPatm / (kRu * T_peer)) : T_peer);
+      const RT T_peer = __shfl_sync(kFull, T, lane & 15);
+      const RT lval = M::log((lane & 16) ? (M::patm() / (M::ru() * T_peer)) : T_peer);
       lnT = __shfl_sync(kFull, lval, lane & 15);
       ln_c0 = __shfl_sync(kFull, lval, (lane & 15) | 16);
     } else {
-      lnT = ab_log(T);
-      ln_c0 = ab_log(kPatm / (kRu * T));
+      lnT = M::log(T);
+      ln_c0 = M::log(M::patm() / (M::ru() * T));
     }
     if (my_slot) {
-      const double RuT = kRu * T;
-      const double c_tot = p / RuT;
-      const double invT = 1.0 / T;
-      inv_ctot = 1.0 / c_tot;
+      const RT RuT = M::ru() * T;
+      const RT c_tot = p / RuT;
+      const RT invT = RT(1) / T;
+      inv_ctot = RT(1) / c_tot;
       // 1/Wbar = sum Y_i/W_i, sequential in species order (contract 5.4); estimator inputs on the way (R18)
-      double inv_wbar = 0.0;
+      RT inv_wbar = RT(0);
       if (EST && LS_D(n_in) > 1) {
         float *cXn = (float *)(cells + LS_L(oXn));
         const float *eshift = (const float *)(tbl + LS_L(o_eshift)), *escale = (const float *)(tbl + LS_L(o_escale));
         cXn[1 * C + mc] = ((float)p - eshift[1]) * escale[1];
         for (int i = 0; i < S; ++i) {
-          const double y = LS_AT(double, LS_L(oY), i, mc);
-          inv_wbar = fma_rn(y, invW[i], inv_wbar);
+          const RT y = LS_AT(RT, LS_L(oY), i, mc);
+          inv_wbar = M::fma(y, invW[i], inv_wbar);
           cXn[(2 + i) * C + mc] = ((float)y - eshift[2 + i]) * escale[2 + i];
         }
       } else {
 #pragma unroll 4
-        for (int i = 0; i < S; ++i) inv_wbar = fma_rn(LS_AT(double, LS_L(oY), i, mc), invW[i], inv_wbar);
+        for (int i = 0; i < S; ++i) inv_wbar = M::fma(LS_AT(RT, LS_L(oY), i, mc), invW[i], inv_wbar);
       }
       if (EST) {
         float *cXn = (float *)(cells + LS_L(oXn));
         cXn[mc] = ((float)T - ((const float *)(tbl + LS_L(o_eshift)))[0]) * ((const float *)(tbl + LS_L(o_escale)))[0];
       }
       rho = c_tot / inv_wbar;
-      LS_SC(double, kF_T, mc) = T;
-      LS_SC(double, kF_P, mc) = p;
-      LS_SC(double, kF_LNT, mc) = lnT;
-      LS_SC(double, kF_LNC0, mc) = ln_c0;
-      LS_SC(double, kF_INVT, mc) = invT;
-      LS_SC(double, kF_ICTOT, mc) = inv_ctot;
-      LS_SC(double, kF_RHO, mc) = rho;
-      LS_SC(double, kF_REM, mc) = a.t_f - t;
-      LS_SC(unsigned long long, kF_TSTAR, mc) = kInfBits;
+      LS_SC(RT, kF_T, mc) = T;
+      LS_SC(RT, kF_P, mc) = p;
+      LS_SC(RT, kF_LNT, mc) = lnT;
+      LS_SC(RT, kF_LNC0, mc) = ln_c0;
+      LS_SC(RT, kF_INVT, mc) = invT;
+      LS_SC(RT, kF_ICTOT, mc) = inv_ctot;
+      LS_SC(RT, kF_RHO, mc) = rho;
+      LS_SC(RT, kF_REM, mc) = t_f - t;
+      LS_SC(bits_t, kF_TSTAR, mc) = kInfBits;
       LS_SC(int, kF_ACTIVE, mc) = active ? 1 : 0;
       LS_SC(int, kF_FRESH, mc) = fresh;
       LS_SC(int, kF_BAD, mc) = 0;
@@ -453,33 +564,33 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
       // the scalar warp's own ringing-filter passes of the step just taken (it spent that step's phase 4 on the serial
       // chain): the previous scalar set and ring position are still intact
       const int set_prev = (sc_set == LS_L(oSc)) ? LS_L(oSc) + LS_L(sc_bytes) : LS_L(oSc);
-      ls_dft<SH>(a, cells, set_prev, trow, (g13 == 0) ? kWindow - 1 : g13 - 1, warp, lane, dt_max, t_tol);
+      ls_dft<SH, RT>(a, cells, set_prev, trow, (g13 == 0) ? kWindow - 1 : g13 - 1, warp, lane, dt_max, t_tol);
     }
     for (unsigned it = (unsigned)tid; it < n_cs; it += kLsThreads) {
       const unsigned i = ls_div_c<SH>(it, C, a.mC), c = it - i * (unsigned)C;
-      const double Tc = LS_SC(double, kF_T, c), invT = LS_SC(double, kF_INVT, c), lnT = LS_SC(double, kF_LNT, c);
-      const double rho_c = LS_SC(double, kF_RHO, c);
+      const RT Tc = LS_SC(RT, kF_T, c), invT = LS_SC(RT, kF_INVT, c), lnT = LS_SC(RT, kF_LNT, c);
+      const RT rho_c = LS_SC(RT, kF_RHO, c);
       // NASA-7 (Eqs 15-16, R17): g/RT and 2 g/RT always, cp/R and h/RT without an estimator
-      const double *ca = nasa + ((Tc < tmid[i]) ? 0 : kNasaRows * S) + i;
-      const double a1a = ca[0], a2a = ca[S];
-      const double hpa = fma_rn(fma_rn(fma_rn(fma_rn(ca[8 * S], Tc, ca[7 * S]), Tc, ca[6 * S]), Tc, ca[5 * S]), Tc, a1a);
-      const double hRTa = fma_rn(ca[9 * S], invT, hpa);
-      const double spa = fma_rn(fma_rn(fma_rn(ca[12 * S], Tc, ca[11 * S]), Tc, ca[10 * S]), Tc, a2a);
-      const double sRa = fma_rn(a1a, lnT, fma_rn(spa, Tc, ca[13 * S]));
-      const double ga = hRTa - sRa;
-      LS_AT(double, LS_L(oG), 1 + i, c) = ga;
-      LS_AT(double, LS_L(oG), 1 + S + i, c) = ga + ga;
+      const RT *ca = nasa + ((Tc < tmid[i]) ? 0 : kNasaRows * S) + i;
+      const RT a1a = ca[0], a2a = ca[S];
+      const RT hpa = M::fma(M::fma(M::fma(M::fma(ca[8 * S], Tc, ca[7 * S]), Tc, ca[6 * S]), Tc, ca[5 * S]), Tc, a1a);
+      const RT hRTa = M::fma(ca[9 * S], invT, hpa);
+      const RT spa = M::fma(M::fma(M::fma(ca[12 * S], Tc, ca[11 * S]), Tc, ca[10 * S]), Tc, a2a);
+      const RT sRa = M::fma(a1a, lnT, M::fma(spa, Tc, ca[13 * S]));
+      const RT ga = hRTa - sRa;
+      LS_AT(RT, LS_L(oG), 1 + i, c) = ga;
+      LS_AT(RT, LS_L(oG), 1 + S + i, c) = ga + ga;
       if (!EST) {
-        LS_AT(double, LS_L(oCp), i, c) = fma_rn(fma_rn(fma_rn(fma_rn(ca[4 * S], Tc, ca[3 * S]), Tc, ca[2 * S]), Tc, a2a), Tc, a1a);
-        LS_AT(double, LS_L(oH), i, c) = hRTa;
+        LS_AT(RT, LS_L(oCp), i, c) = M::fma(M::fma(M::fma(M::fma(ca[4 * S], Tc, ca[3 * S]), Tc, ca[2 * S]), Tc, a2a), Tc, a1a);
+        LS_AT(RT, LS_L(oH), i, c) = hRTa;
       }
       // Y_i/W_i (for the cp sum) and the small-species stabilisation (Eqs 6-7, R7): C** = gamma(y) rho y / W
-      const double y = LS_AT(double, LS_L(oY), i, c), iw = invW[i];
-      const double ypa = (y > 0.0) ? y : 0.0;
-      double cc = (rho_c * ypa) * iw;
-      if (sc.alpha > 0.0) cc = (ypa / (sc.alpha + ypa)) * cc;
-      LS_AT(double, LS_L(oYw), i, c) = y * iw;
-      LS_AT(double, LS_L(oConc), 1 + i, c) = cc;
+      const RT y = LS_AT(RT, LS_L(oY), i, c), iw = invW[i];
+      const RT ypa = (y > RT(0)) ? y : RT(0);
+      RT cc = (rho_c * ypa) * iw;
+      if (alpha > RT(0)) cc = (ypa / (alpha + ypa)) * cc;
+      LS_AT(RT, LS_L(oYw), i, c) = y * iw;
+      LS_AT(RT, LS_L(oConc), 1 + i, c) = cc;
     }
     if (EST) {
       // hidden units, dealt from the last thread downwards (the first threads have the species above)
@@ -507,9 +618,7 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
 #pragma unroll
         for (int u = 0; u < HU; ++u) {
           if (u == 0 || it0 + (unsigned)(u * kLsThreads) < (unsigned)(C * H)) {
-            const double zd = (double)z[u];
-            cHid[cc[u] * LS_L(Hs) + jj[u]] =
-                (tb.act == 0) ? (float)(1.0 - 2.0 / (1.0 + ab_exp(2.0 * zd))) : (float)(1.0 / (1.0 + ab_exp(-zd)));
+            cHid[cc[u] * LS_L(Hs) + jj[u]] = LR::activation(z[u], tb.act);
           }
         }
       }
@@ -519,8 +628,8 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
     LST(5)
 
     // =========================== phase 2: a2 rates ===========================
-    ls_rev_range<SH>(a, tbl, cells, sc_set, trow, 0, kLsSlots, warp, lane);
-    ls_irr_passes<SH>(a, tbl, cells, sc_set, warp, lane);
+    ls_rev_range<SH, RT>(a, tbl, cells, sc_set, trow, 0, ls_slots((int)sizeof(RT)), warp, lane);
+    ls_irr_passes<SH, RT>(a, tbl, cells, sc_set, warp, lane);
     LST(2)
     __syncthreads();
     LST(5)
@@ -535,40 +644,40 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
         const bool valid = it < n_cs;
         it = valid ? it : n_cs - 1;
         const unsigned r = ls_div_c<SH>(it, C, a.mC), c = it - r * (unsigned)C;   // lanes of one species (same list) side by side
-        const unsigned char *cc = cells + (c << 3);
+        const unsigned char *cc = cells + c * (unsigned)sizeof(RT);
         const int i = gsp[r];
         const int row0 = grow[r], rows = glen[r];
         const int max_rows = __reduce_max_sync(kFull, rows);
-        double om = 0.0;
+        RT om = RT(0);
         // entries in the caller's reaction order; a shorter list reads the all-padding row (the 0.0 slot; om is never -0.0).
         // The values of the next row are fetched before this row is added.
         uint4 o = gent[(0 < rows) ? row0 : tb.g_zero_row];
-        double v0 = lds_f64(cc, o.x), v1 = lds_f64(cc, o.y), v2 = lds_f64(cc, o.z), v3 = lds_f64(cc, o.w);
+        RT v0 = *(const RT *)(cc + o.x), v1 = *(const RT *)(cc + o.y), v2 = *(const RT *)(cc + o.z), v3 = *(const RT *)(cc + o.w);
         o = gent[(1 < rows) ? row0 + 1 : tb.g_zero_row];
         for (int e = 0; e < max_rows; ++e) {
-          const double u0 = v0, u1 = v1, u2 = v2, u3 = v3;
-          v0 = lds_f64(cc, o.x);
-          v1 = lds_f64(cc, o.y);
-          v2 = lds_f64(cc, o.z);
-          v3 = lds_f64(cc, o.w);
+          const RT u0 = v0, u1 = v1, u2 = v2, u3 = v3;
+          v0 = *(const RT *)(cc + o.x);
+          v1 = *(const RT *)(cc + o.y);
+          v2 = *(const RT *)(cc + o.z);
+          v3 = *(const RT *)(cc + o.w);
           o = gent[(e + 2 < rows) ? row0 + e + 2 : tb.g_zero_row];
           om = om + u0;
           om = om + u1;
           om = om + u2;
           om = om + u3;
         }
-        const double inv_rho = 1.0 / LS_SC(double, kF_RHO, c);
-        const double r0 = (W[i] * om) * inv_rho;
-        const double y0 = LS_AT(double, LS_L(oY), i, c);
-        const double rs0 = (-r0 > 1.0e-30) ? -r0 : 1.0e-30;                       // Eq 1
-        const double ys0 = (y0 < 1.0e-20) ? 1.0 : 0.9 * y0;                       // Eq 2 (R2)
-        const double lim0 = ((sc.y_step_max < ys0) ? sc.y_step_max : ys0) / rs0;  // Eq 3
+        const RT inv_rho = RT(1) / LS_SC(RT, kF_RHO, c);
+        const RT r0 = (W[i] * om) * inv_rho;
+        const RT y0 = LS_AT(RT, LS_L(oY), i, c);
+        const RT rs0 = (-r0 > M::r_floor()) ? -r0 : M::r_floor();                 // Eq 1
+        const RT ys0 = (y0 < M::y_small()) ? RT(1) : M::ninety() * y0;            // Eq 2 (R2)
+        const RT lim0 = ((y_step_max < ys0) ? y_step_max : ys0) / rs0;            // Eq 3
         if (valid) {
-          LS_AT(double, LS_L(oConc), 1 + i, c) = r0;     // concentrations are dead: reuse for dY_i/dt
-          LS_AT(double, LS_L(oOm), i, c) = om;
+          LS_AT(RT, LS_L(oConc), 1 + i, c) = r0;     // concentrations are dead: reuse for dY_i/dt
+          LS_AT(RT, LS_L(oOm), i, c) = om;
           // min over species: every lim is a positive double, for which the ordering of the bit patterns as unsigned
           // integers is the ordering of the values; NaN is ignored like the contract's plain comparison ignores it
-          if (lim0 < bits_to_double(kInfBits)) atomicMin(&LS_SC(unsigned long long, kF_TSTAR, c), double_to_bits(lim0));
+          if (lim0 < M::inf()) atomicMin(&LS_SC(bits_t, kF_TSTAR, c), LR::to_bits(lim0));
         }
       }
     }
@@ -610,8 +719,8 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
         for (int u = 0; u < CG; ++u) {
           const int c = c0 + u;
           if (c < C) {
-            if (o < (unsigned)S) LS_AT(double, LS_L(oCp), o, c) = (double)y[u];
-            else LS_AT(double, LS_L(oH), o - S, c) = ((double)y[u] * (double)tb.h_ref_T) * LS_SC(double, kF_INVT, c);
+            if (o < (unsigned)S) LS_AT(RT, LS_L(oCp), o, c) = (RT)y[u];
+            else LS_AT(RT, LS_L(oH), o - S, c) = ((RT)y[u] * (RT)tb.h_ref_T) * LS_SC(RT, kF_INVT, c);
           }
         }
       }
@@ -625,26 +734,26 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
     const int g_next = (g13 + 1 == kWindow) ? 0 : g13 + 1;
     if (warp == SW) {
       if (my_slot) {
-        const double t_star = bits_to_double(LS_SC(unsigned long long, kF_TSTAR, mc));
-        double h = (t_star < dt_max) ? t_star : dt_max;   // Eq 5
-        const double rem = a.t_f - t;
+        const RT t_star = LR::from_bits(LS_SC(bits_t, kF_TSTAR, mc));
+        RT h = (t_star < dt_max) ? t_star : dt_max;       // Eq 5
+        const RT rem = t_f - t;
         bool lst = false;
         if (rem - h < t_tol) {                            // landing on t_f (R5)
           h = rem;
           lst = true;
         }
         // temperature equation (R15): sum (Y_i/W_i) cp_i/R and sum (h_i/RT) omega_i, each sequential in species order
-        double sum_cp = 0.0, sum_h = 0.0;
+        RT sum_cp = RT(0), sum_h = RT(0);
 #pragma unroll 4
         for (int i = 0; i < S; ++i) {
-          sum_cp = fma_rn(LS_AT(double, LS_L(oYw), i, mc), LS_AT(double, LS_L(oCp), i, mc), sum_cp);
-          sum_h = fma_rn(LS_AT(double, LS_L(oH), i, mc), LS_AT(double, LS_L(oOm), i, mc), sum_h);
+          sum_cp = M::fma(LS_AT(RT, LS_L(oYw), i, mc), LS_AT(RT, LS_L(oCp), i, mc), sum_cp);
+          sum_h = M::fma(LS_AT(RT, LS_L(oH), i, mc), LS_AT(RT, LS_L(oOm), i, mc), sum_h);
         }
-        const double dTdt = (sc.energy_mode == 0) ? -((sum_h * kRu) * T) / (rho * (kRu * sum_cp)) : 0.0;
+        const RT dTdt = (sc.energy_mode == 0) ? -((sum_h * M::ru()) * T) / (rho * (M::ru() * sum_cp)) : RT(0);
         if (active) {
-          T = fma_rn(h, dTdt, T);
-          bad_T = !(T - T == 0.0);
-          t = lst ? a.t_f : t + h;
+          T = M::fma(h, dTdt, T);
+          bad_T = !(T - T == RT(0));
+          t = lst ? t_f : t + h;
           steps += 1;
           last = lst;
         }
@@ -655,19 +764,19 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
     } else {
       for (unsigned it = (unsigned)tid; it < n_cs; it += kLsItemThreads) {
         const unsigned i = ls_div_c<SH>(it, C, a.mC), c = it - i * (unsigned)C;
-        const double t_star = bits_to_double(LS_SC(unsigned long long, kF_TSTAR, c));
-        double h = (t_star < dt_max) ? t_star : dt_max;       // Eq 5
-        const double rem = LS_SC(double, kF_REM, c);
+        const RT t_star = LR::from_bits(LS_SC(bits_t, kF_TSTAR, c));
+        RT h = (t_star < dt_max) ? t_star : dt_max;            // Eq 5
+        const RT rem = LS_SC(RT, kF_REM, c);
         if (rem - h < t_tol) h = rem;                          // landing on t_f (R5)
         if (LS_SC(int, kF_ACTIVE, c)) {
-          const double y = fma_rn(h, LS_AT(double, LS_L(oConc), 1 + i, c), LS_AT(double, LS_L(oY), i, c));   // Eq 18
-          LS_AT(double, LS_L(oY), i, c) = y;
-          if (!(y - y == 0.0)) atomicOr(&LS_SC(int, kF_BAD, c), 1);
+          const RT y = M::fma(h, LS_AT(RT, LS_L(oConc), 1 + i, c), LS_AT(RT, LS_L(oY), i, c));   // Eq 18
+          LS_AT(RT, LS_L(oY), i, c) = y;
+          if (!(y - y == RT(0))) atomicOr(&LS_SC(int, kF_BAD, c), 1);
         }
       }
       __threadfence_block();
       asm volatile("bar.arrive %0, %1;" ::"n"(kXBar), "n"(kLsThreads) : "memory");
-      ls_dft<SH>(a, cells, sc_set, trow, g13, warp, lane, dt_max, t_tol);
+      ls_dft<SH, RT>(a, cells, sc_set, trow, g13, warp, lane, dt_max, t_tol);
     }
     LST(4)
     __syncthreads();

@@ -37,6 +37,10 @@ def test_rates_bit_exact_in_float(stev, oracle, config, lanes):
 
 
 @pytest.mark.parametrize("config,n,over", [(0, 2000, {}), (1, 600, {}), (2, 300, {}), (3, 96, {}), (4, 200, {}),
+                                           (0, 2000, dict(lanes_per_cell=4)), (1, 600, dict(lanes_per_cell=16)),
+                                           (2, 300, dict(lanes_per_cell=8)), (3, 96, dict(lanes_per_cell=32)),
+                                           (4, 200, dict(lanes_per_cell=32)), (3, 700, dict(lanes_per_cell=513)),
+                                           (3, 1, {}), (3, 19, {}), (4, 1000, dict(lanes_per_cell=513)), (2, 1500, dict(lanes_per_cell=512)),
                                            (3, 64, dict(use_estimator=False)), (1, 200, dict(lanes_per_cell=1)),
                                            (1, 200, dict(lanes_per_cell=32)), (2, 200, dict(chunk_steps=300)),
                                            (1, 100, dict(max_steps=150)), (2, 100, dict(alpha=0.0, dft_first_high_bin=1)),
@@ -53,7 +57,12 @@ def test_integrate_parity_in_float(stev, oracle, config, n, over):
     if est is None:
         case.est = None
     gpu = case.integrate(state_precision=stev.STEV_STATE_FP32, **over, **sched)
-    assert gpu["stats"]["lanes_per_cell"] <= 32
+    if "lanes_per_cell" in sched:
+        assert gpu["stats"]["lanes_per_cell"] == sched["lanes_per_cell"]
+    elif "chunk_steps" in sched:
+        assert gpu["stats"]["lanes_per_cell"] <= 32           # chunked passes: the shared-memory-history kernel
+    else:
+        assert gpu["stats"]["lanes_per_cell"] == 512          # default: the lock-step kernel, binary32 instantiation
     rep = assert_parity(gpu, ref)
     print(f"binary32 config {config}: n={n} {rep} lanes={gpu['stats']['lanes_per_cell']} steps {ref['steps'].min()}..{ref['steps'].max()}")
     assert gpu["rc"] == ref["rc"]
