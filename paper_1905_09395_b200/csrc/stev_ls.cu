@@ -193,9 +193,9 @@ bool build_ls_image(const HostMechanism &m, const HostEstimator *e, std::vector<
 using LsShape0 = LsFix<3, 2, 1, 2, 0, 0, 0, 0, 32>;
 using LsShape1 = LsFix<9, 19, 11, 4, 0, 0, 0, 0, 32>;
 using LsShape2 = LsFix<20, 60, 42, 4, 0, 0, 0, 0, 32>;
-using LsShape3 = LsFix<53, 325, 225, 4, 1, 32, 1, 106, 9>;
+using LsShape3 = LsFix<53, 325, 225, 4, 1, 32, 1, 106, 8>;
 using LsShape4 = LsFix<20, 60, 42, 4, 1, 64, 22, 40, 32>;
-using LsShape3f = LsFix<53, 325, 225, 4, 1, 32, 1, 106, 18, 4>;   // config 3 with the binary32 state: 18 cells per block
+using LsShape3f = LsFix<53, 325, 225, 4, 1, 32, 1, 106, 17, 4>;   // config 3 with the binary32 state: 17 cells per block
 using LsShape4f = LsFix<20, 60, 42, 4, 1, 64, 22, 40, 32, 4>;
 
 static bool same_dims(const LsDims &x, const LsDims &y) {

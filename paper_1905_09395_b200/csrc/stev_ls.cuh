@@ -20,13 +20,13 @@ namespace stev {
 
 constexpr int kLsThreads = 512;                 // 16 warps; warp w reaches TMEM lane quarter w % 4
 constexpr int kLsWarps = kLsThreads / 32;
-constexpr int kLsPassWarps = kLsWarps;          // every warp owns (reaction, cell) passes: pass p belongs to warp p % 16
+constexpr int kLsPassWarps = kLsWarps - 1;      // the last warp is the scalar warp: it owns no reversible (reaction, cell) passes; pass p belongs to warp p % 15
 constexpr int kLsItemThreads = 32 * (kLsWarps - 1);   // threads that update the mass fractions in phase 4 (not the scalar warp)
 // A warp owns 128 tensor-memory columns of its lane quarter (4 warps per quarter x 128 = 512): four 32-column slots of
 // thirteen doubles, or eight 16-column slots of thirteen floats (stev_params.state_precision = STEV_STATE_FP32).
 __host__ __device__ constexpr int ls_slot_pitch(int es) { return es == 8 ? 32 : 16; }
 __host__ __device__ constexpr int ls_slots(int es) { return 128 / ls_slot_pitch(es); }
-__host__ __device__ constexpr int ls_max_passes(int es) { return kLsPassWarps * ls_slots(es); }   // 64 (2048 windows) / 128 (4096)
+__host__ __device__ constexpr int ls_max_passes(int es) { return kLsPassWarps * ls_slots(es); }   // 60 (1920 windows) / 120 (3840)
 constexpr int kLsMaxCells = 32;                 // one lane of the scalar warp per cell
 
 // Scalars of the cell slots, one array of C eight-byte entries per field (entry (f, c) at set + (f C + c) 8).  There are

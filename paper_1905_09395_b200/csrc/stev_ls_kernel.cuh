@@ -12,10 +12,9 @@
 //      to the scalar warp through a named barrier (bar.arrive / bar.sync) and run the whole ringing filter (a5) of the
 //      step: the filter only feeds rOF, which the rates of the next step read, so the fp64-bound filter hides the
 //      latency-bound chain.  The scalars exist in two sets used by alternate steps, so the scalar warp can write the
-//      next step's while the filter still reads this step's; its own filter passes run at the top of the next phase 1,
-//      from the previous set.
+//      next step's while the filter still reads this step's.  The scalar warp owns no reversible (reaction, cell) pairs.
 // The 13-deep history of every reversible reaction lives in TENSOR MEMORY: pass p of 32 consecutive (reaction, cell)
-// pairs belongs to warp p % 16 and sits in one 32-column slot of that warp's TMEM lane quarter.  tcgen05.st writes one
+// pairs belongs to warp p % 15 and sits in one 32-column slot of that warp's TMEM lane quarter.  tcgen05.st writes one
 // column pair for all 32 lanes at once, so all cells of a block share the ring position: a slot is refilled only when
 // the block's step counter is a multiple of 13 (the new cell then starts at physical slot 0, as the contract's R10 wants;
 // a landed cell waits at most 12 steps, < 1.5 % of the shortest integrations of the five configurations).
@@ -351,7 +350,8 @@ __device__ __forceinline__ void ls_irr_passes(const LsArgs &a, const unsigned ch
   const int n_irr_pass = LS_L(n_irr_pass);
   const bool has2 = LS_D(n_var) > 2;
   const unsigned n_irr = (unsigned)(C * Rirr);
-  for (int p = (warp - LS_L(n_rev_pass)) & (kLsWarps - 1); p < n_irr_pass; p += kLsWarps) {
+  // all sixteen warps take these; the first irreversible pass goes to the warp after the last reversible one
+  for (int p = (warp - LS_L(n_rev_pass) % kLsPassWarps) & (kLsWarps - 1); p < n_irr_pass; p += kLsWarps) {
     unsigned f = (unsigned)(p * 32 + lane);
     const bool valid = f < n_irr;
     f = valid ? f : n_irr - 1;
@@ -557,15 +557,8 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
   __syncthreads();
 
   int g13 = 0;   // ring position of the step being taken (block-uniform)
-  bool have_prev = false;
   while (s_go) {
     // =========================== phase 1: a1 thermo, concentrations, first estimator layer ===========================
-    if (warp == SW && have_prev) {
-      // the scalar warp's own ringing-filter passes of the step just taken (it spent that step's phase 4 on the serial
-      // chain): the previous scalar set and ring position are still intact
-      const int set_prev = (sc_set == LS_L(oSc)) ? LS_L(oSc) + LS_L(sc_bytes) : LS_L(oSc);
-      ls_dft<SH, RT>(a, cells, set_prev, trow, (g13 == 0) ? kWindow - 1 : g13 - 1, warp, lane, dt_max, t_tol);
-    }
     for (unsigned it = (unsigned)tid; it < n_cs; it += kLsThreads) {
       const unsigned i = ls_div_c<SH>(it, C, a.mC), c = it - i * (unsigned)C;
       const RT Tc = LS_SC(RT, kF_T, c), invT = LS_SC(RT, kF_INVT, c), lnT = LS_SC(RT, kF_LNT, c);
@@ -628,7 +621,7 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
     LST(5)
 
     // =========================== phase 2: a2 rates ===========================
-    ls_rev_range<SH, RT>(a, tbl, cells, sc_set, trow, 0, ls_slots((int)sizeof(RT)), warp, lane);
+    if (warp != SW) ls_rev_range<SH, RT>(a, tbl, cells, sc_set, trow, 0, ls_slots((int)sizeof(RT)), warp, lane);
     ls_irr_passes<SH, RT>(a, tbl, cells, sc_set, warp, lane);
     LST(2)
     __syncthreads();
@@ -783,7 +776,6 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
     LST(5)
     sc_set = set_next;
     g13 = g_next;
-    have_prev = true;
 #ifdef LS_TIMING
     n_steps_ += 1;
 #endif
