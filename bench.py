@@ -432,10 +432,7 @@ def main():
     sm_max = (clocks or {}).get("sm_max_mhz") or 1965.0
     peak_instr = workmodel.fp64_peak_instr_per_s(sm_max)
     peak_tflops = 2.0 * peak_instr / 1e12
-    kernel_name = {33: "stev_pk_kernel<1> (one warp per cell, DFT history in tensor memory)",
-                   34: "stev_pk_kernel<1, dense> (one warp per cell, 32 cells per SM, DFT history in tensor memory)",
-                   64: "stev_pk_kernel<2> (warp pair per cell, DFT history in tensor memory)",
-                   512: "stev_ls_kernel (lock-step block, DFT history in tensor memory)",
+    kernel_name = {512: "stev_ls_kernel (lock-step block, DFT history in tensor memory)",
                    513: "stev_ls_kernel<LsDyn> (lock-step block, run-time dimensions)"}.get(st["lanes_per_cell"],
                                                                              f"stev_integrate_kernel<{st['lanes_per_cell']}>")
     # DRAM bytes of one launch from ncu (dram__bytes_read.sum + dram__bytes_write.sum), known only for the captured

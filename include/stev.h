@@ -127,16 +127,15 @@ typedef struct {
   int32_t chunk_steps;    /* 0: every cell runs to completion in one pass; > 0: a pass advances each active
                              cell at most this many steps, unfinished cells are spilled to the workspace and the
                              active-cell list is compacted before the next pass */
-  int32_t lanes_per_cell; /* 0 = chosen from (S, R).  1,2,4,8,16,32 = lanes cooperating on one cell, DFT history in
-                             shared memory (any mechanism, any chunk_steps).  Kernels that keep the DFT history in tensor
-                             memory (need chunk_steps = 0, at most two factors per reaction side):
-                             33 = one warp per cell, 16 cells per SM (<= 32 species, 1..128 reversible reactions);
-                             34 = the same at 64 registers, 32 cells per SM (<= 32 species, 1..64 reversible reactions);
-                             64 = a warp pair per cell, 8 cells per SM, both warps split every phase of a step
-                                  (<= 64 species, 1..256 reversible reactions; the default for >= 128 reactions);
+  int32_t lanes_per_cell; /* 0 = the lock-step kernel wherever the call fits it, else the shared-memory-history kernel with the
+                             lane count chosen from (S, R).  1,2,4,8,16,32 = lanes cooperating on one cell, DFT history in
+                             shared memory (any mechanism, any chunk_steps).
                              512 = lock-step block: up to 32 cells of a block step together, work flattened over (reaction,
-                                  cell) and (species, cell) pairs, one warp for the scalar chains (<= 64 species; the
-                                  default for tiny mechanisms); 513 = the same with run-time dimensions only */
+                                  cell) and (species, cell) pairs, one warp for the scalar chains of all cells, DFT history in
+                                  tensor memory.  Needs chunk_steps = 0, at most two factors per reaction side, integer
+                                  coefficients and orders, <= 64 species, <= 1920 reversible reactions (3840 in binary32);
+                                  STEV_EINVAL otherwise.  513 = the same with run-time dimensions only (the instantiation any
+                                  mechanism outside the shape list runs).  Other values: STEV_EINVAL. */
   int32_t nonblocking;    /* 0: stev_integrate returns after the stream has drained, with the final return code.  1: if the call
                              is a single kernel pass (chunk_steps = 0) it only enqueues on the stream and returns STEV_OK;
                              outputs are valid after the caller synchronises the stream, and stev_integrate_finish() returns

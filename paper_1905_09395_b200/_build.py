@@ -9,8 +9,8 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libstev_b200.so")
-SOURCES = ["stev_api.cu", "stev_pk.cu", "stev_ls.cu", "stev_compact.cu", "stev_aux.cu", "stev_mlp_tc.cu"]
-HEADERS = ["stev_math.cuh", "stev_device.cuh", "stev_fast.cuh", "stev_pk.cuh", "stev_pk_kernel.cuh", "stev_ls.cuh", "stev_ls_kernel.cuh", "stev_host.h", os.path.join("..", "..", "include", "stev.h")]
+SOURCES = ["stev_api.cu", "stev_ls.cu", "stev_compact.cu", "stev_aux.cu", "stev_mlp_tc.cu"]
+HEADERS = ["stev_math.cuh", "stev_device.cuh", "stev_fast.cuh", "stev_ls.cuh", "stev_ls_kernel.cuh", "stev_host.h", os.path.join("..", "..", "include", "stev.h")]
 
 # --fmad=false: no implicit FMA contraction anywhere (arithmetic contract); FMAs are explicit.
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "--fmad=false",

@@ -402,16 +402,6 @@ int stev_mechanism_create(const stev_mechanism_desc *d, stev_mechanism **out) {
     e = cudaMalloc(&m->d_table32, image.size());
     if (e == cudaSuccess) e = cudaMemcpy(m->d_table32, image.data(), image.size(), cudaMemcpyHostToDevice);
   }
-  for (int n = 0; n < 2 && e == cudaSuccess; ++n) {   // the pair image first: it chooses the reaction order
-    static const int order[2] = {1, 0}, nw_of[2] = {1, 2};
-    const int w = order[n];
-    std::vector<unsigned char> pk;
-    m->pk_ok[w] = build_pk_image(h, nullptr, nw_of[w], pk, m->pk_tb[w], m->pk_cl[w]);
-    if (m->pk_ok[w]) {
-      e = cudaMalloc(&m->d_pk_table[w], pk.size());
-      if (e == cudaSuccess) e = cudaMemcpy(m->d_pk_table[w], pk.data(), pk.size(), cudaMemcpyHostToDevice);
-    }
-  }
   if (e == cudaSuccess) {
     std::vector<unsigned char> ls;
     m->ls_ok = build_ls_image(h, nullptr, ls, m->ls_tb);
@@ -437,8 +427,6 @@ void stev_mechanism_destroy(stev_mechanism *m) {
   if (!m) return;
   if (m->d_table) cudaFree(m->d_table);
   if (m->d_table32) cudaFree(m->d_table32);
-  for (int w = 0; w < 2; ++w)
-    if (m->d_pk_table[w]) cudaFree(m->d_pk_table[w]);
   if (m->d_ls_table) cudaFree(m->d_ls_table);
   if (m->d_ls_table32) cudaFree(m->d_ls_table32);
   delete m;
@@ -493,16 +481,6 @@ int stev_estimator_load(const stev_mechanism *m, const stev_estimator_desc *d, s
       ce = cudaMalloc(&e->d_table32, image.size());
       if (ce == cudaSuccess) ce = cudaMemcpy(e->d_table32, image.data(), image.size(), cudaMemcpyHostToDevice);
     }
-    for (int n = 0; n < 2 && ce == cudaSuccess; ++n) {
-      static const int order[2] = {1, 0}, nw_of[2] = {1, 2};
-      const int w = order[n];
-      std::vector<unsigned char> pk;
-      e->pk_ok[w] = build_pk_image(m->host, &h, nw_of[w], pk, e->pk_tb[w], e->pk_cl[w]);
-      if (e->pk_ok[w]) {
-        ce = cudaMalloc(&e->d_pk_table[w], pk.size());
-        if (ce == cudaSuccess) ce = cudaMemcpy(e->d_pk_table[w], pk.data(), pk.size(), cudaMemcpyHostToDevice);
-      }
-    }
   }
   if (ce == cudaSuccess && m) {
     std::vector<unsigned char> ls;
@@ -548,8 +526,6 @@ void stev_estimator_destroy(stev_estimator *e) {
   if (!e) return;
   if (e->d_table) cudaFree(e->d_table);
   if (e->d_table32) cudaFree(e->d_table32);
-  for (int w = 0; w < 2; ++w)
-    if (e->d_pk_table[w]) cudaFree(e->d_pk_table[w]);
   if (e->d_ls_table) cudaFree(e->d_ls_table);
   if (e->d_ls_table32) cudaFree(e->d_ls_table32);
   if (e->d_params) cudaFree(e->d_params);
@@ -731,11 +707,6 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
   if (rc) return rc;
   const bool f32 = p->state_precision == STEV_STATE_FP32;
   if ((rc = pick_tables(m, est, &tb, &table, f32))) return rc;
-  if (f32 && p->lanes_per_cell > 32 && p->lanes_per_cell != 512 && p->lanes_per_cell != 513) {
-    set_error("stev_integrate: state_precision = STEV_STATE_FP32 runs on the lock-step kernel (lanes_per_cell 0, 512, 513) or the "
-              "shared-memory-history kernel (1..32)");
-    return STEV_EINVAL;
-  }
   if (n < 0 || n > 0x7fffffff || ld < n || !(dt_cfd > 0.0) || !std::isfinite(dt_cfd)) {
     set_error("stev_integrate: need 0 <= n_cells <= 2^31-1, ld >= n_cells, dt_cfd > 0");
     return STEV_EINVAL;
@@ -752,52 +723,25 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
   cudaStream_t s = (cudaStream_t)cuda_stream;
   Workspace w = carve(workspace, *tb, p, n);
 
-  // The whole-cell-on-chip kernels with the DFT history in tensor memory (all need chunk_steps = 0 and at most two
-  // concentration factors per reaction side):
-  //   lanes_per_cell = 33:  one warp per cell, 16 cells per SM (<= 32 species, <= 128 reversible reactions)
-  //   lanes_per_cell = 34:  the same at 64 registers, 32 cells per SM (<= 64 reversible reactions)
-  //   lanes_per_cell = 64:  warp pair per cell, 8 cells per SM (both warps split every phase; the default for >= 128 reactions)
-  //   lanes_per_cell = 512: lock-step block (all cells of a block step together; the default for tiny mechanisms);
-  //                   513:  the same with the dimensions read at run time even if the shape list has the mechanism
-  int g_request = p->lanes_per_cell;   // group width handed to the shared-memory-history kernel (0: its own heuristic)
+  // The lock-step kernel keeps the DFT history in tensor memory and the whole working set of its cells on chip
+  // (stev_ls_kernel.cuh); it needs chunk_steps = 0, at most two concentration factors per reaction side and integer
+  // coefficients.  lanes_per_cell = 0: that kernel wherever the mechanism fits it; 512: the same, refusing if it does not
+  // fit; 513: the same with the dimensions read at run time even if the shape list has the mechanism; 1..32: the
+  // shared-memory-history kernel below.
+  const int g_request = (p->lanes_per_cell >= 1 && p->lanes_per_cell <= 32) ? p->lanes_per_cell : 0;
   {
-    const bool tm_common = p->chunk_steps == 0;
-    const bool pk1_ok = (est ? est->pk_ok[0] : m->pk_ok[0]) && tm_common;
-    const bool pk2_ok = (est ? est->pk_ok[1] : m->pk_ok[1]) && tm_common;
-    const bool ls_ok = (f32 ? (est ? est->ls32_ok : m->ls32_ok) : (est ? est->ls_ok : m->ls_ok)) && tm_common;
-    const bool dense_ok = pk1_ok && pk_dense_ok(est ? est->pk_tb[0] : m->pk_tb[0]);
-    int kind = 0;   // 0: sub-warp groups (history in shared memory), 1: one warp per cell, 2: warp pair, 6: dense one warp per cell, 7: lock step
-    if (p->lanes_per_cell == 33) kind = 1;
-    else if (p->lanes_per_cell == 64) kind = 2;
-    else if (p->lanes_per_cell == 34) kind = 6;
-    else if (p->lanes_per_cell == 512 || p->lanes_per_cell == 513) kind = 7;
-    else if (p->lanes_per_cell == 0 && f32) {
-      if (ls_ok) kind = 7;   // binary32 state: the lock-step kernel where the mechanism fits it, else sub-warp groups
-    } else if (p->lanes_per_cell == 0) {
-      // Measured on B200: large mechanisms -> warp pair; tiny ones (a step is a few hundred
-      // instructions) -> lock-step block, which flattens (cell, reaction) pairs over the lanes (configs 0, 1: +56 %);
-      // mid-size with an estimator -> lock-step block too (its estimator layers are shared over the cells of the block;
-      // config 4 at full size: +24 %); mid-size without -> one warp per cell, 32 cells per SM when the reversible
-      // reactions fit two 32-blocks, else 16 (config 2: the 200 000-step cells set the time, and a lone warp steps faster).
-      if (tb->R >= 128 && pk2_ok) kind = 2;
-      else if (tb->S <= 16 && tb->R <= 32 && ls_ok) kind = 7;
-      else if (est && tb->S <= 32 && ls_ok) kind = 7;
-      else if (tb->S <= 16 && tb->R <= 32) {
-        kind = 0;
-        g_request = 4;
-        while (g_request < tb->S) g_request *= 2;
-      } else if (dense_ok) kind = 6;
-      else if (pk1_ok) kind = 1;
-      else if (pk2_ok && tb->R >= 64) kind = 2;
-      else if (ls_ok) kind = 7;
-    }
-    if ((kind == 1 && !pk1_ok) || (kind == 2 && !pk2_ok) || (kind == 6 && !dense_ok) || (kind == 7 && !ls_ok)) {
-      set_error("stev_integrate: lanes_per_cell = 33 / 34 / 64 / 512 / 513 (tensor-memory kernels) need chunk_steps = 0, at most two "
-                "factors per reaction side, 1..128 (33), 1..64 (34) or 1..256 (64) reversible reactions, at most 32 (33, 34) or 64 "
-                "species");
+    const bool ls_ok = (f32 ? (est ? est->ls32_ok : m->ls32_ok) : (est ? est->ls_ok : m->ls_ok)) && p->chunk_steps == 0;
+    const bool want_ls = p->lanes_per_cell == 512 || p->lanes_per_cell == 513;
+    if (p->lanes_per_cell != 0 && !want_ls && g_request == 0) {
+      set_error("stev_integrate: lanes_per_cell must be 0, 1, 2, 4, 8, 16, 32, 512 or 513");
       return STEV_EINVAL;
     }
-    if (kind) {
+    if (want_ls && !ls_ok) {
+      set_error("stev_integrate: lanes_per_cell = 512 / 513 (lock-step kernel, DFT history in tensor memory) needs chunk_steps = 0, "
+                "at most two factors per reaction side, integer coefficients, at most 64 species");
+      return STEV_EINVAL;
+    }
+    if (ls_ok && (want_ls || p->lanes_per_cell == 0)) {
       STEV_CUDA(cudaMemsetAsync(w.counters, 0, 256, s));
       const int *order = nullptr;
       if (p->order_cells && n > 1) {
@@ -805,32 +749,21 @@ int stev_integrate(const stev_mechanism *m, const stev_estimator *est, const ste
         if (rc) return rc;
         order = w.order;
       }
-      int blocks = 0, cpb = 0, threads = kPkThreads, specialised = 0;
+      int blocks = 0;
       size_t smem = 0;
-      if (kind == 7) {
-        const stev::LsTables &ltb = f32 ? (est ? est->ls_tb32 : m->ls_tb32) : (est ? est->ls_tb : m->ls_tb);
-        const unsigned char *ltable = f32 ? (est ? est->d_ls_table32 : m->d_ls_table32) : (est ? est->d_ls_table : m->d_ls_table);
-        bool is_static = false;
-        rc = integrate_ls_launch(ltb, ltable, make_consts(p), dt_cfd, n, ld, T, pressure, Y,
-                                 steps_out, status_out, w.counters, s, &blocks, &smem, order, p->lanes_per_cell != 513, &is_static);
-        cpb = ltb.d.C;
-        threads = kLsThreads;
-        specialised = is_static ? 1 : 0;
-      } else {
-        const int wi = (kind == 2) ? 1 : 0;
-        rc = integrate_pk_launch(est ? est->pk_tb[wi] : m->pk_tb[wi], est ? est->pk_cl[wi] : m->pk_cl[wi],
-                                 est ? est->d_pk_table[wi] : m->d_pk_table[wi], make_consts(p), dt_cfd, n, ld, T, pressure, Y,
-                                 steps_out, status_out, w.counters, s, &blocks, &cpb, &smem, kind == 6, order);
-        threads = (kind == 6) ? kPkThreads4 : kPkThreads;
-      }
+      const stev::LsTables &ltb = f32 ? (est ? est->ls_tb32 : m->ls_tb32) : (est ? est->ls_tb : m->ls_tb);
+      const unsigned char *ltable = f32 ? (est ? est->d_ls_table32 : m->d_ls_table32) : (est ? est->d_ls_table : m->d_ls_table);
+      bool is_static = false;
+      rc = integrate_ls_launch(ltb, ltable, make_consts(p), dt_cfd, n, ld, T, pressure, Y, steps_out, status_out, w.counters, s,
+                               &blocks, &smem, order, p->lanes_per_cell != 513, &is_static);
       if (rc) return rc;
       g_stats.passes = 1;
-      g_stats.specialised = specialised;
+      g_stats.specialised = is_static ? 1 : 0;
       g_stats.kernel_launches = 1 + (order ? 3 : 0);   // integrator + histogram, scan, scatter of the launch order
       g_stats.blocks = blocks;
-      g_stats.lanes_per_cell = kind == 1 ? 33 : (kind == 2 ? 64 : (kind == 6 ? 34 : (p->lanes_per_cell == 513 ? 513 : 512)));
-      g_stats.threads_per_block = threads;
-      g_stats.cells_per_block = cpb;
+      g_stats.lanes_per_cell = p->lanes_per_cell == 513 ? 513 : 512;
+      g_stats.threads_per_block = kLsThreads;
+      g_stats.cells_per_block = ltb.d.C;
       g_stats.smem_bytes = (int64_t)smem;
       if (p->nonblocking) return STEV_OK;
       return finish_integrate(w.counters, s);

@@ -7,7 +7,6 @@
 #include <cuda_runtime.h>
 
 #include "../../include/stev.h"
-#include "stev_pk.cuh"
 #include "stev_ls.cuh"
 #include "stev_device.cuh"
 
@@ -39,7 +38,6 @@ struct HostMechanism {
   std::vector<double> reac_coef, prod_coef, reac_order, prod_order;   // per CSR entry, always filled (defaults applied)
   std::vector<int> internal_of;  // caller reaction index -> internal index (reversible first)
   std::vector<int> orig_of;      // internal -> caller
-  mutable std::vector<int> pk_order;     // internal -> caller of the warp-pair kernel (bank-conflict-aware, chosen once)
 };
 
 // Builds the table image for a mechanism and, optionally, an estimator.
@@ -57,16 +55,6 @@ bool choose_config(const DevTables &tb, int lanes_per_cell_request, LaunchConfig
 int device_sm_count();
 
 int estimator_tensor_prepare(stev_estimator *e);
-
-// Warp-pair integrator (stev_pk.cuh / stev_pk.cu): both warps of a cell split every phase.  Same limits as above
-// plus at most 64 species.
-bool build_pk_image(const HostMechanism &m, const HostEstimator *e, int nw, std::vector<unsigned char> &image, PkTables &tb,
-                    PkCell &cl);
-int integrate_pk_launch(const PkTables &tb, const PkCell &cl, const unsigned char *d_table, const SolverConsts &sc, double t_f,
-                        long long n, long long ld, double *T, const double *p, double *Y, int *steps, unsigned char *status,
-                        int *counters, cudaStream_t s, int *blocks_out, int *cells_per_block_out, size_t *smem_out,
-                        bool dense = false, const int *list = nullptr);
-bool pk_dense_ok(const PkTables &tb);
 
 // Lock-step integrator (stev_ls.cuh / stev_ls.cu): all cells of a block step together.  build_ls_image returns false if
 // the mechanism is outside its limits (more than two factors per reaction side, tables too large for shared memory).
@@ -95,10 +83,6 @@ struct stev_mechanism {
   unsigned char *d_table = nullptr;
   stev::DevTables tb32{};                // the same image with every real table rounded to float (state_precision FP32)
   unsigned char *d_table32 = nullptr;
-  bool pk_ok[2] = {false, false};         // images of the tensor-memory kernel: [0] one warp per cell, [1] pair (NASA-7 thermo)
-  stev::PkTables pk_tb[2]{};
-  stev::PkCell pk_cl[2]{};
-  unsigned char *d_pk_table[2] = {nullptr, nullptr};
   bool ls_ok = false;                    // image of the lock-step kernel (NASA-7 thermo)
   stev::LsTables ls_tb{};
   unsigned char *d_ls_table = nullptr;
@@ -114,10 +98,6 @@ struct stev_estimator {
   unsigned char *d_table = nullptr;
   stev::DevTables tb32{};
   unsigned char *d_table32 = nullptr;
-  bool pk_ok[2] = {false, false};         // images of the tensor-memory kernel (MLP thermo)
-  stev::PkTables pk_tb[2]{};
-  stev::PkCell pk_cl[2]{};
-  unsigned char *d_pk_table[2] = {nullptr, nullptr};
   bool ls_ok = false;                    // image of the lock-step kernel (MLP thermo)
   stev::LsTables ls_tb{};
   unsigned char *d_ls_table = nullptr;

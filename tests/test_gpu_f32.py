@@ -88,8 +88,9 @@ def test_bfer_shaped_mechanism_in_float(stev, oracle):
     assert rc == ref["rc"] and rep["bit_exact"] == 1.0, rep
 
 
-def test_float_state_refuses_the_tensor_memory_kernels(stev):
+def test_unknown_kernel_id_is_refused(stev):
     w = make_workload(3, 32)
-    with pytest.raises(stev.StevError) as err:
-        GpuCase(stev, w).integrate(state_precision=stev.STEV_STATE_FP32, lanes_per_cell=64)
-    assert err.value.code == stev.STEV_EINVAL
+    for prec in (stev.STEV_STATE_FP32, stev.STEV_STATE_FP64):
+        with pytest.raises(stev.StevError) as err:
+            GpuCase(stev, w).integrate(state_precision=prec, lanes_per_cell=64)
+        assert err.value.code == stev.STEV_EINVAL

@@ -215,77 +215,24 @@ def test_result_does_not_depend_on_lanes_per_cell(stev, oracle, config, n, lanes
     assert rep["bit_exact"] == 1.0
 
 
-@pytest.mark.parametrize("config,n,over", [(3, 500, {}), (3, 37, {}), (3, 200, dict(use_estimator=False)),
-                                           (1, 400, {}), (2, 300, {}), (4, 300, {}), (0, 600, {}),
-                                           (1, 100, dict(max_steps=150)), (2, 100, dict(alpha=0.0, dft_first_high_bin=1)),
-                                           (2, 100, dict(energy_mode=1, delta_max=0.002, y_step_max=0.05)),
-                                           (1, 100, dict(dft_enable=0, max_steps=3000))])
-@pytest.mark.parametrize("kernel", [33, 34, 64])
-def test_tensor_memory_kernels_parity(stev, oracle, kernel, config, n, over):
-    """lanes_per_cell = 33: one warp per cell (stev_pk_kernel.cuh, NW = 1), the default for small and mid-size mechanisms;
-    lanes_per_cell = 34: the same at 64 registers, 32 cells per SM (at most 64 reversible reactions);
-    lanes_per_cell = 64: the warp-pair kernel (stev_pk_kernel.cuh, NW = 2), the default for large mechanisms (config 3);
-    All keep the DFT history in tensor memory and are bit-exact against the oracle on every config they accept
-    (the lock-step kernel, lanes_per_cell = 512 / 513, has its own file: test_gpu_lockstep.py)."""
-    over = dict(over)
-    if kernel in (33, 34) and config == 3:
-        pytest.skip("one warp per cell holds at most 32 species / 128 reversible reactions (dense: 64)")
-    w = make_workload(config, n)
-    est = w.estimator if over.pop("use_estimator", True) else None
-    prm = dict(w.params, **over)
-    ref = oracle.integrate(w.mech, est, prm, w.T, w.p, w.Y, w.dt_cfd)
-    case = GpuCase(stev, w)
-    if est is None:
-        case.est = None
-    gpu = case.integrate(lanes_per_cell=kernel, **over)
-    assert gpu["stats"]["lanes_per_cell"] == kernel
-    rep = assert_parity(gpu, ref)
-    print(f"kernel {kernel} config {config}: n={n} {rep} stats={gpu['stats']}")
-    assert gpu["rc"] == ref["rc"]
-    assert rep["bit_exact"] == 1.0
-
-
-@pytest.mark.parametrize("config,kernel,n_rev", [(3, 64, 1), (3, 64, 31), (3, 64, 32), (3, 64, 33), (3, 64, 64), (3, 64, 65),
-                                                 (3, 64, 128), (3, 64, 129), (3, 64, 193), (3, 64, 224),
-                                                 (2, 33, 1), (2, 33, 31), (2, 33, 32), (2, 33, 33), (2, 64, 33), (1, 33, 1),
-                                                 (2, 34, 1), (2, 34, 31), (2, 34, 32), (2, 34, 33), (1, 34, 1)])
-def test_tensor_memory_kernels_block_boundaries(stev, oracle, config, kernel, n_rev):
-    """The tensor-memory kernels walk the reversible reactions in 32-blocks split over the warps of a cell; this runs
-    them with the number of reversible reactions at and around every block boundary (the first n_rev reversible
-    reactions of the config's mechanism stay reversible, the others become irreversible)."""
-    import dataclasses
-    w = make_workload(config, 48)
-    rev = np.array(w.mech.reversible).copy()
-    idx = np.nonzero(rev)[0]
-    assert n_rev <= idx.size
-    rev[idx[n_rev:]] = 0
-    mech = dataclasses.replace(w.mech, reversible=rev)
-    prm = dict(w.params, max_steps=4000)
-    ref = oracle.integrate(mech, None, prm, w.T, w.p, w.Y, w.dt_cfd)
-    w2 = dataclasses.replace(w, mech=mech, estimator=None)
-    gpu = GpuCase(stev, w2).integrate(lanes_per_cell=kernel, max_steps=4000)
-    assert gpu["stats"]["lanes_per_cell"] == kernel
-    rep = assert_parity(gpu, ref)
-    assert rep["bit_exact"] == 1.0, rep
-
-
 def test_default_kernel_selection(stev):
-    gpu = GpuCase(stev, make_workload(3, 64)).integrate()
-    assert gpu["stats"]["lanes_per_cell"] == 64 and gpu["stats"]["threads_per_block"] == 512
-    gpu = GpuCase(stev, make_workload(2, 64)).integrate()
-    assert gpu["stats"]["lanes_per_cell"] == 34 and gpu["stats"]["cells_per_block"] == 32   # dense: 42 reversible reactions
-    gpu = GpuCase(stev, make_workload(4, 64)).integrate()
-    assert gpu["stats"]["lanes_per_cell"] == 512 and gpu["stats"]["specialised"] == 1   # mid-size with estimator: lock-step block
-    gpu = GpuCase(stev, make_workload(1, 64)).integrate()
-    assert gpu["stats"]["lanes_per_cell"] == 512 and gpu["stats"]["specialised"] == 1   # tiny mechanism: lock-step block
-    gpu = GpuCase(stev, make_workload(0, 64)).integrate()
-    assert gpu["stats"]["lanes_per_cell"] == 512
+    """lanes_per_cell = 0: the lock-step kernel (test_gpu_lockstep.py) with compile-time dimensions for the five configs,
+    the shared-memory-history kernel for what the lock-step kernel does not take (chunked passes here; three factors per
+    side and real coefficients in test_gpu_edges.py)."""
+    cells = {0: 32, 1: 32, 2: 32, 3: 8, 4: 32}
+    for config in range(5):
+        gpu = GpuCase(stev, make_workload(config, 64)).integrate()
+        st = gpu["stats"]
+        assert st["lanes_per_cell"] == 512 and st["specialised"] == 1 and st["threads_per_block"] == 512, (config, st)
+        assert st["cells_per_block"] == cells[config], (config, st)
     gpu = GpuCase(stev, make_workload(2, 64)).integrate(chunk_steps=50)
     assert gpu["stats"]["lanes_per_cell"] <= 32
+    with pytest.raises(stev.StevError):
+        GpuCase(stev, make_workload(2, 64)).integrate(lanes_per_cell=64)   # the round-1 warp-pair kernel is gone
 
 
 @pytest.mark.parametrize("config,n,over", [(2, 3000, {}), (1, 2000, {}), (3, 300, {}), (4, 500, {}), (2, 700, dict(chunk_steps=400)),
-                                           (2, 900, dict(lanes_per_cell=33)), (0, 5000, {})])
+                                           (2, 900, dict(lanes_per_cell=513)), (0, 5000, {})])
 def test_launch_order_is_pure_scheduling(stev, config, n, over):
     """stev_params.order_cells: the persistent kernels pull the hottest cells first (counting sort on the device);
     nothing of the result may depend on it."""
