@@ -615,7 +615,7 @@ SolverConsts make_consts(const stev_params *p) {
   sc.tol_ring2 = p->tol_ring * p->tol_ring;
   sc.ring_lo = 1.0 - 1.0e-14;
   sc.ring_hi = 1.0 + 1.0e-14;
-  sc.ring_filter_ok = (p->tol_ring > 1.0e-100 && p->tol_ring < 1.0e100) ? 1 : 0;
+  sc.ring_filter_ok = (p->tol_ring > 1.0e-9 && p->tol_ring < 1.0e9) ? 1 : 0;
   sc.nhf = p->dft_first_high_bin;
   sc.dft_enable = p->dft_enable;
   sc.max_steps = p->max_steps;

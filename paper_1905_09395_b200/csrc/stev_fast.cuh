@@ -157,12 +157,13 @@ __device__ __forceinline__ bool ab_ring_exact(double d0, double m2, const Solver
 // The same decision without the square root and the division whenever it is not close: with u = 2^-53,
 // fl(d0/fl(sqrt m2)) = (d0/sqrt m2)(1 + 2.1u) at worst, while d0^2 and Tol_ring^2 m2 are each formed with at most
 // three roundings, so  d0^2 < Tol_ring^2 m2 (1 - 1e-14)  implies f_ring < Tol_ring (1 - 4e-15) < Tol_ring, and
-// symmetrically for >.  `sure` is false inside that band, when m2 or Tol_ring^2 m2 leave [1e-290, 1e290] (so that
-// no underflow, overflow or the 1e-300 guard is involved) and for NaN; the caller then evaluates ab_ring_exact.
+// symmetrically for >.  `sure` is false inside that band, when m2 leaves [2^-900, 2^901) (read off its exponent field:
+// with 1e-9 < Tol_ring < 1e9, checked on the host, neither m2 nor Tol_ring^2 m2 is then near underflow, overflow or the
+// 1e-300 guard) and for NaN (exponent field 0x7ff); the caller then evaluates ab_ring_exact.
 __device__ __forceinline__ bool ab_ring_filter(double d0, double m2, const SolverConsts &sc, bool &sure) {
   const double lhs = d0 * d0, rhs = sc.tol_ring2 * m2;
   const bool below = lhs < rhs * sc.ring_lo, above = lhs > rhs * sc.ring_hi;
-  const bool in_range = (m2 >= 1.0e-280) && (rhs >= 1.0e-290) && (rhs <= 1.0e290);
+  const bool in_range = (((unsigned)__double2hiint(m2) >> 20) - 123u) < 1801u;   // m2 is +0, positive or NaN: no sign bit
   const bool small = d0 < sc.tol_freq;
   sure = !small || (sc.ring_filter_ok && in_range && (below || above));
   return below && small;

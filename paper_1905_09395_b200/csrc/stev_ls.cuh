@@ -21,7 +21,6 @@ namespace stev {
 constexpr int kLsThreads = 512;                 // 16 warps; warp w reaches TMEM lane quarter w % 4
 constexpr int kLsWarps = kLsThreads / 32;
 constexpr int kLsPassWarps = kLsWarps - 1;      // the last warp is the scalar warp: it owns no reversible (reaction, cell) passes; pass p belongs to warp p % 15
-constexpr int kLsItemThreads = 32 * (kLsWarps - 1);   // threads that update the mass fractions in phase 4 (not the scalar warp)
 // A warp owns 128 tensor-memory columns of its lane quarter (4 warps per quarter x 128 = 512): four 32-column slots of
 // thirteen doubles, or eight 16-column slots of thirteen floats (stev_params.state_precision = STEV_STATE_FP32).
 __host__ __device__ constexpr int ls_slot_pitch(int es) { return es == 8 ? 32 : 16; }
@@ -34,12 +33,11 @@ constexpr int kLsMaxCells = 32;                 // one lane of the scalar warp p
 // warp already writes the set of step n + 1.  Written by the cell's lane of the scalar warp unless stated.
 enum LsField {
   kF_T, kF_P,                          // state of the step
-  kF_LNT, kF_LNC0, kF_INVT, kF_ICTOT, kF_RHO,
+  kF_LNT, kF_LNC0, kF_INVT, kF_ICTOT, kF_RHO, kF_INVRHO,
   kF_REM,                              // t_f - t before the step
   kF_TSTAR,                            // u64: running minimum of the limiter (atomicMin of the bit patterns, phase 3)
   kF_ACTIVE,                           // int: 1 the slot integrates a cell; 0 it waits for a refill (or the queue is empty)
   kF_FRESH,                            // int: 1 during the first step of a new cell: window owners zero the history, rOF = 1
-  kF_BAD,                              // int: non-finite mass fraction seen by the update (atomicOr, phase 4)
   kF_COUNT
 };
 

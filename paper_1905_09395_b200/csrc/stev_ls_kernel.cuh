@@ -90,6 +90,15 @@ __device__ __forceinline__ void tmem_st1(uint32_t taddr, float v) {
   asm volatile("tcgen05.st.sync.aligned.32x32b.x1.b32 [%0], {%1};" ::"r"(taddr), "r"(__float_as_uint(v)) : "memory");
 }
 
+// Shared-memory store the compiler does not see as a memory access: the loads of the following loop iterations (other
+// addresses, by construction) may be scheduled above it.  The caller closes the loop with a compiler barrier.
+__device__ __forceinline__ void ls_sts_unordered(double *p, double v) {
+  asm volatile("st.shared.f64 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(p)), "d"(v));
+}
+__device__ __forceinline__ void ls_sts_unordered(float *p, float v) {
+  asm volatile("st.shared.f32 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(p)), "f"(v));
+}
+
 // The pieces of a step that differ between the two precisions (DESIGN.md sections 5 and 5b).
 template <typename RT> struct LsReal;
 template <> struct LsReal<double> {
@@ -202,61 +211,67 @@ template <> struct LsReal<float> {
 // minimum exactly as in the update.  slot13: ring position of the step (the same for every cell of the block).
 // ---------------------------------------------------------------------------------------------------------
 template <class SH, typename RT, int NHF>
-__device__ __forceinline__ void ls_dft_pass(const LsArgs &a, unsigned char *cells, int sc_set, uint32_t trow, int s, int slot13,
-                                            int warp, int lane, RT dt_max, RT t_tol) {
+__device__ __forceinline__ void ls_dft_all(const LsArgs &a, unsigned char *cells, int sc_set, uint32_t trow, int slot13, int prank,
+                                           int lane, RT dt_max, RT t_tol) {
   using LR = LsReal<RT>;
   const SolverConsts &sc = a.sc;
   const int C = LS_D(C);
-  const int p = warp + s * kLsPassWarps;
-  if (p >= LS_L(n_rev_pass)) return;
   const unsigned n_items = (unsigned)(C * LS_D(Rrev));
-  unsigned f = (unsigned)(p * 32 + lane);
-  const bool valid = f < n_items;
-  f = valid ? f : n_items - 1;
-  const unsigned k = ls_div_c<SH>(f, C, a.mC), c = f - k * (unsigned)C;
-  const RT t_star = LR::from_bits(LS_SC(typename LR::bits_t, kF_TSTAR, c));
-  RT h = (t_star < dt_max) ? t_star : dt_max;
-  const RT rem = LS_SC(RT, kF_REM, c);
-  const bool lst = rem - h < t_tol;
-  h = lst ? rem : h;
-  const RT ic = LS_SC(RT, kF_ICTOT, c);
-  const bool on = valid && LS_SC(int, kF_ACTIVE, c) && !lst;   // the landing step's change is never looked at: the cell retires
-  if (!__any_sync(kFull, on)) return;   // landing steps and empty slots store nothing
-  const RT q = LS_AT(RT, LS_L(oQ), k, c);
-  // Eq 8 with R8, R9: the applied change in progress / C_tot.  (Lanes whose cell is not `on` overwrite a window that is
-  // zeroed before its next use.)
-  const bool ringing = LR::template window_rings<NHF>(trow + (uint32_t)(s * ls_slot_pitch((int)sizeof(RT))), slot13, (q * h) * ic, on, sc);
-  if (on) {
-    RT &rof_ref = LS_AT(RT, LS_L(oRof), k, c);
-    RT rof = rof_ref * (ringing ? MathT<RT>::inv_r_fac(sc) : (RT)sc.r_fac);   // Eqs 12-13
-    if (rof > RT(1)) rof = RT(1);
-    if (rof < (RT)sc.rof_min) rof = (RT)sc.rof_min;
-    rof_ref = rof;
-  }
-}
-
-template <class SH, typename RT, int NHF>
-__device__ __forceinline__ void ls_dft_all(const LsArgs &a, unsigned char *cells, int sc_set, uint32_t trow, int slot13, int warp,
-                                           int lane, RT dt_max, RT t_tol) {
+  // what a pass needs of its cell: the step size (from the limiter's minimum, exactly as the update forms it), 1/C_tot,
+  // and whether the step's change is looked at -- not on the landing step (the cell retires), not in an empty slot
+  RT h = RT(0), ic = RT(0);
+  bool cell_on = false;
+  auto load_cell = [&](unsigned c) {
+    const RT t_star = LR::from_bits(LS_SC(typename LR::bits_t, kF_TSTAR, c));
+    h = (t_star < dt_max) ? t_star : dt_max;
+    const RT rem = LS_SC(RT, kF_REM, c);
+    const bool lst = rem - h < t_tol;
+    h = lst ? rem : h;
+    ic = LS_SC(RT, kF_ICTOT, c);
+    cell_on = LS_SC(int, kF_ACTIVE, c) && !lst;
+  };
+  const bool fixed_cell = (32 % C) == 0;   // then a lane holds the same cell in every pass
+  if (fixed_cell) load_cell((unsigned)lane % (unsigned)C);
 #pragma unroll 1
-  for (int s = 0; s < ls_slots((int)sizeof(RT)); ++s) ls_dft_pass<SH, RT, NHF>(a, cells, sc_set, trow, s, slot13, warp, lane, dt_max, t_tol);
+  for (int s = 0; s < ls_slots((int)sizeof(RT)); ++s) {
+    const int p = prank + s * kLsPassWarps;
+    if (p >= LS_L(n_rev_pass)) break;
+    unsigned f = (unsigned)(p * 32 + lane);
+    const bool valid = f < n_items;
+    f = valid ? f : n_items - 1;
+    const unsigned k = ls_div_c<SH>(f, C, a.mC), c = f - k * (unsigned)C;
+    if (!fixed_cell) load_cell(c);
+    const bool on = valid && cell_on;
+    if (!__any_sync(kFull, on)) continue;   // landing steps and empty slots store nothing
+    const RT q = LS_AT(RT, LS_L(oQ), k, c);
+    // Eq 8 with R8, R9: the applied change in progress / C_tot.  (Lanes whose cell is not `on` overwrite a window that is
+    // zeroed before its next use.)
+    const bool ringing = LR::template window_rings<NHF>(trow + (uint32_t)(s * ls_slot_pitch((int)sizeof(RT))), slot13, (q * h) * ic, on, sc);
+    if (on) {
+      RT &rof_ref = LS_AT(RT, LS_L(oRof), k, c);
+      RT rof = rof_ref * (ringing ? MathT<RT>::inv_r_fac(sc) : (RT)sc.r_fac);   // Eqs 12-13
+      if (rof > RT(1)) rof = RT(1);
+      if (rof < (RT)sc.rof_min) rof = (RT)sc.rof_min;
+      rof_ref = rof;
+    }
+  }
 }
 
 template <class SH, typename RT>
-__device__ __forceinline__ void ls_dft(const LsArgs &a, unsigned char *cells, int sc_set, uint32_t trow, int slot13, int warp, int lane,
+__device__ __forceinline__ void ls_dft(const LsArgs &a, unsigned char *cells, int sc_set, uint32_t trow, int slot13, int prank, int lane,
                                        RT dt_max, RT t_tol) {
   if (!a.sc.dft_enable) return;
   if (sizeof(RT) == 4) {   // the binary32 filter reads the first high bin at run time
-    ls_dft_all<SH, RT, 0>(a, cells, sc_set, trow, slot13, warp, lane, dt_max, t_tol);
+    ls_dft_all<SH, RT, 0>(a, cells, sc_set, trow, slot13, prank, lane, dt_max, t_tol);
     return;
   }
   switch (a.sc.nhf) {
-    case 1: ls_dft_all<SH, RT, 1>(a, cells, sc_set, trow, slot13, warp, lane, dt_max, t_tol); break;
-    case 2: ls_dft_all<SH, RT, 2>(a, cells, sc_set, trow, slot13, warp, lane, dt_max, t_tol); break;
-    case 3: ls_dft_all<SH, RT, 3>(a, cells, sc_set, trow, slot13, warp, lane, dt_max, t_tol); break;
-    case 4: ls_dft_all<SH, RT, 4>(a, cells, sc_set, trow, slot13, warp, lane, dt_max, t_tol); break;
-    case 5: ls_dft_all<SH, RT, 5>(a, cells, sc_set, trow, slot13, warp, lane, dt_max, t_tol); break;
-    default: ls_dft_all<SH, RT, 6>(a, cells, sc_set, trow, slot13, warp, lane, dt_max, t_tol); break;
+    case 1: ls_dft_all<SH, RT, 1>(a, cells, sc_set, trow, slot13, prank, lane, dt_max, t_tol); break;
+    case 2: ls_dft_all<SH, RT, 2>(a, cells, sc_set, trow, slot13, prank, lane, dt_max, t_tol); break;
+    case 3: ls_dft_all<SH, RT, 3>(a, cells, sc_set, trow, slot13, prank, lane, dt_max, t_tol); break;
+    case 4: ls_dft_all<SH, RT, 4>(a, cells, sc_set, trow, slot13, prank, lane, dt_max, t_tol); break;
+    case 5: ls_dft_all<SH, RT, 5>(a, cells, sc_set, trow, slot13, prank, lane, dt_max, t_tol); break;
+    default: ls_dft_all<SH, RT, 6>(a, cells, sc_set, trow, slot13, prank, lane, dt_max, t_tol); break;
   }
 }
 
@@ -423,7 +438,9 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
   const unsigned n_cs = (unsigned)(C * S);
   const bits_t kInfBits = LR::inf_bits();
   constexpr int SW = kLsWarps - 1;              // the scalar warp
-  constexpr int kXBar = 1;                      // named barrier: the other warps arrive when the new mass fractions are in place
+  // Passes over the (reversible reaction, cell) pairs are dealt in the order 0 1 2 4 5 6 8 9 10 12 13 14 3 7 11: when the
+  // count is not a multiple of fifteen, the warps that share a scheduler (warp % 4) with the scalar warp get one less.
+  const int prank = ((warp & 3) == 3) ? 12 + (warp >> 2) : (warp >> 2) * 3 + (warp & 3);
 
   // the scalar lane of cell slot `lane` keeps the cell's own scalars in registers for the whole integration
   const bool my_slot = (warp == SW) && lane < C;
@@ -444,14 +461,14 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
 
   // What the scalar warp does between two steps: retirement of the step just taken (a6), write-back and refill at ring
   // position 0, and the scalars of the next step into scalar set `set_next`.  g_next: ring position of the next step.
-  auto scalar_warp_prepare = [&](int set_prev, int set_next, int g_next, bool first) {
+  // inv_wbar: sum Y_i/W_i of the updated mass fractions (from the fused loop of phase 4; recomputed here for a new cell).
+  auto scalar_warp_prepare = [&](int set_next, int g_next, bool first, RT inv_wbar, bool bad_y) {
     const int sc_keep = sc_set;
     if (!first) {
-      sc_set = set_prev;
       // ---- a6: retirement (R20) of the step just taken
       if (my_slot && active) {
         int st = -1;
-        if (bad_T || LS_SC(int, kF_BAD, mc)) st = 2;   // checked first: a non-finite landing step is not "finished"
+        if (bad_T || bad_y) st = 2;   // checked first: a non-finite landing step is not "finished"
         else if (last) st = 0;
         else if (steps >= sc.max_steps) st = 1;
         if (st >= 0) {
@@ -499,29 +516,16 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
     }
     const int go = __any_sync(kFull, my_slot && (active || pending_st >= 0));
     if (lane == 0) s_go = go;
-    // ---- scalars of the next step.  With at most 16 cells the two logarithms run side by side in the two half-warps
-    // (lane c: ln T, lane 16 + c: ln(p_atm / (R_u T)) of the same cell); else one after the other.
-    RT lnT, ln_c0;
-    if (C <= 16) {
-      const RT T_peer = __shfl_sync(kFull, T, lane & 15);
-      const RT lval = M::log((lane & 16) ? (M::patm() / (M::ru() * T_peer)) : T_peer);
-      lnT = __shfl_sync(kFull, lval, lane & 15);
-      ln_c0 = __shfl_sync(kFull, lval, (lane & 15) | 16);
-    } else {
-      lnT = M::log(T);
-      ln_c0 = M::log(M::patm() / (M::ru() * T));
-    }
-    if (my_slot) {
-      const RT RuT = M::ru() * T;
-      const RT c_tot = p / RuT;
-      const RT invT = RT(1) / T;
-      inv_ctot = RT(1) / c_tot;
-      // 1/Wbar = sum Y_i/W_i, sequential in species order (contract 5.4); estimator inputs on the way (R18)
-      RT inv_wbar = RT(0);
+    // ---- scalars of the next step.  The chain per cell is five divisions and two logarithms; the lanes of the scalar warp
+    // beyond the C cell lanes take their share: with C <= 8 four lane groups (lane = group * 8 + cell), with C <= 16 two,
+    // each evaluating one quotient / logarithm of the cell at a time with the same instructions on different operands.
+    // 1/Wbar = sum Y_i/W_i, sequential in species order (contract 5.4), comes from the fused loop of phase 4; a new cell
+    // (and the very first call) computes it here, with the estimator inputs on the way (R18).
+    if (my_slot && (first || fresh)) {
+      inv_wbar = RT(0);
       if (EST && LS_D(n_in) > 1) {
         float *cXn = (float *)(cells + LS_L(oXn));
         const float *eshift = (const float *)(tbl + LS_L(o_eshift)), *escale = (const float *)(tbl + LS_L(o_escale));
-        cXn[1 * C + mc] = ((float)p - eshift[1]) * escale[1];
         for (int i = 0; i < S; ++i) {
           const RT y = LS_AT(RT, LS_L(oY), i, mc);
           inv_wbar = M::fma(y, invW[i], inv_wbar);
@@ -531,11 +535,54 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
 #pragma unroll 4
         for (int i = 0; i < S; ++i) inv_wbar = M::fma(LS_AT(RT, LS_L(oY), i, mc), invW[i], inv_wbar);
       }
+    }
+    RT lnT, ln_c0, invT, c_tot, inv_rho;
+    const int cp = (C <= 8) ? 8 : ((C <= 16) ? 16 : 32);   // lanes per group
+    const int src = lane & (cp - 1);                        // the cell's own lane (group 0)
+    const int grp = lane / cp;
+    const RT Tb = __shfl_sync(kFull, T, src), pb = __shfl_sync(kFull, p, src), iwb = __shfl_sync(kFull, inv_wbar, src);
+    const RT RuT = M::ru() * Tb;
+    if (cp == 8) {
+      // group 0: p_atm / (R_u T), ln of it;  group 1: c_tot = p / (R_u T), 1 / c_tot;  group 2: 1 / T;  groups 1-3: ln T;
+      // groups 0, 2, 3: rho = c_tot / (1/Wbar)
+      const RT q1 = ((grp == 1) ? pb : ((grp == 2) ? RT(1) : M::patm())) / ((grp == 2) ? Tb : RuT);
+      const RT lv = M::log((grp == 0) ? q1 : Tb);
+      c_tot = __shfl_sync(kFull, q1, src + 8);
+      const RT q3 = ((grp == 1) ? RT(1) : c_tot) / ((grp == 1) ? q1 : iwb);
+      ln_c0 = lv;
+      lnT = __shfl_sync(kFull, lv, src + 8);
+      invT = __shfl_sync(kFull, q1, src + 16);
+      inv_ctot = __shfl_sync(kFull, q3, src + 8);
+      rho = q3;
+      inv_rho = RT(1) / rho;
+    } else if (cp == 16) {
+      // group 0: p_atm / (R_u T), ln of it, 1 / T;  group 1: c_tot, ln T, 1 / c_tot;  both: rho
+      const RT q1 = ((grp == 1) ? pb : M::patm()) / RuT;
+      const RT lv = M::log((grp == 0) ? q1 : Tb);
+      const RT q2 = RT(1) / ((grp == 1) ? q1 : Tb);
+      c_tot = __shfl_sync(kFull, q1, src + 16);
+      ln_c0 = lv;
+      lnT = __shfl_sync(kFull, lv, src + 16);
+      invT = q2;
+      inv_ctot = __shfl_sync(kFull, q2, src + 16);
+      rho = c_tot / iwb;
+      inv_rho = RT(1) / rho;
+    } else {
+      lnT = M::log(Tb);
+      ln_c0 = M::log(M::patm() / RuT);
+      c_tot = pb / RuT;
+      invT = RT(1) / Tb;
+      inv_ctot = RT(1) / c_tot;
+      rho = c_tot / iwb;
+      inv_rho = RT(1) / rho;
+    }
+    if (my_slot) {
       if (EST) {
         float *cXn = (float *)(cells + LS_L(oXn));
-        cXn[mc] = ((float)T - ((const float *)(tbl + LS_L(o_eshift)))[0]) * ((const float *)(tbl + LS_L(o_escale)))[0];
+        const float *eshift = (const float *)(tbl + LS_L(o_eshift)), *escale = (const float *)(tbl + LS_L(o_escale));
+        cXn[mc] = ((float)T - eshift[0]) * escale[0];
+        if (LS_D(n_in) > 1) cXn[1 * C + mc] = ((float)p - eshift[1]) * escale[1];
       }
-      rho = c_tot / inv_wbar;
       LS_SC(RT, kF_T, mc) = T;
       LS_SC(RT, kF_P, mc) = p;
       LS_SC(RT, kF_LNT, mc) = lnT;
@@ -543,17 +590,17 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
       LS_SC(RT, kF_INVT, mc) = invT;
       LS_SC(RT, kF_ICTOT, mc) = inv_ctot;
       LS_SC(RT, kF_RHO, mc) = rho;
+      LS_SC(RT, kF_INVRHO, mc) = inv_rho;
       LS_SC(RT, kF_REM, mc) = t_f - t;
       LS_SC(bits_t, kF_TSTAR, mc) = kInfBits;
       LS_SC(int, kF_ACTIVE, mc) = active ? 1 : 0;
       LS_SC(int, kF_FRESH, mc) = fresh;
-      LS_SC(int, kF_BAD, mc) = 0;
     }
     sc_set = sc_keep;
   };
 
   // ---- before the first step: the scalar warp fills the slots and prepares scalar set 0
-  if (warp == SW) scalar_warp_prepare(LS_L(oSc), LS_L(oSc), 0, true);
+  if (warp == SW) scalar_warp_prepare(LS_L(oSc), 0, true, RT(0), false);
   __syncthreads();
 
   int g13 = 0;   // ring position of the step being taken (block-uniform)
@@ -621,8 +668,8 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
     LST(5)
 
     // =========================== phase 2: a2 rates ===========================
-    if (warp != SW) ls_rev_range<SH, RT>(a, tbl, cells, sc_set, trow, 0, ls_slots((int)sizeof(RT)), warp, lane);
-    ls_irr_passes<SH, RT>(a, tbl, cells, sc_set, warp, lane);
+    if (warp != SW) ls_rev_range<SH, RT>(a, tbl, cells, sc_set, trow, 0, ls_slots((int)sizeof(RT)), prank, lane);
+    ls_irr_passes<SH, RT>(a, tbl, cells, sc_set, prank, lane);
     LST(2)
     __syncthreads();
     LST(5)
@@ -659,7 +706,7 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
           om = om + u2;
           om = om + u3;
         }
-        const RT inv_rho = RT(1) / LS_SC(RT, kF_RHO, c);
+        const RT inv_rho = LS_SC(RT, kF_INVRHO, c);
         const RT r0 = (W[i] * om) * inv_rho;
         const RT y0 = LS_AT(RT, LS_L(oY), i, c);
         const RT rs0 = (-r0 > M::r_floor()) ? -r0 : M::r_floor();                 // Eq 1
@@ -668,9 +715,20 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
         if (valid) {
           LS_AT(RT, LS_L(oConc), 1 + i, c) = r0;     // concentrations are dead: reuse for dY_i/dt
           LS_AT(RT, LS_L(oOm), i, c) = om;
-          // min over species: every lim is a positive double, for which the ordering of the bit patterns as unsigned
-          // integers is the ordering of the values; NaN is ignored like the contract's plain comparison ignores it
-          if (lim0 < M::inf()) atomicMin(&LS_SC(bits_t, kF_TSTAR, c), LR::to_bits(lim0));
+        }
+        // min over species: every lim is a positive real, for which the ordering of the bit patterns as unsigned
+        // integers is the ordering of the values; NaN is ignored like the contract's plain comparison ignores it.
+        // When C divides 32 the lanes lane, lane + C, lane + 2C ... hold the same cell: they reduce by shuffles and
+        // one lane per cell goes to the shared atomic.
+        bits_t lb = (valid && lim0 < M::inf()) ? LR::to_bits(lim0) : kInfBits;
+        if ((32 % C) == 0) {
+          for (int off = C; off < 32; off <<= 1) {
+            const bits_t o2 = __shfl_xor_sync(kFull, lb, off);
+            lb = (o2 < lb) ? o2 : lb;
+          }
+          if (lane < C && lb != kInfBits) atomicMin(&LS_SC(bits_t, kF_TSTAR, c), lb);
+        } else if (lb != kInfBits) {
+          atomicMin(&LS_SC(bits_t, kF_TSTAR, c), lb);
         }
       }
     }
@@ -726,6 +784,8 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
     const int set_next = (sc_set == LS_L(oSc)) ? LS_L(oSc) + LS_L(sc_bytes) : LS_L(oSc);
     const int g_next = (g13 + 1 == kWindow) ? 0 : g13 + 1;
     if (warp == SW) {
+      RT inv_wbar = RT(0);
+      bool bad_y = false;
       if (my_slot) {
         const RT t_star = LR::from_bits(LS_SC(bits_t, kF_TSTAR, mc));
         RT h = (t_star < dt_max) ? t_star : dt_max;       // Eq 5
@@ -735,12 +795,29 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
           h = rem;
           lst = true;
         }
-        // temperature equation (R15): sum (Y_i/W_i) cp_i/R and sum (h_i/RT) omega_i, each sequential in species order
+        // One loop over the species carries the three sequential sums of the step side by side: the temperature
+        // equation's sum (Y_i/W_i) cp_i/R and sum (h_i/RT) omega_i (R15), and, behind the update of the mass fractions
+        // (Eq 18), 1/Wbar of the new state -- each in species order (contract 5.4).
+        // The loop body is branch-free (a slot without a cell stores its mass fractions back unchanged), so the loads
+        // of the next species are issued under the fused multiply-adds of this one.
         RT sum_cp = RT(0), sum_h = RT(0);
 #pragma unroll 4
         for (int i = 0; i < S; ++i) {
           sum_cp = M::fma(LS_AT(RT, LS_L(oYw), i, mc), LS_AT(RT, LS_L(oCp), i, mc), sum_cp);
           sum_h = M::fma(LS_AT(RT, LS_L(oH), i, mc), LS_AT(RT, LS_L(oOm), i, mc), sum_h);
+          const RT y_old = LS_AT(RT, LS_L(oY), i, mc);
+          const RT y_new = M::fma(h, LS_AT(RT, LS_L(oConc), 1 + i, mc), y_old);
+          const RT y = active ? y_new : y_old;
+          ls_sts_unordered(&LS_AT(RT, LS_L(oY), i, mc), y);
+          bad_y = bad_y | !(y - y == RT(0));
+          inv_wbar = M::fma(y, invW[i], inv_wbar);
+        }
+        asm volatile("" ::: "memory");
+        if (EST && LS_D(n_in) > 1) {   // estimator inputs of the new state (R18)
+          const float *eshift = (const float *)(tbl + LS_L(o_eshift)), *escale = (const float *)(tbl + LS_L(o_escale));
+          float *cXn = (float *)(cells + LS_L(oXn));
+#pragma unroll 4
+          for (int i = 0; i < S; ++i) cXn[(2 + i) * C + mc] = ((float)LS_AT(RT, LS_L(oY), i, mc) - eshift[2 + i]) * escale[2 + i];
         }
         const RT dTdt = (sc.energy_mode == 0) ? -((sum_h * M::ru()) * T) / (rho * (M::ru() * sum_cp)) : RT(0);
         if (active) {
@@ -751,25 +828,9 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
           last = lst;
         }
       }
-      // the new mass fractions (and the non-finite flags) of all cells are in place once every other warp has arrived
-      asm volatile("bar.sync %0, %1;" ::"n"(kXBar), "n"(kLsThreads) : "memory");
-      scalar_warp_prepare(sc_set, set_next, g_next, false);
+      scalar_warp_prepare(set_next, g_next, false, inv_wbar, bad_y);
     } else {
-      for (unsigned it = (unsigned)tid; it < n_cs; it += kLsItemThreads) {
-        const unsigned i = ls_div_c<SH>(it, C, a.mC), c = it - i * (unsigned)C;
-        const RT t_star = LR::from_bits(LS_SC(bits_t, kF_TSTAR, c));
-        RT h = (t_star < dt_max) ? t_star : dt_max;            // Eq 5
-        const RT rem = LS_SC(RT, kF_REM, c);
-        if (rem - h < t_tol) h = rem;                          // landing on t_f (R5)
-        if (LS_SC(int, kF_ACTIVE, c)) {
-          const RT y = M::fma(h, LS_AT(RT, LS_L(oConc), 1 + i, c), LS_AT(RT, LS_L(oY), i, c));   // Eq 18
-          LS_AT(RT, LS_L(oY), i, c) = y;
-          if (!(y - y == RT(0))) atomicOr(&LS_SC(int, kF_BAD, c), 1);
-        }
-      }
-      __threadfence_block();
-      asm volatile("bar.arrive %0, %1;" ::"n"(kXBar), "n"(kLsThreads) : "memory");
-      ls_dft<SH, RT>(a, cells, sc_set, trow, g13, warp, lane, dt_max, t_tol);
+      ls_dft<SH, RT>(a, cells, sc_set, trow, g13, prank, lane, dt_max, t_tol);
     }
     LST(4)
     __syncthreads();
