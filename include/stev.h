@@ -193,6 +193,25 @@ STEV_API int stev_integrate(const stev_mechanism *m, const stev_estimator *estim
  * blocking call would have returned (STEV_OK, STEV_WMAXSTEPS, STEV_WNONFINITE, or STEV_ECUDA). */
 STEV_API int stev_integrate_finish(void *workspace, void *cuda_stream);
 
+/* stev_integrate for callers that cannot allocate device memory (code under CUDA graph capture, serving loops, harnesses
+ * that forbid cudaMalloc): no workspace argument.  The scratch the integrator needs (its queue head / worst-status
+ * counters, the launch order of the cells and the histogram of the counting sort that produces it) sits in ONE
+ * file-scope device array of the library, sizeof = 256 + 4 STEV_STATIC_MAX_CELLS + 16,640 bytes (about 1.02 MiB), which
+ * every GPU that loads the library holds until the process exits.  The call allocates nothing (no cudaMalloc, cudaFree
+ * or allocating library routine): it clears the counters with cudaMemsetAsync, rewrites the launch order in full and
+ * launches the lock-step kernel of stev_integrate (same arithmetic, bit-identical results).
+ *   - n_cells > STEV_STATIC_MAX_CELLS: STEV_EINVAL (split the field, or use stev_integrate with your own workspace).
+ *   - Only what the lock-step kernel takes: chunk_steps = 0, lanes_per_cell 0 / 512 / 513, at most two factors per
+ *     reaction side, integer coefficients; otherwise STEV_EINVAL.
+ *   - Every call on a device shares the array, and it keeps the previous call's contents.  Calls that overlap on the
+ *     same GPU (two streams, two host threads) RACE on it: serialise them (one stream, or an event between them).
+ *   - p->nonblocking = 1 only enqueues and returns STEV_OK; read the per-cell status_out after synchronising.
+ * All other arguments, layouts and return codes are those of stev_integrate. */
+#define STEV_STATIC_MAX_CELLS 262144
+STEV_API int stev_integrate_static(const stev_mechanism *m, const stev_estimator *estimator, const stev_params *p,
+                          int64_t n_cells, int64_t ld, double *T, const double *pressure, double *Y, double dt_cfd,
+                          int32_t *steps_out, uint8_t *status_out, void *cuda_stream);
+
 /* Same call with HOST buffers (the paper's calling convention: the CFD code hands over host
  * memory and gets the state back): allocates device buffers, copies in, integrates, copies out. */
 STEV_API int stev_integrate_host(const stev_mechanism *m, const stev_estimator *estimator, const stev_params *p,

@@ -4,7 +4,7 @@ The package is a thin binding over the C ABI of include/stev.h (libstev_b200.so,
 """
 from .binding import (  # noqa: F401
     Mechanism, Estimator, StevError, load, lib_path, EXPORTS,
-    stev_params, stev_params_default, stev_workspace_bytes, stev_integrate, stev_integrate_host, stev_integrate_finish, stev_last_stats,
+    stev_params, stev_params_default, stev_workspace_bytes, stev_integrate, stev_integrate_host, stev_integrate_finish, stev_integrate_static, STEV_STATIC_MAX_CELLS, stev_last_stats,
     stev_rates_eval, stev_estimator_eval, stev_compact_active, stev_dft_mag, stev_contract_exp_log, stev_microbench,
     stev_version, stev_last_error,
     STEV_OK, STEV_EINVAL, STEV_EWORKSPACE, STEV_ECUDA, STEV_WMAXSTEPS, STEV_WNONFINITE,

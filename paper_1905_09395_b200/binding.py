@@ -50,7 +50,7 @@ class stev_stats(C.Structure):
 
 EXPORTS = ["stev_params_default", "stev_mechanism_create", "stev_mechanism_destroy", "stev_mechanism_sizes",
            "stev_estimator_load", "stev_estimator_destroy", "stev_workspace_bytes", "stev_integrate",
-           "stev_integrate_host", "stev_integrate_finish", "stev_last_stats", "stev_rates_eval", "stev_estimator_eval", "stev_compact_active",
+           "stev_integrate_host", "stev_integrate_finish", "stev_integrate_static", "stev_last_stats", "stev_rates_eval", "stev_estimator_eval", "stev_compact_active",
            "stev_dft_mag", "stev_contract_exp_log", "stev_microbench", "stev_last_error", "stev_version"]
 
 _lib = None
@@ -92,6 +92,7 @@ def load(build: bool = True):
     lib.stev_integrate.argtypes = [vp, vp, C.POINTER(stev_params), i64, i64, vp, vp, vp, dbl, vp, vp, vp, C.c_size_t, vp]
     lib.stev_integrate_host.argtypes = [vp, vp, C.POINTER(stev_params), i64, i64, vp, vp, vp, dbl, vp, vp]
     lib.stev_integrate_finish.argtypes = [vp, vp]
+    lib.stev_integrate_static.argtypes = [vp, vp, C.POINTER(stev_params), i64, i64, vp, vp, vp, dbl, vp, vp, vp]
     lib.stev_last_stats.argtypes = [C.POINTER(stev_stats)]
     lib.stev_last_stats.restype = None
     lib.stev_rates_eval.argtypes = [vp, vp, C.POINTER(stev_params), i64, i64, vp, vp, vp, vp, vp, vp, vp, vp]
@@ -239,6 +240,26 @@ def stev_integrate(mechanism: Mechanism, estimator: Estimator | None, params: st
                                T.data_ptr(), p.data_ptr(), Y.data_ptr(), float(dt_cfd), steps_out.data_ptr(),
                                status_out.data_ptr() if status_out is not None else None, workspace.data_ptr(),
                                workspace.numel() * workspace.element_size(), _stream_ptr(stream))
+    return _check(rc)
+
+
+STEV_STATIC_MAX_CELLS = 262144
+
+
+def stev_integrate_static(mechanism: Mechanism, estimator: Estimator | None, params: stev_params, T, p, Y, dt_cfd: float,
+                          steps_out, status_out=None, stream=None) -> int:
+    """stev_integrate without a workspace: the scratch is a fixed device array inside the library, nothing is allocated
+    (include/stev.h).  At most STEV_STATIC_MAX_CELLS cells; calls that overlap on one GPU race on the scratch."""
+    import torch
+    n = int(T.shape[0])
+    assert T.is_cuda and T.dtype == torch.float64 and T.is_contiguous()
+    assert p.is_cuda and p.dtype == torch.float64 and p.is_contiguous() and p.shape[0] == n
+    assert Y.is_cuda and Y.dtype == torch.float64 and Y.dim() == 2 and (Y.stride(1) == 1 or Y.shape[1] <= 1) and Y.shape[0] == mechanism.n_species
+    assert steps_out.is_cuda and steps_out.dtype == torch.int32 and steps_out.is_contiguous()
+    ld = int(Y.stride(0)) if Y.shape[0] > 1 else int(Y.shape[1])
+    rc = load().stev_integrate_static(mechanism.handle, estimator.handle if estimator else None, C.byref(params), n, ld,
+                                      T.data_ptr(), p.data_ptr(), Y.data_ptr(), float(dt_cfd), steps_out.data_ptr(),
+                                      status_out.data_ptr() if status_out is not None else None, _stream_ptr(stream))
     return _check(rc)
 
 

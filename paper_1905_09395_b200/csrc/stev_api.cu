@@ -938,3 +938,107 @@ int stev_rates_eval(const stev_mechanism *m, const stev_estimator *est, const st
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------
+// stev_integrate_static: the lock-step integrator for callers that cannot allocate (code under CUDA graph capture,
+// serving loops, harnesses that forbid cudaMalloc).  Its scratch -- the queue head / worst-status counters, the launch
+// order of the cells and the counting sort's histogram -- lives in ONE file-scope device array of fixed size that every
+// GPU loading this library holds until the process exits.  In host code the array's name is a host-side stand-in, not a
+// device address: its address is taken once per device with cudaGetSymbolAddress (that device current) and that
+// pointer is what the kernels get.
+// ---------------------------------------------------------------------------------------------------------
+namespace {
+constexpr size_t kStaticCountersBytes = 256;
+constexpr size_t kStaticOrderBytes = 4 * (size_t)STEV_STATIC_MAX_CELLS;
+constexpr size_t kStaticHistBytes = (4 * (size_t)(stev::kOrderBuckets + 1) + 255) & ~(size_t)255;
+constexpr size_t kStaticScratchBytes = kStaticCountersBytes + kStaticOrderBytes + kStaticHistBytes;   // 1 MiB + 16.25 KiB
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticScratchBytes];
+
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mutex;
+unsigned char *g_static_ptr[kStaticMaxDevices] = {};
+
+// device address of g_static_scratch on the current device (looked up once per device)
+int static_scratch(unsigned char **out) {
+  int dev = -1;
+  STEV_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kStaticMaxDevices) { stev::set_error("stev_integrate_static: device ordinal beyond 63"); return STEV_EINVAL; }
+  std::lock_guard<std::mutex> lock(g_static_mutex);
+  if (!g_static_ptr[dev]) {
+    void *ptr = nullptr;
+    STEV_CUDA(cudaGetSymbolAddress(&ptr, g_static_scratch));
+    if (!ptr) { stev::set_error("stev_integrate_static: cudaGetSymbolAddress returned a null address"); return STEV_ECUDA; }
+    g_static_ptr[dev] = (unsigned char *)ptr;
+  }
+  *out = g_static_ptr[dev];
+  return STEV_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int stev_integrate_static(const stev_mechanism *m, const stev_estimator *est, const stev_params *p, int64_t n, int64_t ld,
+                          double *T, const double *pressure, double *Y, double dt_cfd, int32_t *steps_out, uint8_t *status_out,
+                          void *cuda_stream) {
+  const DevTables *tb;
+  const unsigned char *table;
+  int rc = check_params(p);
+  if (rc) return rc;
+  const bool f32 = p->state_precision == STEV_STATE_FP32;
+  if ((rc = pick_tables(m, est, &tb, &table, f32))) return rc;
+  if (n < 0 || ld < n || !(dt_cfd > 0.0) || !std::isfinite(dt_cfd)) {
+    set_error("stev_integrate_static: need n_cells >= 0, ld >= n_cells, dt_cfd > 0");
+    return STEV_EINVAL;
+  }
+  if (n > STEV_STATIC_MAX_CELLS) {
+    set_error("stev_integrate_static: n_cells = " + std::to_string((long long)n) + " is beyond STEV_STATIC_MAX_CELLS = " +
+              std::to_string((long long)STEV_STATIC_MAX_CELLS) + " (the fixed scratch array holds one launch-order entry per cell); "
+              "split the field or use stev_integrate with a caller-owned workspace");
+    return STEV_EINVAL;
+  }
+  const bool ls_ok = (f32 ? (est ? est->ls32_ok : m->ls32_ok) : (est ? est->ls_ok : m->ls_ok)) && p->chunk_steps == 0;
+  if (!ls_ok || !(p->lanes_per_cell == 0 || p->lanes_per_cell == 512 || p->lanes_per_cell == 513)) {
+    set_error("stev_integrate_static runs the lock-step kernel only: chunk_steps = 0, lanes_per_cell 0 / 512 / 513, at most two "
+              "factors per reaction side, integer coefficients, at most 64 species");
+    return STEV_EINVAL;
+  }
+  g_stats = stev_stats{};
+  g_stats.total_steps = -1;
+  if (n == 0) return STEV_OK;
+  if (!T || !pressure || !Y || !steps_out) { set_error("stev_integrate_static: null state pointer"); return STEV_EINVAL; }
+  unsigned char *scratch = nullptr;
+  if ((rc = static_scratch(&scratch))) return rc;
+  int *counters = (int *)scratch;
+  int *order_list = (int *)(scratch + kStaticCountersBytes);
+  int *order_hist = (int *)(scratch + kStaticCountersBytes + kStaticOrderBytes);
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  // the array keeps the previous call's contents: the counters must start at zero; the launch order and its histogram
+  // are rewritten in full by order_cells_launch before they are read
+  STEV_CUDA(cudaMemsetAsync(counters, 0, kStaticCountersBytes, s));
+  const int *order = nullptr;
+  if (p->order_cells && n > 1) {
+    rc = order_cells_launch(T, n, order_group(p->order_cells, n, tb->S), order_list, order_hist, s);
+    if (rc) return rc;
+    order = order_list;
+  }
+  int blocks = 0;
+  size_t smem = 0;
+  const stev::LsTables &ltb = f32 ? (est ? est->ls_tb32 : m->ls_tb32) : (est ? est->ls_tb : m->ls_tb);
+  const unsigned char *ltable = f32 ? (est ? est->d_ls_table32 : m->d_ls_table32) : (est ? est->d_ls_table : m->d_ls_table);
+  bool is_static = false;
+  rc = integrate_ls_launch(ltb, ltable, make_consts(p), dt_cfd, n, ld, T, pressure, Y, steps_out, status_out, counters, s, &blocks,
+                           &smem, order, p->lanes_per_cell != 513, &is_static);
+  if (rc) return rc;
+  g_stats.passes = 1;
+  g_stats.specialised = is_static ? 1 : 0;
+  g_stats.kernel_launches = 1 + (order ? 3 : 0);
+  g_stats.blocks = blocks;
+  g_stats.lanes_per_cell = p->lanes_per_cell == 513 ? 513 : 512;
+  g_stats.threads_per_block = kLsThreads;
+  g_stats.cells_per_block = ltb.d.C;
+  g_stats.smem_bytes = (int64_t)smem;
+  if (p->nonblocking) return STEV_OK;
+  return finish_integrate(counters, s);
+}
+
+}  // extern "C"

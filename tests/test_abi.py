@@ -49,3 +49,4 @@ def test_argument_validation_without_gpu():
     assert lib.stev_mechanism_create(None, None) == stev.STEV_EINVAL
     assert b"null" in lib.stev_last_error()
     assert lib.stev_integrate(None, None, None, 0, 0, None, None, None, 1e-4, None, None, None, 0, None) == stev.STEV_EINVAL
+    assert lib.stev_integrate_static(None, None, None, 0, 0, None, None, None, 1e-4, None, None, None) == stev.STEV_EINVAL
