@@ -225,7 +225,12 @@ STEV_API void stev_last_stats(stev_stats *out);
 STEV_API int stev_rates_eval(const stev_mechanism *m, const stev_estimator *estimator, const stev_params *p, int64_t n_cells,
                     int64_t ld, const double *T, const double *pressure, const double *Y, const double *rOF,
                     double *dYdt, double *dTdt, double *q, void *cuda_stream);
-/* Estimator forward pass: X [n][n_in] raw inputs (float, device), out [n][n_out] (float, device).  PAPER.md:126. */
+/* Estimator forward pass: X [n][n_in] raw inputs (float, device), out [n][n_out] (float, device).  PAPER.md:126.
+ * The STEV_PREC_FP32 kernel keeps the network and a tile of 128 rows in shared memory:
+ * 4 (n_params + 128 (n_in + n_hidden + n_out + 2)) bytes, n_params = n_hidden (n_in + 1) + n_out (n_hidden + 1) + 2 n_in,
+ * must fit 227 KB, else STEV_EINVAL: the largest sizes the descriptor admits (64-128-256: 387 KB) do not, 22-64-40
+ * (80 KB) and 1-32-106 do.  The TF32 / BF16 paths have their own bound (weight image + one input and one output tile
+ * within 200 KB of shared memory, accumulators within 512 tensor-memory columns) and return STEV_EINVAL beyond it. */
 STEV_API int stev_estimator_eval(const stev_estimator *e, int64_t n, const float *X, float *out, int32_t precision,
                         void *cuda_stream);
 /* Variable-load compaction: list_out = [list_in[k] (or k if list_in is NULL) for k in 0..n-1 if

@@ -102,6 +102,28 @@ bool build_ls_image(const HostMechanism &m, const HostEstimator *e, std::vector<
     if ((size_t)L.cell_bytes <= avail) break;
   }
   if (C < 1) return false;
+  {
+    // irreversible passes dealt by rate work: a reversible pass (two exponentials, the equilibrium sum, evaluated two
+    // passes side by side) counts three, an irreversible one (one exponential, one at a time) two; each pass goes to
+    // the warp with the least work so far, then every warp takes a contiguous range
+    const int n_rev_pass = L.n_rev_pass, n_irr_pass = L.n_irr_pass, PW = kLsPassWarps, NW = kLsWarps;
+    if (n_irr_pass > 255) return false;
+    int load[16] = {}, cnt[16] = {};
+    for (int r = 0; r < PW; ++r) load[r] = 3 * ((n_rev_pass - r + PW - 1) / PW);
+    for (int p = 0; p < n_irr_pass; ++p) {
+      int best = NW - 1;   // ties go to the scalar warp first, then to the highest ranks (the warps with one reversible pass less)
+      for (int r = NW - 2; r >= 0; --r)
+        if (load[r] < load[best]) best = r;
+      load[best] += 2;
+      cnt[best] += 1;
+    }
+    int start = 0;
+    for (int r = 0; r < NW; ++r) {
+      tb.irr_start[r] = (unsigned char)start;
+      tb.irr_count[r] = (unsigned char)cnt[r];
+      start += cnt[r];
+    }
+  }
 
   image.assign(tb.bytes, 0);
   unsigned char *base = image.data();

@@ -126,6 +126,9 @@ struct LsTables {
   int act, input_map;
   float h_ref_T;
   int g_zero_row;                      // index of the all-padding row of o_gent
+  // passes over the (irreversible reaction, cell) pairs of the warp of rank r: irr_start[r] .. + irr_count[r]; dealt on the
+  // host so that every warp carries about the same rate work (the scalar warp, which owns no reversible passes, the most)
+  unsigned char irr_start[16], irr_count[16];
   int bytes;                           // image size
 };
 

@@ -365,8 +365,8 @@ __device__ __forceinline__ void ls_irr_passes(const LsArgs &a, const unsigned ch
   const int n_irr_pass = LS_L(n_irr_pass);
   const bool has2 = LS_D(n_var) > 2;
   const unsigned n_irr = (unsigned)(C * Rirr);
-  // all sixteen warps take these; the first irreversible pass goes to the warp after the last reversible one
-  for (int p = (warp - LS_L(n_rev_pass) % kLsPassWarps) & (kLsWarps - 1); p < n_irr_pass; p += kLsWarps) {
+  (void)n_irr_pass;
+  for (int p = a.tb.irr_start[warp], p_end = p + a.tb.irr_count[warp]; p < p_end; ++p) {
     unsigned f = (unsigned)(p * 32 + lane);
     const bool valid = f < n_irr;
     f = valid ? f : n_irr - 1;
