@@ -119,8 +119,9 @@ typedef struct {
   int32_t energy_mode; /* STEV_ENERGY_* */
   int32_t estimator_precision; /* STEV_PREC_*: precision of the attached estimator INSIDE stev_integrate.  Only STEV_PREC_FP32 (the
                              bit-reproducible CUDA-core path, R18) is accepted there; TF32 / BF16 return STEV_EINVAL: a
-                             tensor-core contraction needs >= 64 cells at the same phase per MMA, and the estimator is 6 % of
-                             the integrator's instructions.  stev_estimator_eval runs all three. */
+                             tensor-core contraction needs >= 64 cells at the same phase per MMA where a block holds at most 32,
+                             and the estimator is 3 % (config 3) to 12 % (config 4) of the integrator's issued instructions
+                             (DESIGN.md section 7.4).  stev_estimator_eval runs all three. */
   int32_t state_precision; /* STEV_STATE_*: FP32 runs the whole step in binary32 with its own arithmetic contract
                              (DESIGN.md section 5b); checked against the oracle's binary32 mode */
   /* scheduling only: results do not depend on these */
