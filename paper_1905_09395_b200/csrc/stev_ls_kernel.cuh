@@ -278,6 +278,24 @@ __device__ __forceinline__ void ls_dft(const LsArgs &a, unsigned char *cells, in
 // two reals / four table offsets of a reaction
 template <typename RT> struct alignas(2 * sizeof(RT)) LsPair { RT x, y; };
 
+// What the rate passes need of a cell.  When C divides 32 a lane holds the same cell (lane % C) in every pass, and the
+// caller loads these once per step (fixed = true); otherwise every pass loads its own.
+template <typename RT> struct LsCellScalars {
+  bool fixed;
+  RT invT, lnT, ln_c0;
+  int fresh;
+};
+template <typename RT>
+__device__ __forceinline__ LsCellScalars<RT> ls_cell_scalars(const unsigned char *cells, int sc_set, int C, unsigned c) {
+  LsCellScalars<RT> v;
+  v.fixed = true;
+  v.invT = *(const RT *)(cells + sc_set + ((unsigned)((int)kF_INVT * C + (int)c) << 3));
+  v.lnT = *(const RT *)(cells + sc_set + ((unsigned)((int)kF_LNT * C + (int)c) << 3));
+  v.ln_c0 = *(const RT *)(cells + sc_set + ((unsigned)((int)kF_LNC0 * C + (int)c) << 3));
+  v.fresh = *(const int *)(cells + sc_set + ((unsigned)((int)kF_FRESH * C + (int)c) << 3));
+  return v;
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // a2: rates of passes s0 .. s0 + U - 1 of this warp over the (reversible reaction, cell) pairs, side by side (2 U
 // independent exponential chains in flight).  The owner of a pair also owns its DFT window and its rOF: on the first
@@ -285,7 +303,7 @@ template <typename RT> struct alignas(2 * sizeof(RT)) LsPair { RT x, y; };
 // ---------------------------------------------------------------------------------------------------------
 template <class SH, typename RT, int U>
 __device__ __forceinline__ void ls_rev_batch(const LsArgs &a, const unsigned char *tbl, unsigned char *cells, int sc_set, uint32_t trow,
-                                             int s0, int warp, int lane) {
+                                             int s0, int warp, int lane, const LsCellScalars<RT> &cs) {
   using M = MathT<RT>;
   using LR = LsReal<RT>;
   const int C = LS_D(C), Rrev = LS_D(Rrev), Rp = LS_L(Rp);
@@ -303,7 +321,7 @@ __device__ __forceinline__ void ls_rev_batch(const LsArgs &a, const unsigned cha
     f = valid[u] ? f : n_rev - 1;
     k[u] = ls_div_c<SH>(f, C, a.mC);
     c[u] = f - k[u] * (unsigned)C;
-    const bool fresh = valid[u] && LS_SC(int, kF_FRESH, c[u]);
+    const bool fresh = valid[u] && (cs.fixed ? cs.fresh : LS_SC(int, kF_FRESH, c[u]));
     if (__any_sync(kFull, fresh)) {   // rare: once per cell
       LR::window_zero_if(trow + (uint32_t)((s0 + u) * ls_slot_pitch((int)sizeof(RT))), fresh);
       if (fresh) LS_AT(RT, LS_L(oRof), k[u], c[u]) = RT(1);
@@ -312,7 +330,8 @@ __device__ __forceinline__ void ls_rev_batch(const LsArgs &a, const unsigned cha
 #pragma unroll
   for (int u = 0; u < U; ++u) {
     const unsigned char *cc = cells + c[u] * (unsigned)sizeof(RT);   // this lane's cell column
-    const RT invT = LS_SC(RT, kF_INVT, c[u]), lnT = LS_SC(RT, kF_LNT, c[u]), ln_c0 = LS_SC(RT, kF_LNC0, c[u]);
+    const RT invT = cs.fixed ? cs.invT : LS_SC(RT, kF_INVT, c[u]), lnT = cs.fixed ? cs.lnT : LS_SC(RT, kF_LNT, c[u]);
+    const RT ln_c0 = cs.fixed ? cs.ln_c0 : LS_SC(RT, kF_LNC0, c[u]);
     const LsPair<RT> p0 = ((const LsPair<RT> *)(tbl + LS_L(o_rkA)))[k[u]], p1 = ((const LsPair<RT> *)(tbl + LS_L(o_rkB)))[k[u]];
     const uint4 d = ((const uint4 *)(tbl + LS_L(o_rdg)))[k[u]];
     fo[u] = ((const uint4 *)(tbl + LS_L(o_rfac)))[k[u]];
@@ -348,18 +367,19 @@ __device__ __forceinline__ void ls_rev_batch(const LsArgs &a, const unsigned cha
 // passes [s0, s1) of this warp, two at a time while two are left
 template <class SH, typename RT>
 __device__ __forceinline__ void ls_rev_range(const LsArgs &a, const unsigned char *tbl, unsigned char *cells, int sc_set, uint32_t trow,
-                                             int s0, int s1, int warp, int lane) {
+                                             int s0, int s1, int warp, int lane, const LsCellScalars<RT> &cs) {
   const int n_mine = (LS_L(n_rev_pass) - warp + kLsPassWarps - 1) / kLsPassWarps;   // passes of this warp
   s1 = (s1 < n_mine) ? s1 : n_mine;
   int s = s0;
-  for (; s + 2 <= s1; s += 2) ls_rev_batch<SH, RT, 2>(a, tbl, cells, sc_set, trow, s, warp, lane);
-  if (s < s1) ls_rev_batch<SH, RT, 1>(a, tbl, cells, sc_set, trow, s, warp, lane);
+  for (; s + 2 <= s1; s += 2) ls_rev_batch<SH, RT, 2>(a, tbl, cells, sc_set, trow, s, warp, lane, cs);
+  if (s < s1) ls_rev_batch<SH, RT, 1>(a, tbl, cells, sc_set, trow, s, warp, lane, cs);
 }
 
 // irreversible reactions: passes continue round robin after the reversible ones, so the warps that had one pass less get
 // these first
 template <class SH, typename RT>
-__device__ __forceinline__ void ls_irr_passes(const LsArgs &a, const unsigned char *tbl, unsigned char *cells, int sc_set, int warp, int lane) {
+__device__ __forceinline__ void ls_irr_passes(const LsArgs &a, const unsigned char *tbl, unsigned char *cells, int sc_set, int warp, int lane,
+                                              const LsCellScalars<RT> &cs) {
   using M = MathT<RT>;
   const int C = LS_D(C), Rrev = LS_D(Rrev), Rp = LS_L(Rp), Rirr = LS_D(R) - LS_D(Rrev);
   const int n_irr_pass = LS_L(n_irr_pass);
@@ -375,7 +395,7 @@ __device__ __forceinline__ void ls_irr_passes(const LsArgs &a, const unsigned ch
     const LsPair<RT> p0 = ((const LsPair<RT> *)(tbl + LS_L(o_rkA)))[k];
     const RT ta = ((const LsPair<RT> *)(tbl + LS_L(o_rkB)))[k].x;
     const uint4 fo = ((const uint4 *)(tbl + LS_L(o_rfac)))[k];
-    const RT lk = M::fma(-ta, LS_SC(RT, kF_INVT, c), M::fma(p0.y, LS_SC(RT, kF_LNT, c), p0.x));
+    const RT lk = M::fma(-ta, cs.fixed ? cs.invT : LS_SC(RT, kF_INVT, c), M::fma(p0.y, cs.fixed ? cs.lnT : LS_SC(RT, kF_LNT, c), p0.x));
     RT fw = LsReal<RT>::exp1(lk);
     fw = fw * *(const RT *)(cc + fo.x);
     fw = fw * *(const RT *)(cc + fo.y);
@@ -668,8 +688,12 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
     LST(5)
 
     // =========================== phase 2: a2 rates ===========================
-    if (warp != SW) ls_rev_range<SH, RT>(a, tbl, cells, sc_set, trow, 0, ls_slots((int)sizeof(RT)), prank, lane);
-    ls_irr_passes<SH, RT>(a, tbl, cells, sc_set, prank, lane);
+    {
+      LsCellScalars<RT> cs{};
+      if ((32 % C) == 0) cs = ls_cell_scalars<RT>(cells, sc_set, C, (unsigned)lane % (unsigned)C);
+      if (warp != SW) ls_rev_range<SH, RT>(a, tbl, cells, sc_set, trow, 0, ls_slots((int)sizeof(RT)), prank, lane, cs);
+      ls_irr_passes<SH, RT>(a, tbl, cells, sc_set, prank, lane, cs);
+    }
     LST(2)
     __syncthreads();
     LST(5)
