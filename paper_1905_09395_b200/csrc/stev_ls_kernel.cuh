@@ -282,6 +282,7 @@ template <typename RT> struct alignas(2 * sizeof(RT)) LsPair { RT x, y; };
 // caller loads these once per step (fixed = true); otherwise every pass loads its own.
 template <typename RT> struct LsCellScalars {
   bool fixed;
+  unsigned c;
   RT invT, lnT, ln_c0;
   int fresh;
 };
@@ -289,6 +290,7 @@ template <typename RT>
 __device__ __forceinline__ LsCellScalars<RT> ls_cell_scalars(const unsigned char *cells, int sc_set, int C, unsigned c) {
   LsCellScalars<RT> v;
   v.fixed = true;
+  v.c = c;
   v.invT = *(const RT *)(cells + sc_set + ((unsigned)((int)kF_INVT * C + (int)c) << 3));
   v.lnT = *(const RT *)(cells + sc_set + ((unsigned)((int)kF_LNT * C + (int)c) << 3));
   v.ln_c0 = *(const RT *)(cells + sc_set + ((unsigned)((int)kF_LNC0 * C + (int)c) << 3));
@@ -311,7 +313,7 @@ __device__ __forceinline__ void ls_rev_batch(const LsArgs &a, const unsigned cha
   const unsigned n_rev = (unsigned)(C * Rrev);
   unsigned k[U], c[U];
   bool valid[U];
-  RT lkf[U], lkr[U];
+  RT lkf[U], lkr[U], cx[U], cy[U], cz[U], cw[U], rof[U];
   uint4 fo[U];
 #pragma unroll
   for (int u = 0; u < U; ++u) {
@@ -320,7 +322,7 @@ __device__ __forceinline__ void ls_rev_batch(const LsArgs &a, const unsigned cha
     valid[u] = f < n_rev;
     f = valid[u] ? f : n_rev - 1;
     k[u] = ls_div_c<SH>(f, C, a.mC);
-    c[u] = f - k[u] * (unsigned)C;
+    c[u] = cs.fixed ? cs.c : f - k[u] * (unsigned)C;   // (a lane beyond the last pair computes on (R_rev - 1, its own cell) and stores nothing)
     const bool fresh = valid[u] && (cs.fixed ? cs.fresh : LS_SC(int, kF_FRESH, c[u]));
     if (__any_sync(kFull, fresh)) {   // rare: once per cell
       LR::window_zero_if(trow + (uint32_t)((s0 + u) * ls_slot_pitch((int)sizeof(RT))), fresh);
@@ -341,17 +343,22 @@ __device__ __forceinline__ void ls_rev_batch(const LsArgs &a, const unsigned cha
     dg = dg + *(const RT *)(cc + d.z);
     dg = dg + *(const RT *)(cc + d.w);
     lkr[u] = lkf[u] - M::fma(p1.y, ln_c0, -dg);
+    // the concentration factors and rOF are fetched here, under the exponentials, not behind them
+    cx[u] = *(const RT *)(cc + fo[u].x);
+    cy[u] = *(const RT *)(cc + fo[u].y);
+    cz[u] = *(const RT *)(cc + fo[u].z);
+    cw[u] = *(const RT *)(cc + fo[u].w);
+    rof[u] = LS_AT(RT, LS_L(oRof), k[u], c[u]);
   }
   RT fwd[U], rev[U];
   LR::template exp_pairs<U>(lkf, lkr, fwd, rev);
 #pragma unroll
   for (int u = 0; u < U; ++u) {
-    const unsigned char *cc = cells + c[u] * (unsigned)sizeof(RT);
-    fwd[u] = fwd[u] * *(const RT *)(cc + fo[u].x);
-    rev[u] = rev[u] * *(const RT *)(cc + fo[u].z);
-    fwd[u] = fwd[u] * *(const RT *)(cc + fo[u].y);
-    rev[u] = rev[u] * *(const RT *)(cc + fo[u].w);
-    const RT q = (fwd[u] - rev[u]) * LS_AT(RT, LS_L(oRof), k[u], c[u]);   // Eq 14
+    fwd[u] = fwd[u] * cx[u];
+    rev[u] = rev[u] * cz[u];
+    fwd[u] = fwd[u] * cy[u];
+    rev[u] = rev[u] * cw[u];
+    const RT q = (fwd[u] - rev[u]) * rof[u];   // Eq 14
     if (valid[u]) {
       LS_AT(RT, LS_L(oQ), k[u], c[u]) = q;
       LS_AT(RT, LS_L(oQ), Rp + k[u], c[u]) = -q;
@@ -390,15 +397,16 @@ __device__ __forceinline__ void ls_irr_passes(const LsArgs &a, const unsigned ch
     unsigned f = (unsigned)(p * 32 + lane);
     const bool valid = f < n_irr;
     f = valid ? f : n_irr - 1;
-    const unsigned kk = ls_div_c<SH>(f, C, a.mC), c = f - kk * (unsigned)C, k = (unsigned)Rrev + kk;
+    const unsigned kk = ls_div_c<SH>(f, C, a.mC), c = cs.fixed ? cs.c : f - kk * (unsigned)C, k = (unsigned)Rrev + kk;
     const unsigned char *cc = cells + c * (unsigned)sizeof(RT);
     const LsPair<RT> p0 = ((const LsPair<RT> *)(tbl + LS_L(o_rkA)))[k];
     const RT ta = ((const LsPair<RT> *)(tbl + LS_L(o_rkB)))[k].x;
     const uint4 fo = ((const uint4 *)(tbl + LS_L(o_rfac)))[k];
     const RT lk = M::fma(-ta, cs.fixed ? cs.invT : LS_SC(RT, kF_INVT, c), M::fma(p0.y, cs.fixed ? cs.lnT : LS_SC(RT, kF_LNT, c), p0.x));
+    const RT cx = *(const RT *)(cc + fo.x), cy = *(const RT *)(cc + fo.y);   // fetched under the exponential
     RT fw = LsReal<RT>::exp1(lk);
-    fw = fw * *(const RT *)(cc + fo.x);
-    fw = fw * *(const RT *)(cc + fo.y);
+    fw = fw * cx;
+    fw = fw * cy;
     if (valid) {
       LS_AT(RT, LS_L(oQ), k, c) = fw;
       LS_AT(RT, LS_L(oQ), Rp + k, c) = -fw;
@@ -623,6 +631,21 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
   if (warp == SW) scalar_warp_prepare(LS_L(oSc), 0, true, RT(0), false);
   __syncthreads();
 
+  // The thread's first (species, cell) item of phase 3 never changes: its species, the rows of its source-term list and
+  // the longest list of its warp are looked up once, not at the head of every step's gather.
+  unsigned g_c = 0;
+  int g_i = 0, g_row0 = 0, g_rows = 0, g_max = 0;
+  {
+    unsigned it = (unsigned)(warp * 32 + lane);
+    it = (it < n_cs) ? it : n_cs - 1;
+    const unsigned r = ls_div_c<SH>(it, C, a.mC);
+    g_c = it - r * (unsigned)C;
+    g_i = (tbl + LS_L(o_gsp))[r];
+    g_row0 = ((const unsigned short *)(tbl + LS_L(o_grow)))[r];
+    g_rows = ((const unsigned short *)(tbl + LS_L(o_glen)))[r];
+    g_max = __reduce_max_sync(kFull, g_rows);
+  }
+
   int g13 = 0;   // ring position of the step being taken (block-uniform)
   while (s_go) {
     // =========================== phase 1: a1 thermo, concentrations, first estimator layer ===========================
@@ -707,11 +730,22 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
         unsigned it = base + (unsigned)lane;
         const bool valid = it < n_cs;
         it = valid ? it : n_cs - 1;
-        const unsigned r = ls_div_c<SH>(it, C, a.mC), c = it - r * (unsigned)C;   // lanes of one species (same list) side by side
+        // lanes of one species (same list) side by side
+        unsigned c;
+        int i, row0, rows, max_rows;
+        if (base == (unsigned)(warp * 32)) {
+          c = g_c; i = g_i; row0 = g_row0; rows = g_rows; max_rows = g_max;
+        } else {
+          const unsigned r = ls_div_c<SH>(it, C, a.mC);
+          c = it - r * (unsigned)C;
+          i = gsp[r];
+          row0 = grow[r];
+          rows = glen[r];
+          max_rows = __reduce_max_sync(kFull, rows);
+        }
         const unsigned char *cc = cells + c * (unsigned)sizeof(RT);
-        const int i = gsp[r];
-        const int row0 = grow[r], rows = glen[r];
-        const int max_rows = __reduce_max_sync(kFull, rows);
+        // what the limiter needs besides the sum is fetched before the gather, not behind it
+        const RT inv_rho = LS_SC(RT, kF_INVRHO, c), w_i = W[i], y0 = LS_AT(RT, LS_L(oY), i, c);
         RT om = RT(0);
         // entries in the caller's reaction order; a shorter list reads the all-padding row (the 0.0 slot; om is never -0.0).
         // The values of the next row are fetched before this row is added.
@@ -730,9 +764,7 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
           om = om + u2;
           om = om + u3;
         }
-        const RT inv_rho = LS_SC(RT, kF_INVRHO, c);
-        const RT r0 = (W[i] * om) * inv_rho;
-        const RT y0 = LS_AT(RT, LS_L(oY), i, c);
+        const RT r0 = (w_i * om) * inv_rho;
         const RT rs0 = (-r0 > M::r_floor()) ? -r0 : M::r_floor();                 // Eq 1
         const RT ys0 = (y0 < M::y_small()) ? RT(1) : M::ninety() * y0;            // Eq 2 (R2)
         const RT lim0 = ((y_step_max < ys0) ? y_step_max : ys0) / rs0;            // Eq 3
