@@ -183,6 +183,12 @@ bool build_ls_image(const HostMechanism &m, const HostEstimator *e, std::vector<
     put(L.o_rkA, 2 * k + 1, m.b[j]);
     put(L.o_rkB, 2 * k, m.Ea[j] / kRcal);
     put(L.o_rkB, 2 * k + 1, f32 ? (double)dnu32 : dnu);
+    // top bit of the fourth offset: some species has a coefficient of 2 in this reaction, i.e. the doubled multiples
+    // +2q, -2q are read by a gather list (the rate passes store them only then)
+    bool uses2 = false;
+    for (int en = m.reac_ptr[j]; en < m.reac_ptr[j + 1]; ++en) uses2 = uses2 || m.reac_nu[en] == 2;
+    for (int en = m.prod_ptr[j]; en < m.prod_ptr[j + 1]; ++en) uses2 = uses2 || m.prod_nu[en] == 2;
+    if (uses2) fac[3] |= 0x80000000u;
     std::memcpy(rfac + 4 * k, fac, 16);
     if (k < Rrev) std::memcpy(rdg + 4 * k, dgo, 16);
   }

@@ -59,7 +59,7 @@ struct LsDims {
 // Table image (from the image base):
 //   o_tmid, o_W, o_invW real [S] | o_nasa real [2][14][S] | o_rkA real2 [R] {ln A, b} | o_rkB real2 [R] {Ea/R_cal, dnu}
 //   o_rfac uint4 [R] offsets (from the cell region, for cell 0) of the two reactant and two product concentration factors
-//          (the 1.0 slot if absent)
+//          (the 1.0 slot if absent); top bit of .w: the reaction has a coefficient of 2, its doubled multiples are read
 //   o_rdg uint4 [Rrev] offsets of nu*g of the <= 2 reactant / <= 2 product entries (0.0 slot if absent)
 //   o_gsp uint8 [S] species with the r-th longest source-term list | o_grow, o_glen uint16 [S] first row / rows of that list
 //   o_eshift, o_escale float [n_in] | o_W1T float [n_in][H] | o_b1 float [H] | o_W2p float [n_out][Hpad] | o_b2 float [n_out]

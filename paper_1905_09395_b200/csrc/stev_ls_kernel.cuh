@@ -347,7 +347,7 @@ __device__ __forceinline__ void ls_rev_batch(const LsArgs &a, const unsigned cha
     cx[u] = *(const RT *)(cc + fo[u].x);
     cy[u] = *(const RT *)(cc + fo[u].y);
     cz[u] = *(const RT *)(cc + fo[u].z);
-    cw[u] = *(const RT *)(cc + fo[u].w);
+    cw[u] = *(const RT *)(cc + (fo[u].w & 0x7fffffffu));
     rof[u] = LS_AT(RT, LS_L(oRof), k[u], c[u]);
   }
   RT fwd[U], rev[U];
@@ -362,7 +362,7 @@ __device__ __forceinline__ void ls_rev_batch(const LsArgs &a, const unsigned cha
     if (valid[u]) {
       LS_AT(RT, LS_L(oQ), k[u], c[u]) = q;
       LS_AT(RT, LS_L(oQ), Rp + k[u], c[u]) = -q;
-      if (has2) {
+      if (has2 && (fo[u].w >> 31)) {   // only a reaction with a coefficient of 2 has readers of these
         const RT q2 = q + q;
         LS_AT(RT, LS_L(oQ), 2 * Rp + k[u], c[u]) = q2;
         LS_AT(RT, LS_L(oQ), 3 * Rp + k[u], c[u]) = -q2;
@@ -410,7 +410,7 @@ __device__ __forceinline__ void ls_irr_passes(const LsArgs &a, const unsigned ch
     if (valid) {
       LS_AT(RT, LS_L(oQ), k, c) = fw;
       LS_AT(RT, LS_L(oQ), Rp + k, c) = -fw;
-      if (has2) {
+      if (has2 && (fo.w >> 31)) {
         const RT f2 = fw + fw;
         LS_AT(RT, LS_L(oQ), 2 * Rp + k, c) = f2;
         LS_AT(RT, LS_L(oQ), 3 * Rp + k, c) = -f2;
