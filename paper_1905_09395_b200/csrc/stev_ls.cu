@@ -70,10 +70,8 @@ bool build_ls_image(const HostMechanism &m, const HostEstimator *e, std::vector<
   d.C = 1;
   LsLayout L = ls_layout_of(d);   // table offsets do not depend on C
 
-  // internal reaction order: reversible first, each group in the caller's order (lanes hold consecutive cells of one
-  // reaction, so the order within a group does not change the shared-memory bank pattern: measured, 850.5 vs 849.4 ms)
+  // internal reaction order: reversible first; within each group the caller's order, re-paired below once C is known
   std::vector<int> orig_of = m.orig_of, internal_of(R);
-  for (int k = 0; k < R; ++k) internal_of[orig_of[k]] = k;
 
   // species sorted by decreasing list length: a warp of phase 3 holds a few neighbouring ranks (times all cells), so its
   // lanes walk lists of nearly equal length
@@ -110,6 +108,57 @@ bool build_ls_image(const HostMechanism &m, const HostEstimator *e, std::vector<
       d.C = C;
       L = ls_layout_of(d);
     }
+  // When a row of the working set (C reals of one species) is 64 bytes -- 8 cells in binary64, 16 in binary32 -- the
+  // lanes that issue one shared-memory access together hold TWO consecutive reactions, and their two rows are served in
+  // one wavefront only if they lie in different halves of the 128-byte bank line, i.e. if the row indices differ by an
+  // odd number.  Consecutive internal indices (2m, 2m + 1) are therefore chosen so that as many as possible of the
+  // eight rows a rate pass reads (two + two concentration factors, two + two nu g terms) have opposite parity.  Any
+  // internal order is valid: every table is indexed through it and the source terms are summed in the caller's order.
+  if (es * C == 64) {
+    auto rows_of = [&](int j, int (&row)[8]) {
+      for (int n = 0; n < 8; ++n) row[n] = 0;   // the 1.0 slot / the 0.0 slot
+      int nf = 0, ne = 4;
+      for (int en = m.reac_ptr[j]; en < m.reac_ptr[j + 1]; ++en, ++ne) {
+        for (int n = 0; n < m.reac_nu[en]; ++n) row[nf++] = 1 + m.reac_sp[en];
+        row[ne] = 1 + (m.reac_nu[en] == 2 ? S : 0) + m.reac_sp[en];
+      }
+      nf = 2;
+      ne = 6;
+      for (int en = m.prod_ptr[j]; en < m.prod_ptr[j + 1]; ++en, ++ne) {
+        for (int n = 0; n < m.prod_nu[en]; ++n) row[nf++] = 1 + m.prod_sp[en];
+        row[ne] = 1 + (m.prod_nu[en] == 2 ? S : 0) + m.prod_sp[en];
+      }
+    };
+    auto pair_up = [&](int lo, int hi, int n_slots) {   // greedy matching inside orig_of[lo, hi)
+      std::vector<int> in(orig_of.begin() + lo, orig_of.begin() + hi), out;
+      std::vector<char> used(in.size(), 0);
+      for (size_t x = 0; x < in.size(); ++x) {
+        if (used[x]) continue;
+        used[x] = 1;
+        out.push_back(in[x]);
+        int ra[8], rb[8], best = -1, best_cost = 1 << 30;
+        rows_of(in[x], ra);
+        for (size_t y = x + 1; y < in.size(); ++y) {
+          if (used[y]) continue;
+          rows_of(in[y], rb);
+          int cost = 0;
+          for (int n = 0; n < n_slots; ++n) cost += ((ra[n] - rb[n]) & 1) ? 0 : 1;
+          if (cost < best_cost) {
+            best_cost = cost;
+            best = (int)y;
+          }
+        }
+        if (best >= 0) {
+          used[best] = 1;
+          out.push_back(in[best]);
+        }
+      }
+      std::copy(out.begin(), out.end(), orig_of.begin() + lo);
+    };
+    pair_up(0, Rrev, 8);
+    pair_up(Rrev, R, 2);   // an irreversible pass reads only its two reactant factors
+  }
+  for (int k = 0; k < R; ++k) internal_of[orig_of[k]] = k;
   {
     // irreversible passes dealt by rate work: a reversible pass (two exponentials, the equilibrium sum, evaluated two
     // passes side by side) counts three, an irreversible one (one exponential, one at a time) two; each pass goes to
