@@ -104,6 +104,8 @@ template <typename RT> struct LsReal;
 template <> struct LsReal<double> {
   using bits_t = unsigned long long;
   static __device__ __forceinline__ bits_t inf_bits() { return 0x7ff0000000000000ull; }
+  // v is infinite or NaN, i.e. !(v - v == 0): the exponent field is all ones (no fp64 instruction)
+  static __device__ __forceinline__ bool nonfinite(double v) { return ((unsigned)__double2hiint(v) & 0x7ff00000u) == 0x7ff00000u; }
   static __device__ __forceinline__ double from_bits(bits_t u) { return bits_to_double(u); }
   static __device__ __forceinline__ bits_t to_bits(double v) { return double_to_bits(v); }
   // forward and reverse exponentials of a batch: the generic routine only if any lane of the warp is out of range
@@ -166,6 +168,7 @@ template <> struct LsReal<double> {
 template <> struct LsReal<float> {
   using bits_t = unsigned int;
   static __device__ __forceinline__ bits_t inf_bits() { return 0x7f800000u; }
+  static __device__ __forceinline__ bool nonfinite(float v) { return (__float_as_uint(v) & 0x7f800000u) == 0x7f800000u; }
   static __device__ __forceinline__ float from_bits(bits_t u) { return __uint_as_float(u); }
   static __device__ __forceinline__ bits_t to_bits(float v) { return __float_as_uint(v); }
   template <int U>
@@ -856,18 +859,23 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
         // (Eq 18), 1/Wbar of the new state -- each in species order (contract 5.4).
         // The loop body is branch-free (a slot without a cell stores its mass fractions back unchanged), so the loads
         // of the next species are issued under the fused multiply-adds of this one.
+        // The scalar warp gets one issue slot in four while the three filter warps of its scheduler stream their
+        // multiply-adds, so what counts here is the number of instructions: a slot without a cell takes a step of
+        // length zero (fma(0, dY, y) = y exactly: its dY is finite, or y is already not) instead of a select, and the
+        // non-finite test reads the exponent field instead of forming y - y.
         RT sum_cp = RT(0), sum_h = RT(0);
+        const RT h_upd = active ? h : RT(0);
+        bool bad_any = false;
 #pragma unroll 4
         for (int i = 0; i < S; ++i) {
           sum_cp = M::fma(LS_AT(RT, LS_L(oYw), i, mc), LS_AT(RT, LS_L(oCp), i, mc), sum_cp);
           sum_h = M::fma(LS_AT(RT, LS_L(oH), i, mc), LS_AT(RT, LS_L(oOm), i, mc), sum_h);
-          const RT y_old = LS_AT(RT, LS_L(oY), i, mc);
-          const RT y_new = M::fma(h, LS_AT(RT, LS_L(oConc), 1 + i, mc), y_old);
-          const RT y = active ? y_new : y_old;
+          const RT y = M::fma(h_upd, LS_AT(RT, LS_L(oConc), 1 + i, mc), LS_AT(RT, LS_L(oY), i, mc));
           ls_sts_unordered(&LS_AT(RT, LS_L(oY), i, mc), y);
-          bad_y = bad_y | !(y - y == RT(0));
+          bad_any = bad_any | LR::nonfinite(y);
           inv_wbar = M::fma(y, invW[i], inv_wbar);
         }
+        bad_y = active && bad_any;
         asm volatile("" ::: "memory");
         if (EST && LS_D(n_in) > 1) {   // estimator inputs of the new state (R18)
           const float *eshift = (const float *)(tbl + LS_L(o_eshift)), *escale = (const float *)(tbl + LS_L(o_escale));
@@ -878,7 +886,7 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
         const RT dTdt = (sc.energy_mode == 0) ? -((sum_h * M::ru()) * T) / (rho * (M::ru() * sum_cp)) : RT(0);
         if (active) {
           T = M::fma(h, dTdt, T);
-          bad_T = !(T - T == RT(0));
+          bad_T = LR::nonfinite(T);
           t = lst ? t_f : t + h;
           steps += 1;
           last = lst;
