@@ -6,15 +6,17 @@
 //   2  (reaction, cell) pairs: rates (a2), q_eff = q rOF, stored multiples
 //   3  (species, cell) pairs: source terms gathered in the caller's reaction order, limiter (a3), atomicMin per cell;
 //      (output, cell) pairs: second estimator layer (it only feeds the temperature equation)
-//   4  the serial chain of the method on the SCALAR WARP, one cell per lane -- the two sequential sums of the temperature
-//      equation, T, t, step count, retirement / refill from the queue (a6), then for the NEXT step the two logarithms, the
-//      divisions and the sequential sum 1/Wbar -- while the fifteen other warps update the mass fractions (a4), hand them
-//      to the scalar warp through a named barrier (bar.arrive / bar.sync) and run the whole ringing filter (a5) of the
-//      step: the filter only feeds rOF, which the rates of the next step read, so the fp64-bound filter hides the
-//      latency-bound chain.  The scalars exist in two sets used by alternate steps, so the scalar warp can write the
-//      next step's while the filter still reads this step's.  The scalar warp owns no reversible (reaction, cell) pairs.
+//   4  the serial chain of the method on the SCALAR WARP, one cell per lane -- step size and landing, one loop over the
+//      species that carries the two sequential sums of the temperature equation and, behind the update of each mass
+//      fraction (a4), 1/Wbar of the new state, then T, t, step count, retirement / refill from the queue (a6) and for
+//      the NEXT step the two logarithms and the divisions (spread over lane groups) -- while the fifteen other warps run
+//      the whole ringing filter (a5) of the step: the filter only feeds rOF, which the rates of the next step read, so
+//      the fp64-bound filter hides the chain.  The scalars exist in two sets used by alternate steps, so the scalar
+//      warp can write the next step's while the filter still reads this step's.  The scalar warp owns no reversible
+//      (reaction, cell) pairs; beside the three filter warps of its scheduler it gets one issue slot in four, so its chain
+//      is bound by its instruction count.
 // The 13-deep history of every reversible reaction lives in TENSOR MEMORY: pass p of 32 consecutive (reaction, cell)
-// pairs belongs to warp p % 15 and sits in one 32-column slot of that warp's TMEM lane quarter.  tcgen05.st writes one
+// pairs belongs to the pass warp of rank p % 15 and sits in one 32-column slot of that warp's TMEM lane quarter.  tcgen05.st writes one
 // column pair for all 32 lanes at once, so all cells of a block share the ring position: a slot is refilled only when
 // the block's step counter is a multiple of 13 (the new cell then starts at physical slot 0, as the contract's R10 wants;
 // a landed cell waits at most 12 steps, < 1.5 % of the shortest integrations of the five configurations).
