@@ -699,9 +699,18 @@ __global__ void __launch_bounds__(kLsThreads, 1) stev_ls_kernel(const __grid_con
           z[u] = b1[jj[u]];
         }
         const float *w = W1T;
-        for (int k = 0; k < n_in; ++k, w += H) {
+        if ((kLsThreads % C) == 0) {   // the thread's units are of one cell: its input is loaded once per unit row
+          const float *xc = cXn + cc[0];
+          for (int k = 0; k < n_in; ++k, w += H) {
+            const float xk = xc[k * C];
 #pragma unroll
-          for (int u = 0; u < HU; ++u) z[u] = __fmaf_rn(w[jj[u]], cXn[k * C + cc[u]], z[u]);
+            for (int u = 0; u < HU; ++u) z[u] = __fmaf_rn(w[jj[u]], xk, z[u]);
+          }
+        } else {
+          for (int k = 0; k < n_in; ++k, w += H) {
+#pragma unroll
+            for (int u = 0; u < HU; ++u) z[u] = __fmaf_rn(w[jj[u]], cXn[k * C + cc[u]], z[u]);
+          }
         }
 #pragma unroll
         for (int u = 0; u < HU; ++u) {
